@@ -1,0 +1,408 @@
+"""Pins for the float64 oracle (oracle/delta_oracle.py) against things other than itself.
+
+The paper prints no spectral values (PAPER.md gives only Eq. 1a-1d, and structural
+constants, L107), so the oracle is pinned by closed forms, invariants, brute-force time-domain
+restatements, independent library routines (numpy.fft / scipy.signal, which are neither the
+oracle nor the CUDA path) and white-noise statistics.  Each pin names the mistake it would catch.
+Pin numbers P1..P10 follow DESIGN.md section 5.
+"""
+import os
+
+import numpy as np
+import pytest
+import scipy.signal as sps
+
+import ecei_synth as es
+from oracle import delta_oracle as o
+
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def read_constants():
+    out = {}
+    with open(os.path.join(GOLDEN, "paper_constants.txt")) as fh:
+        for line in fh:
+            line = line.split("#")[0].split()
+            if len(line) == 2:
+                out[line[0]] = int(line[1])
+    return out
+
+
+# ---------------------------------------------------------------------------- paper constants
+def test_paper_structural_constants():
+    c = read_constants()
+    assert c["grid_rows"] * c["grid_cols"] == c["n_channels"]
+    assert len(o.all_pairs(c["n_channels"])) == c["n_pairs"]
+    assert c["shot_samples"] // c["chunk_samples"] == c["shot_chunks"]
+    # segmentation rule (no padding, tail dropped) is the only one that gives BASELINE's counts
+    assert o.n_segments(2048, 256, 128) == c["tiny_segments"]
+    assert o.n_segments(100_000, 1024, 512) == c["long_segments"]
+    assert len(o.all_pairs(384)) == c["wide_pairs"]
+    assert len(o.all_pairs(8)) == c["tiny_pairs"]
+    # the workload table of the input module agrees
+    assert es.WORKLOADS["single"].P == c["n_pairs"] and es.WORKLOADS["single"].K == 38
+    assert es.WORKLOADS["wide"].K == 94 and es.WORKLOADS["long"].K == c["long_segments"]
+
+
+def test_pair_index_is_lexicographic():
+    for C in (2, 3, 8, 17):
+        pairs = o.all_pairs(C)
+        for p, (i, j) in enumerate(pairs):
+            assert i < j and o.pair_index(int(i), int(j), C) == p
+        assert len(pairs) == C * (C - 1) // 2
+
+
+# ---------------------------------------------------------------------------- window
+@pytest.mark.parametrize("L", [64, 256, 512, 2048])
+def test_hann_closed_forms(L):
+    w = o.hann_periodic(L)
+    assert abs(w.sum() - L / 2) < 1e-9 * L          # sum w   = L/2
+    assert abs((w * w).sum() - 3 * L / 8) < 1e-9 * L  # sum w^2 = 3L/8
+    assert w[0] == 0.0 and abs(w[L // 2] - 1.0) < 1e-15
+    assert np.allclose(w[1:], w[1:][::-1], atol=1e-15)  # periodic: symmetric about L/2, w[L]=w[0]
+    assert abs(o.scale_factor(L) - 8.0 / (3 * L)) < 1e-15
+    # overlap correlation at 50 %: sum_n w[n] w[n+L/2] = L/16  ->  r_1 = 1/6
+    assert abs((w[:L // 2] * w[L // 2:]).sum() / (w * w).sum() - 1.0 / 6.0) < 1e-12
+
+
+# ---------------------------------------------------------------------------- P1: closed form
+@pytest.mark.parametrize("L,H,q", [(256, 128, 10), (256, 64, 37), (512, 256, 5), (128, 100, 20)])
+def test_P1_bin_centred_tone_closed_form(L, H, q):
+    """x_i[t] = cos(2 pi q t / L + phi_i): |X[q]| = L/4, |X[q+-1]| = L/8, all other bins 0;
+    S_ij[q] = s2 (L/4)^2 e^{i(phi_i - phi_j)}, G = 1, A = phi_i - phi_j.
+    Catches: symmetric instead of periodic Hann, wrong DFT sign, conj on the wrong operand,
+    wrong scaling, averaging mistakes, wrong hop handling."""
+    T = 4 * L + 3 * H + 7
+    t = np.arange(T)
+    phi = np.array([0.4, -0.7, 2.9])
+    x = np.stack([np.cos(2 * np.pi * q * t / L + p) for p in phi])
+    X = o.stft(x, L, H)
+    K = o.n_segments(T, L, H)
+    assert X.shape == (3, K, L // 2 + 1)
+    mag = np.abs(X)
+    assert np.allclose(mag[:, :, q], L / 4, atol=1e-9)
+    assert np.allclose(mag[:, :, q - 1], L / 8, atol=1e-9)
+    assert np.allclose(mag[:, :, q + 1], L / 8, atol=1e-9)
+    rest = np.delete(mag, [q - 1, q, q + 1], axis=2)
+    assert rest.max() < 1e-10
+    # phase of X at segment k: phi + 2 pi q k H / L
+    for k in range(K):
+        d = np.angle(X[:, k, q] * np.exp(-1j * (phi + 2 * np.pi * q * k * H / L)))
+        assert np.abs(d).max() < 1e-10
+    s2 = o.scale_factor(L)
+    pairs = o.all_pairs(3)
+    S = o.cross_spectra(X, pairs, s2)
+    Sa = o.auto_spectra(X, s2)
+    for p, (i, j) in enumerate(pairs):
+        expect = s2 * (L / 4) ** 2 * np.exp(1j * (phi[i] - phi[j]))
+        assert abs(S[p, q] - expect) < 1e-9 * abs(expect)
+    G = o.coherence(S, Sa, pairs)
+    A = o.crossphase(S)
+    assert np.allclose(G[:, q], 1.0, atol=1e-12)
+    dphi = np.array([phi[i] - phi[j] for i, j in pairs])
+    assert np.abs(np.angle(np.exp(1j * (A[:, q] - dphi)))).max() < 1e-10
+    assert np.allclose(Sa[:, q], s2 * (L / 4) ** 2, rtol=1e-10)
+    assert np.allclose(o.crosspower(S)[:, q], s2 * (L / 4) ** 2, rtol=1e-10)
+
+
+# ---------------------------------------------------------------------------- P2, P3
+def _rand_chunk(C=5, T=1500, seed=11):
+    return np.random.default_rng(seed).standard_normal((C, T))
+
+
+def test_P2_self_coherence_and_P3_hermitian_symmetry():
+    """G_ii = 1, rho_ii[0] = 1, A_ii = 0;  S_ji = conj S_ij => P, G symmetric, A_ji = -A_ij,
+    rho_ji[m] = rho_ij[-m].  Catches pair-handling and lag-ordering mistakes."""
+    L, H, M = 128, 64, 64
+    x = _rand_chunk()
+    X = o.stft(x, L, H)
+    s2 = o.scale_factor(L)
+    Sa = o.auto_spectra(X, s2)
+    self_pairs = np.array([(c, c) for c in range(5)])
+    S = o.cross_spectra(X, self_pairs, s2)
+    assert np.allclose(S.real, Sa, rtol=1e-12) and np.abs(S.imag).max() < 1e-12
+    assert np.allclose(o.coherence(S, Sa, self_pairs), 1.0, atol=1e-12)
+    assert np.abs(o.crossphase(S)).max() < 1e-12
+    rho = o.crosscorr(S, Sa, self_pairs, L, M)
+    assert np.allclose(rho[:, M], 1.0, atol=1e-12)
+    assert np.abs(rho).max() <= 1.0 + 1e-12
+    fwd = np.array([(0, 3), (1, 4), (2, 3)])
+    rev = fwd[:, ::-1]
+    Sf, Sr = o.cross_spectra(X, fwd, s2), o.cross_spectra(X, rev, s2)
+    assert np.allclose(Sr, np.conj(Sf), rtol=1e-13)
+    assert np.allclose(o.coherence(Sf, Sa, fwd), o.coherence(Sr, Sa, rev))
+    assert np.allclose(o.crossphase(Sr)[:, 1:-1], -o.crossphase(Sf)[:, 1:-1])
+    rf, rr = o.crosscorr(Sf, Sa, fwd, L, M), o.crosscorr(Sr, Sa, rev, L, M)
+    assert np.allclose(rr, rf[:, ::-1], atol=1e-13)
+    assert np.abs(rf).max() <= 1.0 + 1e-12  # Cauchy-Schwarz
+
+
+# ---------------------------------------------------------------------------- P4: Parseval
+def test_P4_parseval_per_segment_and_lag0():
+    """|X0|^2 + 2 sum |Xf|^2 + |X_{L/2}|^2 = L sum (w y)^2 for every segment, and
+    R_ii[0] = s2 (1/K) sum_k sum_n (w y)^2.  Catches a wrong DFT kernel / dropped bins /
+    one-sided doubling / wrong 1/L in the inverse."""
+    L, H = 256, 96
+    x = _rand_chunk(3, 2000, 5)
+    X = o.stft(x, L, H)
+    w = o.hann_periodic(L)
+    K = X.shape[1]
+    e_seg = np.empty((3, K))
+    for c in range(3):
+        for k in range(K):
+            e_seg[c, k] = ((w * x[c, k * H:k * H + L]) ** 2).sum()
+    p = np.abs(X) ** 2
+    lhs = p[:, :, 0] + 2 * p[:, :, 1:L // 2].sum(axis=2) + p[:, :, L // 2]
+    assert np.allclose(lhs, L * e_seg, rtol=1e-12)
+    s2 = o.scale_factor(L)
+    Sa = o.auto_spectra(X, s2)
+    R0 = o.hermitian_extend(Sa.astype(complex), L).real.sum(axis=1) / L
+    assert np.allclose(R0, s2 * e_seg.mean(axis=1), rtol=1e-12)
+    # un-normalised R_ii[0] through crosscorr's own path: rho * R0
+    sp = np.array([(0, 0), (0, 1)])
+    S = o.cross_spectra(X, sp, s2)
+    rho = o.crosscorr(S, Sa, sp, L, 4)
+    assert abs(rho[0, 4] - 1.0) < 1e-12
+
+
+# ---------------------------------------------------------------------------- P5: brute force
+def test_P5_time_domain_circular_correlation_and_lag_sign():
+    """R_ij[m] = s2 (1/K) sum_k sum_n yh_i,k[(n+m) mod L] yh_j,k[n], yh = windowed segment.
+    And: if channel j is channel i delayed by d samples, rho_ij peaks at m = -d and
+    A_ij[f] = +2 pi f d / L.  Catches a wrong sign/conjugate in Eq. 1a or 1d, wrong lag order,
+    missing Hermitian half, wrong 1/L."""
+    L, H, M = 64, 32, 32
+    x = _rand_chunk(3, 400, 2)
+    K = o.n_segments(400, L, H)
+    w = o.hann_periodic(L)
+    s2 = o.scale_factor(L)
+    pairs = np.array([(0, 1), (1, 2), (0, 2), (0, 0), (1, 1), (2, 2)])
+    X = o.stft(x, L, H)
+    S = o.cross_spectra(X, pairs, s2)
+    Sa = o.auto_spectra(X, s2)
+    rho = o.crosscorr(S, Sa, pairs, L, M)
+    Rb = np.zeros((len(pairs), 2 * M + 1))
+    for p, (i, j) in enumerate(pairs):
+        for q, m in enumerate(range(-M, M + 1)):
+            acc = 0.0
+            for k in range(K):
+                yi = w * x[i, k * H:k * H + L]
+                yj = w * x[j, k * H:k * H + L]
+                for n in range(L):
+                    acc += yi[(n + m) % L] * yj[n]
+            Rb[p, q] = s2 * acc / K
+    r0 = {c: Rb[3 + c, M] for c in range(3)}
+    for p, (i, j) in enumerate(pairs):
+        assert np.allclose(rho[p], Rb[p] / np.sqrt(r0[i] * r0[j]), atol=1e-12)
+    # delayed copy
+    d = 5
+    T = 4000
+    base = np.random.default_rng(9).standard_normal(T + d)
+    xi, xj = base[d:], base[:T]          # x_j[t] = x_i[t - d]
+    xx = np.stack([xi, xj])
+    L, H, M = 128, 64, 64
+    r = o.analyze_chunk(xx, L, H, M)
+    assert np.argmax(r["R"][0]) - M == -d
+    f = np.arange(1, L // 2)
+    sel = r["G"][0, 1:L // 2] > 0.8
+    err = np.angle(np.exp(1j * (r["A"][0, 1:L // 2] - 2 * np.pi * f * d / L)))
+    assert sel.sum() > 10 and np.abs(err[sel]).max() < 0.2
+
+
+# ---------------------------------------------------------------------------- P6: library
+@pytest.mark.parametrize("L,H", [(256, 128), (512, 128), (128, 96)])
+def test_P6_library_special_cases(L, H):
+    """numpy rfft / scipy Welch routines are independent code.  Oracle X == rfft(w * segment);
+    scipy csd(x_i, x_j) (density, fs = 1, two-sided, no detrend) == conj(S_ij) [scipy conjugates
+    its FIRST argument]; 'spectrum' scaling == conj(S_ij) sum w^2/(sum w)^2; scipy coherence
+    == G^2.  Catches any deviation of the oracle from the standard Welch estimator."""
+    x = _rand_chunk(4, 3000, 21)
+    C, T = x.shape
+    K = o.n_segments(T, L, H)
+    X = o.stft(x, L, H)
+    w = o.hann_periodic(L)
+    assert np.allclose(w, sps.get_window("hann", L, fftbins=True), atol=1e-15)
+    for c in range(C):
+        for k in (0, K // 2, K - 1):
+            ref = np.fft.rfft(w * x[c, k * H:k * H + L])
+            assert np.allclose(X[c, k], ref, rtol=1e-10, atol=1e-10)
+    pairs = o.all_pairs(C)
+    s2 = o.scale_factor(L)
+    S = o.cross_spectra(X, pairs, s2)
+    Sa = o.auto_spectra(X, s2)
+    G = o.coherence(S, Sa, pairs)
+    kw = dict(fs=1.0, window="hann", nperseg=L, noverlap=L - H, nfft=L, detrend=False,
+              return_onesided=False)
+    F = L // 2 + 1
+    for p, (i, j) in enumerate(pairs):
+        _, Pd = sps.csd(x[i], x[j], scaling="density", **kw)
+        assert np.allclose(np.conj(Pd[:F]), S[p], rtol=1e-9, atol=1e-12)
+        _, Ps = sps.csd(x[i], x[j], scaling="spectrum", **kw)
+        assert np.allclose(np.conj(Ps[:F]), S[p] * (w * w).sum() / w.sum() ** 2, rtol=1e-9, atol=1e-12)
+        _, Coh = sps.coherence(x[i], x[j], fs=1.0, window="hann", nperseg=L, noverlap=L - H,
+                               nfft=L, detrend=False)
+        assert np.allclose(Coh, G[p] ** 2, rtol=1e-9, atol=1e-12)
+    # scaling options against scipy's definitions
+    Ssp = o.cross_spectra(X, pairs[:1], o.scale_factor(L, o.SCALE_SPECTRUM))
+    _, Ps = sps.csd(x[0], x[1], scaling="spectrum", **kw)
+    assert np.allclose(np.conj(Ps[:F]), Ssp[0], rtol=1e-9, atol=1e-12)
+    fs = 500e3
+    Sd = o.cross_spectra(X, pairs[:1], o.scale_factor(L, o.SCALE_DENSITY, fs))
+    kw2 = dict(kw, fs=fs)
+    _, Pd = sps.csd(x[0], x[1], scaling="density", **kw2)
+    assert np.allclose(np.conj(Pd[:F]), Sd[0], rtol=1e-9, atol=1e-18)
+    # inverse transform against numpy irfft (circular lags)
+    M = L // 2
+    rho = o.crosscorr(S, Sa, pairs, L, M)
+    R0 = np.fft.irfft(Sa, n=L)[:, 0]
+    for p, (i, j) in enumerate(pairs):
+        Sp = S[p].copy()
+        r = np.fft.irfft(Sp, n=L)
+        lag = np.array([r[m % L] for m in range(-M, M + 1)]) / np.sqrt(R0[i] * R0[j])
+        assert np.allclose(rho[p], lag, atol=1e-12)
+
+
+# ---------------------------------------------------------------------------- P7: config 1
+def test_P7_injected_phase_offsets_tiny_config():
+    """BASELINE config 1: A_ij = 0.3 (i - j) at the tone bins; coherence there >= 0.999."""
+    wl = es.WORKLOADS["tiny"]
+    x = es.tiny()
+    assert x.shape == (8, 2048) and x.dtype == np.float32
+    r = o.analyze_chunk(x, wl.nfft, wl.hop, wl.max_lag)
+    assert r["G"].shape == (28, 129) and r["R"].shape == (28, 257) and r["Sauto"].shape == (8, 129)
+    pairs = o.all_pairs(8)
+    expect = np.array([0.3 * (i - j) for i, j in pairs])
+    for b in (10, 31):   # 20 kHz -> bin 10.24, 60 kHz -> bin 30.72 (nearest bins)
+        assert np.abs(np.angle(np.exp(1j * (r["A"][:, b] - expect)))).max() < 2e-2
+        assert r["G"][:, b].min() > 0.999
+    # noise-free version: tight
+    t = np.arange(2048) / es.FS
+    xn = np.stack([sum(np.sin(2 * np.pi * f * t + 0.3 * i) for f in (5e3, 20e3, 60e3)) for i in range(8)])
+    rn = o.analyze_chunk(xn, 256, 128, 128)
+    for b, tol in ((3, 1e-3), (10, 1e-5), (31, 1e-5)):
+        assert np.abs(np.angle(np.exp(1j * (rn["A"][:, b] - expect)))).max() < tol
+
+
+# ---------------------------------------------------------------------------- P8: white noise
+def _welch_phi(L, H, K):
+    w = o.hann_periodic(L)
+    phi = 1.0
+    s = 1
+    while s * H < L and s < K:
+        r = (w[:L - s * H] * w[s * H:]).sum() / (w * w).sum()
+        phi += 2 * (1 - s / K) * r * r
+        s += 1
+    return phi
+
+
+@pytest.mark.parametrize("L,H,T,expect", [(256, 128, 2048, 0.235), (512, 256, 10_000, 0.148),
+                                          (2048, 512, 50_000, 0.1265)])
+def test_P8_independent_white_noise(L, H, T, expect):
+    """E S_ii = sigma^2 under WINPOW scaling; mean coherence of independent channels
+    = sqrt(pi phi / 4K) with Welch's overlap factor phi (about 1/sqrt(K_segments)).
+    Catches wrong averaging (sum vs mean), wrong scaling, coherence formed before averaging."""
+    sigma = 0.7
+    C = 24
+    x = es.white(C, T, seed=77, sigma=sigma)
+    K = o.n_segments(T, L, H)
+    X = o.stft(x, L, H)
+    s2 = o.scale_factor(L)
+    Sa = o.auto_spectra(X, s2)
+    assert abs(Sa[:, 2:-2].mean() / sigma ** 2 - 1.0) < 0.02
+    pairs = o.all_pairs(C)
+    G = o.coherence(o.cross_spectra(X, pairs, s2), Sa, pairs)[:, 2:-2]
+    theory = np.sqrt(np.pi * _welch_phi(L, H, K) / (4 * K))
+    assert abs(theory - expect) < 2e-3            # closed form reproduces DESIGN.md's numbers
+    assert abs(G.mean() / theory - 1.0) < 0.03
+    assert 0.6 / np.sqrt(K) < G.mean() < 1.4 / np.sqrt(K)   # north_star: "near 1/sqrt(K_segments)"
+
+
+# ---------------------------------------------------------------------------- P10: scale laws
+def test_P10_scale_laws():
+    L, H, M = 128, 64, 64
+    x = _rand_chunk(3, 1200, 3)
+    a = -2.5
+    x2 = x.copy()
+    x2[1] *= a
+    r1, r2 = o.analyze_chunk(x, L, H, M), o.analyze_chunk(x2, L, H, M)
+    pairs = o.all_pairs(3)
+    for p, (i, j) in enumerate(pairs):
+        touched = 1 in (i, j)
+        assert np.allclose(r2["G"][p], r1["G"][p], atol=1e-12)
+        assert np.allclose(r2["P"][p], r1["P"][p] * (abs(a) if touched else 1.0), rtol=1e-12)
+        if touched:   # negative scale: phase shifts by pi, correlation flips
+            d = np.angle(np.exp(1j * (r2["A"][p] - r1["A"][p] - np.pi)))
+            assert np.abs(d[1:-1]).max() < 1e-9
+            assert np.allclose(r2["R"][p], -r1["R"][p], atol=1e-12)
+        else:
+            assert np.allclose(r2["A"][p], r1["A"][p]) and np.allclose(r2["R"][p], r1["R"][p])
+
+
+# ---------------------------------------------------------------------------- normalisation (step 2)
+def test_offset_normalisation_int16():
+    """y = (x - o_c)/o_c with o_c = mean of the first n samples (reading R1)."""
+    rng = np.random.default_rng(4)
+    o_true = np.array([2100.0, 2950.0])
+    sig = rng.standard_normal((2, 6000))
+    counts = np.rint(o_true[:, None] + 200 * sig).astype(np.int16)
+    offs = o.offsets(counts[:, :5000])
+    # integer-exact mean
+    for c in range(2):
+        assert offs[c] == sum(int(v) for v in counts[c, :5000]) / 5000
+    y = o.normalise(counts, offs, o.NORM_RELATIVE)
+    assert np.allclose(y, (counts.astype(float) - offs[:, None]) / offs[:, None])
+    assert abs(y[:, :5000].mean(axis=1)).max() < 1e-12
+    assert np.allclose(o.normalise(counts, offs, o.NORM_SUBTRACT), counts - offs[:, None])
+    assert np.array_equal(o.normalise(counts, None, o.NORM_NONE), counts.astype(float))
+    # a per-channel scale cancels in G, A, rho and scales P by 1/(o_i o_j)
+    L, H, M = 128, 64, 16
+    r_rel = o.analyze_chunk(counts, L, H, M, norm_mode=o.NORM_RELATIVE, offs=offs)
+    r_sub = o.analyze_chunk(counts, L, H, M, norm_mode=o.NORM_SUBTRACT, offs=offs)
+    assert np.allclose(r_rel["G"], r_sub["G"], atol=1e-12)
+    assert np.allclose(r_rel["R"], r_sub["R"], atol=1e-12)
+    assert np.allclose(r_rel["P"] * offs[0] * offs[1], r_sub["P"], rtol=1e-12)
+
+
+# ---------------------------------------------------------------------------- P9: chunk independence
+def test_P9_chunks_are_independent():
+    """"any calculation is performed individually on each time-chunk"."""
+    x = _rand_chunk(3, 3000, 8)
+    a = o.analyze_chunk(x[:, :1000], 128, 64, 64)
+    b = o.analyze_chunk(x[:, 1000:2000], 128, 64, 64)
+    x2 = x.copy()
+    x2[:, 1000:] += 5.0
+    a2 = o.analyze_chunk(x2[:, :1000], 128, 64, 64)
+    for k in a:
+        assert np.array_equal(a[k], a2[k])
+    assert not np.allclose(a["G"], b["G"])
+
+
+# ---------------------------------------------------------------------------- workload generators
+def test_single_config_signature():
+    """The config-2 stand-in has the structure DESIGN.md section 4 states: a 20 kHz mode (bin 20
+    of 257) coherent over the whole array, advected poloidally: A_ij = +2 pi f (tau_j - tau_i)."""
+    wl = es.WORKLOADS["single"]
+    x = es.single()
+    assert x.shape == (192, 10_000) and x.dtype == np.float32
+    rows = [0, 3, 6, 12]
+    sel = np.array([r * 8 for r in rows])
+    pairs = o.all_pairs(len(sel))
+    r = o.analyze_chunk(x[sel], wl.nfft, wl.hop, wl.max_lag)
+    tau = (0.40 / 24) / 5e3 * es.FS   # samples per row
+    b = 20
+    assert r["G"][:, b].min() > 0.9
+    for p, (i, j) in enumerate(pairs):
+        expect = 2 * np.pi * b / wl.nfft * tau * (rows[j] - rows[i])
+        assert abs(np.angle(np.exp(1j * (r["A"][p, b] - expect)))) < 0.1
+
+
+def test_golden_oracle_regression():
+    """tests/golden/tiny_oracle.txt is written by tests/golden/make_golden.py, which calls only
+    oracle/ and ecei_synth; it guards the oracle against accidental change."""
+    path = os.path.join(GOLDEN, "tiny_oracle.txt")
+    rows = [l.split() for l in open(path) if l.strip() and not l.startswith("#")]
+    wl = es.WORKLOADS["tiny"]
+    r = o.analyze_chunk(es.tiny(), wl.nfft, wl.hop, wl.max_lag)
+    assert len(rows) > 20
+    for name, p, q, val in rows:
+        assert abs(r[name][int(p), int(q)] - float(val)) < 1e-12 * max(1.0, abs(float(val)))
