@@ -1,0 +1,364 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the all-channel-pairs spectral path (delta_analyze_chunk) on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload single]
+
+One "step" = one pass of the whole hot path (STFT -> cross-spectra -> coherence, cross-phase,
+cross-power, cross-correlation for all pairs) over one synthetic ECEi-shaped chunk (BASELINE.json
+configs[1]: 192 channels x 10,000 float32 samples, nfft 512, 50 % overlap, 18,336 pairs).
+Prints ONE JSON line (rank 0).  See DESIGN.md section 8 for what each number means.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+import ecei_synth as es  # noqa: E402
+
+METRIC = "channel_pair_spectra_per_s"
+UNIT = "pair-spectra/s"
+N_IN, N_OUT = 4, 5   # rotating input chunks / output buffer sets (5 x 94.4 MB > 126 MB L2)
+
+
+def load_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as fh:
+            d = json.load(fh)
+        return dict(hbm_gbs=float(d["hbm_gbs"]), bf16_tflops=float(d.get("bf16_tflops", 1590.0)),
+                    bf16_tflops_sustained=float(d.get("bf16_tflops_sustained", 1400.0)),
+                    sm_max_mhz=float(d.get("sm_max_mhz", 1965.0)), source="measured")
+    return dict(hbm_gbs=6650.0, bf16_tflops=1590.0, bf16_tflops_sustained=1400.0, sm_max_mhz=1965.0, source="fallback")
+
+
+class ClockSampler:
+    """Polls NVML for SM clock and throttle reasons while the timed region runs."""
+
+    def __init__(self, index: int, period_s: float = 0.002):
+        self.index, self.period = index, period_s
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self._stop = threading.Event()
+        self._thread = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+        except Exception:
+            self.nv = None
+
+    def _poll(self):
+        nv = self.nv
+        names = {"hw_slowdown": 0x8, "sw_thermal_slowdown": 0x20, "hw_thermal_slowdown": 0x40,
+                 "hw_power_brake_slowdown": 0x80, "sw_power_cap": 0x4, "sync_boost": 0x10}
+        while not self._stop.is_set():
+            try:
+                self.samples.append(float(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+                try:
+                    r = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                except Exception:
+                    r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for k, bit in names.items():
+                    if r & bit:
+                        self.reasons.add(k)
+            except Exception:
+                pass
+            time.sleep(self.period)
+
+    def start(self):
+        if self.nv is not None:
+            self._thread = threading.Thread(target=self._poll, daemon=True)
+            self._thread.start()
+
+    def stop(self):
+        self._stop.set()
+        if self._thread is not None:
+            self._thread.join()
+        if not self.samples and self.nv is not None:   # region shorter than one period: one sample now
+            try:
+                self.samples.append(float(self.nv.nvmlDeviceGetClockInfo(self.h, self.nv.NVML_CLOCK_SM)))
+            except Exception:
+                pass
+        med = float(np.median(self.samples)) if self.samples else None
+        return {"sm_mhz": med, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+def physical_gpu_index(local_rank: int) -> int:
+    vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+    if vis:
+        try:
+            return int(vis.split(",")[local_rank])
+        except Exception:
+            return local_rank
+    return local_rank
+
+
+def alg_bytes(w, in_esz=4):
+    """Algorithmic bytes per chunk: read the chunk once, write every requested
+    output once.  X, S and tables are implementation intermediates and are not counted."""
+    inp = w.C * w.T * in_esz
+    gap = 3 * w.P * w.F * 4
+    rho = w.P * (2 * w.max_lag + 1) * 4
+    auto = w.C * w.F * 4
+    return dict(input=inp, gap=gap, rho=rho, auto=auto, total=inp + gap + rho + auto)
+
+
+def oracle_chunk(x, w):
+    from oracle import delta_oracle as o
+    return o.analyze_chunk(x, w.nfft, w.hop, w.max_lag)
+
+
+def blas_threads():
+    try:
+        import threadpoolctl
+        return max([p.get("num_threads", 1) for p in threadpoolctl.threadpool_info()] or [1])
+    except Exception:
+        return os.cpu_count() or 1
+
+
+def cpu_baseline(w, budget_s=12.0):
+    """The oracle as it stands, timed on this box's host cores on whole chunks of the workload."""
+    xs = [es.turbulence(w.T, 9000 + i) for i in range(2)]
+    t0 = time.perf_counter()
+    n = 0
+    while True:
+        oracle_chunk(xs[n % 2], w)
+        n += 1
+        dt = time.perf_counter() - t0
+        if dt >= budget_s or n >= 64:
+            break
+    return {"value": w.P * n / dt, "unit": UNIT, "cores": blas_threads(), "kind": "oracle",
+            "sample": f"{n} whole chunk(s) of the '{w.name}' workload ({w.C}x{w.T} f32, all {w.P} pairs, G+A+P+rho), "
+                      f"float64 direct-DFT numpy oracle, {dt:.1f} s", "seconds": dt}
+
+
+# --------------------------------------------------------------------------------------------
+def run_reference(args):
+    """--impl reference: for this tier the reference arm is the oracle, timed on host cores."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    w = es.WORKLOADS[args.workload]
+    x_full = es.turbulence(w.T, 2)
+    # bounded sample per step so that (W + K) steps end within a few minutes
+    t0 = time.perf_counter()
+    oracle_chunk(x_full[:48], w)
+    t48 = time.perf_counter() - t0
+    budget = 150.0
+    n_ch = w.C
+    steps_total = args.steps + args.warmup
+    # oracle cost ~ a*C + b*C^2; take the pair term as dominant for the estimate (conservative)
+    est_full = t48 * (w.C / 48.0) ** 2
+    if est_full * steps_total > budget:
+        n_ch = int(max(8, min(w.C, 48.0 * np.sqrt(budget / steps_total / t48))))
+    x = x_full[:n_ch]
+    P = n_ch * (n_ch - 1) // 2
+    for _ in range(args.warmup):
+        oracle_chunk(x, w)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        oracle_chunk(x, w)
+    dt = time.perf_counter() - t0
+    val = P * args.steps / dt
+    sample = (f"each step = the first {n_ch} channels ({P} pairs) of one '{w.name}' chunk "
+              f"({w.T} samples, nfft {w.nfft}), all four quantities")
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": w.name, "channels": w.C, "samples": w.T, "nfft": w.nfft, "hop": w.hop,
+                       "pairs": w.P, "max_lag": w.max_lag, "sample": sample},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": blas_threads(), "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+# --------------------------------------------------------------------------------------------
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: libdelta_b200 has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    from paper_2108_08896_b200 import binding as b
+
+    w = es.WORKLOADS[args.workload]
+    peaks = load_peaks()
+    plan = b.Plan(w.C, w.T, w.nfft, w.hop, w.max_lag)
+    s = plan.sizes
+    # inputs resident in HBM before the timed region; every rank works on its own chunks (weak scaling)
+    xs_host = [es.turbulence(w.T, 2 + 100 * i + 1000 * rank) for i in range(N_IN)]
+    xs = [torch.from_numpy(x).cuda() for x in xs_host]
+    outs = [plan.empty_outputs() for _ in range(N_OUT)]
+    K, W = args.steps, args.warmup
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for k in range(W):
+        plan.analyze_chunk(xs[k % N_IN], outs[k % N_OUT])
+    torch.cuda.synchronize()
+    launches_per_step = plan.last_launch_count
+
+    # ---- timed region: exactly K steps, CUDA events on the launching stream --------------------
+    sampler = ClockSampler(physical_gpu_index(local_rank))
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    sampler.start()
+    e0.record()
+    for k in range(K):
+        plan.analyze_chunk(xs[k % N_IN], outs[k % N_OUT])
+    e1.record()
+    barrier()
+    clocks = sampler.stop()
+    ms = e0.elapsed_time(e1)
+    if world > 1:
+        t = torch.tensor([ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+
+    # ---- per-stage durations (same K steps again, events recorded between the kernels) ----------
+    Ks = min(K, 400)
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(4)] for _ in range(Ks)]
+    for row in evs:
+        for e in row:
+            e.record()
+    torch.cuda.synchronize()
+    for k in range(Ks):
+        plan.set_stage_events(evs[k])
+        plan.analyze_chunk(xs[k % N_IN], outs[k % N_OUT])
+    plan.set_stage_events(None)
+    torch.cuda.synchronize()
+    stage_ms = np.array([[row[i].elapsed_time(row[i + 1]) for i in range(3)] for row in evs])
+    stage_mean = stage_ms.mean(axis=0)
+    ab = alg_bytes(w)
+    tc = s.contraction == b.CONTRACT_TC
+    flops_contract = 8.0 * (w.P + w.C) * w.F * w.K   # useful FP32-equivalent flops of Eq. (1a), Hermitian half
+    alu_peak_tf = 148 * 128 * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
+    stages = [
+        {"kernel": "stft_kernel" + ("+chscale_kernel" if tc else ""), "ms": float(stage_mean[0]), "bound": "hbm",
+         "alg_bytes": ab["input"], "achieved": ab["input"] / (stage_mean[0] * 1e-3) / 1e9, "unit": "GB/s"},
+        {"kernel": "contract_tc_kernel" if tc else "contract_fp32_kernel", "ms": float(stage_mean[1]),
+         "bound": "tensor" if tc else "alu", "alg_flops": flops_contract,
+         "achieved": flops_contract / (stage_mean[1] * 1e-3) / 1e12, "unit": "TFLOP/s"},
+        {"kernel": "pair_epilogue_kernel", "ms": float(stage_mean[2]), "bound": "hbm",
+         "alg_bytes": ab["gap"] + ab["rho"], "achieved": (ab["gap"] + ab["rho"]) / (stage_mean[2] * 1e-3) / 1e9,
+         "unit": "GB/s"},
+    ]
+    dom = int(np.argmax(stage_mean))
+    d = stages[dom]
+    if d["bound"] == "hbm":
+        peak, peak_src = peaks["hbm_gbs"], f"MEASURED_PEAKS.json hbm_gbs ({peaks['source']})"
+    elif d["bound"] == "alu":
+        peak, peak_src = alu_peak_tf, "148 SMs x 128 FP32 lanes x 2 flop x sm_max_mhz (DESIGN.md section 7)"
+    else:
+        peak, peak_src = peaks["bf16_tflops"], f"MEASURED_PEAKS.json bf16_tflops burst ({peaks['source']}); fp16 kind::f16"
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "ncu_traffic.json")
+    if os.path.exists(tpath):
+        try:
+            traffic = json.load(open(tpath)).get(d["kernel"].split("+")[0])
+        except Exception:
+            traffic = None
+    roofline = {"kernel": d["kernel"], "bound": d["bound"], "achieved": d["achieved"], "peak": peak, "unit": d["unit"],
+                "frac": d["achieved"] / peak, "traffic": traffic, "peak_source": peak_src,
+                "kernel_ms": d["ms"], "kernel_share_of_step": float(stage_mean[dom] / stage_mean.sum()),
+                "stages": stages,
+                "pipeline": {"alg_bytes_per_step": ab["total"], "achieved": ab["total"] / (ms / K * 1e-3) / 1e9,
+                             "unit": "GB/s", "frac_of_measured_hbm": ab["total"] / (ms / K * 1e-3) / 1e9 / peaks["hbm_gbs"],
+                             "frac_of_8TBs": ab["total"] / (ms / K * 1e-3) / 1e9 / 8000.0}}
+
+    # ---- end to end through the C ABI with HOST buffers (H2D + D2H inside the timed region) ------
+    n_e2e = max(1, min(K, 12))
+    h_x = torch.from_numpy(np.stack([xs_host[i % N_IN] for i in range(n_e2e)])).pin_memory()
+    host_out = dict(G=torch.empty((n_e2e, s.P, s.F)).pin_memory(), A=torch.empty((n_e2e, s.P, s.F)).pin_memory(),
+                    P=torch.empty((n_e2e, s.P, s.F)).pin_memory(), R=torch.empty((n_e2e, s.P, s.n_lags)).pin_memory(),
+                    Sauto=torch.empty((n_e2e, w.C, s.F)).pin_memory())
+    slots = torch.empty(plan.slot_bytes(), dtype=torch.uint8, device="cuda")
+    dev_out = dict(G=torch.empty((2, s.P, s.F), device="cuda"), A=torch.empty((2, s.P, s.F), device="cuda"),
+                   P=torch.empty((2, s.P, s.F), device="cuda"), R=torch.empty((2, s.P, s.n_lags), device="cuda"),
+                   Sauto=torch.empty((2, w.C, s.F), device="cuda"))
+
+    def e2e_once():
+        # D2H copies run on the launching stream right after each chunk, so one device output set suffices
+        plan.analyze_shot_host(h_x, slots, dev_out, strides=(0, 0, 0), host_out=host_out)
+
+    e2e_once()
+    barrier()
+    f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    f0.record()
+    e2e_once()
+    f1.record()
+    barrier()
+    e2e_ms = f0.elapsed_time(f1)
+    if world > 1:
+        t = torch.tensor([e2e_ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_ms = float(t.item())
+    d2h = ab["gap"] + ab["rho"] + ab["auto"]
+    e2e = {"value": world * w.P * n_e2e / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": ab["input"],
+           "d2h_bytes_per_step": d2h, "steps": n_e2e, "ms_per_step": e2e_ms / n_e2e,
+           "call": "delta_analyze_shot_host: pinned host chunks in, all five outputs copied back to pinned host memory"}
+
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        cpu = cpu_baseline(w)
+
+    if rank == 0:
+        value = world * w.P * K / (ms * 1e-3)
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+                "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                "dtype": "f32", "data": "synthetic",
+                "config": {"workload": w.name, "channels": w.C, "samples": w.T, "nfft": w.nfft, "hop": w.hop,
+                           "segments": w.K, "pairs": w.P, "max_lag": w.max_lag, "outputs": "G,A,P,rho,autospectra",
+                           "contraction": "tcgen05 split-fp16" if tc else "fp32 fma",
+                           "l2_policy": f"inputs rotate over {N_IN} chunks, outputs over {N_OUT} buffer sets "
+                                        f"({N_OUT * (ab['gap'] + ab['rho']) / 1e6:.0f} MB > 126 MB L2)",
+                           "parallelism": f"chunk-parallel replicas x{world}, no collective"},
+                "samples_per_s": world * w.C * w.T * K / (ms * 1e-3),
+                "clocks": clocks, "e2e": e2e, "gpu_launches": launches_per_step * K, "roofline": roofline,
+                "cpu_baseline": cpu}
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=1000)
+    ap.add_argument("--warmup", type=int, default=100)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="single", choices=["single"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        if args.steps == 1000 and args.warmup == 100:   # defaults are sized for the GPU arm
+            args.steps, args.warmup = 20, 3
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,176 @@
+/* delta.h -- C ABI of libdelta_b200: the all-channel-pairs spectral path of the Delta framework
+ * (arxiv 2108.08896, "Near real-time streaming analysis of big fusion data"), hand-written CUDA
+ * for NVIDIA B200 (sm_100a).
+ *
+ * What the library computes, per streamed channel-by-time chunk (citations are line numbers of
+ * the paper text, /root/reference/PAPER.md; DESIGN.md section 3 lists the readings R1..R16 taken
+ * where the paper is silent or garbled):
+ *
+ *   normalisation   y_c[t] = (x_c[t] - o_c)/o_c               "After normalizing each chunk" L107, L89
+ *   STFT            X_c[k,f] = sum_n w[n] y_c[kH+n] e^{-2 pi i f n/L}        L107, L169 (Hann, R2-R5)
+ *   Eq. (1a) L95    S_ij[f]  = s^2 (1/K) sum_k X_i[k,f] conj(X_j[k,f])       (E[.] = mean over segments)
+ *                   P_ij[f]  = |S_ij[f]|                                     cross-power
+ *   Eq. (1b) L97    G_ij[f]  = |S_ij[f]| / sqrt(S_ii[f] S_jj[f])             coherence
+ *   Eq. (1c) L100   A_ij[f]  = atan2(Im S_ij[f], Re S_ij[f])                 cross-phase
+ *   Eq. (1d) L102   rho_ij[m] = IFFT_L(S_ij)[m] / sqrt(R_ii[0] R_jj[0])      cross-correlation, m = -M..M
+ *   for all C(C-1)/2 channel pairs i < j, lexicographic ("18336 ... channel pair combinations" L107).
+ *
+ * Conventions
+ *   - Pointers named d_* are DEVICE pointers, h_* are HOST pointers; all are owned by the caller.
+ *     The library never allocates device memory: scratch comes from delta_plan_set_workspace().
+ *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Every call
+ *     that takes a stream is asynchronous on it and never synchronises, unless stated otherwise.
+ *   - Every function returns DELTA_OK (0) or a negative delta_status; nothing is printed.
+ *   - A plan is bound to the device that is current when delta_plan_set_workspace() is called and
+ *     must not be used from two streams at the same time (it owns the scratch buffers).
+ *   - There is no CPU fallback: without a CUDA device every compute call returns DELTA_ERR_CUDA.
+ *
+ * Symbols: C channels, T samples per chunk, L = nfft, H = hop, K = (T-L)/H + 1 segments (no
+ * padding, tail dropped), F = L/2+1 one-sided bins, P = C(C-1)/2 pairs, M = max_lag.
+ */
+#ifndef DELTA_B200_H
+#define DELTA_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define DELTA_VERSION 100 /* 0.1.0 */
+
+typedef enum {
+  DELTA_OK = 0,
+  DELTA_ERR_INVALID_ARG = -1, /* NULL pointer, non-positive size, unknown enum value               */
+  DELTA_ERR_UNSUPPORTED = -2, /* nfft not a power of two in [64,4096], T < L, hop not in [1,L],
+                                 max_lag > L/2, explicit pair list (not in this version), C > 4096  */
+  DELTA_ERR_ALIGNMENT = -3,   /* a device pointer is not 16-byte aligned                            */
+  DELTA_ERR_NO_WORKSPACE = -4,/* compute call before delta_plan_set_workspace(), or it is too small */
+  DELTA_ERR_CUDA = -5,        /* a CUDA runtime call failed; see delta_last_cuda_error()            */
+  DELTA_ERR_STATE = -6        /* e.g. norm_mode needs offsets and delta_set_offsets() was not called */
+} delta_status;
+
+enum { DELTA_WIN_HANN_PERIODIC = 0 };                /* w[n] = 1/2 - 1/2 cos(2 pi n/L)  (R4)          */
+enum { DELTA_SCALE_WINPOW = 0,                       /* s^2 = 1/sum w^2 (default; white noise of
+                                                        variance v has E S_ii = v)                    */
+       DELTA_SCALE_NONE = 1,                         /* s^2 = 1                                       */
+       DELTA_SCALE_DENSITY = 2,                      /* s^2 = 1/(fs sum w^2)                          */
+       DELTA_SCALE_SPECTRUM = 3 };                   /* s^2 = 1/(sum w)^2                             */
+enum { DELTA_F32 = 0, DELTA_I16 = 1 };               /* element type of the input chunk               */
+enum { DELTA_NORM_NONE = 0,                          /* y = x                                         */
+       DELTA_NORM_SUBTRACT = 1,                      /* y = x - o_c                                   */
+       DELTA_NORM_RELATIVE = 2 };                    /* y = (x - o_c)/o_c   (delta T_e/<T_e>, L89)    */
+enum { DELTA_CONTRACT_AUTO = 0,                      /* library picks (tensor cores when available)   */
+       DELTA_CONTRACT_FP32 = 1,                      /* Eq. (1a) on the FP32 FMA pipe                 */
+       DELTA_CONTRACT_TC = 2 };                      /* Eq. (1a) on tcgen05 tensor cores, split fp16  */
+
+typedef struct {
+  int32_t n_channels;   /* C >= 1                                                                     */
+  int32_t n_samples;    /* T >= nfft, samples per channel per chunk                                   */
+  int32_t nfft;         /* L, power of two in [64, 4096]; segment length == nfft (no zero padding)    */
+  int32_t hop;          /* H in [1, L]; overlap = L - H                                               */
+  int32_t window;       /* DELTA_WIN_HANN_PERIODIC                                                    */
+  int32_t scaling;      /* DELTA_SCALE_*                                                              */
+  float   fs;           /* sampling rate in Hz; only DELTA_SCALE_DENSITY uses it                      */
+  int32_t in_dtype;     /* DELTA_F32 | DELTA_I16                                                      */
+  int32_t norm_mode;    /* DELTA_NORM_*; SUBTRACT and RELATIVE need delta_set_offsets() once per shot */
+  int32_t max_lag;      /* M in [0, L/2]; cross-correlation lags -M..M                                */
+  int32_t n_pairs;      /* 0 => all i < j in lexicographic order                                      */
+  const int32_t *h_pairs; /* host [n_pairs][2] or NULL; explicit lists: DELTA_ERR_UNSUPPORTED for now */
+  int32_t contraction;  /* DELTA_CONTRACT_*                                                           */
+} delta_config;
+
+typedef struct {
+  int32_t n_segments;      /* K */
+  int32_t n_bins;          /* F = L/2 + 1 */
+  int32_t n_lags;          /* 2M + 1 */
+  int32_t contraction;     /* the mode the plan resolved DELTA_CONTRACT_AUTO to */
+  int64_t n_pairs;         /* P */
+  int64_t workspace_bytes; /* minimum size for delta_plan_set_workspace() */
+  int64_t x_bytes;         /* size of a d_X buffer  (delta_stft output, opaque layout) */
+  int64_t s_bytes;         /* size of a d_S buffer  = F * P_pad * 8, complex64 [F][P_pad] */
+  int64_t s_row_stride;    /* P_pad: complex64 elements between consecutive frequencies of d_S */
+} delta_sizes;
+
+typedef struct delta_plan delta_plan; /* opaque; owned by the library */
+
+/* Validates the configuration, copies it, builds host-side tables.  Makes no CUDA call, so it
+ * also works on a machine without a GPU.  *out is set to NULL on failure. */
+int delta_plan_create(const delta_config *cfg, delta_plan **out);
+int delta_plan_destroy(delta_plan *plan);
+int delta_plan_sizes(const delta_plan *plan, delta_sizes *out);
+
+/* Hands the plan its scratch memory (>= workspace_bytes, 256-byte aligned, device memory that
+ * stays valid while the plan is used) and uploads the twiddle / window / pair tables into it on
+ * `stream`.  Binds the plan to the current device. */
+int delta_plan_set_workspace(delta_plan *plan, void *d_workspace, size_t bytes, void *stream);
+
+/* Per-shot offsets for DELTA_NORM_SUBTRACT / RELATIVE (reading R1): o_c = mean of the first
+ * n_first samples of channel c of d_x (the first chunk of the shot), element type = in_dtype,
+ * `ld` = elements between consecutive channels.  For int16 input the sum is exact (integer). */
+int delta_set_offsets(delta_plan *plan, const void *d_x, int64_t ld, int32_t n_first, void *stream);
+/* Copies the C offsets (as float64: integer sum / n_first for int16) to h_out.  Synchronises stream. */
+int delta_get_offsets(delta_plan *plan, double *h_out, void *stream);
+
+/* a0 + a1.  Normalise, window and Fourier-transform every segment of every channel.
+ * d_x: [C][ld] of in_dtype, ld >= T.  d_X: x_bytes, layout opaque (see delta_stft_unpack). */
+int delta_stft(delta_plan *plan, const void *d_x, int64_t ld, void *d_X, void *stream);
+/* Test accessor: expands d_X to complex64 [C][K][F] (interleaved re, im), unscaled as in the
+ * definition above. */
+int delta_stft_unpack(delta_plan *plan, const void *d_X, float *d_out, void *stream);
+
+/* a2 + a3, Eq. (1a).  d_S: complex64 [F][P_pad] (frequency-major: for each bin the upper triangle
+ * of the cross-spectral matrix, pairs in lexicographic order, row stride s_row_stride);
+ * d_Sauto: float [C][F] autospectra S_cc[f].  Either may be NULL. */
+int delta_cross_spectra(delta_plan *plan, const void *d_X, float *d_S, float *d_Sauto, void *stream);
+
+/* a4, Eq. (1b): d_G float [P][F].  0 where S_ii S_jj = 0 (R16). */
+int delta_coherence(delta_plan *plan, const float *d_S, const float *d_Sauto, float *d_G, void *stream);
+/* a4, Eq. (1c): d_A float [P][F], radians in [-pi, pi]. */
+int delta_crossphase(delta_plan *plan, const float *d_S, float *d_A, void *stream);
+/* a4, |Eq. (1a)|: d_P float [P][F]. */
+int delta_crosspower(delta_plan *plan, const float *d_S, float *d_P, void *stream);
+/* a5, Eq. (1d): d_R float [P][2M+1], lags -M..M increasing, normalised by sqrt(R_ii[0] R_jj[0]),
+ * circular in the lag (R12).  0 where the denominator is 0. */
+int delta_crosscorr(delta_plan *plan, const float *d_S, const float *d_Sauto, float *d_R, void *stream);
+
+/* The whole path a0..a5 for one chunk resident in device memory, using the plan's workspace for
+ * X and S.  Any output pointer may be NULL (that quantity is then not computed / stored).
+ * Outputs as in the staged calls: d_G, d_A, d_P [P][F]; d_R [P][2M+1]; d_Sauto [C][F]. */
+int delta_analyze_chunk(delta_plan *plan, const void *d_x, int64_t ld,
+                        float *d_G, float *d_A, float *d_P, float *d_R, float *d_Sauto, void *stream);
+
+/* a6: a whole shot from HOST memory.  h_x: [n_chunks][C][T] of in_dtype (pinned memory for true
+ * overlap), chunk n+1 is copied host->device on an internal side stream while chunk n is analysed on
+ * `stream` (two device input slots taken from d_slots, >= 2*C*T*sizeof(in_dtype) bytes, 256-byte
+ * aligned).  If set_offsets != 0 the offsets are taken from the first n_first samples of chunk 0.
+ * Device outputs: chunk n goes to d_X + n*stride_X elements (stride may be 0 to overwrite; NULL
+ * pointer = skip).  Host outputs (any may be NULL): if non-NULL, chunk n's result is copied
+ * device->host to h_X + n*(its full size) after it is computed.  Returns after enqueuing; the
+ * caller synchronises `stream`. */
+int delta_analyze_shot_host(delta_plan *plan, const void *h_x, int32_t n_chunks, void *d_slots,
+                            int32_t set_offsets, int32_t n_first,
+                            float *d_G, float *d_A, float *d_P, float *d_R, float *d_Sauto,
+                            int64_t stride_GAP, int64_t stride_R, int64_t stride_auto,
+                            float *h_G, float *h_A, float *h_P, float *h_R, float *h_Sauto,
+                            void *stream);
+
+/* Profiling hook.  `events` = 4 cudaEvent_t handles (passed as void*) owned by the caller, or NULL to
+ * switch the hook off.  While set, every delta_analyze_chunk() records events[0] before the STFT
+ * stage, events[1] after it, events[2] after the contraction and events[3] after the pair stage, on
+ * the launching stream (so the caller can time each stage with cudaEventElapsedTime). */
+int delta_plan_set_stage_events(delta_plan *plan, void *const *events);
+
+/* Number of kernels the last delta_analyze_chunk() on this plan launched (for bench accounting). */
+int delta_last_launch_count(const delta_plan *plan);
+
+const char *delta_strerror(int status);
+/* cudaError_t of the last failing CUDA call made by this library in the calling thread (0 if none). */
+int delta_last_cuda_error(void);
+int delta_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DELTA_B200_H */

@@ -1,0 +1,369 @@
+// C-ABI entry points of libdelta_b200 (include/delta.h): argument validation, plan and workspace
+// management, and the launch sequences.  All arithmetic of the path lives in the kernels.
+#include <cmath>
+#include <cstring>
+#include <new>
+
+#include "delta_internal.h"
+
+namespace delta {
+
+static thread_local int g_last_cuda_error = 0;
+void set_cuda_error(cudaError_t e) { g_last_cuda_error = (int)e; }
+
+static inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+static inline bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+static int validate(const delta_config *c) {
+  if (!c) return DELTA_ERR_INVALID_ARG;
+  if (c->n_channels < 1 || c->n_samples < 1 || c->nfft < 1 || c->hop < 1 || c->max_lag < 0) return DELTA_ERR_INVALID_ARG;
+  if (c->window != DELTA_WIN_HANN_PERIODIC) return DELTA_ERR_INVALID_ARG;
+  if (c->scaling < DELTA_SCALE_WINPOW || c->scaling > DELTA_SCALE_SPECTRUM) return DELTA_ERR_INVALID_ARG;
+  if (c->in_dtype != DELTA_F32 && c->in_dtype != DELTA_I16) return DELTA_ERR_INVALID_ARG;
+  if (c->norm_mode < DELTA_NORM_NONE || c->norm_mode > DELTA_NORM_RELATIVE) return DELTA_ERR_INVALID_ARG;
+  if (c->contraction < DELTA_CONTRACT_AUTO || c->contraction > DELTA_CONTRACT_TC) return DELTA_ERR_INVALID_ARG;
+  if (c->scaling == DELTA_SCALE_DENSITY && !(c->fs > 0.f)) return DELTA_ERR_INVALID_ARG;
+  if (c->n_pairs < 0 || (c->n_pairs > 0 && !c->h_pairs)) return DELTA_ERR_INVALID_ARG;
+  const int L = c->nfft;
+  if (L < 64 || L > 4096 || (L & (L - 1)) != 0) return DELTA_ERR_UNSUPPORTED;
+  if (c->hop > L) return DELTA_ERR_UNSUPPORTED;
+  if (c->n_samples < L) return DELTA_ERR_UNSUPPORTED;
+  if (c->max_lag > L / 2) return DELTA_ERR_UNSUPPORTED;
+  if (c->n_channels > 4096) return DELTA_ERR_UNSUPPORTED;
+  if (c->n_pairs > 0) return DELTA_ERR_UNSUPPORTED;  // explicit pair lists: not in this version
+  return DELTA_OK;
+}
+
+static bool tc_supported(const delta_config *) {
+  return false;  // the tcgen05 contraction is not wired in yet
+}
+
+}  // namespace delta
+
+using namespace delta;
+
+extern "C" {
+
+int delta_plan_create(const delta_config *cfg, delta_plan **out) {
+  if (!out) return DELTA_ERR_INVALID_ARG;
+  *out = nullptr;
+  int rc = validate(cfg);
+  if (rc) return rc;
+  if (cfg->contraction == DELTA_CONTRACT_TC && !tc_supported(cfg)) return DELTA_ERR_UNSUPPORTED;
+  delta_plan *p = new (std::nothrow) delta_plan();
+  if (!p) return DELTA_ERR_INVALID_ARG;
+  p->cfg = *cfg;
+  p->cfg.h_pairs = nullptr;
+  p->contraction = (cfg->contraction == DELTA_CONTRACT_AUTO) ? (tc_supported(cfg) ? DELTA_CONTRACT_TC : DELTA_CONTRACT_FP32)
+                                                             : cfg->contraction;
+  Layout &l = p->lay;
+  l.C = cfg->n_channels;
+  l.Cp = (int)align_up((size_t)l.C, 64);
+  if (l.Cp < 128) l.Cp = 128;
+  l.T = cfg->n_samples;
+  l.L = cfg->nfft;
+  l.N = l.L / 2;
+  l.H = cfg->hop;
+  l.K = (l.T - l.L) / l.H + 1;
+  l.Kp = (int)align_up((size_t)l.K, 16);
+  l.Kc = l.Kp / kSegBlock;
+  l.F = l.L / 2 + 1;
+  l.M = cfg->max_lag;
+  l.nlags = 2 * l.M + 1;
+  l.P = (int64_t)l.C * (l.C - 1) / 2;
+  l.Ppad = (int64_t)align_up((size_t)(l.P > 0 ? l.P : 1), 32);
+  // floats (2 parts) or halves (2 precisions x 2 parts) per frequency
+  l.x_elems_per_f = (int64_t)(p->contraction == DELTA_CONTRACT_TC ? 4 : 2) * l.Kc * l.Cp * kSegBlock;
+
+  // host tables in float64, rounded once
+  const int L = l.L;
+  p->h_tw.resize(L);
+  p->h_win.resize(L);
+  double sw = 0.0, sw2 = 0.0;
+  for (int n = 0; n < L; ++n) {
+    const double ang = -2.0 * M_PI * (double)n / (double)L;
+    p->h_tw[n] = make_float2((float)std::cos(ang), (float)std::sin(ang));
+    const double w = 0.5 - 0.5 * std::cos(2.0 * M_PI * (double)n / (double)L);
+    p->h_win[n] = (float)w;
+    sw += w;
+    sw2 += w * w;
+  }
+  switch (cfg->scaling) {
+    case DELTA_SCALE_WINPOW: p->s2 = (float)(1.0 / sw2); break;
+    case DELTA_SCALE_NONE: p->s2 = 1.f; break;
+    case DELTA_SCALE_DENSITY: p->s2 = (float)(1.0 / ((double)cfg->fs * sw2)); break;
+    default: p->s2 = (float)(1.0 / (sw * sw)); break;
+  }
+  p->h_pairs.reserve((size_t)l.P);
+  for (int i = 0; i < l.C; ++i)
+    for (int j = i + 1; j < l.C; ++j) p->h_pairs.push_back(make_ushort2((unsigned short)i, (unsigned short)j));
+
+  Workspace &w = p->wsl;
+  size_t o = 0;
+  auto take = [&](size_t bytes) { size_t at = o; o = align_up(o + bytes, 256); return at; };
+  w.off_tw = take((size_t)L * sizeof(float2));
+  w.off_win = take((size_t)L * sizeof(float));
+  w.off_pairs = take((size_t)(l.P > 0 ? l.P : 1) * sizeof(ushort2));
+  w.off_offs = take((size_t)l.C * sizeof(double));
+  w.off_isum = take((size_t)l.C * sizeof(long long));
+  w.off_chscale = take((size_t)l.C * sizeof(float));
+  w.off_X = take((size_t)l.F * l.x_elems_per_f * (p->contraction == DELTA_CONTRACT_TC ? 2 : 4));
+  w.off_S = take((size_t)l.F * l.Ppad * sizeof(float2));
+  w.off_auto = take((size_t)l.C * l.F * sizeof(float));
+  w.total = o;
+  *out = p;
+  return DELTA_OK;
+}
+
+int delta_plan_destroy(delta_plan *p) {
+  if (!p) return DELTA_ERR_INVALID_ARG;
+  if (p->copy_stream) cudaStreamDestroy(p->copy_stream);
+  for (int s = 0; s < 2; ++s) {
+    if (p->ev_copied[s]) cudaEventDestroy(p->ev_copied[s]);
+    if (p->ev_consumed[s]) cudaEventDestroy(p->ev_consumed[s]);
+    if (p->ev_done[s]) cudaEventDestroy(p->ev_done[s]);
+  }
+  delete p;
+  return DELTA_OK;
+}
+
+int delta_plan_sizes(const delta_plan *p, delta_sizes *out) {
+  if (!p || !out) return DELTA_ERR_INVALID_ARG;
+  const Layout &l = p->lay;
+  out->n_segments = l.K;
+  out->n_bins = l.F;
+  out->n_lags = l.nlags;
+  out->contraction = p->contraction;
+  out->n_pairs = l.P;
+  out->workspace_bytes = (int64_t)p->wsl.total;
+  out->x_bytes = (int64_t)l.F * l.x_elems_per_f * (p->contraction == DELTA_CONTRACT_TC ? 2 : 4);
+  out->s_bytes = (int64_t)l.F * l.Ppad * (int64_t)sizeof(float2);
+  out->s_row_stride = l.Ppad;
+  return DELTA_OK;
+}
+
+int delta_plan_set_workspace(delta_plan *p, void *d_ws, size_t bytes, void *stream) {
+  if (!p || !d_ws) return DELTA_ERR_INVALID_ARG;
+  if ((reinterpret_cast<uintptr_t>(d_ws) & 255u) != 0) return DELTA_ERR_ALIGNMENT;
+  if (bytes < p->wsl.total) return DELTA_ERR_NO_WORKSPACE;
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+  DELTA_CUDA_CHECK(cudaGetDevice(&p->device));
+  p->ws = reinterpret_cast<char *>(d_ws);
+  p->ws_bytes = bytes;
+  p->offsets_set = false;
+  const Layout &l = p->lay;
+  DELTA_CUDA_CHECK(cudaMemcpyAsync(p->ws + p->wsl.off_tw, p->h_tw.data(), (size_t)l.L * sizeof(float2), cudaMemcpyHostToDevice, st));
+  DELTA_CUDA_CHECK(cudaMemcpyAsync(p->ws + p->wsl.off_win, p->h_win.data(), (size_t)l.L * sizeof(float), cudaMemcpyHostToDevice, st));
+  if (l.P > 0)
+    DELTA_CUDA_CHECK(cudaMemcpyAsync(p->ws + p->wsl.off_pairs, p->h_pairs.data(), (size_t)l.P * sizeof(ushort2), cudaMemcpyHostToDevice, st));
+  // zero rows C..Cp-1 of the workspace X once (kernels never write them)
+  DELTA_CUDA_CHECK(cudaMemsetAsync(p->ws + p->wsl.off_X, 0, p->wsl.off_S - p->wsl.off_X, st));
+  DELTA_CUDA_CHECK(cudaMemsetAsync(p->ws + p->wsl.off_offs, 0, p->wsl.off_X - p->wsl.off_offs, st));
+  return DELTA_OK;
+}
+
+static int need_ws(const delta_plan *p) {
+  if (!p) return DELTA_ERR_INVALID_ARG;
+  if (!p->ws) return DELTA_ERR_NO_WORKSPACE;
+  return DELTA_OK;
+}
+
+int delta_set_offsets(delta_plan *p, const void *d_x, int64_t ld, int32_t n_first, void *stream) {
+  int rc = need_ws(p);
+  if (rc) return rc;
+  if (!d_x || n_first < 1 || ld < n_first) return DELTA_ERR_INVALID_ARG;
+  p->n_first = n_first;
+  rc = launch_offsets(p, d_x, ld, n_first, reinterpret_cast<cudaStream_t>(stream));
+  if (rc == DELTA_OK) p->offsets_set = true;
+  return rc;
+}
+
+int delta_get_offsets(delta_plan *p, double *h_out, void *stream) {
+  int rc = need_ws(p);
+  if (rc) return rc;
+  if (!h_out) return DELTA_ERR_INVALID_ARG;
+  if (!p->offsets_set) return DELTA_ERR_STATE;
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+  DELTA_CUDA_CHECK(cudaMemcpyAsync(h_out, p->d_offs(), (size_t)p->lay.C * sizeof(double), cudaMemcpyDeviceToHost, st));
+  DELTA_CUDA_CHECK(cudaStreamSynchronize(st));
+  return DELTA_OK;
+}
+
+static int check_input(const delta_plan *p, const void *d_x, int64_t ld) {
+  if (!d_x || ld < p->lay.T) return DELTA_ERR_INVALID_ARG;
+  if (p->cfg.norm_mode != DELTA_NORM_NONE && !p->offsets_set) return DELTA_ERR_STATE;
+  return DELTA_OK;
+}
+
+int delta_stft(delta_plan *p, const void *d_x, int64_t ld, void *d_X, void *stream) {
+  int rc = need_ws(p);
+  if (rc) return rc;
+  if (!d_X) return DELTA_ERR_INVALID_ARG;
+  rc = check_input(p, d_x, ld);
+  if (rc) return rc;
+  if (!aligned16(d_X)) return DELTA_ERR_ALIGNMENT;
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+  if (p->lay.Cp != p->lay.C && d_X != p->d_X()) {
+    delta_sizes sz;
+    delta_plan_sizes(p, &sz);
+    DELTA_CUDA_CHECK(cudaMemsetAsync(d_X, 0, (size_t)sz.x_bytes, st));
+  }
+  return launch_stft(p, d_x, ld, d_X, st);
+}
+
+int delta_stft_unpack(delta_plan *p, const void *d_X, float *d_out, void *stream) {
+  int rc = need_ws(p);
+  if (rc) return rc;
+  if (!d_X || !d_out) return DELTA_ERR_INVALID_ARG;
+  return launch_stft_unpack(p, d_X, d_out, reinterpret_cast<cudaStream_t>(stream));
+}
+
+int delta_cross_spectra(delta_plan *p, const void *d_X, float *d_S, float *d_Sauto, void *stream) {
+  int rc = need_ws(p);
+  if (rc) return rc;
+  if (!d_X) return DELTA_ERR_INVALID_ARG;
+  if (!aligned16(d_X) || (d_S && !aligned16(d_S))) return DELTA_ERR_ALIGNMENT;
+  if (!d_S && !d_Sauto) return DELTA_OK;
+  return launch_contract_fp32(p, d_X, d_S, d_Sauto, reinterpret_cast<cudaStream_t>(stream));
+}
+
+static int pair_stage(delta_plan *p, const float *d_S, const float *d_Sauto, float *G, float *A, float *P, float *R,
+                      void *stream, bool need_auto) {
+  int rc = need_ws(p);
+  if (rc) return rc;
+  if (!d_S || (need_auto && !d_Sauto)) return DELTA_ERR_INVALID_ARG;
+  if (!G && !A && !P && !R) return DELTA_ERR_INVALID_ARG;
+  if (!aligned16(d_S)) return DELTA_ERR_ALIGNMENT;
+  // the kernel always reads the autospectra (for the r0 sums); without them use the workspace copy
+  const float *au = d_Sauto ? d_Sauto : p->d_auto();
+  return launch_pair_epilogue(p, d_S, au, G, A, P, R, reinterpret_cast<cudaStream_t>(stream));
+}
+
+int delta_coherence(delta_plan *p, const float *d_S, const float *d_Sauto, float *d_G, void *stream) {
+  if (!d_G) return DELTA_ERR_INVALID_ARG;
+  return pair_stage(p, d_S, d_Sauto, d_G, nullptr, nullptr, nullptr, stream, true);
+}
+int delta_crossphase(delta_plan *p, const float *d_S, float *d_A, void *stream) {
+  if (!d_A) return DELTA_ERR_INVALID_ARG;
+  return pair_stage(p, d_S, nullptr, nullptr, d_A, nullptr, nullptr, stream, false);
+}
+int delta_crosspower(delta_plan *p, const float *d_S, float *d_P, void *stream) {
+  if (!d_P) return DELTA_ERR_INVALID_ARG;
+  return pair_stage(p, d_S, nullptr, nullptr, nullptr, d_P, nullptr, stream, false);
+}
+int delta_crosscorr(delta_plan *p, const float *d_S, const float *d_Sauto, float *d_R, void *stream) {
+  if (!d_R) return DELTA_ERR_INVALID_ARG;
+  return pair_stage(p, d_S, d_Sauto, nullptr, nullptr, nullptr, d_R, stream, true);
+}
+
+int delta_analyze_chunk(delta_plan *p, const void *d_x, int64_t ld, float *d_G, float *d_A, float *d_P, float *d_R,
+                        float *d_Sauto, void *stream) {
+  int rc = need_ws(p);
+  if (rc) return rc;
+  rc = check_input(p, d_x, ld);
+  if (rc) return rc;
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+  p->launches = 0;
+  const bool ev = p->stage_events_on;
+  if (ev) DELTA_CUDA_CHECK(cudaEventRecord(p->stage_ev[0], st));
+  rc = launch_stft(p, d_x, ld, p->d_X(), st);
+  if (rc) return rc;
+  if (ev) DELTA_CUDA_CHECK(cudaEventRecord(p->stage_ev[1], st));
+  float *au = d_Sauto ? d_Sauto : p->d_auto();
+  const bool pairs_wanted = (d_G || d_A || d_P || d_R) && p->lay.P > 0;
+  rc = launch_contract_fp32(p, p->d_X(), pairs_wanted ? p->d_S() : nullptr, au, st);
+  if (rc) return rc;
+  if (ev) DELTA_CUDA_CHECK(cudaEventRecord(p->stage_ev[2], st));
+  if (pairs_wanted) rc = launch_pair_epilogue(p, p->d_S(), au, d_G, d_A, d_P, d_R, st);
+  if (rc) return rc;
+  if (ev) DELTA_CUDA_CHECK(cudaEventRecord(p->stage_ev[3], st));
+  return rc;
+}
+
+int delta_plan_set_stage_events(delta_plan *p, void *const *events) {
+  if (!p) return DELTA_ERR_INVALID_ARG;
+  p->stage_events_on = events != nullptr;
+  for (int s = 0; s < 4; ++s) {
+    p->stage_ev[s] = events ? reinterpret_cast<cudaEvent_t>(events[s]) : nullptr;
+    if (events && !events[s]) { p->stage_events_on = false; return DELTA_ERR_INVALID_ARG; }
+  }
+  return DELTA_OK;
+}
+
+int delta_analyze_shot_host(delta_plan *p, const void *h_x, int32_t n_chunks, void *d_slots, int32_t set_offsets,
+                            int32_t n_first, float *d_G, float *d_A, float *d_P, float *d_R, float *d_Sauto,
+                            int64_t stride_GAP, int64_t stride_R, int64_t stride_auto, float *h_G, float *h_A,
+                            float *h_P, float *h_R, float *h_Sauto, void *stream) {
+  int rc = need_ws(p);
+  if (rc) return rc;
+  if (!h_x || !d_slots || n_chunks < 1) return DELTA_ERR_INVALID_ARG;
+  if ((reinterpret_cast<uintptr_t>(d_slots) & 255u) != 0) return DELTA_ERR_ALIGNMENT;
+  if ((h_G && !d_G) || (h_A && !d_A) || (h_P && !d_P) || (h_R && !d_R) || (h_Sauto && !d_Sauto)) return DELTA_ERR_INVALID_ARG;
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+  const Layout &l = p->lay;
+  const size_t esz = p->cfg.in_dtype == DELTA_I16 ? 2 : 4;
+  const size_t chunk_bytes = (size_t)l.C * l.T * esz;
+  const size_t slot_bytes = align_up(chunk_bytes, 256);
+  if (!p->copy_stream) {
+    DELTA_CUDA_CHECK(cudaStreamCreateWithFlags(&p->copy_stream, cudaStreamNonBlocking));
+    for (int s = 0; s < 2; ++s) {
+      DELTA_CUDA_CHECK(cudaEventCreateWithFlags(&p->ev_copied[s], cudaEventDisableTiming));
+      DELTA_CUDA_CHECK(cudaEventCreateWithFlags(&p->ev_consumed[s], cudaEventDisableTiming));
+      DELTA_CUDA_CHECK(cudaEventCreateWithFlags(&p->ev_done[s], cudaEventDisableTiming));
+    }
+  }
+  // the copy stream must not start before work already queued on `stream` (e.g. a previous shot
+  // still reading the slots) has finished
+  DELTA_CUDA_CHECK(cudaEventRecord(p->ev_done[0], st));
+  DELTA_CUDA_CHECK(cudaStreamWaitEvent(p->copy_stream, p->ev_done[0], 0));
+  const size_t gap_bytes = (size_t)l.P * l.F * sizeof(float), r_bytes = (size_t)l.P * l.nlags * sizeof(float);
+  const size_t au_bytes = (size_t)l.C * l.F * sizeof(float);
+  int total_launches = 0;
+  for (int n = 0; n < n_chunks; ++n) {
+    const int s = n & 1;
+    char *slot = reinterpret_cast<char *>(d_slots) + (size_t)s * slot_bytes;
+    if (n >= 2) DELTA_CUDA_CHECK(cudaStreamWaitEvent(p->copy_stream, p->ev_consumed[s], 0));
+    DELTA_CUDA_CHECK(cudaMemcpyAsync(slot, reinterpret_cast<const char *>(h_x) + (size_t)n * chunk_bytes, chunk_bytes,
+                                     cudaMemcpyHostToDevice, p->copy_stream));
+    DELTA_CUDA_CHECK(cudaEventRecord(p->ev_copied[s], p->copy_stream));
+    DELTA_CUDA_CHECK(cudaStreamWaitEvent(st, p->ev_copied[s], 0));
+    if (n == 0 && set_offsets) {
+      rc = delta_set_offsets(p, slot, l.T, n_first, stream);
+      if (rc) return rc;
+    }
+    float *g = d_G ? d_G + (size_t)n * stride_GAP : nullptr, *a = d_A ? d_A + (size_t)n * stride_GAP : nullptr;
+    float *pw = d_P ? d_P + (size_t)n * stride_GAP : nullptr, *r = d_R ? d_R + (size_t)n * stride_R : nullptr;
+    float *au = d_Sauto ? d_Sauto + (size_t)n * stride_auto : nullptr;
+    rc = delta_analyze_chunk(p, slot, l.T, g, a, pw, r, au, stream);
+    if (rc) return rc;
+    total_launches += p->launches;
+    DELTA_CUDA_CHECK(cudaEventRecord(p->ev_consumed[s], st));
+    if (h_G) DELTA_CUDA_CHECK(cudaMemcpyAsync(h_G + (size_t)n * l.P * l.F, g, gap_bytes, cudaMemcpyDeviceToHost, st));
+    if (h_A) DELTA_CUDA_CHECK(cudaMemcpyAsync(h_A + (size_t)n * l.P * l.F, a, gap_bytes, cudaMemcpyDeviceToHost, st));
+    if (h_P) DELTA_CUDA_CHECK(cudaMemcpyAsync(h_P + (size_t)n * l.P * l.F, pw, gap_bytes, cudaMemcpyDeviceToHost, st));
+    if (h_R) DELTA_CUDA_CHECK(cudaMemcpyAsync(h_R + (size_t)n * l.P * l.nlags, r, r_bytes, cudaMemcpyDeviceToHost, st));
+    if (h_Sauto) DELTA_CUDA_CHECK(cudaMemcpyAsync(h_Sauto + (size_t)n * l.C * l.F, au, au_bytes, cudaMemcpyDeviceToHost, st));
+  }
+  p->launches = total_launches;
+  return DELTA_OK;
+}
+
+int delta_last_launch_count(const delta_plan *p) { return p ? p->launches : 0; }
+
+const char *delta_strerror(int status) {
+  switch (status) {
+    case DELTA_OK: return "ok";
+    case DELTA_ERR_INVALID_ARG: return "invalid argument";
+    case DELTA_ERR_UNSUPPORTED: return "unsupported configuration";
+    case DELTA_ERR_ALIGNMENT: return "pointer not sufficiently aligned";
+    case DELTA_ERR_NO_WORKSPACE: return "workspace missing or too small";
+    case DELTA_ERR_CUDA: return "CUDA runtime error (see delta_last_cuda_error)";
+    case DELTA_ERR_STATE: return "call sequence error (offsets not set)";
+    default: return "unknown status";
+  }
+}
+
+int delta_last_cuda_error(void) { return g_last_cuda_error; }
+int delta_version(void) { return DELTA_VERSION; }
+
+}  // extern "C"

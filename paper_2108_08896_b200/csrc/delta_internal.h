@@ -1,0 +1,87 @@
+// Internal declarations of libdelta_b200 (not part of the C ABI; see include/delta.h).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <vector>
+
+#include "delta.h"
+
+namespace delta {
+
+constexpr int kPairTile = 64;     // channel block of the FP32 contraction tiles
+constexpr int kSegBlock = 8;      // segments per K-chunk ("kc") of the X layout
+constexpr int kThreads = 256;
+
+struct Layout {
+  // X (STFT) buffer, frequency-major so that one bin's C x K matrix is one contiguous block:
+  //   FP32 mode : float  X[f][part][kc][c][8]                 part 0 = Re, 1 = Im
+  //   TC   mode : __half X[f][prec][part][kc][c][8]           prec 0 = hi, 1 = lo (split fp16)
+  // k = 8*kc + kk, c < Cp (rows C..Cp-1 are zero), kc < Kc = Kp/8, Kp = K rounded up to 16.
+  int C, Cp, T, L, N, H, K, Kp, Kc, F, M, nlags;
+  int64_t P, Ppad;
+  int64_t x_elems_per_f;  // elements (float or half) per frequency
+};
+
+struct Workspace {
+  size_t off_tw, off_win, off_pairs, off_offs, off_isum, off_chscale, off_X, off_S, off_auto, total;
+};
+
+}  // namespace delta
+
+struct delta_plan {
+  delta_config cfg;
+  delta::Layout lay;
+  delta::Workspace wsl;
+  int contraction;   // resolved mode
+  float s2;          // spectral scaling s^2 (reading R6)
+  // host tables (uploaded by delta_plan_set_workspace)
+  std::vector<float2> h_tw;      // e^{-2 pi i f / L}, f = 0..L-1
+  std::vector<float> h_win;      // periodic Hann
+  std::vector<ushort2> h_pairs;  // (i, j), lexicographic
+  // device state
+  char *ws = nullptr;
+  size_t ws_bytes = 0;
+  int device = -1;
+  bool offsets_set = false;
+  int n_first = 0;
+  int launches = 0;
+  bool stage_events_on = false;
+  cudaEvent_t stage_ev[4] = {nullptr, nullptr, nullptr, nullptr};
+  cudaStream_t copy_stream = nullptr;
+  cudaEvent_t ev_copied[2] = {nullptr, nullptr};
+  cudaEvent_t ev_consumed[2] = {nullptr, nullptr};
+  cudaEvent_t ev_done[2] = {nullptr, nullptr};
+
+  const float2 *d_tw() const { return reinterpret_cast<const float2 *>(ws + wsl.off_tw); }
+  const float *d_win() const { return reinterpret_cast<const float *>(ws + wsl.off_win); }
+  const ushort2 *d_pairs() const { return reinterpret_cast<const ushort2 *>(ws + wsl.off_pairs); }
+  double *d_offs() const { return reinterpret_cast<double *>(ws + wsl.off_offs); }
+  long long *d_isum() const { return reinterpret_cast<long long *>(ws + wsl.off_isum); }
+  float *d_chscale() const { return reinterpret_cast<float *>(ws + wsl.off_chscale); }
+  void *d_X() const { return ws + wsl.off_X; }
+  float *d_S() const { return reinterpret_cast<float *>(ws + wsl.off_S); }
+  float *d_auto() const { return reinterpret_cast<float *>(ws + wsl.off_auto); }
+};
+
+namespace delta {
+
+void set_cuda_error(cudaError_t e);
+#define DELTA_CUDA_CHECK(expr)                 \
+  do {                                         \
+    cudaError_t _e = (expr);                   \
+    if (_e != cudaSuccess) {                   \
+      ::delta::set_cuda_error(_e);             \
+      return DELTA_ERR_CUDA;                   \
+    }                                          \
+  } while (0)
+
+// kernels.cu launchers (each returns a delta_status and counts its launches into plan->launches)
+int launch_offsets(delta_plan *p, const void *d_x, int64_t ld, int n_first, cudaStream_t st);
+int launch_stft(delta_plan *p, const void *d_x, int64_t ld, void *d_X, cudaStream_t st);
+int launch_stft_unpack(delta_plan *p, const void *d_X, float *d_out, cudaStream_t st);
+int launch_contract_fp32(delta_plan *p, const void *d_X, float *d_S, float *d_auto, cudaStream_t st);
+int launch_pair_epilogue(delta_plan *p, const float *d_S, const float *d_auto, float *d_G, float *d_A,
+                         float *d_P, float *d_R, cudaStream_t st);
+
+}  // namespace delta

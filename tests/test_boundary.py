@@ -1,0 +1,116 @@
+"""CPU-side checks of the C-ABI boundary (include/delta.h): the library loads, exports every
+declared symbol, validates arguments with the documented status codes, and reports the sizes
+SURVEY.md section 8 tabulates.  No compute call is made (there is no GPU here)."""
+import ctypes as C
+import os
+import re
+
+import pytest
+
+from paper_2108_08896_b200 import binding as b
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def declared_symbols():
+    text = open(os.path.join(ROOT, "include", "delta.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(delta_[a-z0-9_]+)\s*\(", text)))
+
+
+def test_library_exports_every_declared_symbol():
+    syms = declared_symbols()
+    assert len(syms) >= 19
+    assert set(syms) == set(b.EXPORTS)
+    for s in syms:
+        assert getattr(b.LIB, s) is not None
+    for name in ("delta_stft", "delta_cross_spectra", "delta_coherence", "delta_crossphase", "delta_crosspower",
+                 "delta_crosscorr"):   # the six calls BASELINE.json's north_star names
+        assert name in syms
+    assert b.LIB.delta_version() == 100
+    assert os.path.dirname(b.LIB_PATH).endswith("paper_2108_08896_b200")  # in-tree, not site-packages
+
+
+def mk(**kw):
+    base = dict(n_channels=192, n_samples=10_000, nfft=512, hop=256, window=0, scaling=0, fs=500e3, in_dtype=0,
+                norm_mode=0, max_lag=256, n_pairs=0, h_pairs=None, contraction=0)
+    base.update(kw)
+    return b.DeltaConfig(**base)
+
+
+def create(cfg):
+    h = C.c_void_p()
+    rc = b.LIB.delta_plan_create(C.byref(cfg), C.byref(h))
+    if rc == 0:
+        b.LIB.delta_plan_destroy(h)
+    else:
+        assert not h.value
+    return rc
+
+
+@pytest.mark.parametrize("kw,status", [
+    (dict(), b.OK),
+    (dict(nfft=500), b.ERR_UNSUPPORTED),          # not a power of two
+    (dict(nfft=32, hop=16, max_lag=8), b.ERR_UNSUPPORTED),
+    (dict(nfft=8192, hop=4096, n_samples=100_000), b.ERR_UNSUPPORTED),
+    (dict(n_samples=300), b.ERR_UNSUPPORTED),     # T < L
+    (dict(max_lag=257), b.ERR_UNSUPPORTED),       # M > L/2
+    (dict(hop=513), b.ERR_UNSUPPORTED),
+    (dict(hop=0), b.ERR_INVALID_ARG),
+    (dict(n_channels=0), b.ERR_INVALID_ARG),
+    (dict(n_channels=5000), b.ERR_UNSUPPORTED),
+    (dict(window=3), b.ERR_INVALID_ARG),
+    (dict(scaling=9), b.ERR_INVALID_ARG),
+    (dict(scaling=2, fs=0.0), b.ERR_INVALID_ARG),
+    (dict(in_dtype=7), b.ERR_INVALID_ARG),
+    (dict(norm_mode=-1), b.ERR_INVALID_ARG),
+    (dict(max_lag=-1), b.ERR_INVALID_ARG),
+    (dict(contraction=5), b.ERR_INVALID_ARG),
+    (dict(n_pairs=3), b.ERR_INVALID_ARG),         # list announced but NULL
+])
+def test_plan_create_validation(kw, status):
+    assert create(mk(**kw)) == status
+
+
+def test_null_arguments():
+    assert b.LIB.delta_plan_create(None, None) == b.ERR_INVALID_ARG
+    h = C.c_void_p()
+    assert b.LIB.delta_plan_create(None, C.byref(h)) == b.ERR_INVALID_ARG
+    assert b.LIB.delta_plan_destroy(None) == b.ERR_INVALID_ARG
+    assert b.LIB.delta_plan_sizes(None, None) == b.ERR_INVALID_ARG
+
+
+def test_explicit_pair_list_is_reported_unsupported():
+    arr = (C.c_int32 * 4)(0, 1, 0, 2)
+    assert create(mk(n_pairs=2, h_pairs=C.cast(arr, C.POINTER(C.c_int32)))) == b.ERR_UNSUPPORTED
+
+
+@pytest.mark.parametrize("name,K,F,P,nl", [("tiny", 15, 129, 28, 257), ("single", 38, 257, 18336, 513),
+                                           ("long", 194, 513, 18336, 1025), ("wide", 94, 1025, 73536, 2049)])
+def test_sizes_match_survey_table(name, K, F, P, nl):
+    import ecei_synth as es
+    w = es.WORKLOADS[name]
+    p = b.Plan(w.C, w.T, w.nfft, w.hop, w.max_lag, allocate=False)
+    s = p.sizes
+    assert (s.K, s.F, s.P, s.n_lags) == (K, F, P, nl) == (w.K, w.F, w.P, 2 * w.max_lag + 1)
+    assert s.s_row_stride >= P and s.s_row_stride % 32 == 0
+    assert s.s_bytes == s.F * s.s_row_stride * 8
+    assert s.workspace_bytes >= s.x_bytes + s.s_bytes
+
+
+def test_compute_calls_refuse_without_workspace():
+    p = b.Plan(8, 2048, 256, 128, allocate=False)
+    assert b.LIB.delta_stft(p._h, 16, 2048, 16, None) == b.ERR_NO_WORKSPACE
+    assert b.LIB.delta_analyze_chunk(p._h, 16, 2048, None, None, None, None, None, None) == b.ERR_NO_WORKSPACE
+    assert b.LIB.delta_plan_set_workspace(p._h, None, 0, None) == b.ERR_INVALID_ARG
+    assert b.LIB.delta_plan_set_workspace(p._h, 8, 1 << 30, None) == b.ERR_ALIGNMENT
+    assert b.LIB.delta_plan_set_workspace(p._h, 256, 16, None) == b.ERR_NO_WORKSPACE
+    assert b.LIB.delta_strerror(b.ERR_UNSUPPORTED).decode().startswith("unsupported")
+
+
+def test_plan_needs_a_gpu_for_allocation():
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("GPU present")
+    with pytest.raises(RuntimeError):
+        b.Plan(8, 2048, 256, 128)

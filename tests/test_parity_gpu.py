@@ -1,0 +1,302 @@
+"""GPU parity: the CUDA path (through the C ABI, via the ctypes binding) against the float64 oracle,
+element by element on the same seeded inputs.
+
+Tolerances are BASELINE.json north_star's:
+  cross-power  1e-4 relative      (reading R13: where G_oracle > 0.1 and on autospectra; elsewhere
+                                    |dP| <= 1e-5 sqrt(S_ii S_jj), which is tighter than the coherence bound)
+  coherence    1e-4 absolute
+  cross-phase  1e-3 rad where G_oracle > 0.1, compared modulo 2 pi (R15)
+  cross-corr   1e-4 absolute on the normalised rho
+"""
+import numpy as np
+import pytest
+import torch
+
+import ecei_synth as es
+from oracle import delta_oracle as o
+
+pytestmark = pytest.mark.gpu
+
+TOL_P_REL, TOL_G, TOL_A, TOL_R = 1e-4, 1e-4, 1e-3, 1e-4
+
+
+def binding():
+    from paper_2108_08896_b200 import binding as b
+    return b
+
+
+def dev(x):
+    return torch.from_numpy(np.ascontiguousarray(x)).cuda()
+
+
+def compare(out, ref, pairs, label=""):
+    """out: dict of numpy float32 arrays for `pairs`; ref: oracle dict for the same pairs."""
+    G, A, P, R, Sa = (np.asarray(out[k], dtype=np.float64) for k in ("G", "A", "P", "R", "Sauto"))
+    for k in ("G", "A", "P", "R", "Sauto"):
+        assert np.isfinite(out[k]).all(), f"{label}: non-finite {k}"
+    pairs = np.asarray(pairs).reshape(-1, 2)
+    den = np.sqrt(ref["Sauto"][pairs[:, 0]] * ref["Sauto"][pairs[:, 1]]) if len(pairs) else np.zeros((0, 1))
+    gate = ref["G"] > 0.1
+    stats = {}
+    stats["auto_rel"] = float(np.max(np.abs(Sa - ref["Sauto"]) / np.maximum(ref["Sauto"], 1e-300))) if Sa.size else 0.0
+    assert stats["auto_rel"] <= TOL_P_REL, f"{label}: autospectra rel err {stats['auto_rel']:.3g}"
+    if len(pairs) == 0:
+        return stats
+    dP = np.abs(P - ref["P"])
+    stats["P_rel_gated"] = float(np.max(np.where(gate, dP / np.maximum(ref["P"], 1e-300), 0.0)))
+    stats["P_abs_norm"] = float(np.max(np.where(den > 0, dP / np.where(den > 0, den, 1.0), 0.0)))
+    stats["G_abs"] = float(np.max(np.abs(G - ref["G"])))
+    dA = np.abs(np.angle(np.exp(1j * (A - ref["A"]))))
+    stats["A_gated"] = float(np.max(np.where(gate, dA, 0.0)))
+    stats["R_abs"] = float(np.max(np.abs(R - ref["R"])))
+    assert stats["P_rel_gated"] <= TOL_P_REL, f"{label}: cross-power rel err (G>0.1) {stats['P_rel_gated']:.3g}"
+    assert stats["P_abs_norm"] <= 1e-5, f"{label}: cross-power abs err / sqrt(SiiSjj) {stats['P_abs_norm']:.3g}"
+    assert stats["G_abs"] <= TOL_G, f"{label}: coherence abs err {stats['G_abs']:.3g}"
+    assert stats["A_gated"] <= TOL_A, f"{label}: cross-phase err (G>0.1) {stats['A_gated']:.3g}"
+    assert stats["R_abs"] <= TOL_R, f"{label}: cross-correlation abs err {stats['R_abs']:.3g}"
+    return stats
+
+
+def gpu_analyze(x, L, H, M, in_dtype=None, norm_mode=0, n_first=0, contraction=0, scaling=0, fs=500e3, ld_pad=0):
+    b = binding()
+    C, T = x.shape
+    in_dtype = (b.I16 if x.dtype == np.int16 else b.F32) if in_dtype is None else in_dtype
+    plan = b.Plan(C, T, L, H, M, in_dtype=in_dtype, norm_mode=norm_mode, contraction=contraction, scaling=scaling, fs=fs)
+    if ld_pad:
+        buf = torch.zeros((C, T + ld_pad), dtype=dev(x[:1, :1]).dtype, device="cuda")
+        buf[:, :T] = dev(x)
+        xd = buf[:, :T]
+    else:
+        xd = dev(x)
+    if norm_mode != 0:
+        plan.set_offsets(xd, n_first)
+    out = plan.analyze_chunk(xd)
+    torch.cuda.synchronize()
+    return plan, {k: v.cpu().numpy() for k, v in out.items()}
+
+
+def oracle_for(x, L, H, M, pairs=None, norm_mode=0, offs=None, scaling=0, fs=500e3):
+    return o.analyze_chunk(x, L, H, M, pairs=pairs, norm_mode=norm_mode, offs=offs, scaling=scaling, fs=fs)
+
+
+# ------------------------------------------------------------------------------------------
+def test_library_is_the_cuda_path():
+    b = binding()
+    import os
+    assert os.path.exists(b.LIB_PATH)
+    plan = b.Plan(8, 2048, 256, 128)
+    assert plan.sizes.contraction in (b.CONTRACT_FP32, b.CONTRACT_TC)
+
+
+def test_config1_tiny_full():
+    w = es.WORKLOADS["tiny"]
+    x = es.tiny()
+    _, out = gpu_analyze(x, w.nfft, w.hop, w.max_lag)
+    ref = oracle_for(x, w.nfft, w.hop, w.max_lag)
+    st = compare(out, ref, o.all_pairs(w.C), "tiny")
+    print("tiny", st)
+    # P7: injected phases recovered by the CUDA path itself
+    expect = np.array([0.3 * (i - j) for i, j in o.all_pairs(8)])
+    assert np.abs(np.angle(np.exp(1j * (out["A"][:, 10] - expect)))).max() < 2e-2
+
+
+def test_config2_single_chunk_full():
+    w = es.WORKLOADS["single"]
+    x = es.single()
+    _, out = gpu_analyze(x, w.nfft, w.hop, w.max_lag)
+    ref = oracle_for(x, w.nfft, w.hop, w.max_lag)
+    st = compare(out, ref, o.all_pairs(w.C), "single")
+    print("single", st)
+
+
+def test_stft_stage_against_oracle():
+    b = binding()
+    w = es.WORKLOADS["tiny"]
+    x = es.tiny()
+    plan = b.Plan(w.C, w.T, w.nfft, w.hop, w.max_lag)
+    X = plan.stft_unpack(plan.stft(dev(x))).cpu().numpy()
+    Xo = o.stft(x, w.nfft, w.hop)
+    assert X.shape == Xo.shape
+    scale = np.abs(Xo).max()
+    assert np.abs(X - Xo).max() <= 2e-6 * scale
+
+
+def test_staged_calls_equal_fused_call():
+    b = binding()
+    w = es.WORKLOADS["single"]
+    x = es.single()[:40]
+    plan = b.Plan(40, w.T, w.nfft, w.hop, w.max_lag)
+    xd = dev(x)
+    fused = plan.analyze_chunk(xd)
+    X = plan.stft(xd)
+    S, Sa = plan.cross_spectra(X)
+    G, A, P, R = plan.coherence(S, Sa), plan.crossphase(S), plan.crosspower(S), plan.crosscorr(S, Sa)
+    torch.cuda.synchronize()
+    for name, t in (("G", G), ("A", A), ("P", P), ("R", R), ("Sauto", Sa)):
+        assert torch.equal(t, fused[name]), name
+    # S itself against the oracle, in its documented [F][P_pad] layout
+    Xo = o.stft(x, w.nfft, w.hop)
+    pairs = o.all_pairs(40)
+    So = o.cross_spectra(Xo, pairs, o.scale_factor(w.nfft))
+    Sg = torch.view_as_complex(S).cpu().numpy()[:, :len(pairs)].T
+    den = np.sqrt(o.auto_spectra(Xo, o.scale_factor(w.nfft))[pairs[:, 0]] * o.auto_spectra(Xo, o.scale_factor(w.nfft))[pairs[:, 1]])
+    assert np.max(np.abs(Sg - So) / den) < 1e-5
+
+
+@pytest.mark.parametrize("C,T,L,H,M", [
+    (5, 3000, 128, 100, 40),    # ragged everything: odd C, hop not dividing L, short lags
+    (2, 64, 64, 64, 32),        # T == L: a single segment; smallest transform
+    (3, 700, 64, 1, 0),         # hop 1 (K = 637 segments), lag 0 only
+    (1, 1000, 256, 128, 128),   # a single channel: no pairs, autospectra only
+    (70, 1200, 256, 256, 128),  # no overlap; more than one 64-channel tile with a ragged one
+    (4, 9000, 4096, 2048, 2048),  # largest transform
+    (6, 5000, 1024, 300, 17),
+    (9, 4100, 2048, 1024, 1000),
+    (33, 900, 128, 64, 64),
+])
+def test_edge_shapes(C, T, L, H, M):
+    x = np.random.default_rng(C * 1000 + L).standard_normal((C, T)).astype(np.float32)
+    x += 0.5 * x[0:1]  # some coherence between channels
+    _, out = gpu_analyze(x, L, H, M)
+    ref = oracle_for(x, L, H, M)
+    assert out["G"].shape == ref["G"].shape and out["R"].shape == ref["R"].shape
+    compare(out, ref, o.all_pairs(C), f"edge C={C} L={L}")
+
+
+def test_strided_rows_and_scalings():
+    x = np.random.default_rng(5).standard_normal((6, 2000)).astype(np.float32)
+    b = binding()
+    for scaling in (b.SCALE_NONE, b.SCALE_DENSITY, b.SCALE_SPECTRUM):
+        _, out = gpu_analyze(x, 256, 128, 64, scaling=scaling, fs=500e3, ld_pad=37)
+        ref = oracle_for(x, 256, 128, 64, scaling=scaling, fs=500e3)
+        compare(out, ref, o.all_pairs(6), f"scaling {scaling}")
+
+
+def test_degenerate_zero_channel():
+    """A dead channel: S_ii = 0 -> coherence and rho are 0 by definition (R16), nothing is NaN."""
+    x = np.random.default_rng(6).standard_normal((4, 1500)).astype(np.float32)
+    x[2] = 0.0
+    _, out = gpu_analyze(x, 128, 64, 64)
+    ref = oracle_for(x, 128, 64, 64)
+    compare(out, ref, o.all_pairs(4), "dead channel")
+    dead = [p for p, (i, j) in enumerate(o.all_pairs(4)) if 2 in (i, j)]
+    assert np.all(out["G"][dead] == 0) and np.all(out["R"][dead] == 0) and np.all(out["P"][dead] == 0)
+
+
+@pytest.mark.parametrize("norm_mode", [0, 1, 2])
+def test_int16_and_normalisation_modes(norm_mode):
+    rng = np.random.default_rng(8)
+    o_true = rng.uniform(2000, 3000, size=6)
+    sig = rng.standard_normal((6, 6000))
+    sig[1] += 0.7 * sig[0]
+    counts = np.rint(o_true[:, None] + 200 * sig).astype(np.int16)
+    plan, out = gpu_analyze(counts, 512, 256, 256, norm_mode=norm_mode, n_first=5000)
+    offs = o.offsets(counts[:, :5000])
+    if norm_mode:
+        assert np.array_equal(plan.get_offsets(), offs)   # integer-exact sums
+    ref = oracle_for(counts, 512, 256, 256, norm_mode=norm_mode, offs=offs)
+    compare(out, ref, o.all_pairs(6), f"int16 norm {norm_mode}")
+    # float32 input with offsets
+    xf = counts.astype(np.float32)
+    plan, out = gpu_analyze(xf, 512, 256, 256, norm_mode=norm_mode, n_first=5000)
+    ref = oracle_for(xf, 512, 256, 256, norm_mode=norm_mode, offs=o.offsets(xf[:, :5000]))
+    compare(out, ref, o.all_pairs(6), f"f32 norm {norm_mode}")
+
+
+def test_offsets_required():
+    b = binding()
+    plan = b.Plan(4, 1000, 128, 64, 64, norm_mode=b.NORM_RELATIVE)
+    with pytest.raises(b.DeltaError) as e:
+        plan.analyze_chunk(torch.zeros((4, 1000), device="cuda"))
+    assert e.value.status == b.ERR_STATE
+    with pytest.raises(b.DeltaError) as e:
+        plan.analyze_chunk(torch.zeros((4, 1000), device="cuda")[:, :500])  # ld < T is caught first? T mismatch
+    assert e.value.status in (b.ERR_STATE, b.ERR_INVALID_ARG)
+
+
+def _sampled_pairs(C, n_ch, seed):
+    rng = np.random.default_rng(seed)
+    ch = np.sort(rng.choice(C, size=n_ch, replace=False))
+    ch[0], ch[-1] = 0, C - 1   # include the corners of the pair triangle
+    ch = np.unique(ch)
+    loc = o.all_pairs(len(ch))
+    glob = np.stack([ch[loc[:, 0]], ch[loc[:, 1]]], axis=1)
+    return ch, loc, glob
+
+
+@pytest.mark.parametrize("name,n_ch", [("long", 12), ("wide", 10)])
+def test_full_size_configs_on_sampled_pairs(name, n_ch):
+    """Configs 3 and 5 at BASELINE's full sizes; the oracle's direct DFT is run on a sample of
+    channels (all pairs among them, incl. first/last channel), compared element by element."""
+    w = es.WORKLOADS[name]
+    x = es.make(name)
+    _, out = gpu_analyze(x, w.nfft, w.hop, w.max_lag)
+    assert out["G"].shape == (w.P, w.F) and out["R"].shape == (w.P, 2 * w.max_lag + 1)
+    ch, loc, glob = _sampled_pairs(w.C, n_ch, 42)
+    ref = oracle_for(x[ch], w.nfft, w.hop, w.max_lag)
+    idx = np.array([o.pair_index(int(i), int(j), w.C) for i, j in glob])
+    sub = {k: out[k][idx] for k in ("G", "A", "P", "R")}
+    sub["Sauto"] = out["Sauto"][ch]
+    st = compare(sub, ref, loc, name)
+    print(name, st)
+    # properties that hold at any size, on every output element
+    assert np.isfinite(out["G"]).all() and out["G"].min() >= 0 and out["G"].max() <= 1 + 1e-4
+    assert np.abs(out["R"]).max() <= 1 + 1e-4 and np.abs(out["A"]).max() <= np.pi + 1e-6
+
+
+def test_config4_streamed_shot():
+    """Config 4: int16 counts, offsets from the first 5,000 samples of the shot, 250 chunks streamed
+    from pinned host memory with the H2D copy of chunk n+1 overlapping the analysis of chunk n.
+    Checked chunks: 0, 1, 124, 249 + 4 seeded random ones; also P9 (chunk independence): a chunk
+    analysed alone gives bit-identical results to the same chunk inside the stream."""
+    b = binding()
+    w = es.WORKLOADS["streamed"]
+    n_chunks = w.n_chunks
+    counts, _ = es.streamed(n_chunks=n_chunks)
+    h_x = torch.from_numpy(counts).pin_memory()
+    plan = b.Plan(w.C, w.T, w.nfft, w.hop, w.max_lag, in_dtype=b.I16, norm_mode=b.NORM_RELATIVE)
+    s = plan.sizes
+    check = sorted({0, 1, 124, 249} | set(np.random.default_rng(4).choice(n_chunks, 4, replace=False).tolist()))
+    slots = torch.empty(plan.slot_bytes(), dtype=torch.uint8, device="cuda")
+    # keep every chunk's coherence on the device, the other quantities in a rotating set of 2
+    G = torch.empty((n_chunks, s.P, s.F), dtype=torch.float32, device="cuda")
+    A = torch.empty((n_chunks, s.P, s.F), dtype=torch.float32, device="cuda")
+    P = torch.empty((n_chunks, s.P, s.F), dtype=torch.float32, device="cuda")
+    R = torch.empty((n_chunks, s.P, s.n_lags), dtype=torch.float32, device="cuda")
+    Sa = torch.empty((n_chunks, w.C, s.F), dtype=torch.float32, device="cuda")
+    plan.analyze_shot_host(h_x, slots, dict(G=G, A=A, P=P, R=R, Sauto=Sa),
+                           strides=(s.P * s.F, s.P * s.n_lags, w.C * s.F), set_offsets=True, n_first=w.n_first)
+    torch.cuda.synchronize()
+    offs = o.offsets(counts[0][:, :w.n_first])
+    assert np.array_equal(plan.get_offsets(), offs)
+    pairs = o.all_pairs(w.C)
+    for n in check:
+        ref = oracle_for(counts[n], w.nfft, w.hop, w.max_lag, norm_mode=o.NORM_RELATIVE, offs=offs)
+        out = dict(G=G[n].cpu().numpy(), A=A[n].cpu().numpy(), P=P[n].cpu().numpy(), R=R[n].cpu().numpy(),
+                   Sauto=Sa[n].cpu().numpy())
+        st = compare(out, ref, pairs, f"streamed chunk {n}")
+        print("chunk", n, st)
+    # P9: chunk 124 alone
+    alone = plan.analyze_chunk(dev(counts[124]))
+    torch.cuda.synchronize()
+    for k, t in (("G", G), ("A", A), ("P", P), ("R", R), ("Sauto", Sa)):
+        assert torch.equal(alone[k], t[124]), k
+
+
+def test_host_output_path_roundtrip():
+    """delta_analyze_shot_host with host outputs (the e2e path bench.py times)."""
+    b = binding()
+    x = np.random.default_rng(3).standard_normal((3, 12, 1024)).astype(np.float32)
+    plan = b.Plan(12, 1024, 128, 64, 64)
+    s = plan.sizes
+    h_x = torch.from_numpy(x).pin_memory()
+    slots = torch.empty(plan.slot_bytes(), dtype=torch.uint8, device="cuda")
+    dev_out = plan.empty_outputs()
+    host = dict(G=torch.empty((3, s.P, s.F)).pin_memory(), A=torch.empty((3, s.P, s.F)).pin_memory(),
+                P=torch.empty((3, s.P, s.F)).pin_memory(), R=torch.empty((3, s.P, s.n_lags)).pin_memory(),
+                Sauto=torch.empty((3, 12, s.F)).pin_memory())
+    plan.analyze_shot_host(h_x, slots, dev_out, host_out=host)
+    torch.cuda.synchronize()
+    for n in range(3):
+        ref = oracle_for(x[n], 128, 64, 64)
+        compare({k: host[k][n].numpy() for k in host}, ref, o.all_pairs(12), f"host chunk {n}")
