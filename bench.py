@@ -94,6 +94,27 @@ class ClockSampler:
         return {"sm_mhz": med, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": len(self.samples)}
 
 
+def max_over_ranks(value: float, world: int, device: str = "cuda") -> float:
+    """Timing rule: the step time of a multi-rank run is the MAX over ranks."""
+    if world <= 1:
+        return float(value)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([value], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def rank_chunk_seeds(rank: int, n: int = N_IN):
+    """Weak scaling: every rank analyses its own chunks (disjoint seeds), no data-path collective."""
+    return [2 + 100 * i + 1000 * rank for i in range(n)]
+
+
+def aggregate_value(pairs_per_step: int, steps: int, world: int, ms_max: float) -> float:
+    """Whole-job throughput: units processed by all ranks / max-over-ranks time."""
+    return world * pairs_per_step * steps / (ms_max * 1e-3)
+
+
 def physical_gpu_index(local_rank: int) -> int:
     vis = os.environ.get("CUDA_VISIBLE_DEVICES")
     if vis:
@@ -205,7 +226,7 @@ def run_ours(args):
     plan = b.Plan(w.C, w.T, w.nfft, w.hop, w.max_lag)
     s = plan.sizes
     # inputs resident in HBM before the timed region; every rank works on its own chunks (weak scaling)
-    xs_host = [es.turbulence(w.T, 2 + 100 * i + 1000 * rank) for i in range(N_IN)]
+    xs_host = [es.turbulence(w.T, seed) for seed in rank_chunk_seeds(rank)]
     xs = [torch.from_numpy(x).cuda() for x in xs_host]
     outs = [plan.empty_outputs() for _ in range(N_OUT)]
     K, W = args.steps, args.warmup
@@ -231,11 +252,7 @@ def run_ours(args):
     e1.record()
     barrier()
     clocks = sampler.stop()
-    ms = e0.elapsed_time(e1)
-    if world > 1:
-        t = torch.tensor([ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+    ms = max_over_ranks(e0.elapsed_time(e1), world)
 
     # ---- per-stage durations (same K steps again, events recorded between the kernels) ----------
     Ks = min(K, 400)
@@ -310,13 +327,9 @@ def run_ours(args):
     e2e_once()
     f1.record()
     barrier()
-    e2e_ms = f0.elapsed_time(f1)
-    if world > 1:
-        t = torch.tensor([e2e_ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_ms = float(t.item())
+    e2e_ms = max_over_ranks(f0.elapsed_time(f1), world)
     d2h = ab["gap"] + ab["rho"] + ab["auto"]
-    e2e = {"value": world * w.P * n_e2e / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": ab["input"],
+    e2e = {"value": aggregate_value(w.P, n_e2e, world, e2e_ms), "unit": UNIT, "h2d_bytes_per_step": ab["input"],
            "d2h_bytes_per_step": d2h, "steps": n_e2e, "ms_per_step": e2e_ms / n_e2e,
            "call": "delta_analyze_shot_host: pinned host chunks in, all five outputs copied back to pinned host memory"}
 
@@ -325,7 +338,7 @@ def run_ours(args):
         cpu = cpu_baseline(w)
 
     if rank == 0:
-        value = world * w.P * K / (ms * 1e-3)
+        value = aggregate_value(w.P, K, world, ms)
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
                 "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                 "dtype": "f32", "data": "synthetic",
