@@ -223,7 +223,8 @@ def run_ours(args):
 
     w = es.WORKLOADS[args.workload]
     peaks = load_peaks()
-    plan = b.Plan(w.C, w.T, w.nfft, w.hop, w.max_lag)
+    plan = b.Plan(w.C, w.T, w.nfft, w.hop, w.max_lag,
+                  contraction={"auto": b.CONTRACT_AUTO, "fp32": b.CONTRACT_FP32, "tc": b.CONTRACT_TC}[args.contraction])
     s = plan.sizes
     # inputs resident in HBM before the timed region; every rank works on its own chunks (weak scaling)
     xs_host = [es.turbulence(w.T, seed) for seed in rank_chunk_seeds(rank)]
@@ -364,6 +365,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="single", choices=["single"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--contraction", default="auto", choices=["auto", "fp32", "tc"])
     args = ap.parse_args()
     if args.impl == "reference":
         if args.steps == 1000 and args.warmup == 100:   # defaults are sized for the GPU arm

@@ -120,9 +120,10 @@ int delta_stft(delta_plan *plan, const void *d_x, int64_t ld, void *d_X, void *s
  * definition above. */
 int delta_stft_unpack(delta_plan *plan, const void *d_X, float *d_out, void *stream);
 
-/* a2 + a3, Eq. (1a).  d_S: complex64 [F][P_pad] (frequency-major: for each bin the upper triangle
- * of the cross-spectral matrix, pairs in lexicographic order, row stride s_row_stride);
- * d_Sauto: float [C][F] autospectra S_cc[f].  Either may be NULL. */
+/* a2 + a3, Eq. (1a).  d_S: complex64 [F][P_pad] (frequency-major: for each bin the strict upper
+ * triangle of the cross-spectral matrix packed column by column, S_ij (i < j) at column
+ * j(j-1)/2 + i, row stride s_row_stride); d_Sauto: float [C][F] autospectra S_cc[f].
+ * Either may be NULL.  (The per-pair outputs below are in lexicographic pair order.) */
 int delta_cross_spectra(delta_plan *plan, const void *d_X, float *d_S, float *d_Sauto, void *stream);
 
 /* a4, Eq. (1b): d_G float [P][F].  0 where S_ii S_jj = 0 (R16). */

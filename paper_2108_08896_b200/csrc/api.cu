@@ -34,8 +34,13 @@ static int validate(const delta_config *c) {
   return DELTA_OK;
 }
 
-static bool tc_supported(const delta_config *) {
-  return false;  // the tcgen05 contraction is not wired in yet
+static bool tc_supported(const delta_config *c) {
+  // two pipeline stages of 128*Cp bytes must fit in shared memory, and the tile plan must exist
+  size_t Cp = align_up((size_t)c->n_channels, 64);
+  if (Cp < 128) Cp = 128;
+  if (Cp > 768) return false;
+  TcHostPlan tmp;
+  return tc_plan_tiles((int)Cp, &tmp);
 }
 
 }  // namespace delta
@@ -95,8 +100,10 @@ int delta_plan_create(const delta_config *cfg, delta_plan **out) {
     default: p->s2 = (float)(1.0 / (sw * sw)); break;
   }
   p->h_pairs.reserve((size_t)l.P);
-  for (int i = 0; i < l.C; ++i)
-    for (int j = i + 1; j < l.C; ++j) p->h_pairs.push_back(make_ushort2((unsigned short)i, (unsigned short)j));
+  for (int j = 1; j < l.C; ++j)
+    for (int i = 0; i < j; ++i) p->h_pairs.push_back(make_ushort2((unsigned short)i, (unsigned short)j));
+  memset(&p->tc, 0, sizeof(p->tc));
+  if (p->contraction == DELTA_CONTRACT_TC && !tc_plan_tiles(l.Cp, &p->tc)) { delete p; return DELTA_ERR_UNSUPPORTED; }
 
   Workspace &w = p->wsl;
   size_t o = 0;
@@ -148,6 +155,7 @@ int delta_plan_set_workspace(delta_plan *p, void *d_ws, size_t bytes, void *stre
   if (bytes < p->wsl.total) return DELTA_ERR_NO_WORKSPACE;
   cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
   DELTA_CUDA_CHECK(cudaGetDevice(&p->device));
+  DELTA_CUDA_CHECK(cudaDeviceGetAttribute(&p->num_sms, cudaDevAttrMultiProcessorCount, p->device));
   p->ws = reinterpret_cast<char *>(d_ws);
   p->ws_bytes = bytes;
   p->offsets_set = false;
@@ -218,13 +226,18 @@ int delta_stft_unpack(delta_plan *p, const void *d_X, float *d_out, void *stream
   return launch_stft_unpack(p, d_X, d_out, reinterpret_cast<cudaStream_t>(stream));
 }
 
+static int contract(delta_plan *p, const void *d_X, float *d_S, float *d_auto, cudaStream_t st) {
+  return p->contraction == DELTA_CONTRACT_TC ? launch_contract_tc(p, d_X, d_S, d_auto, st)
+                                             : launch_contract_fp32(p, d_X, d_S, d_auto, st);
+}
+
 int delta_cross_spectra(delta_plan *p, const void *d_X, float *d_S, float *d_Sauto, void *stream) {
   int rc = need_ws(p);
   if (rc) return rc;
   if (!d_X) return DELTA_ERR_INVALID_ARG;
   if (!aligned16(d_X) || (d_S && !aligned16(d_S))) return DELTA_ERR_ALIGNMENT;
   if (!d_S && !d_Sauto) return DELTA_OK;
-  return launch_contract_fp32(p, d_X, d_S, d_Sauto, reinterpret_cast<cudaStream_t>(stream));
+  return contract(p, d_X, d_S, d_Sauto, reinterpret_cast<cudaStream_t>(stream));
 }
 
 static int pair_stage(delta_plan *p, const float *d_S, const float *d_Sauto, float *G, float *A, float *P, float *R,
@@ -271,7 +284,7 @@ int delta_analyze_chunk(delta_plan *p, const void *d_x, int64_t ld, float *d_G, 
   if (ev) DELTA_CUDA_CHECK(cudaEventRecord(p->stage_ev[1], st));
   float *au = d_Sauto ? d_Sauto : p->d_auto();
   const bool pairs_wanted = (d_G || d_A || d_P || d_R) && p->lay.P > 0;
-  rc = launch_contract_fp32(p, p->d_X(), pairs_wanted ? p->d_S() : nullptr, au, st);
+  rc = contract(p, p->d_X(), pairs_wanted ? p->d_S() : nullptr, au, st);
   if (rc) return rc;
   if (ev) DELTA_CUDA_CHECK(cudaEventRecord(p->stage_ev[2], st));
   if (pairs_wanted) rc = launch_pair_epilogue(p, p->d_S(), au, d_G, d_A, d_P, d_R, st);

@@ -12,6 +12,16 @@ namespace delta {
 constexpr int kPairTile = 64;     // channel block of the FP32 contraction tiles
 constexpr int kSegBlock = 8;      // segments per K-chunk ("kc") of the X layout
 constexpr int kThreads = 256;
+constexpr int kTcMaxGroups = 16;  // TMEM-sized groups of accumulator tiles per frequency bin
+constexpr int kTcMaxTiles = 4;    // tiles per group
+
+// tile plan of the tensor-core contraction (host side; see contract_tc.cu)
+struct TcHostPlan {
+  int ngroups;
+  int ntiles[kTcMaxGroups];
+  int tiles[kTcMaxGroups][kTcMaxTiles][6];  // row0, col0, N, lane_lo, tmem col of Re, tmem col of Im
+};
+bool tc_plan_tiles(int Cp, TcHostPlan *out);
 
 struct Layout {
   // X (STFT) buffer, frequency-major so that one bin's C x K matrix is one contiguous block:
@@ -19,7 +29,7 @@ struct Layout {
   //   TC   mode : __half X[f][prec][part][kc][c][8]           prec 0 = hi, 1 = lo (split fp16)
   // k = 8*kc + kk, c < Cp (rows C..Cp-1 are zero), kc < Kc = Kp/8, Kp = K rounded up to 16.
   int C, Cp, T, L, N, H, K, Kp, Kc, F, M, nlags;
-  int64_t P, Ppad;
+  int64_t P, Ppad;        // S is complex64 [F][Ppad], pair (i<j) at column p' = j(j-1)/2 + i
   int64_t x_elems_per_f;  // elements (float or half) per frequency
 };
 
@@ -38,7 +48,9 @@ struct delta_plan {
   // host tables (uploaded by delta_plan_set_workspace)
   std::vector<float2> h_tw;      // e^{-2 pi i f / L}, f = 0..L-1
   std::vector<float> h_win;      // periodic Hann
-  std::vector<ushort2> h_pairs;  // (i, j), lexicographic
+  std::vector<ushort2> h_pairs;  // (i, j) in S order: p' = j(j-1)/2 + i (column-major upper triangle)
+  delta::TcHostPlan tc;
+  int num_sms = 148;
   // device state
   char *ws = nullptr;
   size_t ws_bytes = 0;
@@ -81,6 +93,7 @@ int launch_offsets(delta_plan *p, const void *d_x, int64_t ld, int n_first, cuda
 int launch_stft(delta_plan *p, const void *d_x, int64_t ld, void *d_X, cudaStream_t st);
 int launch_stft_unpack(delta_plan *p, const void *d_X, float *d_out, cudaStream_t st);
 int launch_contract_fp32(delta_plan *p, const void *d_X, float *d_S, float *d_auto, cudaStream_t st);
+int launch_contract_tc(delta_plan *p, const void *d_X, float *d_S, float *d_auto, cudaStream_t st);
 int launch_pair_epilogue(delta_plan *p, const float *d_S, const float *d_auto, float *d_G, float *d_A,
                          float *d_P, float *d_R, cudaStream_t st);
 

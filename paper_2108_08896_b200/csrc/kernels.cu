@@ -306,13 +306,12 @@ contract_fp32_kernel(const float *__restrict__ X, Layout lay, float scale, float
   for (int a = 0; a < 4; ++a) {
     const int i = bi * kPairTile + 4 * ty + a;
     if (i >= C) continue;
-    const int rowbase = i * C - (i * (i + 1)) / 2 - i - 1;  // p = rowbase + j
 #pragma unroll
     for (int b = 0; b < 4; ++b) {
       const int j = bj * kPairTile + 4 * tx + b;
       if (j >= C) continue;
       if (i < j) {
-        if (S) S[(int64_t)f * lay.Ppad + rowbase + j] = make_float2(acc_re[a][b] * scale, acc_im[a][b] * scale);
+        if (S) S[(int64_t)f * lay.Ppad + (j * (j - 1)) / 2 + i] = make_float2(acc_re[a][b] * scale, acc_im[a][b] * scale);
       } else if (i == j) {
         if (Sauto) Sauto[(int64_t)i * lay.F + f] = acc_re[a][b] * scale;
       }
@@ -377,9 +376,11 @@ pair_epilogue_kernel(const float2 *__restrict__ S, const float *__restrict__ Sau
 #pragma unroll 1
   for (int r = 0; r < ROUNDS; ++r) {
     const int pl = r * CONC + g;
-    const int64_t p = p0 + pl;
-    const bool valid = p < lay.P;
-    const ushort2 ij = pairs[valid ? p : 0];
+    const int64_t ps = p0 + pl;  // position in S order (column-major upper triangle)
+    const bool valid = ps < lay.P;
+    const ushort2 ij = pairs[valid ? ps : 0];
+    // output row: lexicographic pair index (reading R9)
+    const int64_t p = (int64_t)ij.x * lay.C - ((int64_t)ij.x * (ij.x + 1)) / 2 + (ij.y - ij.x - 1);
     const float *ai = Sauto + (int64_t)ij.x * F, *aj = Sauto + (int64_t)ij.y * F;
     float si = 0.f, sj = 0.f;
     for (int f = gt; f < F; f += GROUP) {

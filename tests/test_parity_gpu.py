@@ -57,6 +57,13 @@ def compare(out, ref, pairs, label=""):
     return stats
 
 
+@pytest.fixture(params=["fp32", "tc"])
+def mode(request):
+    """Both contraction back ends: FP32 FMA pipe and tcgen05 tensor cores (split fp16)."""
+    b = binding()
+    return b.CONTRACT_FP32 if request.param == "fp32" else b.CONTRACT_TC
+
+
 def gpu_analyze(x, L, H, M, in_dtype=None, norm_mode=0, n_first=0, contraction=0, scaling=0, fs=500e3, ld_pad=0):
     b = binding()
     C, T = x.shape
@@ -88,10 +95,10 @@ def test_library_is_the_cuda_path():
     assert plan.sizes.contraction in (b.CONTRACT_FP32, b.CONTRACT_TC)
 
 
-def test_config1_tiny_full():
+def test_config1_tiny_full(mode):
     w = es.WORKLOADS["tiny"]
     x = es.tiny()
-    _, out = gpu_analyze(x, w.nfft, w.hop, w.max_lag)
+    _, out = gpu_analyze(x, w.nfft, w.hop, w.max_lag, contraction=mode)
     ref = oracle_for(x, w.nfft, w.hop, w.max_lag)
     st = compare(out, ref, o.all_pairs(w.C), "tiny")
     print("tiny", st)
@@ -100,20 +107,20 @@ def test_config1_tiny_full():
     assert np.abs(np.angle(np.exp(1j * (out["A"][:, 10] - expect)))).max() < 2e-2
 
 
-def test_config2_single_chunk_full():
+def test_config2_single_chunk_full(mode):
     w = es.WORKLOADS["single"]
     x = es.single()
-    _, out = gpu_analyze(x, w.nfft, w.hop, w.max_lag)
+    _, out = gpu_analyze(x, w.nfft, w.hop, w.max_lag, contraction=mode)
     ref = oracle_for(x, w.nfft, w.hop, w.max_lag)
     st = compare(out, ref, o.all_pairs(w.C), "single")
     print("single", st)
 
 
-def test_stft_stage_against_oracle():
+def test_stft_stage_against_oracle(mode):
     b = binding()
     w = es.WORKLOADS["tiny"]
     x = es.tiny()
-    plan = b.Plan(w.C, w.T, w.nfft, w.hop, w.max_lag)
+    plan = b.Plan(w.C, w.T, w.nfft, w.hop, w.max_lag, contraction=mode)
     X = plan.stft_unpack(plan.stft(dev(x))).cpu().numpy()
     Xo = o.stft(x, w.nfft, w.hop)
     assert X.shape == Xo.shape
@@ -121,11 +128,11 @@ def test_stft_stage_against_oracle():
     assert np.abs(X - Xo).max() <= 2e-6 * scale
 
 
-def test_staged_calls_equal_fused_call():
+def test_staged_calls_equal_fused_call(mode):
     b = binding()
     w = es.WORKLOADS["single"]
     x = es.single()[:40]
-    plan = b.Plan(40, w.T, w.nfft, w.hop, w.max_lag)
+    plan = b.Plan(40, w.T, w.nfft, w.hop, w.max_lag, contraction=mode)
     xd = dev(x)
     fused = plan.analyze_chunk(xd)
     X = plan.stft(xd)
@@ -134,12 +141,14 @@ def test_staged_calls_equal_fused_call():
     torch.cuda.synchronize()
     for name, t in (("G", G), ("A", A), ("P", P), ("R", R), ("Sauto", Sa)):
         assert torch.equal(t, fused[name]), name
-    # S itself against the oracle, in its documented [F][P_pad] layout
+    # S itself against the oracle, in its documented layout: [F][P_pad], pair (i<j) at column j(j-1)/2 + i
     Xo = o.stft(x, w.nfft, w.hop)
-    pairs = o.all_pairs(40)
-    So = o.cross_spectra(Xo, pairs, o.scale_factor(w.nfft))
+    pairs = np.array([(i, j) for j in range(1, 40) for i in range(j)])
+    s2 = o.scale_factor(w.nfft)
+    So = o.cross_spectra(Xo, pairs, s2)
     Sg = torch.view_as_complex(S).cpu().numpy()[:, :len(pairs)].T
-    den = np.sqrt(o.auto_spectra(Xo, o.scale_factor(w.nfft))[pairs[:, 0]] * o.auto_spectra(Xo, o.scale_factor(w.nfft))[pairs[:, 1]])
+    Sa_o = o.auto_spectra(Xo, s2)
+    den = np.sqrt(Sa_o[pairs[:, 0]] * Sa_o[pairs[:, 1]])
     assert np.max(np.abs(Sg - So) / den) < 1e-5
 
 
@@ -154,29 +163,29 @@ def test_staged_calls_equal_fused_call():
     (9, 4100, 2048, 1024, 1000),
     (33, 900, 128, 64, 64),
 ])
-def test_edge_shapes(C, T, L, H, M):
+def test_edge_shapes(C, T, L, H, M, mode):
     x = np.random.default_rng(C * 1000 + L).standard_normal((C, T)).astype(np.float32)
     x += 0.5 * x[0:1]  # some coherence between channels
-    _, out = gpu_analyze(x, L, H, M)
+    _, out = gpu_analyze(x, L, H, M, contraction=mode)
     ref = oracle_for(x, L, H, M)
     assert out["G"].shape == ref["G"].shape and out["R"].shape == ref["R"].shape
     compare(out, ref, o.all_pairs(C), f"edge C={C} L={L}")
 
 
-def test_strided_rows_and_scalings():
+def test_strided_rows_and_scalings(mode):
     x = np.random.default_rng(5).standard_normal((6, 2000)).astype(np.float32)
     b = binding()
     for scaling in (b.SCALE_NONE, b.SCALE_DENSITY, b.SCALE_SPECTRUM):
-        _, out = gpu_analyze(x, 256, 128, 64, scaling=scaling, fs=500e3, ld_pad=37)
+        _, out = gpu_analyze(x, 256, 128, 64, scaling=scaling, fs=500e3, ld_pad=37, contraction=mode)
         ref = oracle_for(x, 256, 128, 64, scaling=scaling, fs=500e3)
         compare(out, ref, o.all_pairs(6), f"scaling {scaling}")
 
 
-def test_degenerate_zero_channel():
+def test_degenerate_zero_channel(mode):
     """A dead channel: S_ii = 0 -> coherence and rho are 0 by definition (R16), nothing is NaN."""
     x = np.random.default_rng(6).standard_normal((4, 1500)).astype(np.float32)
     x[2] = 0.0
-    _, out = gpu_analyze(x, 128, 64, 64)
+    _, out = gpu_analyze(x, 128, 64, 64, contraction=mode)
     ref = oracle_for(x, 128, 64, 64)
     compare(out, ref, o.all_pairs(4), "dead channel")
     dead = [p for p, (i, j) in enumerate(o.all_pairs(4)) if 2 in (i, j)]
@@ -184,13 +193,13 @@ def test_degenerate_zero_channel():
 
 
 @pytest.mark.parametrize("norm_mode", [0, 1, 2])
-def test_int16_and_normalisation_modes(norm_mode):
+def test_int16_and_normalisation_modes(norm_mode, mode):
     rng = np.random.default_rng(8)
     o_true = rng.uniform(2000, 3000, size=6)
     sig = rng.standard_normal((6, 6000))
     sig[1] += 0.7 * sig[0]
     counts = np.rint(o_true[:, None] + 200 * sig).astype(np.int16)
-    plan, out = gpu_analyze(counts, 512, 256, 256, norm_mode=norm_mode, n_first=5000)
+    plan, out = gpu_analyze(counts, 512, 256, 256, norm_mode=norm_mode, n_first=5000, contraction=mode)
     offs = o.offsets(counts[:, :5000])
     if norm_mode:
         assert np.array_equal(plan.get_offsets(), offs)   # integer-exact sums
@@ -198,7 +207,7 @@ def test_int16_and_normalisation_modes(norm_mode):
     compare(out, ref, o.all_pairs(6), f"int16 norm {norm_mode}")
     # float32 input with offsets
     xf = counts.astype(np.float32)
-    plan, out = gpu_analyze(xf, 512, 256, 256, norm_mode=norm_mode, n_first=5000)
+    plan, out = gpu_analyze(xf, 512, 256, 256, norm_mode=norm_mode, n_first=5000, contraction=mode)
     ref = oracle_for(xf, 512, 256, 256, norm_mode=norm_mode, offs=o.offsets(xf[:, :5000]))
     compare(out, ref, o.all_pairs(6), f"f32 norm {norm_mode}")
 
@@ -225,12 +234,12 @@ def _sampled_pairs(C, n_ch, seed):
 
 
 @pytest.mark.parametrize("name,n_ch", [("long", 12), ("wide", 10)])
-def test_full_size_configs_on_sampled_pairs(name, n_ch):
+def test_full_size_configs_on_sampled_pairs(name, n_ch, mode):
     """Configs 3 and 5 at BASELINE's full sizes; the oracle's direct DFT is run on a sample of
     channels (all pairs among them, incl. first/last channel), compared element by element."""
     w = es.WORKLOADS[name]
     x = es.make(name)
-    _, out = gpu_analyze(x, w.nfft, w.hop, w.max_lag)
+    _, out = gpu_analyze(x, w.nfft, w.hop, w.max_lag, contraction=mode)
     assert out["G"].shape == (w.P, w.F) and out["R"].shape == (w.P, 2 * w.max_lag + 1)
     ch, loc, glob = _sampled_pairs(w.C, n_ch, 42)
     ref = oracle_for(x[ch], w.nfft, w.hop, w.max_lag)
