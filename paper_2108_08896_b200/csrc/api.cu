@@ -5,6 +5,7 @@
 #include <new>
 
 #include "delta_internal.h"
+#include "fft_reg.cuh"
 
 namespace delta {
 
@@ -93,6 +94,8 @@ int delta_plan_create(const delta_config *cfg, delta_plan **out) {
     sw += w;
     sw2 += w * w;
   }
+  p->h_ftab.resize((size_t)fft_table_size(l.N) + 1);
+  fft_twiddle_table(l.N, p->h_ftab.data());
   switch (cfg->scaling) {
     case DELTA_SCALE_WINPOW: p->s2 = (float)(1.0 / sw2); break;
     case DELTA_SCALE_NONE: p->s2 = 1.f; break;
@@ -110,6 +113,7 @@ int delta_plan_create(const delta_config *cfg, delta_plan **out) {
   auto take = [&](size_t bytes) { size_t at = o; o = align_up(o + bytes, 256); return at; };
   w.off_tw = take((size_t)L * sizeof(float2));
   w.off_win = take((size_t)L * sizeof(float));
+  w.off_ftab = take(p->h_ftab.size() * sizeof(float2));
   w.off_pairs = take((size_t)(l.P > 0 ? l.P : 1) * sizeof(ushort2));
   w.off_offs = take((size_t)l.C * sizeof(double));
   w.off_isum = take((size_t)l.C * sizeof(long long));
@@ -162,6 +166,7 @@ int delta_plan_set_workspace(delta_plan *p, void *d_ws, size_t bytes, void *stre
   const Layout &l = p->lay;
   DELTA_CUDA_CHECK(cudaMemcpyAsync(p->ws + p->wsl.off_tw, p->h_tw.data(), (size_t)l.L * sizeof(float2), cudaMemcpyHostToDevice, st));
   DELTA_CUDA_CHECK(cudaMemcpyAsync(p->ws + p->wsl.off_win, p->h_win.data(), (size_t)l.L * sizeof(float), cudaMemcpyHostToDevice, st));
+  DELTA_CUDA_CHECK(cudaMemcpyAsync(p->ws + p->wsl.off_ftab, p->h_ftab.data(), p->h_ftab.size() * sizeof(float2), cudaMemcpyHostToDevice, st));
   if (l.P > 0)
     DELTA_CUDA_CHECK(cudaMemcpyAsync(p->ws + p->wsl.off_pairs, p->h_pairs.data(), (size_t)l.P * sizeof(ushort2), cudaMemcpyHostToDevice, st));
   // zero rows C..Cp-1 of the workspace X once (kernels never write them)

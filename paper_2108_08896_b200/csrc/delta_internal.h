@@ -34,7 +34,7 @@ struct Layout {
 };
 
 struct Workspace {
-  size_t off_tw, off_win, off_pairs, off_offs, off_isum, off_chscale, off_X, off_S, off_auto, total;
+  size_t off_tw, off_win, off_ftab, off_pairs, off_offs, off_isum, off_chscale, off_X, off_S, off_auto, total;
 };
 
 }  // namespace delta
@@ -48,6 +48,7 @@ struct delta_plan {
   // host tables (uploaded by delta_plan_set_workspace)
   std::vector<float2> h_tw;      // e^{-2 pi i f / L}, f = 0..L-1
   std::vector<float> h_win;      // periodic Hann
+  std::vector<float2> h_ftab;    // per-pass twiddles of the register FFT (fft_reg.cuh), N = L/2
   std::vector<ushort2> h_pairs;  // (i, j) in S order: p' = j(j-1)/2 + i (column-major upper triangle)
   delta::TcHostPlan tc;
   int num_sms = 148;
@@ -67,6 +68,7 @@ struct delta_plan {
 
   const float2 *d_tw() const { return reinterpret_cast<const float2 *>(ws + wsl.off_tw); }
   const float *d_win() const { return reinterpret_cast<const float *>(ws + wsl.off_win); }
+  const float2 *d_ftab() const { return reinterpret_cast<const float2 *>(ws + wsl.off_ftab); }
   const ushort2 *d_pairs() const { return reinterpret_cast<const ushort2 *>(ws + wsl.off_pairs); }
   double *d_offs() const { return reinterpret_cast<double *>(ws + wsl.off_offs); }
   long long *d_isum() const { return reinterpret_cast<long long *>(ws + wsl.off_isum); }
@@ -88,7 +90,33 @@ void set_cuda_error(cudaError_t e);
     }                                          \
   } while (0)
 
-// kernels.cu launchers (each returns a delta_status and counts its launches into plan->launches)
+// opt in to more than 48 KB of dynamic shared memory
+template <typename Kern>
+static inline int opt_in_smem(Kern kern, size_t bytes) {
+  if (bytes > 48 * 1024) {
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+    if (e != cudaSuccess) {
+      set_cuda_error(e);
+      return DELTA_ERR_CUDA;
+    }
+  }
+  return DELTA_OK;
+}
+
+// dispatch on the transform length (validate() admits powers of two in [64, 4096])
+#define DELTA_SWITCH_L(L_, CALL)           \
+  switch (L_) {                            \
+    case 64: return CALL(64);              \
+    case 128: return CALL(128);            \
+    case 256: return CALL(256);            \
+    case 512: return CALL(512);            \
+    case 1024: return CALL(1024);          \
+    case 2048: return CALL(2048);          \
+    case 4096: return CALL(4096);          \
+    default: return DELTA_ERR_UNSUPPORTED; \
+  }
+
+// launchers (each returns a delta_status and counts its launches into plan->launches)
 int launch_offsets(delta_plan *p, const void *d_x, int64_t ld, int n_first, cudaStream_t st);
 int launch_stft(delta_plan *p, const void *d_x, int64_t ld, void *d_X, cudaStream_t st);
 int launch_stft_unpack(delta_plan *p, const void *d_X, float *d_out, cudaStream_t st);

@@ -1,7 +1,4 @@
 // CUDA-core kernels of libdelta_b200 (sm_100a):
-//   offsets_kernel        a0  per-shot channel offsets                      (R1)
-//   stft_kernel           a0+a1 normalise + Hann + real FFT of every segment
-//   stft_unpack_kernel    test accessor
 //   contract_fp32_kernel  a2+a3 Eq. (1a) on the FP32 FMA pipe
 //   pair_epilogue_kernel  a4+a5 Eq. (1b), (1c), |1a|, (1d) per pair
 #include <cuda_fp16.h>
@@ -12,49 +9,6 @@
 namespace delta {
 
 // ------------------------------------------------------------------------------------------
-// a0: o_c = mean of the first n_first samples (integer-exact sum for int16)
-__global__ void __launch_bounds__(kThreads) offsets_kernel(const void *__restrict__ x, int64_t ld, int in_dtype,
-                                                           int n_first, double *__restrict__ offs,
-                                                           long long *__restrict__ isum) {
-  const int c = blockIdx.x;
-  __shared__ double red_d[kThreads / 32];
-  __shared__ long long red_i[kThreads / 32];
-  double sd = 0.0;
-  long long si = 0;
-  if (in_dtype == DELTA_I16) {
-    const short *row = reinterpret_cast<const short *>(x) + (int64_t)c * ld;
-    for (int t = threadIdx.x; t < n_first; t += kThreads) si += row[t];
-  } else {
-    const float *row = reinterpret_cast<const float *>(x) + (int64_t)c * ld;
-    for (int t = threadIdx.x; t < n_first; t += kThreads) sd += (double)row[t];
-  }
-  for (int o = 16; o > 0; o >>= 1) {
-    sd += __shfl_xor_sync(0xffffffffu, sd, o);
-    si += __shfl_xor_sync(0xffffffffu, si, o);
-  }
-  if ((threadIdx.x & 31) == 0) {
-    red_d[threadIdx.x >> 5] = sd;
-    red_i[threadIdx.x >> 5] = si;
-  }
-  __syncthreads();
-  if (threadIdx.x == 0) {
-    double td = 0.0;
-    long long ti = 0;
-    for (int w = 0; w < kThreads / 32; ++w) {
-      td += red_d[w];
-      ti += red_i[w];
-    }
-    if (in_dtype == DELTA_I16) {
-      isum[c] = ti;
-      offs[c] = (double)ti / (double)n_first;
-    } else {
-      isum[c] = 0;
-      offs[c] = td / (double)n_first;
-    }
-  }
-}
-
-// ------------------------------------------------------------------------------------------
 template <int L>
 struct FftCfg {
   static constexpr int N = L / 2;
@@ -62,185 +16,6 @@ struct FftCfg {
   static constexpr int CONC = kThreads / GROUP;  // transforms in flight per CTA
   static constexpr int FS = N + 4;               // staging row stride (floats); == 4 mod 8
 };
-
-struct SampleLoader {
-  const void *x;
-  int in_dtype, norm_mode;
-  float o, inv_o;        // float input: offset and 1/offset
-  long long isum;        // int16 input: integer sum over n_first samples
-  float inv_isum, inv_n; // 1/isum, 1/n_first
-  int n_first;
-  __device__ __forceinline__ float operator()(int64_t idx) const {
-    if (in_dtype == DELTA_I16) {
-      const int v = reinterpret_cast<const short *>(x)[idx];
-      if (norm_mode == DELTA_NORM_NONE) return (float)v;
-      // (x - o) = (x n - sum)/n exactly in integers; one rounding at the conversion
-      const float num = __ll2float_rn((long long)v * n_first - isum);
-      return norm_mode == DELTA_NORM_RELATIVE ? num * inv_isum : num * inv_n;
-    }
-    const float v = reinterpret_cast<const float *>(x)[idx];
-    if (norm_mode == DELTA_NORM_NONE) return v;
-    const float d = v - o;
-    return norm_mode == DELTA_NORM_RELATIVE ? d * inv_o : d;
-  }
-};
-
-// a0+a1.  grid = (ceil(K/8), C); one CTA transforms 8 consecutive segments of one channel and
-// writes, for every bin, one 8-segment piece of the frequency-major X layout.
-template <int L>
-__global__ void __launch_bounds__(kThreads)
-stft_kernel(const void *__restrict__ x, int64_t ld, int in_dtype, int norm_mode, int n_first,
-            const double *__restrict__ offs, const long long *__restrict__ isum,
-            const float2 *__restrict__ tw, const float *__restrict__ win, Layout lay, void *__restrict__ Xout,
-            int tc_mode, const float *__restrict__ chscale) {
-  using Cfg = FftCfg<L>;
-  constexpr int N = Cfg::N, GROUP = Cfg::GROUP, CONC = Cfg::CONC, FS = Cfg::FS;
-  constexpr int ROUNDS = kSegBlock / CONC;
-  extern __shared__ __align__(16) unsigned char smem_raw[];
-  float2 *bufA = reinterpret_cast<float2 *>(smem_raw);
-  float2 *bufB = bufA + CONC * N;
-  float *stage = reinterpret_cast<float *>(bufB + CONC * N);  // [2][8][FS]
-
-  const int c = blockIdx.y, kb = blockIdx.x;
-  const int tid = threadIdx.x, g = tid / GROUP, gt = tid % GROUP;
-
-  SampleLoader ldr;
-  ldr.x = x;
-  ldr.in_dtype = in_dtype;
-  ldr.norm_mode = norm_mode;
-  ldr.n_first = n_first;
-  ldr.o = 0.f; ldr.inv_o = 0.f; ldr.isum = 0; ldr.inv_isum = 0.f; ldr.inv_n = 0.f;
-  if (norm_mode != DELTA_NORM_NONE) {
-    const double od = offs[c];
-    ldr.o = (float)od;
-    ldr.inv_o = (float)(1.0 / od);
-    ldr.isum = isum[c];
-    ldr.inv_isum = (float)(1.0 / (double)ldr.isum);
-    ldr.inv_n = (float)(1.0 / (double)n_first);
-  }
-  const int64_t row0 = (int64_t)c * ld;
-
-#pragma unroll 1
-  for (int r = 0; r < ROUNDS; ++r) {
-    const int kk = r * CONC + g;
-    const int k = kb * kSegBlock + kk;
-    float2 *a = bufA + g * N, *b = bufB + g * N;
-    if (k < lay.K) {
-      const int64_t t0 = row0 + (int64_t)k * lay.H;
-      for (int n = gt; n < N; n += GROUP) {
-        const float2 w = __ldg(reinterpret_cast<const float2 *>(win) + n);
-        a[n] = make_float2(ldr(t0 + 2 * n) * w.x, ldr(t0 + 2 * n + 1) * w.y);
-      }
-    } else {
-      for (int n = gt; n < N; n += GROUP) a[n] = make_float2(0.f, 0.f);
-    }
-    group_sync<GROUP>();
-    const float2 *Z = fft_stockham<N, GROUP, false>(a, b, tw, gt);
-    for (int f = gt; f <= N; f += GROUP) {
-      const float2 X = rfft_split<N>(Z, tw, f);
-      stage[(0 * kSegBlock + kk) * FS + f] = X.x;
-      stage[(1 * kSegBlock + kk) * FS + f] = X.y;
-    }
-    group_sync<GROUP>();
-  }
-  __syncthreads();
-
-  const int F = N + 1;
-  if (!tc_mode) {
-    float *X = reinterpret_cast<float *>(Xout);
-    for (int idx = tid; idx < 4 * F; idx += kThreads) {
-      const int h = idx & 1, pf = idx >> 1;
-      const int part = pf / F, f = pf - part * F;
-      const float *s = stage + (part * kSegBlock + 4 * h) * FS + f;
-      const float4 v = make_float4(s[0], s[FS], s[2 * FS], s[3 * FS]);
-      const int64_t o = (int64_t)f * lay.x_elems_per_f +
-                        (((int64_t)part * lay.Kc + kb) * lay.Cp + c) * kSegBlock + 4 * h;
-      *reinterpret_cast<float4 *>(X + o) = v;
-    }
-  } else {
-    // split fp16: v * scale = hi + lo (scale = power of two chosen by chscale_kernel)
-    __half *X = reinterpret_cast<__half *>(Xout);
-    const float sc = chscale[c];
-    for (int idx = tid; idx < 2 * F; idx += kThreads) {
-      const int part = idx / F, f = idx - part * F;
-      const float *s = stage + (part * kSegBlock) * FS + f;
-      __align__(16) __half hi[8], lo[8];
-#pragma unroll
-      for (int q = 0; q < 8; ++q) {
-        const float v = s[q * FS] * sc;
-        hi[q] = __float2half_rn(v);
-        lo[q] = __float2half_rn(v - __half2float(hi[q]));
-      }
-      const int64_t base = (int64_t)f * lay.x_elems_per_f;
-      const int64_t plane = (int64_t)lay.Kc * lay.Cp * kSegBlock;  // one [kc][c][8] block
-      const int64_t within = ((int64_t)kb * lay.Cp + c) * kSegBlock;
-      *reinterpret_cast<uint4 *>(X + base + (0 * 2 + part) * plane + within) = *reinterpret_cast<uint4 *>(hi);
-      *reinterpret_cast<uint4 *>(X + base + (1 * 2 + part) * plane + within) = *reinterpret_cast<uint4 *>(lo);
-    }
-  }
-}
-
-// per-channel power-of-two scale for the split-fp16 operands: |X| <= (L/2) max|y|  =>  scale * |X| <= 2^14
-__global__ void __launch_bounds__(kThreads)
-chscale_kernel(const void *__restrict__ x, int64_t ld, int in_dtype, int norm_mode, int n_first,
-               const double *__restrict__ offs, const long long *__restrict__ isum, int T, int L,
-               float *__restrict__ chscale) {
-  const int c = blockIdx.x;
-  SampleLoader ldr;
-  ldr.x = x; ldr.in_dtype = in_dtype; ldr.norm_mode = norm_mode; ldr.n_first = n_first;
-  ldr.o = 0.f; ldr.inv_o = 0.f; ldr.isum = 0; ldr.inv_isum = 0.f; ldr.inv_n = 0.f;
-  if (norm_mode != DELTA_NORM_NONE) {
-    const double od = offs[c];
-    ldr.o = (float)od; ldr.inv_o = (float)(1.0 / od);
-    ldr.isum = isum[c]; ldr.inv_isum = (float)(1.0 / (double)ldr.isum);
-    ldr.inv_n = (float)(1.0 / (double)n_first);
-  }
-  const int64_t row0 = (int64_t)c * ld;
-  float m = 0.f;
-  for (int t = threadIdx.x; t < T; t += kThreads) m = fmaxf(m, fabsf(ldr(row0 + t)));
-  for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
-  __shared__ float red[kThreads / 32];
-  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = m;
-  __syncthreads();
-  if (threadIdx.x == 0) {
-    for (int w = 0; w < kThreads / 32; ++w) m = fmaxf(m, red[w]);
-    const float bound = m * (0.5f * (float)L);  // sum_n w[n] |y| <= (L/2) max|y|
-    float sc = 1.f;
-    if (bound > 0.f && isfinite(bound)) {
-      int e;
-      frexpf(bound, &e);            // bound = mant * 2^e, mant in [0.5, 1)  =>  bound < 2^e
-      sc = ldexpf(1.f, 14 - e);     // scale * bound < 2^14
-    }
-    chscale[c] = sc;
-  }
-}
-
-// test accessor: X layout -> complex64 [C][K][F]
-__global__ void __launch_bounds__(kThreads)
-stft_unpack_kernel(const void *__restrict__ Xin, Layout lay, int tc_mode, const float *__restrict__ chscale,
-                   float2 *__restrict__ out) {
-  const int64_t total = (int64_t)lay.C * lay.K * lay.F;
-  for (int64_t idx = (int64_t)blockIdx.x * kThreads + threadIdx.x; idx < total; idx += (int64_t)gridDim.x * kThreads) {
-    const int f = (int)(idx % lay.F);
-    const int64_t ck = idx / lay.F;
-    const int k = (int)(ck % lay.K), c = (int)(ck / lay.K);
-    const int kc = k / kSegBlock, kk = k % kSegBlock;
-    const int64_t plane = (int64_t)lay.Kc * lay.Cp * kSegBlock;
-    const int64_t within = ((int64_t)kc * lay.Cp + c) * kSegBlock + kk;
-    const int64_t base = (int64_t)f * lay.x_elems_per_f;
-    float2 v;
-    if (!tc_mode) {
-      const float *X = reinterpret_cast<const float *>(Xin);
-      v = make_float2(X[base + within], X[base + plane + within]);
-    } else {
-      const __half *X = reinterpret_cast<const __half *>(Xin);
-      const float inv = 1.f / chscale[c];
-      v.x = (__half2float(X[base + 0 * plane + within]) + __half2float(X[base + 2 * plane + within])) * inv;
-      v.y = (__half2float(X[base + 1 * plane + within]) + __half2float(X[base + 3 * plane + within])) * inv;
-    }
-    out[idx] = v;
-  }
-}
 
 // ------------------------------------------------------------------------------------------
 // a2+a3, Eq. (1a) on the FP32 pipe.  grid = (upper-triangular 64x64 channel tiles, F).
@@ -422,72 +197,6 @@ pair_epilogue_kernel(const float2 *__restrict__ S, const float *__restrict__ Sau
 
 // ------------------------------------------------------------------------------------------
 // launchers
-template <typename Kern>
-static int opt_in_smem(Kern kern, size_t bytes) {
-  if (bytes > 48 * 1024) {
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
-    if (e != cudaSuccess) { set_cuda_error(e); return DELTA_ERR_CUDA; }
-  }
-  return DELTA_OK;
-}
-
-int launch_offsets(delta_plan *p, const void *d_x, int64_t ld, int n_first, cudaStream_t st) {
-  offsets_kernel<<<p->lay.C, kThreads, 0, st>>>(d_x, ld, p->cfg.in_dtype, n_first, p->d_offs(), p->d_isum());
-  p->launches++;
-  DELTA_CUDA_CHECK(cudaGetLastError());
-  return DELTA_OK;
-}
-
-template <int L>
-static int launch_stft_L(delta_plan *p, const void *d_x, int64_t ld, void *d_X, cudaStream_t st) {
-  using Cfg = FftCfg<L>;
-  const Layout &lay = p->lay;
-  const int tc = p->contraction == DELTA_CONTRACT_TC;
-  if (tc) {
-    chscale_kernel<<<lay.C, kThreads, 0, st>>>(d_x, ld, p->cfg.in_dtype, p->cfg.norm_mode, p->n_first, p->d_offs(),
-                                               p->d_isum(), lay.T, lay.L, p->d_chscale());
-    p->launches++;
-    DELTA_CUDA_CHECK(cudaGetLastError());
-  }
-  const size_t smem = (size_t)2 * Cfg::CONC * Cfg::N * sizeof(float2) + (size_t)2 * kSegBlock * Cfg::FS * sizeof(float);
-  int rc = opt_in_smem(stft_kernel<L>, smem);
-  if (rc) return rc;
-  dim3 grid(lay.Kc, lay.C);
-  stft_kernel<L><<<grid, kThreads, smem, st>>>(d_x, ld, p->cfg.in_dtype, p->cfg.norm_mode, p->n_first, p->d_offs(),
-                                               p->d_isum(), p->d_tw(), p->d_win(), lay, d_X, tc, p->d_chscale());
-  p->launches++;
-  DELTA_CUDA_CHECK(cudaGetLastError());
-  return DELTA_OK;
-}
-
-#define DELTA_SWITCH_L(L_, CALL)                      \
-  switch (L_) {                                       \
-    case 64: return CALL(64);                         \
-    case 128: return CALL(128);                       \
-    case 256: return CALL(256);                       \
-    case 512: return CALL(512);                       \
-    case 1024: return CALL(1024);                     \
-    case 2048: return CALL(2048);                     \
-    case 4096: return CALL(4096);                     \
-    default: return DELTA_ERR_UNSUPPORTED;            \
-  }
-
-int launch_stft(delta_plan *p, const void *d_x, int64_t ld, void *d_X, cudaStream_t st) {
-#define CALL(LL) launch_stft_L<LL>(p, d_x, ld, d_X, st)
-  DELTA_SWITCH_L(p->lay.L, CALL)
-#undef CALL
-}
-
-int launch_stft_unpack(delta_plan *p, const void *d_X, float *d_out, cudaStream_t st) {
-  const int64_t total = (int64_t)p->lay.C * p->lay.K * p->lay.F;
-  const int blocks = (int)((total + kThreads - 1) / kThreads < 148 * 16 ? (total + kThreads - 1) / kThreads : 148 * 16);
-  stft_unpack_kernel<<<blocks, kThreads, 0, st>>>(d_X, p->lay, p->contraction == DELTA_CONTRACT_TC, p->d_chscale(),
-                                                  reinterpret_cast<float2 *>(d_out));
-  p->launches++;
-  DELTA_CUDA_CHECK(cudaGetLastError());
-  return DELTA_OK;
-}
-
 int launch_contract_fp32(delta_plan *p, const void *d_X, float *d_S, float *d_auto, cudaStream_t st) {
   const Layout &lay = p->lay;
   const int nb = (lay.C + kPairTile - 1) / kPairTile;

@@ -1,0 +1,351 @@
+// a0 + a1 of the hot path:
+//   offsets_kernel   a0  per-shot channel offsets o_c = mean of the first n_first samples   (R1)
+//   chscale_kernel       per-channel power-of-two scale of the split-fp16 operands (tensor-core mode)
+//   stft_kernel      a0+a1  normalise + periodic Hann + L-point real FFT of every segment
+//   stft_unpack_kernel   test accessor: X layout -> complex64 [C][K][F]
+//
+// The real transform of a segment is an N = L/2 point complex FFT of z[n] = x[2n] + i x[2n+1] held in
+// registers (fft_reg.cuh) followed by the split step; the split is fused into the transposed write-out.
+#include <cuda_fp16.h>
+
+#include "delta_internal.h"
+#include "fft_reg.cuh"
+
+namespace delta {
+
+// ------------------------------------------------------------------------------------------
+// a0: o_c = mean of the first n_first samples (integer-exact sum for int16)
+__global__ void __launch_bounds__(256) offsets_kernel(const void *__restrict__ x, int64_t ld, int in_dtype, int n_first,
+                                                      double *__restrict__ offs, long long *__restrict__ isum) {
+  const int c = blockIdx.x;
+  __shared__ double red_d[8];
+  __shared__ long long red_i[8];
+  double sd = 0.0;
+  long long si = 0;
+  if (in_dtype == DELTA_I16) {
+    const short *row = reinterpret_cast<const short *>(x) + (int64_t)c * ld;
+    for (int t = threadIdx.x; t < n_first; t += 256) si += row[t];
+  } else {
+    const float *row = reinterpret_cast<const float *>(x) + (int64_t)c * ld;
+    for (int t = threadIdx.x; t < n_first; t += 256) sd += (double)row[t];
+  }
+  for (int o = 16; o > 0; o >>= 1) {
+    sd += __shfl_xor_sync(0xffffffffu, sd, o);
+    si += __shfl_xor_sync(0xffffffffu, si, o);
+  }
+  if ((threadIdx.x & 31) == 0) {
+    red_d[threadIdx.x >> 5] = sd;
+    red_i[threadIdx.x >> 5] = si;
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double td = 0.0;
+    long long ti = 0;
+    for (int w = 0; w < 8; ++w) {
+      td += red_d[w];
+      ti += red_i[w];
+    }
+    if (in_dtype == DELTA_I16) {
+      isum[c] = ti;
+      offs[c] = (double)ti / (double)n_first;
+    } else {
+      isum[c] = 0;
+      offs[c] = td / (double)n_first;
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------
+// Sample access with the offset normalisation of reading R1 fused into the load.
+struct SampleLoader {
+  const void *x;
+  int in_dtype, norm_mode;
+  float o, inv_o;         // float input: offset and 1/offset
+  long long isum;         // int16 input: integer sum over n_first samples
+  float inv_isum, inv_n;  // 1/isum, 1/n_first
+  int n_first;
+
+  __device__ __forceinline__ void init(const void *x_, int in_dtype_, int norm_mode_, int n_first_,
+                                       const double *__restrict__ offs, const long long *__restrict__ isums, int c) {
+    x = x_; in_dtype = in_dtype_; norm_mode = norm_mode_; n_first = n_first_;
+    o = 0.f; inv_o = 0.f; isum = 0; inv_isum = 0.f; inv_n = 0.f;
+    if (norm_mode != DELTA_NORM_NONE) {
+      const double od = offs[c];
+      o = (float)od;
+      inv_o = (float)(1.0 / od);
+      isum = isums[c];
+      inv_isum = (float)(1.0 / (double)isum);
+      inv_n = (float)(1.0 / (double)n_first);
+    }
+  }
+  __device__ __forceinline__ float conv_i16(int v) const {
+    if (norm_mode == DELTA_NORM_NONE) return (float)v;
+    // (x - o) = (x n - sum)/n exactly in integers; one rounding at the conversion
+    const float num = __ll2float_rn((long long)v * n_first - isum);
+    return norm_mode == DELTA_NORM_RELATIVE ? num * inv_isum : num * inv_n;
+  }
+  __device__ __forceinline__ float conv_f32(float v) const {
+    if (norm_mode == DELTA_NORM_NONE) return v;
+    const float d = v - o;
+    return norm_mode == DELTA_NORM_RELATIVE ? d * inv_o : d;
+  }
+  __device__ __forceinline__ float operator()(int64_t idx) const {
+    if (in_dtype == DELTA_I16) return conv_i16(reinterpret_cast<const short *>(x)[idx]);
+    return conv_f32(reinterpret_cast<const float *>(x)[idx]);
+  }
+  // samples idx, idx+1; `pair_ok`: the element pair is naturally aligned (one vector load)
+  __device__ __forceinline__ float2 two(int64_t idx, bool pair_ok) const {
+    if (in_dtype == DELTA_I16) {
+      if (pair_ok) {
+        const short2 v = *reinterpret_cast<const short2 *>(reinterpret_cast<const short *>(x) + idx);
+        return make_float2(conv_i16(v.x), conv_i16(v.y));
+      }
+      const short *p = reinterpret_cast<const short *>(x) + idx;
+      return make_float2(conv_i16(p[0]), conv_i16(p[1]));
+    }
+    if (pair_ok) {
+      const float2 v = *reinterpret_cast<const float2 *>(reinterpret_cast<const float *>(x) + idx);
+      return make_float2(conv_f32(v.x), conv_f32(v.y));
+    }
+    const float *p = reinterpret_cast<const float *>(x) + idx;
+    return make_float2(conv_f32(p[0]), conv_f32(p[1]));
+  }
+};
+
+// per-channel power-of-two scale for the split-fp16 operands: |X| <= (L/2) max|y|  =>  scale * |X| <= 2^14.
+// One CTA of 1024 threads per channel; one pass over the chunk.
+__global__ void __launch_bounds__(1024)
+chscale_kernel(const void *__restrict__ x, int64_t ld, int in_dtype, int norm_mode, int n_first,
+               const double *__restrict__ offs, const long long *__restrict__ isum, int T, int L,
+               float *__restrict__ chscale) {
+  const int c = blockIdx.x;
+  SampleLoader ldr;
+  ldr.init(x, in_dtype, norm_mode, n_first, offs, isum, c);
+  const int64_t row0 = (int64_t)c * ld;
+  const size_t esz = in_dtype == DELTA_I16 ? 2 : 4;
+  const bool pair_ok = ((row0 & 1) == 0) && ((reinterpret_cast<uintptr_t>(x) & (2 * esz - 1)) == 0);
+  float m = 0.f;
+  const int npairs = T >> 1;
+  for (int t = threadIdx.x; t < npairs; t += 1024) {
+    const float2 v = ldr.two(row0 + 2 * t, pair_ok);
+    m = fmaxf(m, fmaxf(fabsf(v.x), fabsf(v.y)));
+  }
+  if ((T & 1) && threadIdx.x == 0) m = fmaxf(m, fabsf(ldr(row0 + T - 1)));
+  for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
+  __shared__ float red[32];
+  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = m;
+  __syncthreads();
+  if (threadIdx.x < 32) {
+    m = red[threadIdx.x];
+    for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
+    if (threadIdx.x == 0) {
+      const float bound = m * (0.5f * (float)L);  // sum_n w[n] |y| <= (L/2) max|y|
+      float sc = 1.f;
+      if (bound > 0.f && isfinite(bound)) {
+        int e;
+        frexpf(bound, &e);         // bound = mant * 2^e, mant in [0.5, 1)  =>  bound < 2^e
+        sc = ldexpf(1.f, 14 - e);  // scale * bound < 2^14
+      }
+      chscale[c] = sc;
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------
+template <int L>
+struct StftCfg {
+  static constexpr int N = L / 2;
+  using G = FftGeom<N>;
+  static constexpr int T = G::T;
+  static constexpr int CH = (N <= 256) ? 4 : (N == 512 ? 2 : 1);  // channels per CTA
+  static constexpr int NFFT = CH * kSegBlock;                      // transforms per CTA
+  static constexpr int THREADS = NFFT * T;
+  static constexpr int CHPAD = CH > 1 ? 16 / CH : 0;                 // float2 skew between channels (bank spread)
+  static constexpr int SMEM_F2 = NFFT * G::BUF + CH * CHPAD;
+};
+
+// Real forward transform, split step: Z = FFT_N(z), z[n] = x[2n] + i x[2n+1]  ->
+//   X[f] = (Z[f] + conj Z[N-f])/2 - (i/2) e^{-2 pi i f/L} (Z[f] - conj Z[N-f]),  f = 0..N, Z[N] = Z[0].
+__device__ __forceinline__ float2 rfft_split(float2 zf, float2 zr, float2 w) {
+  const float2 e = make_float2(0.5f * (zf.x + zr.x), 0.5f * (zf.y - zr.y));  // (Z[f] + conj Zr)/2
+  const float2 d = make_float2(0.5f * (zf.x - zr.x), 0.5f * (zf.y + zr.y));  // (Z[f] - conj Zr)/2
+  const float2 wd = cmul(w, d);
+  return make_float2(e.x + wd.y, e.y - wd.x);  // e - i * (w d)
+}
+
+// grid = (ceil(K/8), ceil(C/CH)).  Phase 1: one group of T threads per (channel, segment) transform.
+// Phase 2: one thread per (channel, bin) gathers the 8 segments of the CTA and writes one 16-byte
+// (fp16) or 32-byte (fp32) piece per operand plane of the frequency-major X layout.
+template <int L, bool TC>
+__global__ void __launch_bounds__(StftCfg<L>::THREADS)
+stft_kernel(const void *__restrict__ x, int64_t ld, int in_dtype, int norm_mode, int n_first,
+            const double *__restrict__ offs, const long long *__restrict__ isum, const float2 *__restrict__ tw,
+            const float *__restrict__ win, const float2 *__restrict__ ftab, Layout lay, void *__restrict__ Xout,
+            const float *__restrict__ chscale) {
+  using Cfg = StftCfg<L>;
+  using G = typename Cfg::G;
+  constexpr int N = Cfg::N, T = Cfg::T, E = G::E, CH = Cfg::CH;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  float2 *zb = reinterpret_cast<float2 *>(smem_raw);
+
+  const int tid = threadIdx.x, g = tid / T, gt = tid % T;
+  const int cl = g / kSegBlock, kk = g % kSegBlock;
+  const int kb = blockIdx.x, c0 = blockIdx.y * CH;
+  float2 *buf = zb + g * G::BUF + cl * Cfg::CHPAD;
+
+  {
+    const int c = c0 + cl, k = kb * kSegBlock + kk;
+    float2 v[E];
+    if (c < lay.C && k < lay.K) {
+      SampleLoader ldr;
+      ldr.init(x, in_dtype, norm_mode, n_first, offs, isum, c);
+      const int64_t t0 = (int64_t)c * ld + (int64_t)k * lay.H;
+      const size_t esz = in_dtype == DELTA_I16 ? 2 : 4;
+      const bool pair_ok = ((t0 & 1) == 0) && ((reinterpret_cast<uintptr_t>(x) & (2 * esz - 1)) == 0);
+#pragma unroll
+      for (int u = 0; u < E; ++u) {
+        const int n = gt + T * u;
+        const float2 s = ldr.two(t0 + 2 * n, pair_ok);
+        const float2 w = __ldg(reinterpret_cast<const float2 *>(win) + n);
+        v[u] = make_float2(s.x * w.x, s.y * w.y);
+      }
+    } else {
+#pragma unroll
+      for (int u = 0; u < E; ++u) v[u] = make_float2(0.f, 0.f);
+    }
+    fft_inplace<N, false>(v, buf, ftab, gt);
+    fft_group_sync<T>();  // every read-back of the group is done before Z overwrites the buffer
+#pragma unroll
+    for (int u = 0; u < E; ++u) buf[fft_pad(gt + T * u)] = v[u];
+  }
+  __syncthreads();
+
+  constexpr int F = N + 1;
+  const int64_t plane = (int64_t)lay.Kc * lay.Cp * kSegBlock;  // one [kc][c][8] block
+  for (int idx = tid; idx < CH * F; idx += Cfg::THREADS) {
+    const int pcl = idx % CH, f = idx / CH;
+    const int c = c0 + pcl;
+    if (c >= lay.C) continue;
+    const float2 w = __ldg(tw + f);  // e^{-2 pi i f/L}
+    const float2 *zc = zb + pcl * (kSegBlock * G::BUF + Cfg::CHPAD);
+    const int i_f = fft_pad(f & (N - 1)), i_r = fft_pad((N - f) & (N - 1));
+    float re[kSegBlock], im[kSegBlock];
+#pragma unroll
+    for (int s = 0; s < kSegBlock; ++s) {
+      const float2 X = rfft_split(zc[s * G::BUF + i_f], zc[s * G::BUF + i_r], w);
+      re[s] = X.x;
+      im[s] = X.y;
+    }
+    const int64_t within = ((int64_t)kb * lay.Cp + c) * kSegBlock;
+    const int64_t base = (int64_t)f * lay.x_elems_per_f + within;
+    if (TC) {
+      // split fp16: v * scale = hi + lo (scale = power of two chosen by chscale_kernel)
+      __half *X = reinterpret_cast<__half *>(Xout);
+      const float sc = chscale[c];
+      __align__(16) __half2 hr[4], hi_[4], lr[4], li[4];
+#pragma unroll
+      for (int q = 0; q < 4; ++q) {
+        const float r0 = re[2 * q] * sc, r1 = re[2 * q + 1] * sc, i0 = im[2 * q] * sc, i1 = im[2 * q + 1] * sc;
+        hr[q] = __floats2half2_rn(r0, r1);
+        hi_[q] = __floats2half2_rn(i0, i1);
+        const float2 hrf = __half22float2(hr[q]), hif = __half22float2(hi_[q]);
+        lr[q] = __floats2half2_rn(r0 - hrf.x, r1 - hrf.y);
+        li[q] = __floats2half2_rn(i0 - hif.x, i1 - hif.y);
+      }
+      *reinterpret_cast<uint4 *>(X + base + 0 * plane) = *reinterpret_cast<const uint4 *>(hr);
+      *reinterpret_cast<uint4 *>(X + base + 1 * plane) = *reinterpret_cast<const uint4 *>(hi_);
+      *reinterpret_cast<uint4 *>(X + base + 2 * plane) = *reinterpret_cast<const uint4 *>(lr);
+      *reinterpret_cast<uint4 *>(X + base + 3 * plane) = *reinterpret_cast<const uint4 *>(li);
+    } else {
+      float *X = reinterpret_cast<float *>(Xout);
+      *reinterpret_cast<float4 *>(X + base) = make_float4(re[0], re[1], re[2], re[3]);
+      *reinterpret_cast<float4 *>(X + base + 4) = make_float4(re[4], re[5], re[6], re[7]);
+      *reinterpret_cast<float4 *>(X + base + plane) = make_float4(im[0], im[1], im[2], im[3]);
+      *reinterpret_cast<float4 *>(X + base + plane + 4) = make_float4(im[4], im[5], im[6], im[7]);
+    }
+  }
+}
+
+// test accessor: X layout -> complex64 [C][K][F]
+__global__ void __launch_bounds__(256)
+stft_unpack_kernel(const void *__restrict__ Xin, Layout lay, int tc_mode, const float *__restrict__ chscale,
+                   float2 *__restrict__ out) {
+  const int64_t total = (int64_t)lay.C * lay.K * lay.F;
+  for (int64_t idx = (int64_t)blockIdx.x * 256 + threadIdx.x; idx < total; idx += (int64_t)gridDim.x * 256) {
+    const int f = (int)(idx % lay.F);
+    const int64_t ck = idx / lay.F;
+    const int k = (int)(ck % lay.K), c = (int)(ck / lay.K);
+    const int kc = k / kSegBlock, kk = k % kSegBlock;
+    const int64_t plane = (int64_t)lay.Kc * lay.Cp * kSegBlock;
+    const int64_t within = ((int64_t)kc * lay.Cp + c) * kSegBlock + kk;
+    const int64_t base = (int64_t)f * lay.x_elems_per_f;
+    float2 v;
+    if (!tc_mode) {
+      const float *X = reinterpret_cast<const float *>(Xin);
+      v = make_float2(X[base + within], X[base + plane + within]);
+    } else {
+      const __half *X = reinterpret_cast<const __half *>(Xin);
+      const float inv = 1.f / chscale[c];
+      v.x = (__half2float(X[base + 0 * plane + within]) + __half2float(X[base + 2 * plane + within])) * inv;
+      v.y = (__half2float(X[base + 1 * plane + within]) + __half2float(X[base + 3 * plane + within])) * inv;
+    }
+    out[idx] = v;
+  }
+}
+
+// ------------------------------------------------------------------------------------------
+// launchers
+int launch_offsets(delta_plan *p, const void *d_x, int64_t ld, int n_first, cudaStream_t st) {
+  offsets_kernel<<<p->lay.C, 256, 0, st>>>(d_x, ld, p->cfg.in_dtype, n_first, p->d_offs(), p->d_isum());
+  p->launches++;
+  DELTA_CUDA_CHECK(cudaGetLastError());
+  return DELTA_OK;
+}
+
+template <int L, bool TC>
+static int launch_stft_LT(delta_plan *p, const void *d_x, int64_t ld, void *d_X, cudaStream_t st) {
+  using Cfg = StftCfg<L>;
+  const Layout &lay = p->lay;
+  const size_t smem = (size_t)Cfg::SMEM_F2 * sizeof(float2);
+  int rc = opt_in_smem(stft_kernel<L, TC>, smem);
+  if (rc) return rc;
+  dim3 grid((lay.K + kSegBlock - 1) / kSegBlock, (lay.C + Cfg::CH - 1) / Cfg::CH);
+  stft_kernel<L, TC><<<grid, Cfg::THREADS, smem, st>>>(d_x, ld, p->cfg.in_dtype, p->cfg.norm_mode, p->n_first, p->d_offs(),
+                                                       p->d_isum(), p->d_tw(), p->d_win(), p->d_ftab(), lay, d_X,
+                                                       p->d_chscale());
+  p->launches++;
+  DELTA_CUDA_CHECK(cudaGetLastError());
+  return DELTA_OK;
+}
+
+template <int L>
+static int launch_stft_L(delta_plan *p, const void *d_x, int64_t ld, void *d_X, cudaStream_t st) {
+  const Layout &lay = p->lay;
+  if (p->contraction == DELTA_CONTRACT_TC) {
+    chscale_kernel<<<lay.C, 1024, 0, st>>>(d_x, ld, p->cfg.in_dtype, p->cfg.norm_mode, p->n_first, p->d_offs(), p->d_isum(),
+                                           lay.T, lay.L, p->d_chscale());
+    p->launches++;
+    DELTA_CUDA_CHECK(cudaGetLastError());
+    return launch_stft_LT<L, true>(p, d_x, ld, d_X, st);
+  }
+  return launch_stft_LT<L, false>(p, d_x, ld, d_X, st);
+}
+
+int launch_stft(delta_plan *p, const void *d_x, int64_t ld, void *d_X, cudaStream_t st) {
+#define CALL(LL) launch_stft_L<LL>(p, d_x, ld, d_X, st)
+  DELTA_SWITCH_L(p->lay.L, CALL)
+#undef CALL
+}
+
+int launch_stft_unpack(delta_plan *p, const void *d_X, float *d_out, cudaStream_t st) {
+  const int64_t total = (int64_t)p->lay.C * p->lay.K * p->lay.F;
+  const int64_t want = (total + 255) / 256;
+  const int blocks = (int)(want < 148 * 16 ? want : 148 * 16);
+  stft_unpack_kernel<<<blocks, 256, 0, st>>>(d_X, p->lay, p->contraction == DELTA_CONTRACT_TC, p->d_chscale(),
+                                             reinterpret_cast<float2 *>(d_out));
+  p->launches++;
+  DELTA_CUDA_CHECK(cudaGetLastError());
+  return DELTA_OK;
+}
+
+}  // namespace delta
