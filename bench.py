@@ -279,7 +279,7 @@ def run_ours(args):
         {"kernel": "contract_tc_kernel" if tc else "contract_fp32_kernel", "ms": float(stage_mean[1]),
          "bound": "tensor" if tc else "alu", "alg_flops": flops_contract,
          "achieved": flops_contract / (stage_mean[1] * 1e-3) / 1e12, "unit": "TFLOP/s"},
-        {"kernel": "pair_epilogue_kernel", "ms": float(stage_mean[2]), "bound": "hbm",
+        {"kernel": "pair_kernel", "ms": float(stage_mean[2]), "bound": "hbm",
          "alg_bytes": ab["gap"] + ab["rho"], "achieved": (ab["gap"] + ab["rho"]) / (stage_mean[2] * 1e-3) / 1e9,
          "unit": "GB/s"},
     ]

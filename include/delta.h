@@ -89,8 +89,8 @@ typedef struct {
   int64_t n_pairs;         /* P */
   int64_t workspace_bytes; /* minimum size for delta_plan_set_workspace() */
   int64_t x_bytes;         /* size of a d_X buffer  (delta_stft output, opaque layout) */
-  int64_t s_bytes;         /* size of a d_S buffer  = F * P_pad * 8, complex64 [F][P_pad] */
-  int64_t s_row_stride;    /* P_pad: complex64 elements between consecutive frequencies of d_S */
+  int64_t s_bytes;         /* size of a d_S buffer (delta_cross_spectra output, opaque layout) */
+  int64_t s_block_pairs;   /* pairs per block of the d_S layout (see delta_cross_spectra) */
 } delta_sizes;
 
 typedef struct delta_plan delta_plan; /* opaque; owned by the library */
@@ -120,11 +120,13 @@ int delta_stft(delta_plan *plan, const void *d_x, int64_t ld, void *d_X, void *s
  * definition above. */
 int delta_stft_unpack(delta_plan *plan, const void *d_X, float *d_out, void *stream);
 
-/* a2 + a3, Eq. (1a).  d_S: complex64 [F][P_pad] (frequency-major: for each bin the strict upper
- * triangle of the cross-spectral matrix packed column by column, S_ij (i < j) at column
- * j(j-1)/2 + i, row stride s_row_stride); d_Sauto: float [C][F] autospectra S_cc[f].
- * Either may be NULL.  (The per-pair outputs below are in lexicographic pair order.) */
+/* a2 + a3, Eq. (1a).  d_S: s_bytes of complex64 in the library's pair-block layout
+ * [ceil(P/B)][F][B], B = s_block_pairs: lexicographic pair p is in block p / B, and inside row f of
+ * the block in slot (p ^ f) mod B (use delta_cross_spectra_unpack to read it); d_Sauto: float [C][F]
+ * autospectra S_cc[f].  Either may be NULL. */
 int delta_cross_spectra(delta_plan *plan, const void *d_X, float *d_S, float *d_Sauto, void *stream);
+/* Test accessor: expands d_S to complex64 [P][F] (interleaved re, im), pairs lexicographic. */
+int delta_cross_spectra_unpack(delta_plan *plan, const float *d_S, float *d_out, void *stream);
 
 /* a4, Eq. (1b): d_G float [P][F].  0 where S_ii S_jj = 0 (R16). */
 int delta_coherence(delta_plan *plan, const float *d_S, const float *d_Sauto, float *d_G, void *stream);
@@ -162,6 +164,10 @@ int delta_analyze_shot_host(delta_plan *plan, const void *h_x, int32_t n_chunks,
  * stage, events[1] after it, events[2] after the contraction and events[3] after the pair stage, on
  * the launching stream (so the caller can time each stage with cudaEventElapsedTime). */
 int delta_plan_set_stage_events(delta_plan *plan, void *const *events);
+
+/* Debug hook.  d_trace: device buffer of 3*512 int64 (or NULL to switch off).  While set, CTA 0 of the
+ * tensor-core contraction writes SM clock stamps of its producer / MMA / epilogue roles into it. */
+int delta_debug_set_trace(delta_plan *plan, void *d_trace);
 
 /* Number of kernels the last delta_analyze_chunk() on this plan launched (for bench accounting). */
 int delta_last_launch_count(const delta_plan *plan);

@@ -33,11 +33,12 @@ class DeltaConfig(C.Structure):
 class DeltaSizes(C.Structure):
     _fields_ = [("n_segments", C.c_int32), ("n_bins", C.c_int32), ("n_lags", C.c_int32), ("contraction", C.c_int32),
                 ("n_pairs", C.c_int64), ("workspace_bytes", C.c_int64), ("x_bytes", C.c_int64),
-                ("s_bytes", C.c_int64), ("s_row_stride", C.c_int64)]
+                ("s_bytes", C.c_int64), ("s_block_pairs", C.c_int64)]
 
 
 EXPORTS = ["delta_plan_create", "delta_plan_destroy", "delta_plan_sizes", "delta_plan_set_workspace",
            "delta_set_offsets", "delta_get_offsets", "delta_stft", "delta_stft_unpack", "delta_cross_spectra",
+           "delta_cross_spectra_unpack", "delta_debug_set_trace",
            "delta_coherence", "delta_crossphase", "delta_crosspower", "delta_crosscorr", "delta_analyze_chunk",
            "delta_analyze_shot_host", "delta_plan_set_stage_events", "delta_last_launch_count", "delta_strerror", "delta_last_cuda_error",
            "delta_version"]
@@ -58,6 +59,8 @@ def _load() -> C.CDLL:
     lib.delta_stft.argtypes = [vp, vp, i64, vp, vp]
     lib.delta_stft_unpack.argtypes = [vp, vp, vp, vp]
     lib.delta_cross_spectra.argtypes = [vp, vp, vp, vp, vp]
+    lib.delta_cross_spectra_unpack.argtypes = [vp, vp, vp, vp]
+    lib.delta_debug_set_trace.argtypes = [vp, vp]
     lib.delta_coherence.argtypes = [vp, vp, vp, vp, vp]
     lib.delta_crossphase.argtypes = [vp, vp, vp, vp]
     lib.delta_crosspower.argtypes = [vp, vp, vp, vp]
@@ -110,7 +113,7 @@ class Sizes:
     workspace_bytes: int
     x_bytes: int
     s_bytes: int
-    s_row_stride: int
+    s_block_pairs: int
 
 
 class Plan:
@@ -126,7 +129,7 @@ class Plan:
         sz = DeltaSizes()
         _check(LIB.delta_plan_sizes(self._h, C.byref(sz)), "delta_plan_sizes")
         self.sizes = Sizes(sz.n_segments, sz.n_bins, sz.n_lags, sz.contraction, sz.n_pairs, sz.workspace_bytes,
-                           sz.x_bytes, sz.s_bytes, sz.s_row_stride)
+                           sz.x_bytes, sz.s_bytes, sz.s_block_pairs)
         self.C, self.T = n_channels, n_samples
         self.workspace = None
         if allocate:
@@ -148,7 +151,7 @@ class Plan:
         return torch.empty(self.sizes.x_bytes, dtype=torch.uint8, device=self.device)
 
     def empty_S(self):
-        return torch.empty((self.sizes.F, self.sizes.s_row_stride, 2), dtype=torch.float32, device=self.device)
+        return torch.empty(self.sizes.s_bytes // 4, dtype=torch.float32, device=self.device)
 
     def empty_outputs(self, G=True, A=True, P=True, R=True, Sauto=True):
         s = self.sizes
@@ -183,6 +186,15 @@ class Plan:
         _check(LIB.delta_cross_spectra(self._h, X.data_ptr(), S.data_ptr(), Sauto.data_ptr(), _stream()),
                "delta_cross_spectra")
         return S, Sauto
+
+    def cross_spectra_unpack(self, S):
+        out = torch.empty((self.sizes.P, self.sizes.F, 2), dtype=torch.float32, device=self.device)
+        _check(LIB.delta_cross_spectra_unpack(self._h, S.data_ptr(), out.data_ptr(), _stream()),
+               "delta_cross_spectra_unpack")
+        return torch.view_as_complex(out)
+
+    def set_trace(self, buf):
+        _check(LIB.delta_debug_set_trace(self._h, None if buf is None else buf.data_ptr()), "delta_debug_set_trace")
 
     def coherence(self, S, Sauto, G=None):
         G = torch.empty((self.sizes.P, self.sizes.F), dtype=torch.float32, device=self.device) if G is None else G

@@ -77,7 +77,9 @@ int delta_plan_create(const delta_config *cfg, delta_plan **out) {
   l.M = cfg->max_lag;
   l.nlags = 2 * l.M + 1;
   l.P = (int64_t)l.C * (l.C - 1) / 2;
-  l.Ppad = (int64_t)align_up((size_t)(l.P > 0 ? l.P : 1), 32);
+  l.PB = pair_block(l.L);
+  l.pb_shift = l.PB == 16 ? 4 : (l.PB == 8 ? 3 : 2);
+  l.Pblk = (l.P + l.PB - 1) / l.PB;
   // floats (2 parts) or halves (2 precisions x 2 parts) per frequency
   l.x_elems_per_f = (int64_t)(p->contraction == DELTA_CONTRACT_TC ? 4 : 2) * l.Kc * l.Cp * kSegBlock;
 
@@ -103,8 +105,8 @@ int delta_plan_create(const delta_config *cfg, delta_plan **out) {
     default: p->s2 = (float)(1.0 / (sw * sw)); break;
   }
   p->h_pairs.reserve((size_t)l.P);
-  for (int j = 1; j < l.C; ++j)
-    for (int i = 0; i < j; ++i) p->h_pairs.push_back(make_ushort2((unsigned short)i, (unsigned short)j));
+  for (int i = 0; i < l.C; ++i)
+    for (int j = i + 1; j < l.C; ++j) p->h_pairs.push_back(make_ushort2((unsigned short)i, (unsigned short)j));
   memset(&p->tc, 0, sizeof(p->tc));
   if (p->contraction == DELTA_CONTRACT_TC && !tc_plan_tiles(l.Cp, &p->tc)) { delete p; return DELTA_ERR_UNSUPPORTED; }
 
@@ -119,8 +121,9 @@ int delta_plan_create(const delta_config *cfg, delta_plan **out) {
   w.off_isum = take((size_t)l.C * sizeof(long long));
   w.off_chscale = take((size_t)l.C * sizeof(float));
   w.off_X = take((size_t)l.F * l.x_elems_per_f * (p->contraction == DELTA_CONTRACT_TC ? 2 : 4));
-  w.off_S = take((size_t)l.F * l.Ppad * sizeof(float2));
+  w.off_S = take((size_t)(l.Pblk > 0 ? l.Pblk : 1) * l.F * l.PB * sizeof(float2));
   w.off_auto = take((size_t)l.C * l.F * sizeof(float));
+  w.off_rsq = take((size_t)l.C * l.F * sizeof(float));
   w.total = o;
   *out = p;
   return DELTA_OK;
@@ -148,8 +151,8 @@ int delta_plan_sizes(const delta_plan *p, delta_sizes *out) {
   out->n_pairs = l.P;
   out->workspace_bytes = (int64_t)p->wsl.total;
   out->x_bytes = (int64_t)l.F * l.x_elems_per_f * (p->contraction == DELTA_CONTRACT_TC ? 2 : 4);
-  out->s_bytes = (int64_t)l.F * l.Ppad * (int64_t)sizeof(float2);
-  out->s_row_stride = l.Ppad;
+  out->s_bytes = (int64_t)(l.Pblk > 0 ? l.Pblk : 1) * l.F * l.PB * (int64_t)sizeof(float2);
+  out->s_block_pairs = l.PB;
   return DELTA_OK;
 }
 
@@ -224,6 +227,19 @@ int delta_stft(delta_plan *p, const void *d_x, int64_t ld, void *d_X, void *stre
   return launch_stft(p, d_x, ld, d_X, st);
 }
 
+int delta_cross_spectra_unpack(delta_plan *p, const float *d_S, float *d_out, void *stream) {
+  int rc = need_ws(p);
+  if (rc) return rc;
+  if (!d_S || !d_out) return DELTA_ERR_INVALID_ARG;
+  return launch_s_unpack(p, d_S, d_out, reinterpret_cast<cudaStream_t>(stream));
+}
+
+int delta_debug_set_trace(delta_plan *p, void *d_trace) {
+  if (!p) return DELTA_ERR_INVALID_ARG;
+  p->d_trace = reinterpret_cast<long long *>(d_trace);
+  return DELTA_OK;
+}
+
 int delta_stft_unpack(delta_plan *p, const void *d_X, float *d_out, void *stream) {
   int rc = need_ws(p);
   if (rc) return rc;
@@ -232,8 +248,8 @@ int delta_stft_unpack(delta_plan *p, const void *d_X, float *d_out, void *stream
 }
 
 static int contract(delta_plan *p, const void *d_X, float *d_S, float *d_auto, cudaStream_t st) {
-  return p->contraction == DELTA_CONTRACT_TC ? launch_contract_tc(p, d_X, d_S, d_auto, st)
-                                             : launch_contract_fp32(p, d_X, d_S, d_auto, st);
+  return p->contraction == DELTA_CONTRACT_TC ? launch_contract_tc(p, d_X, d_S, d_auto, p->d_rsq(), st)
+                                             : launch_contract_fp32(p, d_X, d_S, d_auto, p->d_rsq(), st);
 }
 
 int delta_cross_spectra(delta_plan *p, const void *d_X, float *d_S, float *d_Sauto, void *stream) {
@@ -252,9 +268,12 @@ static int pair_stage(delta_plan *p, const float *d_S, const float *d_Sauto, flo
   if (!d_S || (need_auto && !d_Sauto)) return DELTA_ERR_INVALID_ARG;
   if (!G && !A && !P && !R) return DELTA_ERR_INVALID_ARG;
   if (!aligned16(d_S)) return DELTA_ERR_ALIGNMENT;
-  // the kernel always reads the autospectra (for the r0 sums); without them use the workspace copy
-  const float *au = d_Sauto ? d_Sauto : p->d_auto();
-  return launch_pair_epilogue(p, d_S, au, G, A, P, R, reinterpret_cast<cudaStream_t>(stream));
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+  if (need_auto) {  // coherence and rho need 1/sqrt(S_cc[f]) of the caller's autospectra
+    rc = launch_auto_prep(p, d_Sauto, p->d_rsq(), st);
+    if (rc) return rc;
+  }
+  return launch_pair(p, d_S, d_Sauto, p->d_rsq(), G, A, P, R, st);
 }
 
 int delta_coherence(delta_plan *p, const float *d_S, const float *d_Sauto, float *d_G, void *stream) {
@@ -292,7 +311,7 @@ int delta_analyze_chunk(delta_plan *p, const void *d_x, int64_t ld, float *d_G, 
   rc = contract(p, p->d_X(), pairs_wanted ? p->d_S() : nullptr, au, st);
   if (rc) return rc;
   if (ev) DELTA_CUDA_CHECK(cudaEventRecord(p->stage_ev[2], st));
-  if (pairs_wanted) rc = launch_pair_epilogue(p, p->d_S(), au, d_G, d_A, d_P, d_R, st);
+  if (pairs_wanted) rc = launch_pair(p, p->d_S(), au, p->d_rsq(), d_G, d_A, d_P, d_R, st);
   if (rc) return rc;
   if (ev) DELTA_CUDA_CHECK(cudaEventRecord(p->stage_ev[3], st));
   return rc;

@@ -1,10 +1,10 @@
 // a2+a3 on the 5th-generation tensor cores: Eq. (1a), as a batched Hermitian rank-K
 // contraction  S_f = s^2/K * X_f X_f^H  with tcgen05.mma (kind::f16) and TMEM accumulators.
 //
-//   X_f = A + iB (C x K, A = Re, B = Im).   Re S = A A^T + B B^T,   Im S = B A^T - A B^T.
+//   X_f = A + iB (C x K, A = Re, B = Im).   Re S = A A^T + B B^T,   Im S_ij = B_i A_j - A_i B_j.
 //   Operands are split fp16:  x * s_c = hi + lo  (s_c a per-channel power of two, |x s_c| <= 2^14), and every
 //   real product is formed as hi*hi + hi*lo + lo*hi (the dropped lo*lo term is 2^-22 relative): 3 MMAs.
-//   The -A B^T term uses the negate-A bit of the instruction descriptor, so one copy of the operands in
+//   The subtracted term uses the negate-A bit of the instruction descriptor, so one copy of the operands in
 //   shared memory serves all twelve MMAs of a K=16 step.
 //
 // Operand layout (written by stft_kernel, see delta_internal.h): half X[f][plane][kc][Cp][8], plane = hi_re,
@@ -14,8 +14,15 @@
 // cp.async.bulk copies (no tensor map) and any 8-aligned row range is addressed by moving the descriptor's
 // start address.
 //
+// Accumulator tiles ("units"): TMEM lanes = channel j (128 rows of the A operand), TMEM columns = channel i
+// (N <= 128 rows of the B operand), Re in columns [tm, tm+N), Im in [tm+N, tm+2N).  Only i < j is kept, so the
+// units cover the lower triangle; a lane (fixed j) then walks consecutive lexicographic pairs when the
+// epilogue fixes i and lets the 32 lanes of a warp store: S leaves the SM in 256-byte runs.
+//
 // Roles (one CTA per SM, persistent over (bin, group) items): warp 8 lane 0 = bulk-copy producer,
-// warp 9 lane 0 = MMA issuer, warps 0-7 = epilogue (TMEM -> registers -> scale -> coalesced S stores).
+// warp 9 lane 0 = MMA issuer, warps 0-7 = epilogue (TMEM -> registers -> scale -> S stores).  Every unit has
+// its own TMEM region and full/empty mbarrier pair, so the epilogue of unit u overlaps the MMAs of the
+// following units (and, when all K steps of a bin fit in the operand ring, of the next bin: "unit-major").
 #include <cuda_fp16.h>
 
 #include "delta_internal.h"
@@ -86,37 +93,45 @@ __device__ __forceinline__ void tmem_ld16(uint32_t taddr, float *v) {
 #pragma unroll
   for (int q = 0; q < 16; ++q) v[q] = __uint_as_float(r[q]);
 }
+__device__ __forceinline__ void fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 
 }  // namespace
 
-struct TcTile {
-  int row0;     // first channel of the 128-row A operand (multiple of 64)
-  int col0;     // first channel of the N-row B operand
-  int N;        // multiple of 16, <= 256
-  int lane_lo;  // rows below row0 + lane_lo are owned by another tile (0 or 64)
-  int tm_re, tm_im;  // TMEM column offsets of the two accumulators
+struct TcUnit {
+  int row0;              // first channel of the 128-row A operand = channel of TMEM lane 0 (multiple of 8)
+  int lane_lo, lane_hi;  // lanes [lane_lo, lane_hi) are owned by this unit (multiples of 32)
+  int col0, N;           // B operand rows = channels [col0, col0 + N), N in {32, 64, 96, 128}
+  int tm;                // TMEM column of Re; Im follows at tm + N
 };
 struct TcParams {
   int ngroups;
-  int ntiles[kTcMaxGroups];
-  TcTile tiles[kTcMaxGroups][kTcMaxTiles];
-  int nstage, ksteps;
+  int nunits[kTcMaxGroups];
+  TcUnit units[kTcMaxGroups][kTcMaxUnits];
+  int nstage, ksteps, unit_major;
   uint32_t stage_bytes, plane_bytes;  // per stage: 4 planes of 2*Cp*16 bytes
   int64_t plane_elems;                // halves between planes in global memory: Kc*Cp*8
   int64_t kstep_elems;                // halves per K=16 step inside a plane: 2*Cp*8
 };
 
+// trace[role * 512 + n] = clock64 stamps of CTA 0 (role 0 producer, 1 MMA issuer, 2 epilogue warp 0)
+#define TC_TRACE(role, slot)                                                        \
+  do {                                                                              \
+    if (TRACE && blockIdx.x == 0 && (slot) < 512) trace[(role) * 512 + (slot)] = clock64(); \
+  } while (0)
+
+template <bool TRACE>
 __global__ void __launch_bounds__(kTcThreads, 1)
 contract_tc_kernel(const __half *__restrict__ X, Layout lay, TcParams prm, float scale, const float *__restrict__ chscale,
-                   float2 *__restrict__ S, float *__restrict__ Sauto) {
+                   float2 *__restrict__ S, float *__restrict__ Sauto, float *__restrict__ Srsq, long long *trace) {
   extern __shared__ __align__(1024) unsigned char smem_raw[];
   unsigned char *stages = smem_raw;
   float *inv_scale = reinterpret_cast<float *>(stages + (size_t)prm.nstage * prm.stage_bytes);  // [Cp]
   uint64_t *full_bar = reinterpret_cast<uint64_t *>(inv_scale + lay.Cp);
   uint64_t *empty_bar = full_bar + prm.nstage;
-  uint64_t *tmem_full = empty_bar + prm.nstage;
-  uint64_t *tmem_empty = tmem_full + 1;
-  uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(tmem_empty + 1);
+  uint64_t *tfull = empty_bar + prm.nstage;  // [kTcMaxUnits]
+  uint64_t *tempty = tfull + kTcMaxUnits;    // [kTcMaxUnits]
+  uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(tempty + kTcMaxUnits);
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int nitems = lay.F * prm.ngroups;
@@ -127,29 +142,31 @@ contract_tc_kernel(const __half *__restrict__ X, Layout lay, TcParams prm, float
       mbar_init(full_bar + s, 1);
       mbar_init(empty_bar + s, 1);
     }
-    mbar_init(tmem_full, 1);
-    mbar_init(tmem_empty, kEpiWarps);
+    for (int u = 0; u < kTcMaxUnits; ++u) {
+      mbar_init(tfull + u, 1);
+      mbar_init(tempty + u, kEpiWarps);
+    }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   if (warp == 0) {
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_slot)), "r"(512));
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
   }
-  asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+  fence_before();
   __syncthreads();
-  asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+  fence_after();
   const uint32_t tmem_base = *tmem_slot;
 
   if (warp == kEpiWarps) {
     // ===== producer: stream the four operand planes of every K=16 step =====
     if (lane == 0) {
-      uint32_t step = 0;
+      uint32_t kidx = 0;
       for (int item = blockIdx.x; item < nitems; item += gridDim.x) {
         const int f = item / prm.ngroups;
         const __half *Xf = X + (int64_t)f * lay.x_elems_per_f;
-        for (int ks = 0; ks < prm.ksteps; ++ks, ++step) {
-          const int s = step % prm.nstage;
-          const uint32_t use = step / prm.nstage;
+        for (int ks = 0; ks < prm.ksteps; ++ks, ++kidx) {
+          const int s = kidx % prm.nstage;
+          const uint32_t use = kidx / prm.nstage;
           if (use > 0) mbar_wait(empty_bar + s, (use - 1) & 1);
           mbar_expect_tx(full_bar + s, prm.stage_bytes);
           unsigned char *dst = stages + (size_t)s * prm.stage_bytes;
@@ -157,6 +174,7 @@ contract_tc_kernel(const __half *__restrict__ X, Layout lay, TcParams prm, float
           for (int pl = 0; pl < 4; ++pl)
             bulk_g2s(dst + (size_t)pl * prm.plane_bytes, Xf + pl * prm.plane_elems + ks * prm.kstep_elems, prm.plane_bytes,
                      full_bar + s);
+          TC_TRACE(0, kidx);
         }
       }
     }
@@ -164,149 +182,190 @@ contract_tc_kernel(const __half *__restrict__ X, Layout lay, TcParams prm, float
     // ===== MMA issuer =====
     if (lane == 0) {
       const uint32_t lbo = (uint32_t)lay.Cp * 16u, sbo = 128u;
-      uint32_t step = 0, it = 0;
-      for (int item = blockIdx.x; item < nitems; item += gridDim.x, ++it) {
-        const int g = item % prm.ngroups;
-        if (it > 0) mbar_wait(tmem_empty, (it - 1) & 1);  // epilogue has drained the accumulators
-        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-        for (int ks = 0; ks < prm.ksteps; ++ks, ++step) {
-          const int s = step % prm.nstage;
-          mbar_wait(full_bar + s, (step / prm.nstage) & 1);
-          asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-          const uint32_t sb = smem_u32(stages + (size_t)s * prm.stage_bytes);
-          const uint32_t p_hr = sb, p_hi = sb + prm.plane_bytes, p_lr = sb + 2 * prm.plane_bytes, p_li = sb + 3 * prm.plane_bytes;
-          for (int t = 0; t < prm.ntiles[g]; ++t) {
-            const TcTile tl = prm.tiles[g][t];
-            const uint32_t ao = (uint32_t)(tl.row0 / 8) * 128u, bo = (uint32_t)(tl.col0 / 8) * 128u;
-            const uint32_t id = make_idesc(tl.N, 0), idn = make_idesc(tl.N, 1);
-            const uint32_t acc = ks > 0 ? 1u : 0u;
-            const uint32_t d_re = tmem_base + (uint32_t)tl.tm_re, d_im = tmem_base + (uint32_t)tl.tm_im;
+      uint32_t kbase = 0, tr = 0;
+      uint32_t ucnt[kTcMaxUnits];
+#pragma unroll
+      for (int u = 0; u < kTcMaxUnits; ++u) ucnt[u] = 0;
+
+      // the twelve MMAs of one (unit, K step): Re += A_j A_i + B_j B_i;  Im += A_j B_i - B_j A_i  (rows j, cols i)
+      auto issue = [&](const TcUnit &un, int s, int ks) {
+        const uint32_t sb = smem_u32(stages + (size_t)s * prm.stage_bytes);
+        const uint32_t p_hr = sb, p_hi = sb + prm.plane_bytes, p_lr = sb + 2 * prm.plane_bytes, p_li = sb + 3 * prm.plane_bytes;
+        const uint32_t ao = (uint32_t)(un.row0 / 8) * 128u, bo = (uint32_t)(un.col0 / 8) * 128u;
+        const uint32_t id = make_idesc(un.N, 0), idn = make_idesc(un.N, 1);
+        const uint32_t acc = ks > 0 ? 1u : 0u;
+        const uint32_t d_re = tmem_base + (uint32_t)un.tm, d_im = d_re + (uint32_t)un.N;
 #define SD(plane, off) make_sdesc((plane) + (off), lbo, sbo)
-            // Re S += A A^T + B B^T
-            mma_f16(d_re, SD(p_hr, ao), SD(p_hr, bo), id, acc);
-            mma_f16(d_re, SD(p_hr, ao), SD(p_lr, bo), id, 1u);
-            mma_f16(d_re, SD(p_lr, ao), SD(p_hr, bo), id, 1u);
-            mma_f16(d_re, SD(p_hi, ao), SD(p_hi, bo), id, 1u);
-            mma_f16(d_re, SD(p_hi, ao), SD(p_li, bo), id, 1u);
-            mma_f16(d_re, SD(p_li, ao), SD(p_hi, bo), id, 1u);
-            // Im S += B A^T - A B^T
-            mma_f16(d_im, SD(p_hi, ao), SD(p_hr, bo), id, acc);
-            mma_f16(d_im, SD(p_hi, ao), SD(p_lr, bo), id, 1u);
-            mma_f16(d_im, SD(p_li, ao), SD(p_hr, bo), id, 1u);
-            mma_f16(d_im, SD(p_hr, ao), SD(p_hi, bo), idn, 1u);
-            mma_f16(d_im, SD(p_hr, ao), SD(p_li, bo), idn, 1u);
-            mma_f16(d_im, SD(p_lr, ao), SD(p_hi, bo), idn, 1u);
+        mma_f16(d_re, SD(p_hr, ao), SD(p_hr, bo), id, acc);
+        mma_f16(d_re, SD(p_hr, ao), SD(p_lr, bo), id, 1u);
+        mma_f16(d_re, SD(p_lr, ao), SD(p_hr, bo), id, 1u);
+        mma_f16(d_re, SD(p_hi, ao), SD(p_hi, bo), id, 1u);
+        mma_f16(d_re, SD(p_hi, ao), SD(p_li, bo), id, 1u);
+        mma_f16(d_re, SD(p_li, ao), SD(p_hi, bo), id, 1u);
+        mma_f16(d_im, SD(p_hr, ao), SD(p_hi, bo), id, acc);
+        mma_f16(d_im, SD(p_hr, ao), SD(p_li, bo), id, 1u);
+        mma_f16(d_im, SD(p_lr, ao), SD(p_hi, bo), id, 1u);
+        mma_f16(d_im, SD(p_hi, ao), SD(p_hr, bo), idn, 1u);
+        mma_f16(d_im, SD(p_hi, ao), SD(p_lr, bo), idn, 1u);
+        mma_f16(d_im, SD(p_li, ao), SD(p_hr, bo), idn, 1u);
 #undef SD
+      };
+      auto wait_unit_free = [&](int u) {
+        if (ucnt[u] > 0) mbar_wait(tempty + u, (ucnt[u] - 1) & 1);  // epilogue has drained the previous use
+        fence_after();
+      };
+
+      for (int item = blockIdx.x; item < nitems; item += gridDim.x) {
+        const int g = item % prm.ngroups, nu = prm.nunits[g];
+        if (prm.unit_major) {
+          for (int u = 0; u < nu; ++u) {
+            const TcUnit un = prm.units[g][u];
+            wait_unit_free(u);
+            for (int ks = 0; ks < prm.ksteps; ++ks) {
+              const uint32_t kidx = kbase + ks;
+              const int s = kidx % prm.nstage;
+              if (u == 0) {
+                mbar_wait(full_bar + s, (kidx / prm.nstage) & 1);
+                fence_after();
+              }
+              issue(un, s, ks);
+              if (u == nu - 1) mma_commit(empty_bar + s);  // stage reusable once every unit has read it
+            }
+            mma_commit(tfull + u);
+            ucnt[u]++;
+            TC_TRACE(1, tr); ++tr;
           }
-          mma_commit(empty_bar + s);  // stage reusable once these MMAs have read it
+        } else {
+          for (int ks = 0; ks < prm.ksteps; ++ks) {
+            const uint32_t kidx = kbase + ks;
+            const int s = kidx % prm.nstage;
+            mbar_wait(full_bar + s, (kidx / prm.nstage) & 1);
+            fence_after();
+            for (int u = 0; u < nu; ++u) {
+              if (ks == 0) wait_unit_free(u);
+              issue(prm.units[g][u], s, ks);
+            }
+            mma_commit(empty_bar + s);
+          }
+          for (int u = 0; u < nu; ++u) {
+            mma_commit(tfull + u);
+            ucnt[u]++;
+          }
+          TC_TRACE(1, tr); ++tr;
         }
-        mma_commit(tmem_full);  // accumulators of this item complete
+        kbase += prm.ksteps;
       }
     }
   } else {
-    // ===== epilogue warps: warp = quadrant (lanes of TMEM) + 4 * column half =====
+    // ===== epilogue warps: warp = lane quadrant of TMEM + 4 * column half =====
     const int q = warp & 3, h = warp >> 2;
-    const int C = lay.C;
-    uint32_t it = 0;
-    for (int item = blockIdx.x; item < nitems; item += gridDim.x, ++it) {
-      const int f = item / prm.ngroups, g = item % prm.ngroups;
-      mbar_wait(tmem_full, it & 1);
-      asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-      float2 *Sf = S ? S + (int64_t)f * lay.Ppad : nullptr;
-      for (int t = 0; t < prm.ntiles[g]; ++t) {
-        const TcTile tl = prm.tiles[g][t];
-        if (32 * q < tl.lane_lo) continue;
-        const int i = tl.row0 + 32 * q + lane;
-        const float si = scale * inv_scale[i];
-        const int nhalf = tl.N / 2;
-        const uint32_t lane_addr = (uint32_t)(32 * q) << 16;
-        for (int c0 = h * nhalf; c0 < (h + 1) * nhalf; c0 += 16) {
-          float re[16], im[16];
-          tmem_ld16(tmem_base + lane_addr + (uint32_t)(tl.tm_re + c0), re);
-          tmem_ld16(tmem_base + lane_addr + (uint32_t)(tl.tm_im + c0), im);
-          asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-          const int jbase = tl.col0 + c0;
-          if (jbase + 15 < i || i >= C) continue;   // whole chunk below the diagonal for this lane
+    const int C = lay.C, F = lay.F;
+    const int pb_mask = lay.PB - 1;
+    uint32_t ucnt[kTcMaxUnits], tr = 0;
 #pragma unroll
-          for (int u = 0; u < 16; ++u) {
-            const int j = jbase + u;
-            if (j >= C) break;
-            if (i < j) {
-              if (Sf) {
-                const float sc = si * inv_scale[j];
-                Sf[(j * (j - 1)) / 2 + i] = make_float2(re[u] * sc, im[u] * sc);
+    for (int u = 0; u < kTcMaxUnits; ++u) ucnt[u] = 0;
+    for (int item = blockIdx.x; item < nitems; item += gridDim.x) {
+      const int f = item / prm.ngroups, g = item % prm.ngroups, nu = prm.nunits[g];
+      const int fx = f & pb_mask;
+      for (int u = 0; u < nu; ++u) {
+        const TcUnit un = prm.units[g][u];
+        mbar_wait(tfull + u, ucnt[u] & 1);
+        ucnt[u]++;
+        fence_after();
+        if (warp == 0) { TC_TRACE(2, tr); ++tr; }
+        if (32 * q >= un.lane_lo && 32 * q < un.lane_hi) {
+          const int j = un.row0 + 32 * q + lane;
+          const bool jok = j < C;
+          const float sj = scale * inv_scale[j];
+          const int nhalf = un.N / 2;
+          const uint32_t lane_addr = (uint32_t)(32 * q) << 16;
+          for (int c0 = h * nhalf; c0 < (h + 1) * nhalf; c0 += 16) {
+            const int ibase = un.col0 + c0;
+            if (ibase > un.row0 + 32 * q + 31) continue;  // i > j for every lane of this warp
+            float re[16], im[16];
+            tmem_ld16(tmem_base + lane_addr + (uint32_t)(un.tm + c0), re);
+            tmem_ld16(tmem_base + lane_addr + (uint32_t)(un.tm + un.N + c0), im);
+            asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+            for (int e = 0; e < 16; ++e) {
+              const int i = ibase + e;
+              if (i < j && jok) {
+                if (S) {
+                  // lexicographic pair index p = i C - i(i+1)/2 + (j - i - 1); block-major, slot swizzled by bin
+                  const int p = i * C - (i * (i + 1)) / 2 - i - 1 + j;
+                  const int64_t off = ((int64_t)(p >> lay.pb_shift) * F + f) * lay.PB + ((p ^ fx) & pb_mask);
+                  const float sc = sj * inv_scale[i];
+                  S[off] = make_float2(re[e] * sc, im[e] * sc);
+                }
+              } else if (i == j && jok) {
+                const float a = re[e] * sj * inv_scale[i];
+                if (Sauto) Sauto[(int64_t)j * F + f] = a;
+                if (Srsq) Srsq[(int64_t)j * F + f] = a > 0.f ? rsqrtf(a) : 0.f;
               }
-            } else if (i == j && Sauto) {
-              Sauto[(int64_t)i * lay.F + f] = re[u] * si * inv_scale[j];
             }
           }
         }
+        fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(tempty + u);
+        if (warp == 0) { TC_TRACE(2, tr); ++tr; }
       }
-      asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-      __syncwarp();
-      if (lane == 0) mbar_arrive(tmem_empty);
     }
   }
 
-  asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+  fence_before();
   __syncthreads();
   if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(512));
 }
 
 // ------------------------------------------------------------------------------------------
+// Host: cover the lower triangle (i < j) and the diagonal with units of 128 lanes (j) x N <= 128 columns (i),
+// then pack the units into groups whose accumulators (Re + Im = 2N columns each) fit the 512 TMEM columns.
 bool tc_plan_tiles(int Cp, TcHostPlan *out) {
-  // rows are covered by M = 128 tiles over pairs of 64-channel blocks; each tile's columns start at its
-  // own first row (upper triangle) and are cut into slabs of <= 256; tiles are packed into groups whose
-  // accumulators (Re + Im = 2N columns) fit the 512 TMEM columns.
-  struct T { int row0, col0, N, lane_lo; };
-  T list[64];
+  struct U { int row0, lane_lo, lane_hi, col0, N; };
+  U list[kTcMaxGroups * kTcMaxUnits];
   int n = 0;
-  const int nb = Cp / 64;
-  for (int m = 0; 2 * m + 1 < nb; ++m)
-    for (int c = 128 * m; c < Cp; c += 256) {
-      if (n >= 64) return false;
-      list[n++] = {128 * m, c, (Cp - c) < 256 ? (Cp - c) : 256, 0};
+  auto add_row_tile = [&](int r0, int lane_hi, int col_end) {
+    for (int c = 0; c < col_end; c += 128) {
+      if (n >= kTcMaxGroups * kTcMaxUnits) return false;
+      const int N = (col_end - c) < 128 ? (col_end - c) : 128;
+      int lane_lo = c > r0 ? ((c - r0) & ~31) : 0;  // lanes below have j < col0: nothing to keep
+      list[n++] = {r0, lane_lo, lane_hi, c, N};
     }
-  if (nb & 1) {
-    if (n >= 64) return false;
-    list[n++] = {64 * (nb - 2), 64 * (nb - 1), 64, 64};
-  }
-  // first-fit decreasing by N
-  for (int a = 0; a < n; ++a)
-    for (int b = a + 1; b < n; ++b)
-      if (list[b].N > list[a].N) { T t = list[a]; list[a] = list[b]; list[b] = t; }
+    return true;
+  };
+  if (Cp < 128 || (Cp & 63) != 0) return false;
+  for (int r0 = Cp - 128; r0 >= 0; r0 -= 128)
+    if (!add_row_tile(r0, 128, r0 + 128)) return false;
+  if ((Cp & 127) == 64 && !add_row_tile(0, 64, 64)) return false;
+
   int used[kTcMaxGroups];
   out->ngroups = 0;
-  for (int g = 0; g < kTcMaxGroups; ++g) { used[g] = 0; out->ntiles[g] = 0; }
+  for (int g = 0; g < kTcMaxGroups; ++g) { used[g] = 0; out->nunits[g] = 0; }
   for (int a = 0; a < n; ++a) {
     int g = 0;
     for (; g < kTcMaxGroups; ++g)
-      if (used[g] + 2 * list[a].N <= 512 && out->ntiles[g] < kTcMaxTiles) break;
+      if (used[g] + 2 * list[a].N <= 512 && out->nunits[g] < kTcMaxUnits) break;
     if (g == kTcMaxGroups) return false;
-    int *slot = &out->ntiles[g];
-    out->tiles[g][*slot][0] = list[a].row0;
-    out->tiles[g][*slot][1] = list[a].col0;
-    out->tiles[g][*slot][2] = list[a].N;
-    out->tiles[g][*slot][3] = list[a].lane_lo;
-    out->tiles[g][*slot][4] = used[g];
-    out->tiles[g][*slot][5] = used[g] + list[a].N;
+    int *u = out->units[g][out->nunits[g]++];
+    u[0] = list[a].row0; u[1] = list[a].lane_lo; u[2] = list[a].lane_hi;
+    u[3] = list[a].col0; u[4] = list[a].N; u[5] = used[g];
     used[g] += 2 * list[a].N;
-    ++*slot;
     if (g + 1 > out->ngroups) out->ngroups = g + 1;
   }
   return true;
 }
 
-int launch_contract_tc(delta_plan *p, const void *d_X, float *d_S, float *d_auto, cudaStream_t st) {
+int launch_contract_tc(delta_plan *p, const void *d_X, float *d_S, float *d_auto, float *d_rsq, cudaStream_t st) {
   const Layout &lay = p->lay;
   TcParams prm;
   memset(&prm, 0, sizeof(prm));
   prm.ngroups = p->tc.ngroups;
   for (int g = 0; g < kTcMaxGroups; ++g) {
-    prm.ntiles[g] = p->tc.ntiles[g];
-    for (int t = 0; t < kTcMaxTiles; ++t) {
-      const int *s = p->tc.tiles[g][t];
-      prm.tiles[g][t] = {s[0], s[1], s[2], s[3], s[4], s[5]};
+    prm.nunits[g] = p->tc.nunits[g];
+    for (int u = 0; u < kTcMaxUnits; ++u) {
+      const int *s = p->tc.units[g][u];
+      prm.units[g][u] = {s[0], s[1], s[2], s[3], s[4], s[5]};
     }
   }
   prm.ksteps = lay.Kp / 16;
@@ -319,14 +378,25 @@ int launch_contract_tc(delta_plan *p, const void *d_X, float *d_S, float *d_auto
   if (nstage > 8) nstage = 8;
   if (nstage < 2) return DELTA_ERR_UNSUPPORTED;
   prm.nstage = nstage;
+  prm.unit_major = (2 * prm.ksteps <= nstage) ? 1 : 0;
   size_t smem = (size_t)nstage * prm.stage_bytes + fixed;
   if (smem < 120 * 1024) smem = 120 * 1024;  // one CTA per SM: each CTA allocates all 512 TMEM columns
-  cudaError_t e = cudaFuncSetAttribute(contract_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  if (e != cudaSuccess) { set_cuda_error(e); return DELTA_ERR_CUDA; }
   const int nitems = lay.F * prm.ngroups;
   const int grid = nitems < p->num_sms ? nitems : p->num_sms;
-  contract_tc_kernel<<<grid, kTcThreads, smem, st>>>(reinterpret_cast<const __half *>(d_X), lay, prm, p->s2 / (float)lay.K,
-                                                      p->d_chscale(), reinterpret_cast<float2 *>(d_S), d_auto);
+  const float scale = p->s2 / (float)lay.K;
+  if (p->d_trace) {
+    int rc = opt_in_smem(contract_tc_kernel<true>, smem);
+    if (rc) return rc;
+    contract_tc_kernel<true><<<grid, kTcThreads, smem, st>>>(reinterpret_cast<const __half *>(d_X), lay, prm, scale,
+                                                             p->d_chscale(), reinterpret_cast<float2 *>(d_S), d_auto, d_rsq,
+                                                             p->d_trace);
+  } else {
+    int rc = opt_in_smem(contract_tc_kernel<false>, smem);
+    if (rc) return rc;
+    contract_tc_kernel<false><<<grid, kTcThreads, smem, st>>>(reinterpret_cast<const __half *>(d_X), lay, prm, scale,
+                                                              p->d_chscale(), reinterpret_cast<float2 *>(d_S), d_auto, d_rsq,
+                                                              nullptr);
+  }
   p->launches++;
   DELTA_CUDA_CHECK(cudaGetLastError());
   return DELTA_OK;

@@ -12,16 +12,19 @@ namespace delta {
 constexpr int kPairTile = 64;     // channel block of the FP32 contraction tiles
 constexpr int kSegBlock = 8;      // segments per K-chunk ("kc") of the X layout
 constexpr int kThreads = 256;
-constexpr int kTcMaxGroups = 16;  // TMEM-sized groups of accumulator tiles per frequency bin
-constexpr int kTcMaxTiles = 4;    // tiles per group
+constexpr int kTcMaxGroups = 16;  // TMEM-sized groups of accumulator units per frequency bin
+constexpr int kTcMaxUnits = 4;    // units per group
 
-// tile plan of the tensor-core contraction (host side; see contract_tc.cu)
+// unit plan of the tensor-core contraction (host side; see contract_tc.cu)
 struct TcHostPlan {
   int ngroups;
-  int ntiles[kTcMaxGroups];
-  int tiles[kTcMaxGroups][kTcMaxTiles][6];  // row0, col0, N, lane_lo, tmem col of Re, tmem col of Im
+  int nunits[kTcMaxGroups];
+  int units[kTcMaxGroups][kTcMaxUnits][6];  // row0, lane_lo, lane_hi, col0, N, tmem column of Re
 };
 bool tc_plan_tiles(int Cp, TcHostPlan *out);
+
+// pairs per block of the S layout = pairs per CTA of the pair kernel (its S tile must fit shared memory)
+constexpr int pair_block(int L) { return L <= 1024 ? 16 : (L == 2048 ? 8 : 4); }
 
 struct Layout {
   // X (STFT) buffer, frequency-major so that one bin's C x K matrix is one contiguous block:
@@ -29,12 +32,16 @@ struct Layout {
   //   TC   mode : __half X[f][prec][part][kc][c][8]           prec 0 = hi, 1 = lo (split fp16)
   // k = 8*kc + kk, c < Cp (rows C..Cp-1 are zero), kc < Kc = Kp/8, Kp = K rounded up to 16.
   int C, Cp, T, L, N, H, K, Kp, Kc, F, M, nlags;
-  int64_t P, Ppad;        // S is complex64 [F][Ppad], pair (i<j) at column p' = j(j-1)/2 + i
+  // S (cross-spectra) is complex64 [Pblk][F][PB]: pairs in lexicographic order p = iC - i(i+1)/2 + (j-i-1),
+  // block = p / PB, and inside row f of a block pair p sits in slot (p ^ f) & (PB-1).  One block is one
+  // contiguous tile for the pair kernel; the XOR makes its column (fixed pair) reads bank-conflict free.
+  int PB, pb_shift;
+  int64_t P, Pblk;
   int64_t x_elems_per_f;  // elements (float or half) per frequency
 };
 
 struct Workspace {
-  size_t off_tw, off_win, off_ftab, off_pairs, off_offs, off_isum, off_chscale, off_X, off_S, off_auto, total;
+  size_t off_tw, off_win, off_ftab, off_pairs, off_offs, off_isum, off_chscale, off_X, off_S, off_auto, off_rsq, total;
 };
 
 }  // namespace delta
@@ -49,7 +56,7 @@ struct delta_plan {
   std::vector<float2> h_tw;      // e^{-2 pi i f / L}, f = 0..L-1
   std::vector<float> h_win;      // periodic Hann
   std::vector<float2> h_ftab;    // per-pass twiddles of the register FFT (fft_reg.cuh), N = L/2
-  std::vector<ushort2> h_pairs;  // (i, j) in S order: p' = j(j-1)/2 + i (column-major upper triangle)
+  std::vector<ushort2> h_pairs;  // (i, j) of pair p, lexicographic
   delta::TcHostPlan tc;
   int num_sms = 148;
   // device state
@@ -59,6 +66,7 @@ struct delta_plan {
   bool offsets_set = false;
   int n_first = 0;
   int launches = 0;
+  long long *d_trace = nullptr;  // debug: clock stamps of the tensor-core contraction (delta_debug_set_trace)
   bool stage_events_on = false;
   cudaEvent_t stage_ev[4] = {nullptr, nullptr, nullptr, nullptr};
   cudaStream_t copy_stream = nullptr;
@@ -76,6 +84,7 @@ struct delta_plan {
   void *d_X() const { return ws + wsl.off_X; }
   float *d_S() const { return reinterpret_cast<float *>(ws + wsl.off_S); }
   float *d_auto() const { return reinterpret_cast<float *>(ws + wsl.off_auto); }
+  float *d_rsq() const { return reinterpret_cast<float *>(ws + wsl.off_rsq); }
 };
 
 namespace delta {
@@ -120,9 +129,12 @@ static inline int opt_in_smem(Kern kern, size_t bytes) {
 int launch_offsets(delta_plan *p, const void *d_x, int64_t ld, int n_first, cudaStream_t st);
 int launch_stft(delta_plan *p, const void *d_x, int64_t ld, void *d_X, cudaStream_t st);
 int launch_stft_unpack(delta_plan *p, const void *d_X, float *d_out, cudaStream_t st);
-int launch_contract_fp32(delta_plan *p, const void *d_X, float *d_S, float *d_auto, cudaStream_t st);
-int launch_contract_tc(delta_plan *p, const void *d_X, float *d_S, float *d_auto, cudaStream_t st);
-int launch_pair_epilogue(delta_plan *p, const float *d_S, const float *d_auto, float *d_G, float *d_A,
-                         float *d_P, float *d_R, cudaStream_t st);
+// both contractions write S (may be null), the autospectra and 1/sqrt(autospectra) (either may be null)
+int launch_contract_fp32(delta_plan *p, const void *d_X, float *d_S, float *d_auto, float *d_rsq, cudaStream_t st);
+int launch_contract_tc(delta_plan *p, const void *d_X, float *d_S, float *d_auto, float *d_rsq, cudaStream_t st);
+int launch_auto_prep(delta_plan *p, const float *d_auto, float *d_rsq, cudaStream_t st);
+int launch_pair(delta_plan *p, const float *d_S, const float *d_auto, const float *d_rsq, float *d_G, float *d_A,
+                float *d_P, float *d_R, cudaStream_t st);
+int launch_s_unpack(delta_plan *p, const float *d_S, float *d_out, cudaStream_t st);
 
 }  // namespace delta

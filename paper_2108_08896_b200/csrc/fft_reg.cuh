@@ -1,8 +1,9 @@
 // Register-resident mixed-radix FFT for a group of T = N/E threads (N = L/2 complex points).
 //
 // Every thread keeps E points in registers; a pass is a radix-R butterfly done entirely in registers
-// (R in {4, 8, 16}); between passes the group transposes through a private, padded shared-memory
-// buffer.  Used for the forward transform of the STFT and for the inverse
+// (R in {4, 8, 16}); between passes the group transposes through shared memory, addressed through an
+// index map `m(e)` (any bijection of 0..N-1 onto distinct float2 slots that the group owns): FftPadMap is
+// a private buffer padded by one slot per 16, the pair kernel maps onto the slots of its S tile.  Used for the forward transform of the STFT and for the inverse
 // transform of the cross-correlation (Eq. 1d).  No cuFFT: every butterfly is here.
 //
 // Register/array correspondence, before AND after fft_inplace():   v[u]  <->  x[tid + T*u],  u < E,
@@ -128,6 +129,10 @@ DELTA_FFT_GEOM(2048, 16, 3, 16, 16, 8)
 #undef DELTA_FFT_GEOM
 
 DELTA_HD int fft_pad(int i) { return i + (i >> 4); }
+struct FftPadMap {
+  float2 *buf;  // FftGeom<N>::BUF entries
+  DELTA_HD float2 &operator()(int e) const { return buf[fft_pad(e)]; }
+};
 
 DELTA_HD float2 fft_ld_tw(const float2 *p) {
 #ifdef __CUDA_ARCH__
@@ -138,8 +143,8 @@ DELTA_HD float2 fft_ld_tw(const float2 *p) {
 }
 
 // One pass.  LAST: results stay in registers (natural order, see header); otherwise they go to `buf`.
-template <int N, int R, int S, bool LAST, bool INV>
-DELTA_HD void fft_pass(float2 *v, float2 *buf, const float2 *tp, int tid) {
+template <int N, int R, int S, bool LAST, bool INV, class Map>
+DELTA_HD void fft_pass(float2 *v, const Map &m, const float2 *tp, int tid) {
   using G = FftGeom<N>;
   constexpr int NB = G::E / R, CNT = N / (R * S);
 #pragma unroll
@@ -161,16 +166,16 @@ DELTA_HD void fft_pass(float2 *v, float2 *buf, const float2 *tp, int tid) {
         a[k] = cmul(a[k], w);
       }
 #pragma unroll
-      for (int k = 0; k < R; ++k) buf[fft_pad(q + S * (R * r + k))] = a[k];
+      for (int k = 0; k < R; ++k) m(q + S * (R * r + k)) = a[k];
     }
   }
 }
 
-template <int N>
-DELTA_HD void fft_readback(float2 *v, const float2 *buf, int tid) {
+template <int N, class Map>
+DELTA_HD void fft_readback(float2 *v, const Map &m, int tid) {
   using G = FftGeom<N>;
 #pragma unroll
-  for (int u = 0; u < G::E; ++u) v[u] = buf[fft_pad(tid + G::T * u)];
+  for (int u = 0; u < G::E; ++u) v[u] = m(tid + G::T * u);
 }
 
 #ifdef __CUDACC__
@@ -181,23 +186,23 @@ __device__ __forceinline__ void fft_group_sync() {
   if (T <= 32) __syncwarp(); else __syncthreads();
 }
 
-// v[u] <-> x[tid + T*u] in, X[tid + T*u] out (unnormalised).  `buf`: FftGeom<N>::BUF float2 of shared
-// memory private to the group; it may be reused as soon as the call returns... by this group only
-// after another fft_group_sync (the last read-back is followed by one).
-template <int N, bool INV>
-__device__ __forceinline__ void fft_inplace(float2 *v, float2 *buf, const float2 *__restrict__ tp, int tid) {
+// v[u] <-> x[tid + T*u] in, X[tid + T*u] out (unnormalised).  The slots behind `m` are shared memory owned
+// by the group; other threads of the group may still be reading them when the call returns, so the group
+// must pass another fft_group_sync before it writes them again.
+template <int N, bool INV, class Map>
+__device__ __forceinline__ void fft_inplace(float2 *v, const Map &m, const float2 *__restrict__ tp, int tid) {
   using G = FftGeom<N>;
-  fft_pass<N, G::R0, 1, false, INV>(v, buf, tp, tid);
+  fft_pass<N, G::R0, 1, false, INV>(v, m, tp, tid);
   fft_group_sync<G::T>();
-  fft_readback<N>(v, buf, tid);
+  fft_readback<N>(v, m, tid);
   if constexpr (G::NP == 2) {
-    fft_pass<N, G::R1, G::R0, true, INV>(v, buf, tp, tid);
+    fft_pass<N, G::R1, G::R0, true, INV>(v, m, tp, tid);
   } else {
     fft_group_sync<G::T>();
-    fft_pass<N, G::R1, G::R0, false, INV>(v, buf, tp + G::OFF1, tid);
+    fft_pass<N, G::R1, G::R0, false, INV>(v, m, tp + G::OFF1, tid);
     fft_group_sync<G::T>();
-    fft_readback<N>(v, buf, tid);
-    fft_pass<N, G::R2, G::R0 * G::R1, true, INV>(v, buf, tp, tid);
+    fft_readback<N>(v, m, tid);
+    fft_pass<N, G::R2, G::R0 * G::R1, true, INV>(v, m, tp, tid);
   }
 }
 #endif

@@ -213,7 +213,7 @@ stft_kernel(const void *__restrict__ x, int64_t ld, int in_dtype, int norm_mode,
 #pragma unroll
       for (int u = 0; u < E; ++u) v[u] = make_float2(0.f, 0.f);
     }
-    fft_inplace<N, false>(v, buf, ftab, gt);
+    fft_inplace<N, false>(v, FftPadMap{buf}, ftab, gt);
     fft_group_sync<T>();  // every read-back of the group is done before Z overwrites the buffer
 #pragma unroll
     for (int u = 0; u < E; ++u) buf[fft_pad(gt + T * u)] = v[u];

@@ -93,8 +93,9 @@ def test_sizes_match_survey_table(name, K, F, P, nl):
     p = b.Plan(w.C, w.T, w.nfft, w.hop, w.max_lag, allocate=False)
     s = p.sizes
     assert (s.K, s.F, s.P, s.n_lags) == (K, F, P, nl) == (w.K, w.F, w.P, 2 * w.max_lag + 1)
-    assert s.s_row_stride >= P and s.s_row_stride % 32 == 0
-    assert s.s_bytes == s.F * s.s_row_stride * 8
+    B = s.s_block_pairs
+    assert B in (4, 8, 16)
+    assert s.s_bytes == -(-P // B) * s.F * B * 8
     assert s.workspace_bytes >= s.x_bytes + s.s_bytes
 
 

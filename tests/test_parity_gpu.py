@@ -141,12 +141,12 @@ def test_staged_calls_equal_fused_call(mode):
     torch.cuda.synchronize()
     for name, t in (("G", G), ("A", A), ("P", P), ("R", R), ("Sauto", Sa)):
         assert torch.equal(t, fused[name]), name
-    # S itself against the oracle, in its documented layout: [F][P_pad], pair (i<j) at column j(j-1)/2 + i
+    # S itself against the oracle (through the unpack accessor: [P][F], lexicographic pairs)
     Xo = o.stft(x, w.nfft, w.hop)
-    pairs = np.array([(i, j) for j in range(1, 40) for i in range(j)])
+    pairs = o.all_pairs(40)
     s2 = o.scale_factor(w.nfft)
     So = o.cross_spectra(Xo, pairs, s2)
-    Sg = torch.view_as_complex(S).cpu().numpy()[:, :len(pairs)].T
+    Sg = plan.cross_spectra_unpack(S).cpu().numpy()
     Sa_o = o.auto_spectra(Xo, s2)
     den = np.sqrt(Sa_o[pairs[:, 0]] * Sa_o[pairs[:, 1]])
     assert np.max(np.abs(Sg - So) / den) < 1e-5
