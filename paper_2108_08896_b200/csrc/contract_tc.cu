@@ -31,8 +31,9 @@ namespace delta {
 
 namespace {
 
-constexpr int kTcThreads = 320;
-constexpr int kEpiWarps = 8;
+constexpr int kColSplit = 4;              // column slices of a unit, one per epilogue warp of a lane quadrant
+constexpr int kEpiWarps = 4 * kColSplit;
+constexpr int kTcThreads = 32 * (kEpiWarps + 2);
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
@@ -93,6 +94,11 @@ __device__ __forceinline__ void tmem_ld16(uint32_t taddr, float *v) {
 #pragma unroll
   for (int q = 0; q < 16; ++q) v[q] = __uint_as_float(r[q]);
 }
+__device__ __forceinline__ bool elect_one() {
+  uint32_t pred;
+  asm volatile("{\n\t.reg .pred p;\n\telect.sync _|p, 0xffffffff;\n\tselp.u32 %0, 1, 0, p;\n\t}" : "=r"(pred));
+  return pred != 0;
+}
 __device__ __forceinline__ void fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 
@@ -126,17 +132,21 @@ contract_tc_kernel(const __half *__restrict__ X, Layout lay, TcParams prm, float
                    float2 *__restrict__ S, float *__restrict__ Sauto, float *__restrict__ Srsq, long long *trace) {
   extern __shared__ __align__(1024) unsigned char smem_raw[];
   unsigned char *stages = smem_raw;
-  float *inv_scale = reinterpret_cast<float *>(stages + (size_t)prm.nstage * prm.stage_bytes);  // [Cp]
-  uint64_t *full_bar = reinterpret_cast<uint64_t *>(inv_scale + lay.Cp);
+  // itab[c] = {rowbase(c) = c C - c(c+1)/2 - c - 1 (int bits), 1/chscale[c]}: pair index p(i, j) = rowbase(i) + j
+  float2 *itab = reinterpret_cast<float2 *>(stages + (size_t)prm.nstage * prm.stage_bytes);  // [Cp]
+  uint64_t *full_bar = reinterpret_cast<uint64_t *>(itab + lay.Cp);
   uint64_t *empty_bar = full_bar + prm.nstage;
   uint64_t *tfull = empty_bar + prm.nstage;  // [kTcMaxUnits]
   uint64_t *tempty = tfull + kTcMaxUnits;    // [kTcMaxUnits]
   uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(tempty + kTcMaxUnits);
 
-  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int tid = threadIdx.x, lane = tid & 31;
+  const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);  // provably warp-uniform
   const int nitems = lay.F * prm.ngroups;
+  if (tid == 0) TC_TRACE(3, 0);
 
-  for (int c = tid; c < lay.Cp; c += kTcThreads) inv_scale[c] = (c < lay.C) ? 1.f / chscale[c] : 0.f;
+  for (int c = tid; c < lay.Cp; c += kTcThreads)
+    itab[c] = make_float2(__int_as_float(c * lay.C - (c * (c + 1)) / 2 - c - 1), (c < lay.C) ? 1.f / chscale[c] : 0.f);
   if (tid == 0) {
     for (int s = 0; s < prm.nstage; ++s) {
       mbar_init(full_bar + s, 1);
@@ -156,18 +166,21 @@ contract_tc_kernel(const __half *__restrict__ X, Layout lay, TcParams prm, float
   __syncthreads();
   fence_after();
   const uint32_t tmem_base = *tmem_slot;
+  if (tid == 0) TC_TRACE(3, 1);
 
   if (warp == kEpiWarps) {
     // ===== producer: stream the four operand planes of every K=16 step =====
-    if (lane == 0) {
-      uint32_t kidx = 0;
-      for (int item = blockIdx.x; item < nitems; item += gridDim.x) {
-        const int f = item / prm.ngroups;
-        const __half *Xf = X + (int64_t)f * lay.x_elems_per_f;
-        for (int ks = 0; ks < prm.ksteps; ++ks, ++kidx) {
-          const int s = kidx % prm.nstage;
-          const uint32_t use = kidx / prm.nstage;
-          if (use > 0) mbar_wait(empty_bar + s, (use - 1) & 1);
+    // The whole warp walks the loop (warp-uniform values live in uniform registers, which is what the bulk-copy
+    // and MMA instructions take); one elected lane issues.
+    uint32_t kidx = 0;
+    for (int item = blockIdx.x; item < nitems; item += gridDim.x) {
+      const int f = item / prm.ngroups;
+      const __half *Xf = X + (int64_t)f * lay.x_elems_per_f;
+      for (int ks = 0; ks < prm.ksteps; ++ks, ++kidx) {
+        const int s = kidx % prm.nstage;
+        const uint32_t use = kidx / prm.nstage;
+        if (use > 0) mbar_wait(empty_bar + s, (use - 1) & 1);
+        if (elect_one()) {
           mbar_expect_tx(full_bar + s, prm.stage_bytes);
           unsigned char *dst = stages + (size_t)s * prm.stage_bytes;
 #pragma unroll
@@ -176,129 +189,144 @@ contract_tc_kernel(const __half *__restrict__ X, Layout lay, TcParams prm, float
                      full_bar + s);
           TC_TRACE(0, kidx);
         }
+        __syncwarp();
       }
     }
   } else if (warp == kEpiWarps + 1) {
     // ===== MMA issuer =====
-    if (lane == 0) {
-      const uint32_t lbo = (uint32_t)lay.Cp * 16u, sbo = 128u;
-      uint32_t kbase = 0, tr = 0;
-      uint32_t ucnt[kTcMaxUnits];
-#pragma unroll
-      for (int u = 0; u < kTcMaxUnits; ++u) ucnt[u] = 0;
+    const uint32_t lbo = (uint32_t)lay.Cp * 16u, sbo = 128u;
+    uint32_t kbase = 0, tr = 0;
+    uint32_t used = 0, par = 0;  // per-unit bits: unit has been used; parity of its use count
 
-      // the twelve MMAs of one (unit, K step): Re += A_j A_i + B_j B_i;  Im += A_j B_i - B_j A_i  (rows j, cols i)
-      auto issue = [&](const TcUnit &un, int s, int ks) {
-        const uint32_t sb = smem_u32(stages + (size_t)s * prm.stage_bytes);
-        const uint32_t p_hr = sb, p_hi = sb + prm.plane_bytes, p_lr = sb + 2 * prm.plane_bytes, p_li = sb + 3 * prm.plane_bytes;
-        const uint32_t ao = (uint32_t)(un.row0 / 8) * 128u, bo = (uint32_t)(un.col0 / 8) * 128u;
-        const uint32_t id = make_idesc(un.N, 0), idn = make_idesc(un.N, 1);
-        const uint32_t acc = ks > 0 ? 1u : 0u;
-        const uint32_t d_re = tmem_base + (uint32_t)un.tm, d_im = d_re + (uint32_t)un.N;
-#define SD(plane, off) make_sdesc((plane) + (off), lbo, sbo)
-        mma_f16(d_re, SD(p_hr, ao), SD(p_hr, bo), id, acc);
-        mma_f16(d_re, SD(p_hr, ao), SD(p_lr, bo), id, 1u);
-        mma_f16(d_re, SD(p_lr, ao), SD(p_hr, bo), id, 1u);
-        mma_f16(d_re, SD(p_hi, ao), SD(p_hi, bo), id, 1u);
-        mma_f16(d_re, SD(p_hi, ao), SD(p_li, bo), id, 1u);
-        mma_f16(d_re, SD(p_li, ao), SD(p_hi, bo), id, 1u);
-        mma_f16(d_im, SD(p_hr, ao), SD(p_hi, bo), id, acc);
-        mma_f16(d_im, SD(p_hr, ao), SD(p_li, bo), id, 1u);
-        mma_f16(d_im, SD(p_lr, ao), SD(p_hi, bo), id, 1u);
-        mma_f16(d_im, SD(p_hi, ao), SD(p_hr, bo), idn, 1u);
-        mma_f16(d_im, SD(p_hi, ao), SD(p_lr, bo), idn, 1u);
-        mma_f16(d_im, SD(p_li, ao), SD(p_hr, bo), idn, 1u);
-#undef SD
-      };
-      auto wait_unit_free = [&](int u) {
-        if (ucnt[u] > 0) mbar_wait(tempty + u, (ucnt[u] - 1) & 1);  // epilogue has drained the previous use
-        fence_after();
-      };
+    // the twelve MMAs of one (unit, K step): Re += A_j A_i + B_j B_i;  Im += A_j B_i - B_j A_i  (rows j, cols i)
+    auto issue = [&](const TcUnit &un, int s, int ks) {
+      const uint32_t sb = smem_u32(stages + (size_t)s * prm.stage_bytes);
+      const uint32_t p_hr = sb, p_hi = sb + prm.plane_bytes, p_lr = sb + 2 * prm.plane_bytes, p_li = sb + 3 * prm.plane_bytes;
+      const uint32_t ao = (uint32_t)(un.row0 / 8) * 128u, bo = (uint32_t)(un.col0 / 8) * 128u;
+      const uint32_t id = make_idesc(un.N, 0), idn = make_idesc(un.N, 1);
+      const uint32_t acc = ks > 0 ? 1u : 0u;
+      const uint32_t d_re = tmem_base + (uint32_t)un.tm, d_im = d_re + (uint32_t)un.N;
+      const uint64_t a_hr = make_sdesc(p_hr + ao, lbo, sbo), a_hi = make_sdesc(p_hi + ao, lbo, sbo);
+      const uint64_t a_lr = make_sdesc(p_lr + ao, lbo, sbo), a_li = make_sdesc(p_li + ao, lbo, sbo);
+      const uint64_t b_hr = make_sdesc(p_hr + bo, lbo, sbo), b_hi = make_sdesc(p_hi + bo, lbo, sbo);
+      const uint64_t b_lr = make_sdesc(p_lr + bo, lbo, sbo), b_li = make_sdesc(p_li + bo, lbo, sbo);
+      if (elect_one()) {
+        mma_f16(d_re, a_hr, b_hr, id, acc);
+        mma_f16(d_re, a_hr, b_lr, id, 1u);
+        mma_f16(d_re, a_lr, b_hr, id, 1u);
+        mma_f16(d_re, a_hi, b_hi, id, 1u);
+        mma_f16(d_re, a_hi, b_li, id, 1u);
+        mma_f16(d_re, a_li, b_hi, id, 1u);
+        mma_f16(d_im, a_hr, b_hi, id, acc);
+        mma_f16(d_im, a_hr, b_li, id, 1u);
+        mma_f16(d_im, a_lr, b_hi, id, 1u);
+        mma_f16(d_im, a_hi, b_hr, idn, 1u);
+        mma_f16(d_im, a_hi, b_lr, idn, 1u);
+        mma_f16(d_im, a_li, b_hr, idn, 1u);
+      }
+      __syncwarp();
+    };
+    auto wait_unit_free = [&](int u) {
+      if ((used >> u) & 1u) mbar_wait(tempty + u, ((par >> u) & 1u) ^ 1u);  // epilogue has drained the previous use
+      fence_after();
+    };
+    auto unit_done = [&](int u) {
+      if (elect_one()) mma_commit(tfull + u);
+      __syncwarp();
+      used |= 1u << u;
+      par ^= 1u << u;
+    };
 
-      for (int item = blockIdx.x; item < nitems; item += gridDim.x) {
-        const int g = item % prm.ngroups, nu = prm.nunits[g];
-        if (prm.unit_major) {
-          for (int u = 0; u < nu; ++u) {
-            const TcUnit un = prm.units[g][u];
-            wait_unit_free(u);
-            for (int ks = 0; ks < prm.ksteps; ++ks) {
-              const uint32_t kidx = kbase + ks;
-              const int s = kidx % prm.nstage;
-              if (u == 0) {
-                mbar_wait(full_bar + s, (kidx / prm.nstage) & 1);
-                fence_after();
-              }
-              issue(un, s, ks);
-              if (u == nu - 1) mma_commit(empty_bar + s);  // stage reusable once every unit has read it
-            }
-            mma_commit(tfull + u);
-            ucnt[u]++;
-            TC_TRACE(1, tr); ++tr;
-          }
-        } else {
+    for (int item = blockIdx.x; item < nitems; item += gridDim.x) {
+      const int g = item % prm.ngroups, nu = prm.nunits[g];
+      if (prm.unit_major) {
+        for (int u = 0; u < nu; ++u) {
+          const TcUnit un = prm.units[g][u];
+          wait_unit_free(u);
           for (int ks = 0; ks < prm.ksteps; ++ks) {
             const uint32_t kidx = kbase + ks;
             const int s = kidx % prm.nstage;
-            mbar_wait(full_bar + s, (kidx / prm.nstage) & 1);
-            fence_after();
-            for (int u = 0; u < nu; ++u) {
-              if (ks == 0) wait_unit_free(u);
-              issue(prm.units[g][u], s, ks);
+            if (u == 0) {
+              mbar_wait(full_bar + s, (kidx / prm.nstage) & 1);
+              fence_after();
+              if (lane == 0) TC_TRACE(4, kidx);
             }
-            mma_commit(empty_bar + s);
+            issue(un, s, ks);
+            if (u == nu - 1) {  // stage reusable once every unit has read it
+              if (elect_one()) mma_commit(empty_bar + s);
+              __syncwarp();
+            }
           }
-          for (int u = 0; u < nu; ++u) {
-            mma_commit(tfull + u);
-            ucnt[u]++;
-          }
-          TC_TRACE(1, tr); ++tr;
+          unit_done(u);
+          if (lane == 0) { TC_TRACE(1, tr); } ++tr;
         }
-        kbase += prm.ksteps;
+      } else {
+        for (int ks = 0; ks < prm.ksteps; ++ks) {
+          const uint32_t kidx = kbase + ks;
+          const int s = kidx % prm.nstage;
+          mbar_wait(full_bar + s, (kidx / prm.nstage) & 1);
+          fence_after();
+          for (int u = 0; u < nu; ++u) {
+            if (ks == 0) wait_unit_free(u);
+            issue(prm.units[g][u], s, ks);
+          }
+          if (elect_one()) mma_commit(empty_bar + s);
+          __syncwarp();
+        }
+        for (int u = 0; u < nu; ++u) unit_done(u);
+        if (lane == 0) { TC_TRACE(1, tr); } ++tr;
       }
+      kbase += prm.ksteps;
     }
   } else {
-    // ===== epilogue warps: warp = lane quadrant of TMEM + 4 * column half =====
+    // ===== epilogue warps: warp = lane quadrant of TMEM + 4 * column slice =====
+    // Lane = channel j, TMEM column = channel i.  For a fixed i the 32 lanes of a warp hold 32 consecutive
+    // lexicographic pairs p = rowbase(i) + j, so every store instruction writes two or three full 128-byte
+    // lines of S.  The loop body is branch-free (predicated store) so the 16 elements of a chunk interleave.
     const int q = warp & 3, h = warp >> 2;
     const int C = lay.C, F = lay.F;
     const int pb_mask = lay.PB - 1;
-    uint32_t ucnt[kTcMaxUnits], tr = 0;
-#pragma unroll
-    for (int u = 0; u < kTcMaxUnits; ++u) ucnt[u] = 0;
+    const int blk_stride = F * lay.PB;  // float2 elements between pair blocks
+    uint32_t par = 0, tr = 0;  // per-unit parity of the use count
     for (int item = blockIdx.x; item < nitems; item += gridDim.x) {
       const int f = item / prm.ngroups, g = item % prm.ngroups, nu = prm.nunits[g];
       const int fx = f & pb_mask;
+      float2 *Sf = S + (int64_t)f * lay.PB;
       for (int u = 0; u < nu; ++u) {
         const TcUnit un = prm.units[g][u];
-        mbar_wait(tfull + u, ucnt[u] & 1);
-        ucnt[u]++;
+        mbar_wait(tfull + u, (par >> u) & 1u);
+        par ^= 1u << u;
         fence_after();
         if (warp == 0) { TC_TRACE(2, tr); ++tr; }
         if (32 * q >= un.lane_lo && 32 * q < un.lane_hi) {
-          const int j = un.row0 + 32 * q + lane;
+          const int jw0 = un.row0 + 32 * q, j = jw0 + lane;
           const bool jok = j < C;
-          const float sj = scale * inv_scale[j];
-          const int nhalf = un.N / 2;
+          const float sj = scale * itab[j].y;
+          const int ncols = un.N / kColSplit;
           const uint32_t lane_addr = (uint32_t)(32 * q) << 16;
-          for (int c0 = h * nhalf; c0 < (h + 1) * nhalf; c0 += 16) {
+          for (int c0 = h * ncols; c0 < (h + 1) * ncols; c0 += 16) {
             const int ibase = un.col0 + c0;
-            if (ibase > un.row0 + 32 * q + 31) continue;  // i > j for every lane of this warp
+            if (ibase > jw0 + 31) continue;  // i > j for every lane of this warp
             float re[16], im[16];
             tmem_ld16(tmem_base + lane_addr + (uint32_t)(un.tm + c0), re);
             tmem_ld16(tmem_base + lane_addr + (uint32_t)(un.tm + un.N + c0), im);
             asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+            if (S) {
 #pragma unroll
-            for (int e = 0; e < 16; ++e) {
-              const int i = ibase + e;
-              if (i < j && jok) {
-                if (S) {
-                  // lexicographic pair index p = i C - i(i+1)/2 + (j - i - 1); block-major, slot swizzled by bin
-                  const int p = i * C - (i * (i + 1)) / 2 - i - 1 + j;
-                  const int64_t off = ((int64_t)(p >> lay.pb_shift) * F + f) * lay.PB + ((p ^ fx) & pb_mask);
-                  const float sc = sj * inv_scale[i];
-                  S[off] = make_float2(re[e] * sc, im[e] * sc);
-                }
-              } else if (i == j && jok) {
-                const float a = re[e] * sj * inv_scale[i];
+              for (int e = 0; e < 16; ++e) {
+                const float2 t = itab[ibase + e];          // {rowbase(i) as int bits, 1/scale_i}
+                const int p = __float_as_int(t.x) + j;     // lexicographic pair index of (i, j)
+                const float sc = sj * t.y;
+                const int off = (p >> lay.pb_shift) * blk_stride + ((p ^ fx) & pb_mask);
+                if (ibase + e < j && jok) Sf[off] = make_float2(re[e] * sc, im[e] * sc);
+              }
+            }
+            if (ibase + 15 >= jw0) {  // this chunk crosses the diagonal: autospectrum of channel j
+              float a = 0.f;
+#pragma unroll
+              for (int e = 0; e < 16; ++e) a = (ibase + e == j) ? re[e] : a;
+              if (j >= ibase && j < ibase + 16 && jok) {
+                a *= sj * itab[j].y;
                 if (Sauto) Sauto[(int64_t)j * F + f] = a;
                 if (Srsq) Srsq[(int64_t)j * F + f] = a > 0.f ? rsqrtf(a) : 0.f;
               }
@@ -315,6 +343,7 @@ contract_tc_kernel(const __half *__restrict__ X, Layout lay, TcParams prm, float
 
   fence_before();
   __syncthreads();
+  if (tid == 0) TC_TRACE(3, 2);
   if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(512));
 }
 
@@ -373,7 +402,7 @@ int launch_contract_tc(delta_plan *p, const void *d_X, float *d_S, float *d_auto
   prm.stage_bytes = 4u * prm.plane_bytes;
   prm.plane_elems = (int64_t)lay.Kc * lay.Cp * kSegBlock;
   prm.kstep_elems = (int64_t)2 * lay.Cp * kSegBlock;
-  const size_t fixed = (size_t)lay.Cp * sizeof(float) + 64 * sizeof(uint64_t) + 64;
+  const size_t fixed = (size_t)lay.Cp * sizeof(float2) + 64 * sizeof(uint64_t) + 64;
   int nstage = (int)((200 * 1024 - fixed) / prm.stage_bytes);
   if (nstage > 8) nstage = 8;
   if (nstage < 2) return DELTA_ERR_UNSUPPORTED;
