@@ -144,6 +144,7 @@ contract_tc_kernel(const __half *__restrict__ X, Layout lay, TcParams prm, float
   const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);  // provably warp-uniform
   const int nitems = lay.F * prm.ngroups;
   if (tid == 0) TC_TRACE(3, 0);
+  if (TRACE && tid == 0) { long long g; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g)); trace[5 * 512 + 2 * blockIdx.x] = g; }
 
   for (int c = tid; c < lay.Cp; c += kTcThreads)
     itab[c] = make_float2(__int_as_float(c * lay.C - (c * (c + 1)) / 2 - c - 1), (c < lay.C) ? 1.f / chscale[c] : 0.f);
@@ -172,14 +173,14 @@ contract_tc_kernel(const __half *__restrict__ X, Layout lay, TcParams prm, float
     // ===== producer: stream the four operand planes of every K=16 step =====
     // The whole warp walks the loop (warp-uniform values live in uniform registers, which is what the bulk-copy
     // and MMA instructions take); one elected lane issues.
-    uint32_t kidx = 0;
+    // stage index and use count advance incrementally: no division by the (run-time) stage count in the loop
+    uint32_t s = 0, pass = 0, kidx = 0;  // pass = completed trips around the stage ring
+    int f = blockIdx.x / prm.ngroups, g = blockIdx.x % prm.ngroups;
+    const int fstep = gridDim.x / prm.ngroups, gstep = gridDim.x % prm.ngroups;
     for (int item = blockIdx.x; item < nitems; item += gridDim.x) {
-      const int f = item / prm.ngroups;
       const __half *Xf = X + (int64_t)f * lay.x_elems_per_f;
       for (int ks = 0; ks < prm.ksteps; ++ks, ++kidx) {
-        const int s = kidx % prm.nstage;
-        const uint32_t use = kidx / prm.nstage;
-        if (use > 0) mbar_wait(empty_bar + s, (use - 1) & 1);
+        if (pass) mbar_wait(empty_bar + s, (pass - 1) & 1u);
         if (elect_one()) {
           mbar_expect_tx(full_bar + s, prm.stage_bytes);
           unsigned char *dst = stages + (size_t)s * prm.stage_bytes;
@@ -190,45 +191,46 @@ contract_tc_kernel(const __half *__restrict__ X, Layout lay, TcParams prm, float
           TC_TRACE(0, kidx);
         }
         __syncwarp();
+        if (++s == (uint32_t)prm.nstage) { s = 0; ++pass; }
       }
+      f += fstep; g += gstep;
+      if (g >= prm.ngroups) { g -= prm.ngroups; ++f; }
     }
   } else if (warp == kEpiWarps + 1) {
     // ===== MMA issuer =====
     const uint32_t lbo = (uint32_t)lay.Cp * 16u, sbo = 128u;
-    uint32_t kbase = 0, tr = 0;
+    uint32_t tr = 0;
     uint32_t used = 0, par = 0;  // per-unit bits: unit has been used; parity of its use count
+    // descriptor = dbase + (shared address >> 4): all addresses are 16-byte aligned and below 256 KB
+    const uint64_t dbase = make_sdesc(0, lbo, sbo);
+    const uint32_t st16 = smem_u32(stages) >> 4, stage16 = prm.stage_bytes >> 4, plane16 = prm.plane_bytes >> 4;
 
     // the twelve MMAs of one (unit, K step): Re += A_j A_i + B_j B_i;  Im += A_j B_i - B_j A_i  (rows j, cols i)
-    auto issue = [&](const TcUnit &un, int s, int ks) {
-      const uint32_t sb = smem_u32(stages + (size_t)s * prm.stage_bytes);
-      const uint32_t p_hr = sb, p_hi = sb + prm.plane_bytes, p_lr = sb + 2 * prm.plane_bytes, p_li = sb + 3 * prm.plane_bytes;
-      const uint32_t ao = (uint32_t)(un.row0 / 8) * 128u, bo = (uint32_t)(un.col0 / 8) * 128u;
-      const uint32_t id = make_idesc(un.N, 0), idn = make_idesc(un.N, 1);
-      const uint32_t acc = ks > 0 ? 1u : 0u;
-      const uint32_t d_re = tmem_base + (uint32_t)un.tm, d_im = d_re + (uint32_t)un.N;
-      const uint64_t a_hr = make_sdesc(p_hr + ao, lbo, sbo), a_hi = make_sdesc(p_hi + ao, lbo, sbo);
-      const uint64_t a_lr = make_sdesc(p_lr + ao, lbo, sbo), a_li = make_sdesc(p_li + ao, lbo, sbo);
-      const uint64_t b_hr = make_sdesc(p_hr + bo, lbo, sbo), b_hi = make_sdesc(p_hi + bo, lbo, sbo);
-      const uint64_t b_lr = make_sdesc(p_lr + bo, lbo, sbo), b_li = make_sdesc(p_li + bo, lbo, sbo);
+    auto issue = [&](uint32_t ao16, uint32_t bo16, uint32_t id, uint32_t idn, uint32_t d_re, uint32_t d_im, uint32_t s, uint32_t acc) {
+      const uint64_t sb = dbase + (st16 + s * stage16);
+      const uint64_t a_hr = sb + ao16, a_hi = a_hr + plane16, a_lr = a_hi + plane16, a_li = a_lr + plane16;
+      const uint64_t b_hr = sb + bo16, b_hi = b_hr + plane16, b_lr = b_hi + plane16, b_li = b_lr + plane16;
       if (elect_one()) {
         mma_f16(d_re, a_hr, b_hr, id, acc);
-        mma_f16(d_re, a_hr, b_lr, id, 1u);
-        mma_f16(d_re, a_lr, b_hr, id, 1u);
-        mma_f16(d_re, a_hi, b_hi, id, 1u);
-        mma_f16(d_re, a_hi, b_li, id, 1u);
-        mma_f16(d_re, a_li, b_hi, id, 1u);
         mma_f16(d_im, a_hr, b_hi, id, acc);
+        mma_f16(d_re, a_hr, b_lr, id, 1u);
         mma_f16(d_im, a_hr, b_li, id, 1u);
+        mma_f16(d_re, a_lr, b_hr, id, 1u);
         mma_f16(d_im, a_lr, b_hi, id, 1u);
+        mma_f16(d_re, a_hi, b_hi, id, 1u);
         mma_f16(d_im, a_hi, b_hr, idn, 1u);
+        mma_f16(d_re, a_hi, b_li, id, 1u);
         mma_f16(d_im, a_hi, b_lr, idn, 1u);
+        mma_f16(d_re, a_li, b_hi, id, 1u);
         mma_f16(d_im, a_li, b_hr, idn, 1u);
       }
       __syncwarp();
     };
     auto wait_unit_free = [&](int u) {
-      if ((used >> u) & 1u) mbar_wait(tempty + u, ((par >> u) & 1u) ^ 1u);  // epilogue has drained the previous use
-      fence_after();
+      if ((used >> u) & 1u) {  // epilogue has drained the previous use
+        mbar_wait(tempty + u, ((par >> u) & 1u) ^ 1u);
+        fence_after();
+      }
     };
     auto unit_done = [&](int u) {
       if (elect_one()) mma_commit(tfull + u);
@@ -237,46 +239,57 @@ contract_tc_kernel(const __half *__restrict__ X, Layout lay, TcParams prm, float
       par ^= 1u << u;
     };
 
+    uint32_t s0 = 0, pass0 = 0;  // stage and ring pass of the item's first K step
+    int g = blockIdx.x % prm.ngroups;
+    const int gstep = gridDim.x % prm.ngroups;
     for (int item = blockIdx.x; item < nitems; item += gridDim.x) {
-      const int g = item % prm.ngroups, nu = prm.nunits[g];
+      const int nu = prm.nunits[g];
       if (prm.unit_major) {
         for (int u = 0; u < nu; ++u) {
           const TcUnit un = prm.units[g][u];
+          const uint32_t ao16 = (uint32_t)(un.row0 / 8) * 8u, bo16 = (uint32_t)(un.col0 / 8) * 8u;
+          const uint32_t id = make_idesc(un.N, 0), idn = make_idesc(un.N, 1);
+          const uint32_t d_re = tmem_base + (uint32_t)un.tm, d_im = d_re + (uint32_t)un.N;
           wait_unit_free(u);
+          uint32_t s = s0, pass = pass0;
           for (int ks = 0; ks < prm.ksteps; ++ks) {
-            const uint32_t kidx = kbase + ks;
-            const int s = kidx % prm.nstage;
             if (u == 0) {
-              mbar_wait(full_bar + s, (kidx / prm.nstage) & 1);
+              mbar_wait(full_bar + s, pass & 1u);
               fence_after();
-              if (lane == 0) TC_TRACE(4, kidx);
+              if (lane == 0) TC_TRACE(4, tr);
             }
-            issue(un, s, ks);
+            issue(ao16, bo16, id, idn, d_re, d_im, s, ks > 0 ? 1u : 0u);
             if (u == nu - 1) {  // stage reusable once every unit has read it
               if (elect_one()) mma_commit(empty_bar + s);
               __syncwarp();
             }
+            if (++s == (uint32_t)prm.nstage) { s = 0; ++pass; }
           }
           unit_done(u);
           if (lane == 0) { TC_TRACE(1, tr); } ++tr;
+          if (u == nu - 1) { s0 = s; pass0 = pass; }
         }
       } else {
+        uint32_t s = s0, pass = pass0;
         for (int ks = 0; ks < prm.ksteps; ++ks) {
-          const uint32_t kidx = kbase + ks;
-          const int s = kidx % prm.nstage;
-          mbar_wait(full_bar + s, (kidx / prm.nstage) & 1);
+          mbar_wait(full_bar + s, pass & 1u);
           fence_after();
           for (int u = 0; u < nu; ++u) {
+            const TcUnit un = prm.units[g][u];
             if (ks == 0) wait_unit_free(u);
-            issue(prm.units[g][u], s, ks);
+            issue((uint32_t)(un.row0 / 8) * 8u, (uint32_t)(un.col0 / 8) * 8u, make_idesc(un.N, 0), make_idesc(un.N, 1),
+                  tmem_base + (uint32_t)un.tm, tmem_base + (uint32_t)(un.tm + un.N), s, ks > 0 ? 1u : 0u);
           }
           if (elect_one()) mma_commit(empty_bar + s);
           __syncwarp();
+          if (++s == (uint32_t)prm.nstage) { s = 0; ++pass; }
         }
         for (int u = 0; u < nu; ++u) unit_done(u);
         if (lane == 0) { TC_TRACE(1, tr); } ++tr;
+        s0 = s; pass0 = pass;
       }
-      kbase += prm.ksteps;
+      g += gstep;
+      if (g >= prm.ngroups) g -= prm.ngroups;
     }
   } else {
     // ===== epilogue warps: warp = lane quadrant of TMEM + 4 * column slice =====
@@ -288,8 +301,10 @@ contract_tc_kernel(const __half *__restrict__ X, Layout lay, TcParams prm, float
     const int pb_mask = lay.PB - 1;
     const int blk_stride = F * lay.PB;  // float2 elements between pair blocks
     uint32_t par = 0, tr = 0;  // per-unit parity of the use count
-    for (int item = blockIdx.x; item < nitems; item += gridDim.x) {
-      const int f = item / prm.ngroups, g = item % prm.ngroups, nu = prm.nunits[g];
+    int f = blockIdx.x / prm.ngroups, g = blockIdx.x % prm.ngroups;
+    const int fstep = gridDim.x / prm.ngroups, gstep = gridDim.x % prm.ngroups;
+    for (int item = blockIdx.x; item < nitems; item += gridDim.x, f += fstep + (g + gstep >= prm.ngroups), g = (g + gstep) % prm.ngroups) {
+      const int nu = prm.nunits[g];
       const int fx = f & pb_mask;
       float2 *Sf = S + (int64_t)f * lay.PB;
       for (int u = 0; u < nu; ++u) {
@@ -344,6 +359,7 @@ contract_tc_kernel(const __half *__restrict__ X, Layout lay, TcParams prm, float
   fence_before();
   __syncthreads();
   if (tid == 0) TC_TRACE(3, 2);
+  if (TRACE && tid == 0) { long long g; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g)); trace[5 * 512 + 2 * blockIdx.x + 1] = g; }
   if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(512));
 }
 
