@@ -42,6 +42,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
         return LIB
     cmd = [nvcc_path(), *ARCH, "-O3", "-std=c++17", "-lineinfo", "-shared", "-Xcompiler", "-fPIC",
            "-I", os.path.join(ROOT, "include"), "-I", CSRC, "-o", LIB, *sources()]
+    cmd[1:1] = os.environ.get("DELTA_NVCC_FLAGS", "").split()  # tuning experiments only (e.g. -DDELTA_PAIR_WARPS=32)
     if verbose:
         cmd.insert(1, "-Xptxas=-v")
         print(" ".join(cmd))

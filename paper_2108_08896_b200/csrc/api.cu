@@ -73,7 +73,9 @@ int delta_plan_create(const delta_config *cfg, delta_plan **out) {
   l.K = (l.T - l.L) / l.H + 1;
   l.Kp = (int)align_up((size_t)l.K, 16);
   l.Kc = l.Kp / kSegBlock;
+  l.nkb = (l.K + kSegBlock - 1) / kSegBlock;
   l.F = l.L / 2 + 1;
+  l.Fp = (l.F + 3) & ~3;
   l.M = cfg->max_lag;
   l.nlags = 2 * l.M + 1;
   l.P = (int64_t)l.C * (l.C - 1) / 2;
@@ -98,6 +100,15 @@ int delta_plan_create(const delta_config *cfg, delta_plan **out) {
   }
   p->h_ftab.resize((size_t)fft_table_size(l.N) + 1);
   fft_twiddle_table(l.N, p->h_ftab.data());
+  {
+    const int E = l.N <= 64 ? 8 : 16;  // FftGeom<N>::E
+    const int Tg = l.N / E;
+    for (int u = 0; u < 16; ++u) {
+      const long long e = ((long long)Tg * u) % L;
+      const double ang = -2.0 * M_PI * (double)e / (double)L;
+      p->h_wstep[u] = make_float2((float)std::cos(ang), (float)std::sin(ang));
+    }
+  }
   switch (cfg->scaling) {
     case DELTA_SCALE_WINPOW: p->s2 = (float)(1.0 / sw2); break;
     case DELTA_SCALE_NONE: p->s2 = 1.f; break;
@@ -123,7 +134,9 @@ int delta_plan_create(const delta_config *cfg, delta_plan **out) {
   w.off_X = take((size_t)l.F * l.x_elems_per_f * (p->contraction == DELTA_CONTRACT_TC ? 2 : 4));
   w.off_S = take((size_t)(l.Pblk > 0 ? l.Pblk : 1) * l.F * l.PB * sizeof(float2));
   w.off_auto = take((size_t)l.C * l.F * sizeof(float));
-  w.off_rsq = take((size_t)l.C * l.F * sizeof(float));
+  w.off_rsq = take((size_t)l.C * l.Fp * sizeof(float));
+  w.off_wpart = take((size_t)l.C * l.nkb * sizeof(float));
+  w.off_rsum = take((size_t)l.C * sizeof(float));
   w.total = o;
   *out = p;
   return DELTA_OK;
@@ -270,10 +283,10 @@ static int pair_stage(delta_plan *p, const float *d_S, const float *d_Sauto, flo
   if (!aligned16(d_S)) return DELTA_ERR_ALIGNMENT;
   cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
   if (need_auto) {  // coherence and rho need 1/sqrt(S_cc[f]) of the caller's autospectra
-    rc = launch_auto_prep(p, d_Sauto, p->d_rsq(), st);
+    rc = launch_auto_prep(p, d_Sauto, p->d_rsq(), p->d_rsum(), st);
     if (rc) return rc;
   }
-  return launch_pair(p, d_S, d_Sauto, p->d_rsq(), G, A, P, R, st);
+  return launch_pair(p, d_S, p->d_rsq(), p->d_rsum(), 1, 1, 1.f, G, A, P, R, st);
 }
 
 int delta_coherence(delta_plan *p, const float *d_S, const float *d_Sauto, float *d_G, void *stream) {
@@ -311,7 +324,10 @@ int delta_analyze_chunk(delta_plan *p, const void *d_x, int64_t ld, float *d_G, 
   rc = contract(p, p->d_X(), pairs_wanted ? p->d_S() : nullptr, au, st);
   if (rc) return rc;
   if (ev) DELTA_CUDA_CHECK(cudaEventRecord(p->stage_ev[2], st));
-  if (pairs_wanted) rc = launch_pair(p, p->d_S(), au, p->d_rsq(), d_G, d_A, d_P, d_R, st);
+  // zero-lag autocorrelations for rho come from the windowed signal energy the STFT kernel left in wpart (Parseval)
+  if (pairs_wanted)
+    rc = launch_pair(p, p->d_S(), p->d_rsq(), p->d_wpart(), p->lay.nkb, p->lay.nkb, (float)p->lay.L * p->s2 / (float)p->lay.K,
+                     d_G, d_A, d_P, d_R, st);
   if (rc) return rc;
   if (ev) DELTA_CUDA_CHECK(cudaEventRecord(p->stage_ev[3], st));
   return rc;

@@ -82,7 +82,7 @@ contract_fp32_kernel(const float *__restrict__ X, Layout lay, float scale, float
       } else if (i == j) {
         const float v = acc_re[a][b] * scale;
         if (Sauto) Sauto[(int64_t)i * lay.F + f] = v;
-        if (Srsq) Srsq[(int64_t)i * lay.F + f] = v > 0.f ? rsqrtf(v) : 0.f;
+        if (Srsq) Srsq[(int64_t)i * lay.Fp + f] = v > 0.f ? rsqrtf(v) : 0.f;
       }
     }
   }

@@ -343,7 +343,7 @@ contract_tc_kernel(const __half *__restrict__ X, Layout lay, TcParams prm, float
               if (j >= ibase && j < ibase + 16 && jok) {
                 a *= sj * itab[j].y;
                 if (Sauto) Sauto[(int64_t)j * F + f] = a;
-                if (Srsq) Srsq[(int64_t)j * F + f] = a > 0.f ? rsqrtf(a) : 0.f;
+                if (Srsq) Srsq[(int64_t)j * lay.Fp + f] = a > 0.f ? rsqrtf(a) : 0.f;
               }
             }
           }

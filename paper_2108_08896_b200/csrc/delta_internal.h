@@ -32,6 +32,8 @@ struct Layout {
   //   TC   mode : __half X[f][prec][part][kc][c][8]           prec 0 = hi, 1 = lo (split fp16)
   // k = 8*kc + kk, c < Cp (rows C..Cp-1 are zero), kc < Kc = Kp/8, Kp = K rounded up to 16.
   int C, Cp, T, L, N, H, K, Kp, Kc, F, M, nlags;
+  int Fp;   // row pitch of the rsq table: F rounded up to 4 floats (rows are 16-byte aligned bulk-copy sources)
+  int nkb;  // segment blocks per channel = ceil(K / 8): one partial of the windowed signal energy each (wpart)
   // S (cross-spectra) is complex64 [Pblk][F][PB]: pairs in lexicographic order p = iC - i(i+1)/2 + (j-i-1),
   // block = p / PB, and inside row f of a block pair p sits in slot (p ^ f) & (PB-1).  One block is one
   // contiguous tile for the pair kernel; the XOR makes its column (fixed pair) reads bank-conflict free.
@@ -41,7 +43,7 @@ struct Layout {
 };
 
 struct Workspace {
-  size_t off_tw, off_win, off_ftab, off_pairs, off_offs, off_isum, off_chscale, off_X, off_S, off_auto, off_rsq, total;
+  size_t off_tw, off_win, off_ftab, off_pairs, off_offs, off_isum, off_chscale, off_X, off_S, off_auto, off_rsq, off_wpart, off_rsum, total;
 };
 
 }  // namespace delta
@@ -55,6 +57,7 @@ struct delta_plan {
   // host tables (uploaded by delta_plan_set_workspace)
   std::vector<float2> h_tw;      // e^{-2 pi i f / L}, f = 0..L-1
   std::vector<float> h_win;      // periodic Hann
+  float2 h_wstep[16];            // e^{-2 pi i T u / L}, u < E: bin f = gt + T u of a thread has twiddle tw[gt] * wstep[u]
   std::vector<float2> h_ftab;    // per-pass twiddles of the register FFT (fft_reg.cuh), N = L/2
   std::vector<ushort2> h_pairs;  // (i, j) of pair p, lexicographic
   delta::TcHostPlan tc;
@@ -85,6 +88,11 @@ struct delta_plan {
   float *d_S() const { return reinterpret_cast<float *>(ws + wsl.off_S); }
   float *d_auto() const { return reinterpret_cast<float *>(ws + wsl.off_auto); }
   float *d_rsq() const { return reinterpret_cast<float *>(ws + wsl.off_rsq); }
+  // wpart[c][kb] = sum over the 8 segments of block kb of sum_n (w[n] y_c[kH+n])^2  (written by stft_kernel);
+  // by Parseval  sum over all L bins of S_cc = L s^2/K * sum_kb wpart[c][kb] = L R_cc[0]   (pin P4)
+  float *d_wpart() const { return reinterpret_cast<float *>(ws + wsl.off_wpart); }
+  // rsum[c] = sum over all L bins of caller-supplied autospectra (staged calls; auto_prep_kernel)
+  float *d_rsum() const { return reinterpret_cast<float *>(ws + wsl.off_rsum); }
 };
 
 namespace delta {
@@ -132,9 +140,10 @@ int launch_stft_unpack(delta_plan *p, const void *d_X, float *d_out, cudaStream_
 // both contractions write S (may be null), the autospectra and 1/sqrt(autospectra) (either may be null)
 int launch_contract_fp32(delta_plan *p, const void *d_X, float *d_S, float *d_auto, float *d_rsq, cudaStream_t st);
 int launch_contract_tc(delta_plan *p, const void *d_X, float *d_S, float *d_auto, float *d_rsq, cudaStream_t st);
-int launch_auto_prep(delta_plan *p, const float *d_auto, float *d_rsq, cudaStream_t st);
-int launch_pair(delta_plan *p, const float *d_S, const float *d_auto, const float *d_rsq, float *d_G, float *d_A,
-                float *d_P, float *d_R, cudaStream_t st);
+int launch_auto_prep(delta_plan *p, const float *d_auto, float *d_rsq, float *d_rsum, cudaStream_t st);
+// rpart/nrp/rp_stride/rscale: sum over all L bins of S_cc = rscale * sum_{k<nrp} rpart[c * rp_stride + k]
+int launch_pair(delta_plan *p, const float *d_S, const float *d_rsq, const float *rpart, int nrp, int rp_stride, float rscale,
+                float *d_G, float *d_A, float *d_P, float *d_R, cudaStream_t st);
 int launch_s_unpack(delta_plan *p, const float *d_S, float *d_out, cudaStream_t st);
 
 }  // namespace delta

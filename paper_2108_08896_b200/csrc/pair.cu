@@ -5,11 +5,12 @@
 //   s_unpack_kernel   test accessor: S layout -> complex64 [P][F]
 //
 // One CTA owns one block of PB consecutive (lexicographic) pairs, i.e. one contiguous [F][PB] tile of S and one
-// contiguous run of rows in each output array.  The tile arrives with a single cp.async.bulk copy.  Phase A
-// sweeps it with lanes along frequency (coalesced 128-byte stores of G, A, P).  Phase B gives every pair a
-// group of T = N/E threads which form the half-length complex input of the inverse real transform in
-// registers, run the register FFT of fft_reg.cuh using the pair's own (now dead) tile slots as exchange
-// space, leave the 2N real lags there and sweep them out with lanes along the lag (coalesced stores of rho).
+// contiguous run of rows in each output array.  The tile arrives with a single cp.async.bulk copy.  Every pair
+// has a group of T = N/E threads; thread gt of the group owns the bins f = gt + T u (u < E), which is exactly the
+// register layout the inverse FFT of fft_reg.cuh starts from.  Each S value is therefore read from shared memory
+// once for G, A, P (stored straight away, 16 lanes = 64 contiguous bytes per row) and for the merge step of the
+// inverse real transform; the transform exchanges through a private padded buffer that aliases the (by then
+// dead) tile, ends in registers in natural order, and rho is stored from registers as float2.
 #include "delta_internal.h"
 #include "fft_reg.cuh"
 
@@ -19,6 +20,10 @@ namespace {
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
+struct PairConsts {
+  float2 wstep[16];  // e^{-2 pi i T u / L}
+};
+
 template <int L>
 struct PairCfg {
   static constexpr int N = L / 2, F = N + 1;
@@ -26,24 +31,19 @@ struct PairCfg {
   static constexpr int T = G::T, E = G::E;
   static constexpr int PB = pair_block(L);
   static constexpr int THREADS = PB * T;
-  static constexpr int SW = T < 32 ? 32 : T;  // threads that sweep one pair's row together
-  static constexpr int PU = SW / T;           // pairs per sweep unit
+#ifndef DELTA_PAIR_WARPS
+#define DELTA_PAIR_WARPS 32  // resident warps per SM the register budget is sized for
+#endif
+  static constexpr int MIN_CTAS = (DELTA_PAIR_WARPS * 32) / THREADS > 0 ? (DELTA_PAIR_WARPS * 32) / THREADS : 1;
   static constexpr size_t TILE_BYTES = (size_t)F * PB * sizeof(float2);
-  static constexpr size_t SMEM = TILE_BYTES + 2 * PB * sizeof(float) + PB * sizeof(ushort2) + 16;
+  static constexpr size_t EXCH_BYTES = (size_t)PB * G::BUF * sizeof(float2);
+  static constexpr size_t BUF_BYTES = ((TILE_BYTES > EXCH_BYTES ? TILE_BYTES : EXCH_BYTES) + 15) & ~(size_t)15;
+  static constexpr int FP = (F + 3) & ~3;                                   // pitch of the rsq table
+  static constexpr size_t ROWS_BYTES = (size_t)PB * FP * sizeof(float);     // 1/sqrt(S_jj) row of every pair's j
+  static constexpr size_t SMEM = BUF_BYTES + ROWS_BYTES + 2 * PB * sizeof(float) + PB * sizeof(ushort2) + 16;
   static_assert(THREADS % 32 == 0 && THREADS <= 1024, "block shape");
   static_assert(TILE_BYTES % 16 == 0, "bulk copy size");
-};
-
-// exchange space of the register FFT = the tile slots of pair `pl` (one per row), rows permuted so that the
-// strided accesses of the passes spread over the banks
-template <int PB>
-struct TileMap {
-  float2 *tile;
-  int pl;
-  __device__ __forceinline__ float2 &operator()(int e) const {
-    const int r = e ^ ((e >> 4) & 15);
-    return tile[r * PB + ((pl ^ r) & (PB - 1))];
-  }
+  static_assert((T & (T - 1)) == 0 && (PB & (PB - 1)) == 0, "powers of two");
 };
 
 // atan2 from a degree-13 odd minimax polynomial on [0, 1] (max error 3.2e-7 rad), octant folding
@@ -82,51 +82,62 @@ __device__ __forceinline__ float2 irfft_merge(float2 sf, float2 sr, float2 w_con
   return make_float2(e.x - wd.y, e.y + wd.x);  // e + i * (w d)
 }
 
-template <int W>
-__device__ __forceinline__ void unit_sync() {
-  if (W <= 32) __syncwarp(); else __syncthreads();
-}
-
 }  // namespace
 
-template <int L>
-__global__ void __launch_bounds__(PairCfg<L>::THREADS)
-pair_kernel(const float2 *__restrict__ S, const float *__restrict__ Sauto, const float *__restrict__ Srsq,
-            const ushort2 *__restrict__ pairs, const float2 *__restrict__ tw, const float2 *__restrict__ ftab,
-            Layout lay, float *__restrict__ G, float *__restrict__ A, float *__restrict__ Pw, float *__restrict__ R) {
+// FULL: max_lag == L/2 (every lag of the circular correlation is stored; the two end points are the same sample)
+// Zero-lag autocorrelations (R12): sum over all L bins of S_cc = rscale * sum_{k<nrp} rpart[c rp_stride + k].
+template <int L, bool FULL>
+__global__ void __launch_bounds__(PairCfg<L>::THREADS, PairCfg<L>::MIN_CTAS)
+pair_kernel(const float2 *__restrict__ S, const float *__restrict__ Srsq, const float *__restrict__ rpart, int nrp,
+            int rp_stride, float rscale, const ushort2 *__restrict__ pairs, const float2 *__restrict__ tw,
+            const float2 *__restrict__ ftab, Layout lay, PairConsts pc, float *__restrict__ G_, float *__restrict__ A_,
+            float *__restrict__ Pw_, float *__restrict__ R_) {
   using Cfg = PairCfg<L>;
-  constexpr int N = Cfg::N, F = Cfg::F, T = Cfg::T, E = Cfg::E, PB = Cfg::PB, SW = Cfg::SW, PU = Cfg::PU;
-  constexpr int THREADS = Cfg::THREADS, NW = THREADS / 32;
+  using Geo = typename Cfg::G;
+  constexpr int N = Cfg::N, F = Cfg::F, T = Cfg::T, E = Cfg::E, PB = Cfg::PB;
+  constexpr int THREADS = Cfg::THREADS;
   extern __shared__ __align__(128) unsigned char smem_raw[];
-  float2 *tile = reinterpret_cast<float2 *>(smem_raw);                        // [F][PB], slot = (pl ^ f) & (PB-1)
-  float *rs = reinterpret_cast<float *>(smem_raw + Cfg::TILE_BYTES);          // [PB][2]: 1/sqrt(L R_cc[0]) of i, j
-  ushort2 *ij_s = reinterpret_cast<ushort2 *>(rs + 2 * PB);                   // [PB]
-  uint64_t *bar = reinterpret_cast<uint64_t *>(smem_raw + ((Cfg::TILE_BYTES + 2 * PB * sizeof(float) + PB * sizeof(ushort2) + 7) & ~(size_t)7));
+  float2 *tile = reinterpret_cast<float2 *>(smem_raw);                     // [F][PB], slot = (pl ^ f) & (PB-1)
+  float2 *exch = reinterpret_cast<float2 *>(smem_raw);                     // [PB][BUF] once the tile is dead
+  float *rowj = reinterpret_cast<float *>(smem_raw + Cfg::BUF_BYTES);      // [PB][FP]: 1/sqrt(S_jj[f]) of pair pl's j
+  float *rs = reinterpret_cast<float *>(smem_raw + Cfg::BUF_BYTES + Cfg::ROWS_BYTES);  // [2][PB]: 1/sqrt(L R_cc[0]) of i, j
+  ushort2 *ij_s = reinterpret_cast<ushort2 *>(rs + 2 * PB);                // [PB]
+  uint64_t *bar = reinterpret_cast<uint64_t *>(smem_raw + ((Cfg::BUF_BYTES + Cfg::ROWS_BYTES + 2 * PB * sizeof(float) + PB * sizeof(ushort2) + 7) & ~(size_t)7));
 
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  float *const G = G_, *const A = A_, *const Pw = Pw_, *const R = R_;
+  const bool wantG = G, wantR = R;
+  const int tid = threadIdx.x;
   const int64_t p0 = (int64_t)blockIdx.x * PB;
 
   if (tid == 0) {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(1));
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"((uint32_t)Cfg::TILE_BYTES) : "memory");
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)),
+                 "r"((uint32_t)(Cfg::TILE_BYTES + (wantG ? Cfg::ROWS_BYTES : 0))) : "memory");
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(tile)),
                  "l"(S + (int64_t)blockIdx.x * F * PB), "r"((uint32_t)Cfg::TILE_BYTES), "r"(smem_u32(bar))
                  : "memory");
   }
-  if (tid < PB) ij_s[tid] = (p0 + tid < lay.P) ? pairs[p0 + tid] : make_ushort2(0, 0);
+  if (tid < PB) {
+    const ushort2 ij = (p0 + tid < lay.P) ? pairs[p0 + tid] : make_ushort2(0, 0);
+    ij_s[tid] = ij;
+  }
   __syncthreads();
+  if (tid < PB && wantG) {  // this pair's 1/sqrt(S_jj) row (the expect_tx above is ordered before these copies by the barrier)
+    const ushort2 ij = ij_s[tid];
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(rowj + tid * Cfg::FP)),
+                 "l"(Srsq + (int64_t)ij.y * Cfg::FP), "r"((uint32_t)(Cfg::FP * sizeof(float))), "r"(smem_u32(bar))
+                 : "memory");
+  }
 
-  // R_cc[0] = (1/L) sum over all L bins of S_cc = (1/L) (S_cc[0] + 2 sum_{0<f<N} S_cc[f] + S_cc[N])
-  if (R) {
-    for (int idx = warp; idx < 2 * PB; idx += NW) {
-      const ushort2 ij = ij_s[idx >> 1];
-      const float *a = Sauto + (int64_t)((idx & 1) ? ij.y : ij.x) * F;
-      float sum = 0.f;
-      for (int f = lane; f < F; f += 32) sum = fmaf((f == 0 || f == N) ? 1.f : 2.f, __ldg(a + f), sum);
-      for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
-      if (lane == 0) rs[idx] = sum > 0.f ? rsqrtf(sum) : 0.f;
-    }
+  // rs[role][pl] = 1/sqrt(sum over all L bins of S_cc) = 1/sqrt(L R_cc[0]),  c = i (role 0) or j (role 1) of pair pl
+  if (R && tid < 2 * PB) {
+    const ushort2 ij = ij_s[tid % PB];
+    const float *a = rpart + (int64_t)(tid / PB ? ij.y : ij.x) * rp_stride;
+    float sum = 0.f;
+    for (int k = 0; k < nrp; ++k) sum += __ldg(a + k);
+    sum *= rscale;
+    rs[tid] = sum > 0.f ? rsqrtf(sum) : 0.f;
   }
   __syncthreads();
 
@@ -137,87 +148,116 @@ pair_kernel(const float2 *__restrict__ S, const float *__restrict__ Sauto, const
                    : "=r"(ok) : "r"(smem_u32(bar)), "r"(0) : "memory");
   }
 
-  const int unit = tid / SW, lu = tid % SW;
+  const int pl = tid / T, gt = tid % T;
+  const int64_t p = p0 + pl;
+  const bool valid = p < lay.P;
+  const ushort2 ij = ij_s[pl];
+  const bool gap = (G || A || Pw) && valid;
+  const float *ri = Srsq + (int64_t)ij.x * Cfg::FP, *rj = rowj + pl * Cfg::FP;
+  const float2 wg = __ldg(tw + gt);  // e^{-2 pi i gt / L}
+  const int64_t o = p * F;
 
-  // ---- phase A: G, A, P for bins 0..N-1, lanes along frequency --------------------------------
-  if (G || A || Pw) {
-#pragma unroll 1
-    for (int pi = 0; pi < PU; ++pi) {
-      const int pl = unit * PU + pi;
-      const int64_t p = p0 + pl;
-      if (p >= lay.P) continue;
-      const ushort2 ij = ij_s[pl];
-      const float *ri = Srsq + (int64_t)ij.x * F, *rj = Srsq + (int64_t)ij.y * F;
-      const int64_t o = p * F;
-#pragma unroll 4
-      for (int f = lu; f < N; f += SW) {
-        const float2 s = tile[f * PB + ((pl ^ f) & (PB - 1))];
-        const float mag = sqrt_approx(fmaf(s.x, s.x, s.y * s.y));
-        if (Pw) Pw[o + f] = mag;
-        if (G) G[o + f] = mag * __ldg(ri + f) * __ldg(rj + f);
-        if (A) A[o + f] = atan2_poly(s.y, s.x);
+  // ---- G, A, P of the thread's bins, and the merge step of the inverse real transform --------------------
+  // Loads of a batch of UB bins are issued together so that their latencies overlap.
+  auto emit = [&](float2 s, float gi, float gj, int f) {
+    const float mag = sqrt_approx(fmaf(s.x, s.x, s.y * s.y));
+    if (Pw) Pw[o + f] = mag;
+    if (G) G[o + f] = mag * gi * gj;
+    if (A) A[o + f] = atan2_poly(s.y, s.x);
+  };
+  float2 v[E];
+  const int pg = pl ^ gt;
+  #ifndef DELTA_PAIR_UB
+#define DELTA_PAIR_UB 4
+#endif
+  constexpr int UB = DELTA_PAIR_UB < E ? DELTA_PAIR_UB : E;
+#pragma unroll
+  for (int ub = 0; ub < E; ub += UB) {
+    float2 sf[UB], sr[UB], w[UB];
+    float gi[UB], gj[UB];
+#pragma unroll
+    for (int k = 0; k < UB; ++k) {
+      const int u = ub + k;
+      const int f = gt + T * u;  // gt < T and T is a power of two, so f = gt | T u
+      const int fr = N - f;
+      sf[k] = tile[f * PB + ((pg ^ (T * u)) & (PB - 1))];
+      sr[k] = tile[fr * PB + ((pl ^ fr) & (PB - 1))];
+      gi[k] = wantG ? __ldg(ri + f) : 0.f;
+      gj[k] = wantG ? rj[f] : 0.f;
+      w[k] = cmul(wg, pc.wstep[u]);  // e^{-2 pi i f / L}
+    }
+#pragma unroll
+    for (int k = 0; k < UB; ++k) {
+      const int u = ub + k;
+      const int f = gt + T * u;
+      if (gap) {
+        emit(sf[k], gi[k], gj[k], f);
+        if (u == 0 && gt == 0) emit(sr[k], wantG ? __ldg(ri + N) : 0.f, wantG ? rj[N] : 0.f, N);  // the Nyquist bin
+      }
+      if (wantR) {
+        if (u == 0 && gt == 0) { sf[k].y = 0.f; sr[k].y = 0.f; }  // Im S[0], Im S[N] do not enter the real transform
+        v[u] = irfft_merge(sf[k], sr[k], make_float2(w[k].x, -w[k].y));  // e^{+2 pi i f / L}
       }
     }
+    asm volatile("" ::: "memory");  // keep the next batch's loads from being hoisted (register pressure)
   }
-  // Nyquist bin (row N is never used as exchange space, so it can be done by one thread per pair)
-  if (tid < PB && p0 + tid < lay.P && (G || A || Pw)) {
-    const int pl = tid;
-    const ushort2 ij = ij_s[pl];
-    const float2 s = tile[N * PB + ((pl ^ N) & (PB - 1))];
-    const float mag = sqrt_approx(fmaf(s.x, s.x, s.y * s.y));
-    const int64_t o = (p0 + pl) * F + N;
-    if (Pw) Pw[o] = mag;
-    if (G) G[o] = mag * __ldg(Srsq + (int64_t)ij.x * F + N) * __ldg(Srsq + (int64_t)ij.y * F + N);
-    if (A) A[o] = atan2_poly(s.y, s.x);
-  }
-  if (!R) return;
-  unit_sync<SW>();
+  if (!wantR) return;
+  __syncthreads();  // every S value is in registers: the tile becomes exchange space
 
-  // ---- phase B: rho = irfft(S) / sqrt(R_ii[0] R_jj[0]) -------------------------------------------
-  {
-    const int pl = tid / T, gt = tid % T;
-    const TileMap<PB> map{tile, pl};
-    float2 v[E];
+  // ---- rho = irfft(S) / sqrt(R_ii[0] R_jj[0]) ----------------------------------------------------------------
+  fft_inplace<N, true>(v, FftPadMap{exch + pl * Geo::BUF}, ftab, gt);  // z[n] = (x[2n], x[2n+1]) * N, n = gt + T u
+  if (!valid) return;
+  int ki = pl, kj = pl;  // entries that hold the sums of this pair's channels
+  while (ki > 0 && ij_s[ki - 1].x == ij.x) --ki;
+  while (kj > 0 && ij_s[kj - 1].y == ij.y) --kj;
+  // rho = x / sqrt(R_ii[0] R_jj[0]),  x = z/N,  R_cc[0] = (sum over all L bins of S_cc)/L
+  const float norm = 2.f * rs[ki] * rs[PB + kj];
+  float *Rp = R + p * lay.nlags;
+  if (FULL) {
+    // lag m = xi for xi <= L/2 and xi - L for xi >= L/2; row position q = m + L/2
+    const bool vec = (reinterpret_cast<uintptr_t>(Rp) & 7) == 0;  // q is even: float2 stores iff the row is 8-byte aligned
 #pragma unroll
     for (int u = 0; u < E; ++u) {
-      const int f = gt + T * u;
-      float2 sf = tile[f * PB + ((pl ^ f) & (PB - 1))];
-      float2 sr = tile[(N - f) * PB + ((pl ^ (N - f)) & (PB - 1))];
-      if (f == 0) { sf.y = 0.f; sr.y = 0.f; }
-      float2 w = __ldg(tw + f);
-      w.y = -w.y;  // e^{+2 pi i f / L}
-      v[u] = irfft_merge(sf, sr, w);
+      const int n = gt + T * u;
+      const float a = v[u].x * norm, b = v[u].y * norm;
+      const int q = (u < E / 2) ? 2 * n + N : 2 * n - N;
+      if (vec) {
+        *reinterpret_cast<float2 *>(Rp + q) = make_float2(a, b);
+      } else {
+        Rp[q] = a;
+        Rp[q + 1] = b;
+      }
+      if (u == E / 2 && gt == 0) Rp[L] = a;  // xi = L/2 is lag -L/2 and lag +L/2
     }
-    fft_group_sync<T>();  // every S value of the pair is in registers before its slots become exchange space
-    fft_inplace<N, true>(v, map, ftab, gt);
-    fft_group_sync<T>();
+  } else {
+    const int M = lay.M;
 #pragma unroll
-    for (int u = 0; u < E; ++u) map(gt + T * u) = v[u];  // z[n] = (x[2n], x[2n+1]) * N, natural order
-  }
-  unit_sync<SW>();
-#pragma unroll 1
-  for (int pi = 0; pi < PU; ++pi) {
-    const int pl = unit * PU + pi;
-    const int64_t p = p0 + pl;
-    if (p >= lay.P) continue;
-    const TileMap<PB> map{tile, pl};
-    // rho = x / sqrt(R_ii[0] R_jj[0]),  x = z/N,  R_cc[0] = (sum over all L bins of S_cc)/L
-    const float norm = 2.f * rs[2 * pl] * rs[2 * pl + 1];
-    float *Rp = R + p * lay.nlags;
-    for (int q = lu; q < lay.nlags; q += SW) {
-      const int xi = (q - lay.M) & (L - 1);
-      Rp[q] = reinterpret_cast<const float *>(&map(xi >> 1))[xi & 1] * norm;
+    for (int u = 0; u < E; ++u) {
+      const int n = gt + T * u;
+#pragma unroll
+      for (int h = 0; h < 2; ++h) {
+        const int xi = 2 * n + h;
+        const float val = (h ? v[u].y : v[u].x) * norm;
+        if (xi <= M) Rp[xi + M] = val;
+        if (xi >= L - M) Rp[xi - L + M] = val;
+      }
     }
   }
 }
 
-// rsq[c][f] = 1/sqrt(S_cc[f]) (0 where S_cc[f] <= 0, reading R16)
-__global__ void __launch_bounds__(256) auto_prep_kernel(const float *__restrict__ Sauto, float *__restrict__ rsq, int64_t n) {
-  const int64_t idx = (int64_t)blockIdx.x * 256 + threadIdx.x;
-  if (idx < n) {
-    const float a = Sauto[idx];
-    rsq[idx] = a > 0.f ? rsqrtf(a) : 0.f;
+// rsq[c][f] = 1/sqrt(S_cc[f]) (0 where S_cc[f] <= 0, reading R16) and
+// rsum[c] = S_cc[0] + 2 sum_{0<f<N} S_cc[f] + S_cc[N] = sum over all L bins = L R_cc[0].  One warp per channel.
+__global__ void __launch_bounds__(32) auto_prep_kernel(const float *__restrict__ Sauto, float *__restrict__ rsq,
+                                                       float *__restrict__ rsum, int F, int Fp) {
+  const int c = blockIdx.x, lane = threadIdx.x;
+  float sum = 0.f;
+  for (int f = lane; f < F; f += 32) {
+    const float a = Sauto[(int64_t)c * F + f];
+    rsq[(int64_t)c * Fp + f] = a > 0.f ? rsqrtf(a) : 0.f;
+    sum = fmaf((f == 0 || f == F - 1) ? 1.f : 2.f, a, sum);
   }
+  for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
+  if (lane == 0) rsum[c] = sum;
 }
 
 // test accessor: S layout -> complex64 [P][F], lexicographic pairs
@@ -232,31 +272,39 @@ __global__ void __launch_bounds__(256) s_unpack_kernel(const float2 *__restrict_
 
 // ------------------------------------------------------------------------------------------
 template <int L>
-static int launch_pair_L(delta_plan *p, const float *d_S, const float *d_auto, const float *d_rsq, float *d_G, float *d_A,
-                         float *d_P, float *d_R, cudaStream_t st) {
+static int launch_pair_L(delta_plan *p, const float *d_S, const float *d_rsq, const float *rpart, int nrp, int rp_stride,
+                         float rscale, float *d_G, float *d_A, float *d_P, float *d_R, cudaStream_t st) {
   using Cfg = PairCfg<L>;
   const Layout &lay = p->lay;
   if (lay.Pblk == 0 || lay.P == 0) return DELTA_OK;
-  int rc = opt_in_smem(pair_kernel<L>, Cfg::SMEM);
-  if (rc) return rc;
-  pair_kernel<L><<<(unsigned)lay.Pblk, Cfg::THREADS, Cfg::SMEM, st>>>(reinterpret_cast<const float2 *>(d_S), d_auto, d_rsq,
-                                                                    p->d_pairs(), p->d_tw(), p->d_ftab(), lay, d_G, d_A, d_P,
-                                                                    d_R);
+  PairConsts pc;
+  for (int u = 0; u < 16; ++u) pc.wstep[u] = p->h_wstep[u];
+  const bool full = lay.M == L / 2;
+#define DELTA_PAIR_LAUNCH(FULL_)                                                                                    \
+  do {                                                                                                              \
+    int rc = opt_in_smem(pair_kernel<L, FULL_>, Cfg::SMEM);                                                         \
+    if (rc) return rc;                                                                                              \
+    pair_kernel<L, FULL_><<<(unsigned)lay.Pblk, Cfg::THREADS, Cfg::SMEM, st>>>(                                     \
+        reinterpret_cast<const float2 *>(d_S), d_rsq, rpart, nrp, rp_stride, rscale, p->d_pairs(), p->d_tw(),       \
+        p->d_ftab(), lay, pc, d_G, d_A, d_P, d_R);                                                                  \
+  } while (0)
+  if (full) DELTA_PAIR_LAUNCH(true);
+  else DELTA_PAIR_LAUNCH(false);
+#undef DELTA_PAIR_LAUNCH
   p->launches++;
   DELTA_CUDA_CHECK(cudaGetLastError());
   return DELTA_OK;
 }
 
-int launch_pair(delta_plan *p, const float *d_S, const float *d_auto, const float *d_rsq, float *d_G, float *d_A, float *d_P,
-                float *d_R, cudaStream_t st) {
-#define CALL(LL) launch_pair_L<LL>(p, d_S, d_auto, d_rsq, d_G, d_A, d_P, d_R, st)
+int launch_pair(delta_plan *p, const float *d_S, const float *d_rsq, const float *rpart, int nrp, int rp_stride, float rscale,
+                float *d_G, float *d_A, float *d_P, float *d_R, cudaStream_t st) {
+#define CALL(LL) launch_pair_L<LL>(p, d_S, d_rsq, rpart, nrp, rp_stride, rscale, d_G, d_A, d_P, d_R, st)
   DELTA_SWITCH_L(p->lay.L, CALL)
 #undef CALL
 }
 
-int launch_auto_prep(delta_plan *p, const float *d_auto, float *d_rsq, cudaStream_t st) {
-  const int64_t n = (int64_t)p->lay.C * p->lay.F;
-  auto_prep_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(d_auto, d_rsq, n);
+int launch_auto_prep(delta_plan *p, const float *d_auto, float *d_rsq, float *d_rsum, cudaStream_t st) {
+  auto_prep_kernel<<<(unsigned)p->lay.C, 32, 0, st>>>(d_auto, d_rsq, d_rsum, p->lay.F, p->lay.Fp);
   p->launches++;
   DELTA_CUDA_CHECK(cudaGetLastError());
   return DELTA_OK;

@@ -181,12 +181,13 @@ __global__ void __launch_bounds__(StftCfg<L>::THREADS)
 stft_kernel(const void *__restrict__ x, int64_t ld, int in_dtype, int norm_mode, int n_first,
             const double *__restrict__ offs, const long long *__restrict__ isum, const float2 *__restrict__ tw,
             const float *__restrict__ win, const float2 *__restrict__ ftab, Layout lay, void *__restrict__ Xout,
-            const float *__restrict__ chscale) {
+            const float *__restrict__ chscale, float *__restrict__ wpart) {
   using Cfg = StftCfg<L>;
   using G = typename Cfg::G;
   constexpr int N = Cfg::N, T = Cfg::T, E = G::E, CH = Cfg::CH;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   float2 *zb = reinterpret_cast<float2 *>(smem_raw);
+  __shared__ float wred[Cfg::THREADS / 32];  // per-warp energy of the windowed samples
 
   const int tid = threadIdx.x, g = tid / T, gt = tid % T;
   const int cl = g / kSegBlock, kk = g % kSegBlock;
@@ -213,12 +214,27 @@ stft_kernel(const void *__restrict__ x, int64_t ld, int in_dtype, int norm_mode,
 #pragma unroll
       for (int u = 0; u < E; ++u) v[u] = make_float2(0.f, 0.f);
     }
+    {  // energy of the windowed segment (zero-lag autocorrelation of Eq. 1d by Parseval), fixed summation order
+      float ss = 0.f;
+#pragma unroll
+      for (int u = 0; u < E; ++u) ss = fmaf(v[u].x, v[u].x, fmaf(v[u].y, v[u].y, ss));
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) ss += __shfl_xor_sync(0xffffffffu, ss, o);
+      if ((tid & 31) == 0) wred[tid >> 5] = ss;
+    }
     fft_inplace<N, false>(v, FftPadMap{buf}, ftab, gt);
     fft_group_sync<T>();  // every read-back of the group is done before Z overwrites the buffer
 #pragma unroll
     for (int u = 0; u < E; ++u) buf[fft_pad(gt + T * u)] = v[u];
   }
   __syncthreads();
+  if (tid < CH && c0 + tid < lay.C) {  // the 8 T threads of a channel are 8 T / 32 consecutive warps
+    constexpr int WPC = kSegBlock * T / 32;
+    float e = 0.f;
+#pragma unroll
+    for (int w = 0; w < WPC; ++w) e += wred[tid * WPC + w];
+    wpart[(int64_t)(c0 + tid) * lay.nkb + kb] = e;
+  }
 
   constexpr int F = N + 1;
   const int64_t plane = (int64_t)lay.Kc * lay.Cp * kSegBlock;  // one [kc][c][8] block
@@ -312,7 +328,7 @@ static int launch_stft_LT(delta_plan *p, const void *d_x, int64_t ld, void *d_X,
   dim3 grid((lay.K + kSegBlock - 1) / kSegBlock, (lay.C + Cfg::CH - 1) / Cfg::CH);
   stft_kernel<L, TC><<<grid, Cfg::THREADS, smem, st>>>(d_x, ld, p->cfg.in_dtype, p->cfg.norm_mode, p->n_first, p->d_offs(),
                                                        p->d_isum(), p->d_tw(), p->d_win(), p->d_ftab(), lay, d_X,
-                                                       p->d_chscale());
+                                                       p->d_chscale(), p->d_wpart());
   p->launches++;
   DELTA_CUDA_CHECK(cudaGetLastError());
   return DELTA_OK;
