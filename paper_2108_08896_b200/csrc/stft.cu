@@ -6,10 +6,13 @@
 //
 // The real transform of a segment is an N = L/2 point complex FFT of z[n] = x[2n] + i x[2n+1] held in
 // registers (fft_reg.cuh) followed by the split step; the split is fused into the transposed write-out.
+#include <cooperative_groups.h>
 #include <cuda_fp16.h>
 
 #include "delta_internal.h"
 #include "fft_reg.cuh"
+
+namespace cg = cooperative_groups;
 
 namespace delta {
 
@@ -64,11 +67,14 @@ struct SampleLoader {
   long long isum;         // int16 input: integer sum over n_first samples
   float inv_isum, inv_n;  // 1/isum, 1/n_first
   int n_first;
+  long long i_mul, i_sub;  // int16: numerator = x * i_mul - i_sub
+  float i_scale, f_sub, f_scale;
 
   __device__ __forceinline__ void init(const void *x_, int in_dtype_, int norm_mode_, int n_first_,
                                        const double *__restrict__ offs, const long long *__restrict__ isums, int c) {
     x = x_; in_dtype = in_dtype_; norm_mode = norm_mode_; n_first = n_first_;
     o = 0.f; inv_o = 0.f; isum = 0; inv_isum = 0.f; inv_n = 0.f;
+    i_mul = 1; i_sub = 0; i_scale = 1.f; f_sub = 0.f; f_scale = 1.f;
     if (norm_mode != DELTA_NORM_NONE) {
       const double od = offs[c];
       o = (float)od;
@@ -76,19 +82,16 @@ struct SampleLoader {
       isum = isums[c];
       inv_isum = (float)(1.0 / (double)isum);
       inv_n = (float)(1.0 / (double)n_first);
+      i_mul = n_first; i_sub = isum; i_scale = norm_mode == DELTA_NORM_RELATIVE ? inv_isum : inv_n;
+      f_sub = o; f_scale = norm_mode == DELTA_NORM_RELATIVE ? inv_o : 1.f;
     }
   }
+  // branch-free forms (NONE: multiplier 1, subtrahend 0, scale 1: bit-identical to the plain conversion)
   __device__ __forceinline__ float conv_i16(int v) const {
-    if (norm_mode == DELTA_NORM_NONE) return (float)v;
     // (x - o) = (x n - sum)/n exactly in integers; one rounding at the conversion
-    const float num = __ll2float_rn((long long)v * n_first - isum);
-    return norm_mode == DELTA_NORM_RELATIVE ? num * inv_isum : num * inv_n;
+    return __ll2float_rn((long long)v * i_mul - i_sub) * i_scale;
   }
-  __device__ __forceinline__ float conv_f32(float v) const {
-    if (norm_mode == DELTA_NORM_NONE) return v;
-    const float d = v - o;
-    return norm_mode == DELTA_NORM_RELATIVE ? d * inv_o : d;
-  }
+  __device__ __forceinline__ float conv_f32(float v) const { return (v - f_sub) * f_scale; }
   __device__ __forceinline__ float operator()(int64_t idx) const {
     if (in_dtype == DELTA_I16) return conv_i16(reinterpret_cast<const short *>(x)[idx]);
     return conv_f32(reinterpret_cast<const float *>(x)[idx]);
@@ -157,7 +160,10 @@ struct StftCfg {
   static constexpr int N = L / 2;
   using G = FftGeom<N>;
   static constexpr int T = G::T;
-  static constexpr int CH = (N <= 256) ? 4 : (N == 512 ? 2 : 1);  // channels per CTA
+#ifndef DELTA_STFT_CH
+#define DELTA_STFT_CH 2
+#endif
+  static constexpr int CH = (N <= 256) ? DELTA_STFT_CH : (N == 512 ? 2 : 1);  // channels per CTA
   static constexpr int NFFT = CH * kSegBlock;                      // transforms per CTA
   static constexpr int THREADS = NFFT * T;
   static constexpr int CHPAD = CH > 1 ? 16 / CH : 0;                 // float2 skew between channels (bank spread)
@@ -173,21 +179,27 @@ __device__ __forceinline__ float2 rfft_split(float2 zf, float2 zr, float2 w) {
   return make_float2(e.x + wd.y, e.y - wd.x);  // e - i * (w d)
 }
 
+// CLUSTER (tensor-core mode, at most 8 segment blocks): the CTAs of one channel group form a thread-block cluster
+// and agree on the per-channel fp16 scale through distributed shared memory, so no separate pass over the chunk
+// (chscale_kernel) is needed.
 // grid = (ceil(K/8), ceil(C/CH)).  Phase 1: one group of T threads per (channel, segment) transform.
 // Phase 2: one thread per (channel, bin) gathers the 8 segments of the CTA and writes one 16-byte
 // (fp16) or 32-byte (fp32) piece per operand plane of the frequency-major X layout.
-template <int L, bool TC>
+template <int L, bool TC, bool CLUSTER>
 __global__ void __launch_bounds__(StftCfg<L>::THREADS)
 stft_kernel(const void *__restrict__ x, int64_t ld, int in_dtype, int norm_mode, int n_first,
             const double *__restrict__ offs, const long long *__restrict__ isum, const float2 *__restrict__ tw,
             const float *__restrict__ win, const float2 *__restrict__ ftab, Layout lay, void *__restrict__ Xout,
-            const float *__restrict__ chscale, float *__restrict__ wpart) {
+            float *__restrict__ chscale, float *__restrict__ wpart) {
   using Cfg = StftCfg<L>;
   using G = typename Cfg::G;
   constexpr int N = Cfg::N, T = Cfg::T, E = G::E, CH = Cfg::CH;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   float2 *zb = reinterpret_cast<float2 *>(smem_raw);
   __shared__ float wred[Cfg::THREADS / 32];  // per-warp energy of the windowed samples
+  __shared__ float wmax[Cfg::THREADS / 32];  // per-warp max |y|
+  __shared__ float cmax[CH];                 // per-channel max |y| over this CTA's segments (read by the cluster)
+  __shared__ float csc[CH];                  // per-channel fp16 scale
 
   const int tid = threadIdx.x, g = tid / T, gt = tid % T;
   const int cl = g / kSegBlock, kk = g % kSegBlock;
@@ -197,18 +209,46 @@ stft_kernel(const void *__restrict__ x, int64_t ld, int in_dtype, int norm_mode,
   {
     const int c = c0 + cl, k = kb * kSegBlock + kk;
     float2 v[E];
+    float amax = 0.f;
     if (c < lay.C && k < lay.K) {
       SampleLoader ldr;
       ldr.init(x, in_dtype, norm_mode, n_first, offs, isum, c);
       const int64_t t0 = (int64_t)c * ld + (int64_t)k * lay.H;
       const size_t esz = in_dtype == DELTA_I16 ? 2 : 4;
       const bool pair_ok = ((t0 & 1) == 0) && ((reinterpret_cast<uintptr_t>(x) & (2 * esz - 1)) == 0);
+      // all loads of the segment are issued before the first use (one DRAM latency per thread, not E)
+      float2 smp[E], wv[E];
+      if (in_dtype == DELTA_I16) {
+        const short *xs = reinterpret_cast<const short *>(x) + t0;
+        short2 raw[E];
+        if (pair_ok) {
+#pragma unroll
+          for (int u = 0; u < E; ++u) raw[u] = *reinterpret_cast<const short2 *>(xs + 2 * (gt + T * u));
+        } else {
+#pragma unroll
+          for (int u = 0; u < E; ++u) raw[u] = make_short2(xs[2 * (gt + T * u)], xs[2 * (gt + T * u) + 1]);
+        }
+#pragma unroll
+        for (int u = 0; u < E; ++u) smp[u] = make_float2(ldr.conv_i16(raw[u].x), ldr.conv_i16(raw[u].y));
+      } else {
+        const float *xf = reinterpret_cast<const float *>(x) + t0;
+        float2 raw[E];
+        if (pair_ok) {
+#pragma unroll
+          for (int u = 0; u < E; ++u) raw[u] = *reinterpret_cast<const float2 *>(xf + 2 * (gt + T * u));
+        } else {
+#pragma unroll
+          for (int u = 0; u < E; ++u) raw[u] = make_float2(xf[2 * (gt + T * u)], xf[2 * (gt + T * u) + 1]);
+        }
+#pragma unroll
+        for (int u = 0; u < E; ++u) smp[u] = make_float2(ldr.conv_f32(raw[u].x), ldr.conv_f32(raw[u].y));
+      }
+#pragma unroll
+      for (int u = 0; u < E; ++u) wv[u] = __ldg(reinterpret_cast<const float2 *>(win) + gt + T * u);
 #pragma unroll
       for (int u = 0; u < E; ++u) {
-        const int n = gt + T * u;
-        const float2 s = ldr.two(t0 + 2 * n, pair_ok);
-        const float2 w = __ldg(reinterpret_cast<const float2 *>(win) + n);
-        v[u] = make_float2(s.x * w.x, s.y * w.y);
+        if (CLUSTER) amax = fmaxf(amax, fmaxf(fabsf(smp[u].x), fabsf(smp[u].y)));
+        v[u] = make_float2(smp[u].x * wv[u].x, smp[u].y * wv[u].y);
       }
     } else {
 #pragma unroll
@@ -220,7 +260,14 @@ stft_kernel(const void *__restrict__ x, int64_t ld, int in_dtype, int norm_mode,
       for (int u = 0; u < E; ++u) ss = fmaf(v[u].x, v[u].x, fmaf(v[u].y, v[u].y, ss));
 #pragma unroll
       for (int o = 16; o > 0; o >>= 1) ss += __shfl_xor_sync(0xffffffffu, ss, o);
-      if ((tid & 31) == 0) wred[tid >> 5] = ss;
+      if (CLUSTER) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, o));
+      }
+      if ((tid & 31) == 0) {
+        wred[tid >> 5] = ss;
+        if (CLUSTER) wmax[tid >> 5] = amax;
+      }
     }
     fft_inplace<N, false>(v, FftPadMap{buf}, ftab, gt);
     fft_group_sync<T>();  // every read-back of the group is done before Z overwrites the buffer
@@ -234,6 +281,33 @@ stft_kernel(const void *__restrict__ x, int64_t ld, int in_dtype, int norm_mode,
 #pragma unroll
     for (int w = 0; w < WPC; ++w) e += wred[tid * WPC + w];
     wpart[(int64_t)(c0 + tid) * lay.nkb + kb] = e;
+  }
+  if (CLUSTER) {
+    // per-channel power-of-two scale: sum_n w[n] |y| <= (L/2) max|y|  =>  scale * |X| < 2^14 (same rule as chscale_kernel)
+    cg::cluster_group cluster = cg::this_cluster();
+    if (tid < CH) {
+      constexpr int WPC = kSegBlock * T / 32;
+      float m = 0.f;
+#pragma unroll
+      for (int w = 0; w < WPC; ++w) m = fmaxf(m, wmax[tid * WPC + w]);
+      cmax[tid] = m;
+    }
+    cluster.sync();
+    if (tid < CH) {
+      float m = 0.f;
+      const unsigned nb = cluster.num_blocks();
+      for (unsigned r = 0; r < nb; ++r) m = fmaxf(m, *cluster.map_shared_rank(&cmax[tid], r));
+      const float bound = m * (0.5f * (float)L);
+      float sc = 1.f;
+      if (bound > 0.f && isfinite(bound)) {
+        int e;
+        frexpf(bound, &e);
+        sc = ldexpf(1.f, 14 - e);
+      }
+      csc[tid] = sc;
+      if (kb == 0 && c0 + tid < lay.C) chscale[c0 + tid] = sc;
+    }
+    cluster.sync();  // remote reads of cmax are done (no CTA may exit before), and csc is visible to the CTA
   }
 
   constexpr int F = N + 1;
@@ -257,7 +331,7 @@ stft_kernel(const void *__restrict__ x, int64_t ld, int in_dtype, int norm_mode,
     if (TC) {
       // split fp16: v * scale = hi + lo (scale = power of two chosen by chscale_kernel)
       __half *X = reinterpret_cast<__half *>(Xout);
-      const float sc = chscale[c];
+      const float sc = CLUSTER ? csc[pcl] : chscale[c];
       __align__(16) __half2 hr[4], hi_[4], lr[4], li[4];
 #pragma unroll
       for (int q = 0; q < 4; ++q) {
@@ -318,17 +392,30 @@ int launch_offsets(delta_plan *p, const void *d_x, int64_t ld, int n_first, cuda
   return DELTA_OK;
 }
 
-template <int L, bool TC>
+template <int L, bool TC, bool CLUSTER>
 static int launch_stft_LT(delta_plan *p, const void *d_x, int64_t ld, void *d_X, cudaStream_t st) {
   using Cfg = StftCfg<L>;
   const Layout &lay = p->lay;
   const size_t smem = (size_t)Cfg::SMEM_F2 * sizeof(float2);
-  int rc = opt_in_smem(stft_kernel<L, TC>, smem);
+  int rc = opt_in_smem(stft_kernel<L, TC, CLUSTER>, smem);
   if (rc) return rc;
-  dim3 grid((lay.K + kSegBlock - 1) / kSegBlock, (lay.C + Cfg::CH - 1) / Cfg::CH);
-  stft_kernel<L, TC><<<grid, Cfg::THREADS, smem, st>>>(d_x, ld, p->cfg.in_dtype, p->cfg.norm_mode, p->n_first, p->d_offs(),
-                                                       p->d_isum(), p->d_tw(), p->d_win(), p->d_ftab(), lay, d_X,
-                                                       p->d_chscale(), p->d_wpart());
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(lay.nkb, (lay.C + Cfg::CH - 1) / Cfg::CH);
+  cfg.blockDim = dim3(Cfg::THREADS);
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = st;
+  cudaLaunchAttribute attr[1];
+  if (CLUSTER) {  // the segment blocks of one channel group are one cluster
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = lay.nkb;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+  }
+  DELTA_CUDA_CHECK(cudaLaunchKernelEx(&cfg, stft_kernel<L, TC, CLUSTER>, d_x, ld, p->cfg.in_dtype, p->cfg.norm_mode, p->n_first,
+                                      (const double *)p->d_offs(), (const long long *)p->d_isum(), p->d_tw(), p->d_win(),
+                                      p->d_ftab(), lay, d_X, p->d_chscale(), p->d_wpart()));
   p->launches++;
   DELTA_CUDA_CHECK(cudaGetLastError());
   return DELTA_OK;
@@ -338,13 +425,14 @@ template <int L>
 static int launch_stft_L(delta_plan *p, const void *d_x, int64_t ld, void *d_X, cudaStream_t st) {
   const Layout &lay = p->lay;
   if (p->contraction == DELTA_CONTRACT_TC) {
+    if (lay.nkb <= 8) return launch_stft_LT<L, true, true>(p, d_x, ld, d_X, st);  // scale agreed inside the cluster
     chscale_kernel<<<lay.C, 1024, 0, st>>>(d_x, ld, p->cfg.in_dtype, p->cfg.norm_mode, p->n_first, p->d_offs(), p->d_isum(),
                                            lay.T, lay.L, p->d_chscale());
     p->launches++;
     DELTA_CUDA_CHECK(cudaGetLastError());
-    return launch_stft_LT<L, true>(p, d_x, ld, d_X, st);
+    return launch_stft_LT<L, true, false>(p, d_x, ld, d_X, st);
   }
-  return launch_stft_LT<L, false>(p, d_x, ld, d_X, st);
+  return launch_stft_LT<L, false, false>(p, d_x, ld, d_X, st);
 }
 
 int launch_stft(delta_plan *p, const void *d_x, int64_t ld, void *d_X, cudaStream_t st) {
