@@ -50,7 +50,9 @@ struct PairCfg {
 __device__ __forceinline__ float atan2_poly(float y, float x) {
   const float ax = fabsf(x), ay = fabsf(y);
   const float mx = fmaxf(ax, ay), mn = fminf(ax, ay);
-  const float t = __fdividef(mn, fmaxf(mx, 1e-37f));
+  float rc;
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(rc) : "f"(fmaxf(mx, 1e-37f)));
+  const float t = mn * rc;
   const float u = t * t;
   float p = 0.006811792496591806f;
   p = fmaf(p, u, -0.0336042195558548f);
@@ -75,18 +77,20 @@ __device__ __forceinline__ float sqrt_approx(float v) {
 //   Zin[f] = (S[f] + conj S[N-f])/2 + i e^{+2 pi i f/L} (S[f] - conj S[N-f])/2,   f = 0..N-1
 // then z = IFFT_N(Zin) (unnormalised) gives x[2n] = Re z[n]/N, x[2n+1] = Im z[n]/N  where
 // x[m] = (1/L) sum_{f<L} S_full[f] e^{+2 pi i f m/L}.
-__device__ __forceinline__ float2 irfft_merge(float2 sf, float2 sr, float2 w_conj) {
-  const float2 e = make_float2(0.5f * (sf.x + sr.x), 0.5f * (sf.y - sr.y));
-  const float2 d = make_float2(0.5f * (sf.x - sr.x), 0.5f * (sf.y + sr.y));
+// irfft_merge2 returns twice that Zin (the halvings are left to the caller's normalisation).
+__device__ __forceinline__ float2 irfft_merge2(float2 sf, float2 sr, float2 w_conj) {
+  const float2 e = make_float2(sf.x + sr.x, sf.y - sr.y);
+  const float2 d = make_float2(sf.x - sr.x, sf.y + sr.y);
   const float2 wd = cmul(w_conj, d);
   return make_float2(e.x - wd.y, e.y + wd.x);  // e + i * (w d)
 }
 
 }  // namespace
 
+// GAPALL: G, A and Pw are all requested (no per-element pointer tests)
 // FULL: max_lag == L/2 (every lag of the circular correlation is stored; the two end points are the same sample)
 // Zero-lag autocorrelations (R12): sum over all L bins of S_cc = rscale * sum_{k<nrp} rpart[c rp_stride + k].
-template <int L, bool FULL>
+template <int L, bool FULL, bool GAPALL>
 __global__ void __launch_bounds__(PairCfg<L>::THREADS, PairCfg<L>::MIN_CTAS)
 pair_kernel(const float2 *__restrict__ S, const float *__restrict__ Srsq, const float *__restrict__ rpart, int nrp,
             int rp_stride, float rscale, const ushort2 *__restrict__ pairs, const float2 *__restrict__ tw,
@@ -157,51 +161,51 @@ pair_kernel(const float2 *__restrict__ S, const float *__restrict__ Srsq, const 
   const float2 wg = __ldg(tw + gt);  // e^{-2 pi i gt / L}
   const int64_t o = p * F;
 
-  // ---- G, A, P of the thread's bins, and the merge step of the inverse real transform --------------------
-  // Loads of a batch of UB bins are issued together so that their latencies overlap.
-  auto emit = [&](float2 s, float gi, float gj, int f) {
-    const float mag = sqrt_approx(fmaf(s.x, s.x, s.y * s.y));
-    if (Pw) Pw[o + f] = mag;
-    if (G) G[o + f] = mag * gi * gj;
-    if (A) A[o + f] = atan2_poly(s.y, s.x);
-  };
-  float2 v[E];
+  // ---- pass 1: G, A, P of the thread's bins -----------------------------------------------------------------
+  // The loads of a batch of UB bins (S from the tile, 1/sqrt(S_ii) from global memory, 1/sqrt(S_jj) from the staged
+  // row) are issued together; nothing else is live in registers yet, so their latencies overlap.
   const int pg = pl ^ gt;
-  #ifndef DELTA_PAIR_UB
-#define DELTA_PAIR_UB 4
-#endif
-  constexpr int UB = DELTA_PAIR_UB < E ? DELTA_PAIR_UB : E;
+  if (gap) {
+    auto emit = [&](float2 s, float gi, float gj, int f) {
+      const float mag = sqrt_approx(fmaf(s.x, s.x, s.y * s.y));
+      if (GAPALL || Pw) Pw[o + f] = mag;
+      if (GAPALL || G) G[o + f] = mag * gi * gj;
+      if (GAPALL || A) A[o + f] = atan2_poly(s.y, s.x);
+    };
+    constexpr int UB = E < 8 ? E : 8;
 #pragma unroll
-  for (int ub = 0; ub < E; ub += UB) {
-    float2 sf[UB], sr[UB], w[UB];
-    float gi[UB], gj[UB];
+    for (int ub = 0; ub < E; ub += UB) {
+      float2 sf[UB];
+      float gi[UB], gj[UB];
 #pragma unroll
-    for (int k = 0; k < UB; ++k) {
-      const int u = ub + k;
-      const int f = gt + T * u;  // gt < T and T is a power of two, so f = gt | T u
-      const int fr = N - f;
-      sf[k] = tile[f * PB + ((pg ^ (T * u)) & (PB - 1))];
-      sr[k] = tile[fr * PB + ((pl ^ fr) & (PB - 1))];
-      gi[k] = wantG ? __ldg(ri + f) : 0.f;
-      gj[k] = wantG ? rj[f] : 0.f;
-      w[k] = cmul(wg, pc.wstep[u]);  // e^{-2 pi i f / L}
-    }
-#pragma unroll
-    for (int k = 0; k < UB; ++k) {
-      const int u = ub + k;
-      const int f = gt + T * u;
-      if (gap) {
-        emit(sf[k], gi[k], gj[k], f);
-        if (u == 0 && gt == 0) emit(sr[k], wantG ? __ldg(ri + N) : 0.f, wantG ? rj[N] : 0.f, N);  // the Nyquist bin
+      for (int k = 0; k < UB; ++k) {
+        const int u = ub + k;
+        const int f = gt + T * u;  // gt < T and T is a power of two, so f = gt | T u
+        sf[k] = tile[f * PB + ((pg ^ (T * u)) & (PB - 1))];
+        gi[k] = wantG ? __ldg(ri + f) : 0.f;
+        gj[k] = wantG ? rj[f] : 0.f;
       }
-      if (wantR) {
-        if (u == 0 && gt == 0) { sf[k].y = 0.f; sr[k].y = 0.f; }  // Im S[0], Im S[N] do not enter the real transform
-        v[u] = irfft_merge(sf[k], sr[k], make_float2(w[k].x, -w[k].y));  // e^{+2 pi i f / L}
-      }
+#pragma unroll
+      for (int k = 0; k < UB; ++k) emit(sf[k], gi[k], gj[k], gt + T * (ub + k));
     }
-    asm volatile("" ::: "memory");  // keep the next batch's loads from being hoisted (register pressure)
+    if (gt == 0)  // the Nyquist bin
+      emit(tile[N * PB + ((pl ^ N) & (PB - 1))], wantG ? __ldg(ri + N) : 0.f, wantG ? rj[N] : 0.f, N);
   }
   if (!wantR) return;
+
+  // ---- pass 2: merge step of the inverse real transform (S read again from the tile; twice the merge of
+  // irfft_merge, the factor 1/2 goes into the normalisation) ------------------------------------------------
+  float2 v[E];
+#pragma unroll
+  for (int u = 0; u < E; ++u) {
+    const int f = gt + T * u;
+    const int fr = N - f;
+    float2 sf = tile[f * PB + ((pg ^ (T * u)) & (PB - 1))];
+    float2 sr = tile[fr * PB + ((pl ^ fr) & (PB - 1))];
+    if (u == 0 && gt == 0) { sf.y = 0.f; sr.y = 0.f; }  // Im S[0], Im S[N] do not enter the real transform
+    const float2 w = cmul(wg, pc.wstep[u]);               // e^{-2 pi i f / L}; the inverse uses its conjugate
+    v[u] = irfft_merge2(sf, sr, make_float2(w.x, -w.y));
+  }
   __syncthreads();  // every S value is in registers: the tile becomes exchange space
 
   // ---- rho = irfft(S) / sqrt(R_ii[0] R_jj[0]) ----------------------------------------------------------------
@@ -211,7 +215,7 @@ pair_kernel(const float2 *__restrict__ S, const float *__restrict__ Srsq, const 
   while (ki > 0 && ij_s[ki - 1].x == ij.x) --ki;
   while (kj > 0 && ij_s[kj - 1].y == ij.y) --kj;
   // rho = x / sqrt(R_ii[0] R_jj[0]),  x = z/N,  R_cc[0] = (sum over all L bins of S_cc)/L
-  const float norm = 2.f * rs[ki] * rs[PB + kj];
+  const float norm = rs[ki] * rs[PB + kj];  // 2 (L/N) x 1/2 (irfft_merge2)
   float *Rp = R + p * lay.nlags;
   if (FULL) {
     // lag m = xi for xi <= L/2 and xi - L for xi >= L/2; row position q = m + L/2
@@ -280,16 +284,19 @@ static int launch_pair_L(delta_plan *p, const float *d_S, const float *d_rsq, co
   PairConsts pc;
   for (int u = 0; u < 16; ++u) pc.wstep[u] = p->h_wstep[u];
   const bool full = lay.M == L / 2;
-#define DELTA_PAIR_LAUNCH(FULL_)                                                                                    \
+#define DELTA_PAIR_LAUNCH(FULL_, GAPALL_)                                                                           \
   do {                                                                                                              \
-    int rc = opt_in_smem(pair_kernel<L, FULL_>, Cfg::SMEM);                                                         \
+    int rc = opt_in_smem(pair_kernel<L, FULL_, GAPALL_>, Cfg::SMEM);                                                \
     if (rc) return rc;                                                                                              \
-    pair_kernel<L, FULL_><<<(unsigned)lay.Pblk, Cfg::THREADS, Cfg::SMEM, st>>>(                                     \
+    pair_kernel<L, FULL_, GAPALL_><<<(unsigned)lay.Pblk, Cfg::THREADS, Cfg::SMEM, st>>>(                            \
         reinterpret_cast<const float2 *>(d_S), d_rsq, rpart, nrp, rp_stride, rscale, p->d_pairs(), p->d_tw(),       \
         p->d_ftab(), lay, pc, d_G, d_A, d_P, d_R);                                                                  \
   } while (0)
-  if (full) DELTA_PAIR_LAUNCH(true);
-  else DELTA_PAIR_LAUNCH(false);
+  const bool gapall = d_G && d_A && d_P;
+  if (full && gapall) DELTA_PAIR_LAUNCH(true, true);
+  else if (full) DELTA_PAIR_LAUNCH(true, false);
+  else if (gapall) DELTA_PAIR_LAUNCH(false, true);
+  else DELTA_PAIR_LAUNCH(false, false);
 #undef DELTA_PAIR_LAUNCH
   p->launches++;
   DELTA_CUDA_CHECK(cudaGetLastError());
