@@ -1,6 +1,7 @@
 // C-ABI entry points of libdelta_b200 (include/delta.h): argument validation, plan and workspace
 // management, and the launch sequences.  All arithmetic of the path lives in the kernels.
 #include <cmath>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 
@@ -59,6 +60,7 @@ int delta_plan_create(const delta_config *cfg, delta_plan **out) {
   delta_plan *p = new (std::nothrow) delta_plan();
   if (!p) return DELTA_ERR_INVALID_ARG;
   p->cfg = *cfg;
+  p->use_pdl = std::getenv("DELTA_NO_PDL") == nullptr;
   p->cfg.h_pairs = nullptr;
   p->contraction = (cfg->contraction == DELTA_CONTRACT_AUTO) ? (tc_supported(cfg) ? DELTA_CONTRACT_TC : DELTA_CONTRACT_FP32)
                                                              : cfg->contraction;

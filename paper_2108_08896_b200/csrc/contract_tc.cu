@@ -146,8 +146,6 @@ contract_tc_kernel(const __half *__restrict__ X, Layout lay, TcParams prm, float
   if (tid == 0) TC_TRACE(3, 0);
   if (TRACE && tid == 0) { long long g; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g)); trace[5 * 512 + 2 * blockIdx.x] = g; }
 
-  for (int c = tid; c < lay.Cp; c += kTcThreads)
-    itab[c] = make_float2(__int_as_float(c * lay.C - (c * (c + 1)) / 2 - c - 1), (c < lay.C) ? 1.f / chscale[c] : 0.f);
   if (tid == 0) {
     for (int s = 0; s < prm.nstage; ++s) {
       mbar_init(full_bar + s, 1);
@@ -163,6 +161,10 @@ contract_tc_kernel(const __half *__restrict__ X, Layout lay, TcParams prm, float
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_slot)), "r"(512));
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
   }
+  pdl_launch_dependents();
+  pdl_wait();  // X and chscale come from the STFT kernel; S, Sauto, Srsq of the previous chunk are still being read
+  for (int c = tid; c < lay.Cp; c += kTcThreads)
+    itab[c] = make_float2(__int_as_float(c * lay.C - (c * (c + 1)) / 2 - c - 1), (c < lay.C) ? 1.f / chscale[c] : 0.f);
   fence_before();
   __syncthreads();
   fence_after();
@@ -432,15 +434,16 @@ int launch_contract_tc(delta_plan *p, const void *d_X, float *d_S, float *d_auto
   if (p->d_trace) {
     int rc = opt_in_smem(contract_tc_kernel<true>, smem);
     if (rc) return rc;
-    contract_tc_kernel<true><<<grid, kTcThreads, smem, st>>>(reinterpret_cast<const __half *>(d_X), lay, prm, scale,
-                                                             p->d_chscale(), reinterpret_cast<float2 *>(d_S), d_auto, d_rsq,
-                                                             p->d_trace);
+    LaunchCfg lc(dim3(grid), dim3(kTcThreads), smem, st, p->use_pdl);
+    DELTA_CUDA_CHECK(cudaLaunchKernelEx(&lc.cfg, contract_tc_kernel<true>, reinterpret_cast<const __half *>(d_X), lay, prm, scale,
+                                        (const float *)p->d_chscale(), reinterpret_cast<float2 *>(d_S), d_auto, d_rsq, p->d_trace));
   } else {
     int rc = opt_in_smem(contract_tc_kernel<false>, smem);
     if (rc) return rc;
-    contract_tc_kernel<false><<<grid, kTcThreads, smem, st>>>(reinterpret_cast<const __half *>(d_X), lay, prm, scale,
-                                                              p->d_chscale(), reinterpret_cast<float2 *>(d_S), d_auto, d_rsq,
-                                                              nullptr);
+    LaunchCfg lc(dim3(grid), dim3(kTcThreads), smem, st, p->use_pdl);
+    DELTA_CUDA_CHECK(cudaLaunchKernelEx(&lc.cfg, contract_tc_kernel<false>, reinterpret_cast<const __half *>(d_X), lay, prm, scale,
+                                        (const float *)p->d_chscale(), reinterpret_cast<float2 *>(d_S), d_auto, d_rsq,
+                                        (long long *)nullptr));
   }
   p->launches++;
   DELTA_CUDA_CHECK(cudaGetLastError());

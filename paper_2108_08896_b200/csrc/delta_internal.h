@@ -70,6 +70,7 @@ struct delta_plan {
   int n_first = 0;
   int launches = 0;
   long long *d_trace = nullptr;  // debug: clock stamps of the tensor-core contraction (delta_debug_set_trace)
+  bool use_pdl = true;  // programmatic dependent launch between the hot-path kernels (DELTA_NO_PDL=1 switches it off)
   bool stage_events_on = false;
   cudaEvent_t stage_ev[4] = {nullptr, nullptr, nullptr, nullptr};
   cudaStream_t copy_stream = nullptr;
@@ -106,6 +107,40 @@ void set_cuda_error(cudaError_t e);
       return DELTA_ERR_CUDA;                   \
     }                                          \
   } while (0)
+
+// Programmatic dependent launch: a kernel launched with the attribute may become resident while its predecessor in
+// the stream is still running; it must call pdl_wait() before it reads anything the predecessor wrote or writes
+// anything the predecessor reads.  pdl_launch_dependents() lets the successor start its own prologue early.
+#ifdef __CUDACC__
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+#endif
+struct LaunchCfg {
+  cudaLaunchConfig_t cfg;
+  cudaLaunchAttribute attr[2];
+  LaunchCfg(dim3 grid, dim3 block, size_t smem, cudaStream_t st, bool pdl, unsigned cluster_x = 0) {
+    cfg = cudaLaunchConfig_t{};
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    unsigned n = 0;
+    if (pdl) {
+      attr[n].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+      attr[n].val.programmaticStreamSerializationAllowed = 1;
+      ++n;
+    }
+    if (cluster_x > 1) {
+      attr[n].id = cudaLaunchAttributeClusterDimension;
+      attr[n].val.clusterDim.x = cluster_x;
+      attr[n].val.clusterDim.y = 1;
+      attr[n].val.clusterDim.z = 1;
+      ++n;
+    }
+    cfg.attrs = attr;
+    cfg.numAttrs = n;
+  }
+};
 
 // opt in to more than 48 KB of dynamic shared memory
 template <typename Kern>

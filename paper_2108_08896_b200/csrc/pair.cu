@@ -113,9 +113,13 @@ pair_kernel(const float2 *__restrict__ S, const float *__restrict__ Srsq, const 
   const int tid = threadIdx.x;
   const int64_t p0 = (int64_t)blockIdx.x * PB;
 
+  pdl_launch_dependents();
   if (tid == 0) {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(1));
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  pdl_wait();  // S, rsq and the energy partials come from the preceding kernels; the outputs may still be read by a consumer
+  if (tid == 0) {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)),
                  "r"((uint32_t)(Cfg::TILE_BYTES + (wantG ? Cfg::ROWS_BYTES : 0))) : "memory");
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(tile)),
@@ -288,9 +292,10 @@ static int launch_pair_L(delta_plan *p, const float *d_S, const float *d_rsq, co
   do {                                                                                                              \
     int rc = opt_in_smem(pair_kernel<L, FULL_, GAPALL_>, Cfg::SMEM);                                                \
     if (rc) return rc;                                                                                              \
-    pair_kernel<L, FULL_, GAPALL_><<<(unsigned)lay.Pblk, Cfg::THREADS, Cfg::SMEM, st>>>(                            \
-        reinterpret_cast<const float2 *>(d_S), d_rsq, rpart, nrp, rp_stride, rscale, p->d_pairs(), p->d_tw(),       \
-        p->d_ftab(), lay, pc, d_G, d_A, d_P, d_R);                                                                  \
+    LaunchCfg lc(dim3((unsigned)lay.Pblk), dim3(Cfg::THREADS), Cfg::SMEM, st, p->use_pdl);                          \
+    DELTA_CUDA_CHECK(cudaLaunchKernelEx(&lc.cfg, pair_kernel<L, FULL_, GAPALL_>, reinterpret_cast<const float2 *>(d_S), \
+                                        d_rsq, rpart, nrp, rp_stride, rscale, p->d_pairs(), p->d_tw(), p->d_ftab(), lay, pc, \
+                                        d_G, d_A, d_P, d_R));                                                       \
   } while (0)
   const bool gapall = d_G && d_A && d_P;
   if (full && gapall) DELTA_PAIR_LAUNCH(true, true);

@@ -186,7 +186,7 @@ __device__ __forceinline__ float2 rfft_split(float2 zf, float2 zr, float2 w) {
 // Phase 2: one thread per (channel, bin) gathers the 8 segments of the CTA and writes one 16-byte
 // (fp16) or 32-byte (fp32) piece per operand plane of the frequency-major X layout.
 template <int L, bool TC, bool CLUSTER>
-__global__ void __launch_bounds__(StftCfg<L>::THREADS)
+__global__ void __launch_bounds__(StftCfg<L>::THREADS, 1024 / StftCfg<L>::THREADS)
 stft_kernel(const void *__restrict__ x, int64_t ld, int in_dtype, int norm_mode, int n_first,
             const double *__restrict__ offs, const long long *__restrict__ isum, const float2 *__restrict__ tw,
             const float *__restrict__ win, const float2 *__restrict__ ftab, Layout lay, void *__restrict__ Xout,
@@ -200,6 +200,9 @@ stft_kernel(const void *__restrict__ x, int64_t ld, int in_dtype, int norm_mode,
   __shared__ float wmax[Cfg::THREADS / 32];  // per-warp max |y|
   __shared__ float cmax[CH];                 // per-channel max |y| over this CTA's segments (read by the cluster)
   __shared__ float csc[CH];                  // per-channel fp16 scale
+
+  pdl_launch_dependents();
+  pdl_wait();  // the chunk may come from the caller's previous kernel; X, wpart and chscale are read by ours
 
   const int tid = threadIdx.x, g = tid / T, gt = tid % T;
   const int cl = g / kSegBlock, kk = g % kSegBlock;
@@ -269,6 +272,19 @@ stft_kernel(const void *__restrict__ x, int64_t ld, int in_dtype, int norm_mode,
         if (CLUSTER) wmax[tid >> 5] = amax;
       }
     }
+    if (CLUSTER) {
+      // publish this CTA's per-channel max |y| to the cluster now; the matching wait comes after the FFT, so the
+      // cluster barrier's latency is hidden behind the transform
+      __syncthreads();
+      if (tid < CH) {
+        constexpr int WPC = kSegBlock * T / 32;
+        float m = 0.f;
+#pragma unroll
+        for (int w = 0; w < WPC; ++w) m = fmaxf(m, wmax[tid * WPC + w]);
+        cmax[tid] = m;
+      }
+      cg::this_cluster().barrier_arrive();
+    }
     fft_inplace<N, false>(v, FftPadMap{buf}, ftab, gt);
     fft_group_sync<T>();  // every read-back of the group is done before Z overwrites the buffer
 #pragma unroll
@@ -285,14 +301,7 @@ stft_kernel(const void *__restrict__ x, int64_t ld, int in_dtype, int norm_mode,
   if (CLUSTER) {
     // per-channel power-of-two scale: sum_n w[n] |y| <= (L/2) max|y|  =>  scale * |X| < 2^14 (same rule as chscale_kernel)
     cg::cluster_group cluster = cg::this_cluster();
-    if (tid < CH) {
-      constexpr int WPC = kSegBlock * T / 32;
-      float m = 0.f;
-#pragma unroll
-      for (int w = 0; w < WPC; ++w) m = fmaxf(m, wmax[tid * WPC + w]);
-      cmax[tid] = m;
-    }
-    cluster.sync();
+    cluster.barrier_wait();  // every CTA of the channel group has published cmax
     if (tid < CH) {
       float m = 0.f;
       const unsigned nb = cluster.num_blocks();
@@ -307,29 +316,19 @@ stft_kernel(const void *__restrict__ x, int64_t ld, int in_dtype, int norm_mode,
       csc[tid] = sc;
       if (kb == 0 && c0 + tid < lay.C) chscale[c0 + tid] = sc;
     }
-    cluster.sync();  // remote reads of cmax are done (no CTA may exit before), and csc is visible to the CTA
+    cluster.barrier_arrive();  // remote reads of cmax are done; waited for just before the CTA exits
+    __syncthreads();           // csc is visible to the CTA
   }
 
-  constexpr int F = N + 1;
+  // Phase 2.  Bins f and N - f come from the same pair Z[f], Z[N-f]:  with e = (Z[f] + conj Z[N-f])/2,
+  // d = (Z[f] - conj Z[N-f])/2 and (a, b) = e^{-2 pi i f/L} d:  X[f] = (e.x + b, e.y - a),  X[N-f] = (e.x - b, -e.y - a).
+  // One thread does both for the 8 segments of the CTA; bin N/2 (its own partner) is done once.
   const int64_t plane = (int64_t)lay.Kc * lay.Cp * kSegBlock;  // one [kc][c][8] block
-  for (int idx = tid; idx < CH * F; idx += Cfg::THREADS) {
-    const int pcl = idx % CH, f = idx / CH;
-    const int c = c0 + pcl;
-    if (c >= lay.C) continue;
-    const float2 w = __ldg(tw + f);  // e^{-2 pi i f/L}
-    const float2 *zc = zb + pcl * (kSegBlock * G::BUF + Cfg::CHPAD);
-    const int i_f = fft_pad(f & (N - 1)), i_r = fft_pad((N - f) & (N - 1));
-    float re[kSegBlock], im[kSegBlock];
-#pragma unroll
-    for (int s = 0; s < kSegBlock; ++s) {
-      const float2 X = rfft_split(zc[s * G::BUF + i_f], zc[s * G::BUF + i_r], w);
-      re[s] = X.x;
-      im[s] = X.y;
-    }
+  auto store_bin = [&](int c, int pcl, int f, const float *re, const float *im) {
     const int64_t within = ((int64_t)kb * lay.Cp + c) * kSegBlock;
     const int64_t base = (int64_t)f * lay.x_elems_per_f + within;
     if (TC) {
-      // split fp16: v * scale = hi + lo (scale = power of two chosen by chscale_kernel)
+      // split fp16: v * scale = hi + lo (scale = the channel's power of two)
       __half *X = reinterpret_cast<__half *>(Xout);
       const float sc = CLUSTER ? csc[pcl] : chscale[c];
       __align__(16) __half2 hr[4], hi_[4], lr[4], li[4];
@@ -353,7 +352,31 @@ stft_kernel(const void *__restrict__ x, int64_t ld, int in_dtype, int norm_mode,
       *reinterpret_cast<float4 *>(X + base + plane) = make_float4(im[0], im[1], im[2], im[3]);
       *reinterpret_cast<float4 *>(X + base + plane + 4) = make_float4(im[4], im[5], im[6], im[7]);
     }
+  };
+  constexpr int HB = N / 2 + 1;  // f = 0 .. N/2
+  for (int idx = tid; idx < CH * HB; idx += Cfg::THREADS) {
+    const int pcl = idx % CH, f = idx / CH;
+    const int c = c0 + pcl;
+    if (c >= lay.C) continue;
+    const float2 w = __ldg(tw + f);  // e^{-2 pi i f/L}
+    const float2 *zc = zb + pcl * (kSegBlock * G::BUF + Cfg::CHPAD);
+    const int i_f = fft_pad(f), i_r = fft_pad((N - f) & (N - 1));
+    float re[kSegBlock], im[kSegBlock], re2[kSegBlock], im2[kSegBlock];
+#pragma unroll
+    for (int s = 0; s < kSegBlock; ++s) {
+      const float2 zf = zc[s * G::BUF + i_f], zr = zc[s * G::BUF + i_r];
+      const float2 e = make_float2(0.5f * (zf.x + zr.x), 0.5f * (zf.y - zr.y));
+      const float2 d = make_float2(0.5f * (zf.x - zr.x), 0.5f * (zf.y + zr.y));
+      const float2 wd = cmul(w, d);
+      re[s] = e.x + wd.y;
+      im[s] = e.y - wd.x;
+      re2[s] = e.x - wd.y;
+      im2[s] = -e.y - wd.x;
+    }
+    store_bin(c, pcl, f, re, im);
+    if (2 * f != N) store_bin(c, pcl, N - f, re2, im2);
   }
+  if (CLUSTER) cg::this_cluster().barrier_wait();  // no CTA exits while its cmax may still be read
 }
 
 // test accessor: X layout -> complex64 [C][K][F]
@@ -399,21 +422,9 @@ static int launch_stft_LT(delta_plan *p, const void *d_x, int64_t ld, void *d_X,
   const size_t smem = (size_t)Cfg::SMEM_F2 * sizeof(float2);
   int rc = opt_in_smem(stft_kernel<L, TC, CLUSTER>, smem);
   if (rc) return rc;
-  cudaLaunchConfig_t cfg = {};
-  cfg.gridDim = dim3(lay.nkb, (lay.C + Cfg::CH - 1) / Cfg::CH);
-  cfg.blockDim = dim3(Cfg::THREADS);
-  cfg.dynamicSmemBytes = smem;
-  cfg.stream = st;
-  cudaLaunchAttribute attr[1];
-  if (CLUSTER) {  // the segment blocks of one channel group are one cluster
-    attr[0].id = cudaLaunchAttributeClusterDimension;
-    attr[0].val.clusterDim.x = lay.nkb;
-    attr[0].val.clusterDim.y = 1;
-    attr[0].val.clusterDim.z = 1;
-    cfg.attrs = attr;
-    cfg.numAttrs = 1;
-  }
-  DELTA_CUDA_CHECK(cudaLaunchKernelEx(&cfg, stft_kernel<L, TC, CLUSTER>, d_x, ld, p->cfg.in_dtype, p->cfg.norm_mode, p->n_first,
+  // the segment blocks of one channel group are one cluster
+  LaunchCfg lc(dim3(lay.nkb, (lay.C + Cfg::CH - 1) / Cfg::CH), dim3(Cfg::THREADS), smem, st, p->use_pdl, CLUSTER ? lay.nkb : 0);
+  DELTA_CUDA_CHECK(cudaLaunchKernelEx(&lc.cfg, stft_kernel<L, TC, CLUSTER>, d_x, ld, p->cfg.in_dtype, p->cfg.norm_mode, p->n_first,
                                       (const double *)p->d_offs(), (const long long *)p->d_isum(), p->d_tw(), p->d_win(),
                                       p->d_ftab(), lay, d_X, p->d_chscale(), p->d_wpart()));
   p->launches++;
