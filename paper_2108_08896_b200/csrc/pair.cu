@@ -85,6 +85,18 @@ __device__ __forceinline__ float2 irfft_merge2(float2 sf, float2 sr, float2 w_co
   return make_float2(e.x - wd.y, e.y + wd.x);  // e + i * (w d)
 }
 
+// (i, j) of lexicographic pair p: row i holds the pairs [start(i), start(i+1)), start(i) = i C - i (i + 1) / 2.
+// Float estimate of the root, then exact integer correction.
+__device__ __forceinline__ ushort2 pair_of(int64_t p, int C) {
+  const float b = 2.f * (float)C - 1.f;
+  int i = (int)((b - sqrtf(fmaxf(b * b - 8.f * (float)p, 0.f))) * 0.5f);
+  i = i < 0 ? 0 : (i > C - 2 ? C - 2 : i);
+  auto start = [C](int r) { return (int64_t)r * C - ((int64_t)r * (r + 1)) / 2; };
+  while (i < C - 2 && start(i + 1) <= p) ++i;
+  while (i > 0 && start(i) > p) --i;
+  return make_ushort2((unsigned short)i, (unsigned short)(p - start(i) + i + 1));
+}
+
 }  // namespace
 
 // GAPALL: G, A and Pw are all requested (no per-element pointer tests)
@@ -93,7 +105,7 @@ __device__ __forceinline__ float2 irfft_merge2(float2 sf, float2 sr, float2 w_co
 template <int L, bool FULL, bool GAPALL>
 __global__ void __launch_bounds__(PairCfg<L>::THREADS, PairCfg<L>::MIN_CTAS)
 pair_kernel(const float2 *__restrict__ S, const float *__restrict__ Srsq, const float *__restrict__ rpart, int nrp,
-            int rp_stride, float rscale, const ushort2 *__restrict__ pairs, const float2 *__restrict__ tw,
+            int rp_stride, float rscale, const float2 *__restrict__ tw,
             const float2 *__restrict__ ftab, Layout lay, PairConsts pc, float *__restrict__ G_, float *__restrict__ A_,
             float *__restrict__ Pw_, float *__restrict__ R_) {
   using Cfg = PairCfg<L>;
@@ -114,11 +126,13 @@ pair_kernel(const float2 *__restrict__ S, const float *__restrict__ Srsq, const 
   const int64_t p0 = (int64_t)blockIdx.x * PB;
 
   pdl_launch_dependents();
+  if (tid < PB) ij_s[tid] = (p0 + tid < lay.P) ? pair_of(p0 + tid, lay.C) : make_ushort2(0, 0);
   if (tid == 0) {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(1));
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   pdl_wait();  // S, rsq and the energy partials come from the preceding kernels; the outputs may still be read by a consumer
+  __syncthreads();
   if (tid == 0) {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)),
                  "r"((uint32_t)(Cfg::TILE_BYTES + (wantG ? Cfg::ROWS_BYTES : 0))) : "memory");
@@ -126,12 +140,8 @@ pair_kernel(const float2 *__restrict__ S, const float *__restrict__ Srsq, const 
                  "l"(S + (int64_t)blockIdx.x * F * PB), "r"((uint32_t)Cfg::TILE_BYTES), "r"(smem_u32(bar))
                  : "memory");
   }
-  if (tid < PB) {
-    const ushort2 ij = (p0 + tid < lay.P) ? pairs[p0 + tid] : make_ushort2(0, 0);
-    ij_s[tid] = ij;
-  }
-  __syncthreads();
-  if (tid < PB && wantG) {  // this pair's 1/sqrt(S_jj) row (the expect_tx above is ordered before these copies by the barrier)
+  if (tid < PB && wantG) {  // this pair's 1/sqrt(S_jj) row; a lane's complete_tx may precede lane 0's expect_tx: the
+                            // transaction count is signed and the phase cannot complete before lane 0's arrival
     const ushort2 ij = ij_s[tid];
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(rowj + tid * Cfg::FP)),
                  "l"(Srsq + (int64_t)ij.y * Cfg::FP), "r"((uint32_t)(Cfg::FP * sizeof(float))), "r"(smem_u32(bar))
@@ -294,7 +304,7 @@ static int launch_pair_L(delta_plan *p, const float *d_S, const float *d_rsq, co
     if (rc) return rc;                                                                                              \
     LaunchCfg lc(dim3((unsigned)lay.Pblk), dim3(Cfg::THREADS), Cfg::SMEM, st, p->use_pdl);                          \
     DELTA_CUDA_CHECK(cudaLaunchKernelEx(&lc.cfg, pair_kernel<L, FULL_, GAPALL_>, reinterpret_cast<const float2 *>(d_S), \
-                                        d_rsq, rpart, nrp, rp_stride, rscale, p->d_pairs(), p->d_tw(), p->d_ftab(), lay, pc, \
+                                        d_rsq, rpart, nrp, rp_stride, rscale, p->d_tw(), p->d_ftab(), lay, pc, \
                                         d_G, d_A, d_P, d_R));                                                       \
   } while (0)
   const bool gapall = d_G && d_A && d_P;
