@@ -102,8 +102,10 @@ int delta_plan_create(const delta_config *cfg, delta_plan **out) {
   }
   p->h_ftab.resize((size_t)fft_table_size(l.N) + 1);
   fft_twiddle_table(l.N, p->h_ftab.data());
+  p->h_ftab2.resize((size_t)fft_table_size(l.N, pair_fft_variant(l.N)) + 1);
+  fft_twiddle_table(l.N, p->h_ftab2.data(), pair_fft_variant(l.N));
   {
-    const int E = l.N <= 64 ? 8 : 16;  // FftGeom<N>::E
+    const int E = pair_fft_points(l.N);  // E of the pair kernel's FFT geometry
     const int Tg = l.N / E;
     for (int u = 0; u < 16; ++u) {
       const long long e = ((long long)Tg * u) % L;
@@ -129,6 +131,7 @@ int delta_plan_create(const delta_config *cfg, delta_plan **out) {
   w.off_tw = take((size_t)L * sizeof(float2));
   w.off_win = take((size_t)L * sizeof(float));
   w.off_ftab = take(p->h_ftab.size() * sizeof(float2));
+  w.off_ftab2 = take(p->h_ftab2.size() * sizeof(float2));
   w.off_pairs = take((size_t)(l.P > 0 ? l.P : 1) * sizeof(ushort2));
   w.off_offs = take((size_t)l.C * sizeof(double));
   w.off_isum = take((size_t)l.C * sizeof(long long));
@@ -185,6 +188,7 @@ int delta_plan_set_workspace(delta_plan *p, void *d_ws, size_t bytes, void *stre
   DELTA_CUDA_CHECK(cudaMemcpyAsync(p->ws + p->wsl.off_tw, p->h_tw.data(), (size_t)l.L * sizeof(float2), cudaMemcpyHostToDevice, st));
   DELTA_CUDA_CHECK(cudaMemcpyAsync(p->ws + p->wsl.off_win, p->h_win.data(), (size_t)l.L * sizeof(float), cudaMemcpyHostToDevice, st));
   DELTA_CUDA_CHECK(cudaMemcpyAsync(p->ws + p->wsl.off_ftab, p->h_ftab.data(), p->h_ftab.size() * sizeof(float2), cudaMemcpyHostToDevice, st));
+  DELTA_CUDA_CHECK(cudaMemcpyAsync(p->ws + p->wsl.off_ftab2, p->h_ftab2.data(), p->h_ftab2.size() * sizeof(float2), cudaMemcpyHostToDevice, st));
   if (l.P > 0)
     DELTA_CUDA_CHECK(cudaMemcpyAsync(p->ws + p->wsl.off_pairs, p->h_pairs.data(), (size_t)l.P * sizeof(ushort2), cudaMemcpyHostToDevice, st));
   // zero rows C..Cp-1 of the workspace X once (kernels never write them)

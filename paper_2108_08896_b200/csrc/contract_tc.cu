@@ -422,7 +422,10 @@ int launch_contract_tc(delta_plan *p, const void *d_X, float *d_S, float *d_auto
   prm.kstep_elems = (int64_t)2 * lay.Cp * kSegBlock;
   const size_t fixed = (size_t)lay.Cp * sizeof(float2) + 64 * sizeof(uint64_t) + 64;
   int nstage = (int)((200 * 1024 - fixed) / prm.stage_bytes);
-  if (nstage > 8) nstage = 8;
+#ifndef DELTA_TC_MAX_STAGES
+#define DELTA_TC_MAX_STAGES 8
+#endif
+  if (nstage > DELTA_TC_MAX_STAGES) nstage = DELTA_TC_MAX_STAGES;
   if (nstage < 2) return DELTA_ERR_UNSUPPORTED;
   prm.nstage = nstage;
   prm.unit_major = (2 * prm.ksteps <= nstage) ? 1 : 0;

@@ -24,6 +24,12 @@ struct TcHostPlan {
 bool tc_plan_tiles(int Cp, TcHostPlan *out);
 
 // pairs per block of the S layout = pairs per CTA of the pair kernel (its S tile must fit shared memory)
+// FFT geometry variant of the pair kernel (fft_reg.cuh): narrow (8 points per thread, one warp per pair) where it exists
+#ifndef DELTA_PAIR_NARROW
+#define DELTA_PAIR_NARROW 0  // measured on B200: 35.6 us (narrow, 48 warps/SM) against 34.3 us (wide, 32 warps/SM) at config 2
+#endif
+constexpr int pair_fft_variant(int N) { return (DELTA_PAIR_NARROW && N == 256) ? 1 : 0; }
+constexpr int pair_fft_points(int N) { return (N <= 64 || pair_fft_variant(N) == 1) ? 8 : 16; }  // E of that geometry
 constexpr int pair_block(int L) { return L <= 1024 ? 16 : (L == 2048 ? 8 : 4); }
 
 struct Layout {
@@ -43,7 +49,7 @@ struct Layout {
 };
 
 struct Workspace {
-  size_t off_tw, off_win, off_ftab, off_pairs, off_offs, off_isum, off_chscale, off_X, off_S, off_auto, off_rsq, off_wpart, off_rsum, total;
+  size_t off_tw, off_win, off_ftab, off_ftab2, off_pairs, off_offs, off_isum, off_chscale, off_X, off_S, off_auto, off_rsq, off_wpart, off_rsum, total;
 };
 
 }  // namespace delta
@@ -59,6 +65,7 @@ struct delta_plan {
   std::vector<float> h_win;      // periodic Hann
   float2 h_wstep[16];            // e^{-2 pi i T u / L}, u < E: bin f = gt + T u of a thread has twiddle tw[gt] * wstep[u]
   std::vector<float2> h_ftab;    // per-pass twiddles of the register FFT (fft_reg.cuh), N = L/2
+  std::vector<float2> h_ftab2;   // the same for the pair kernel's geometry variant
   std::vector<ushort2> h_pairs;  // (i, j) of pair p, lexicographic
   delta::TcHostPlan tc;
   int num_sms = 148;
@@ -81,6 +88,7 @@ struct delta_plan {
   const float2 *d_tw() const { return reinterpret_cast<const float2 *>(ws + wsl.off_tw); }
   const float *d_win() const { return reinterpret_cast<const float *>(ws + wsl.off_win); }
   const float2 *d_ftab() const { return reinterpret_cast<const float2 *>(ws + wsl.off_ftab); }
+  const float2 *d_ftab2() const { return reinterpret_cast<const float2 *>(ws + wsl.off_ftab2); }
   const ushort2 *d_pairs() const { return reinterpret_cast<const ushort2 *>(ws + wsl.off_pairs); }
   double *d_offs() const { return reinterpret_cast<double *>(ws + wsl.off_offs); }
   long long *d_isum() const { return reinterpret_cast<long long *>(ws + wsl.off_isum); }

@@ -109,23 +109,27 @@ struct Dft<16, INV> {
 };
 
 // ---------------------------------------------------------------------------------------------
-template <int N>
+// Geometry of a transform: E points per thread, NP passes of radices R0, R1, R2.  Variant V = 0 is the default
+// (E = 16 where possible: fewest exchanges, used by the STFT); V = 1 is the narrow variant (E = 8: half the registers per
+// thread and a whole warp per 256-point transform, used by the pair kernel where occupancy matters more).
+template <int N, int V = 0>
 struct FftGeom;
-#define DELTA_FFT_GEOM(N_, E_, NP_, R0_, R1_, R2_)                                          \
+#define DELTA_FFT_GEOM(N_, V_, E_, NP_, R0_, R1_, R2_)                                      \
   template <>                                                                               \
-  struct FftGeom<N_> {                                                                      \
-    static constexpr int E = E_, NP = NP_, R0 = R0_, R1 = R1_, R2 = R2_, T = N_ / E_;       \
+  struct FftGeom<N_, V_> {                                                                  \
+    static constexpr int N = N_, E = E_, NP = NP_, R0 = R0_, R1 = R1_, R2 = R2_, T = N_ / E_; \
     static constexpr int BUF = N_ + N_ / 16;                      /* padded exchange buffer */ \
     static constexpr int OFF1 = (R0_ - 1) * (N_ / R0_);           /* table offset of pass 1 */ \
     static constexpr int TABLE = OFF1 + (NP_ == 3 ? (R1_ - 1) * (N_ / (R0_ * R1_)) : 0);      \
   };
-DELTA_FFT_GEOM(32, 8, 2, 8, 4, 1)
-DELTA_FFT_GEOM(64, 8, 2, 8, 8, 1)
-DELTA_FFT_GEOM(128, 16, 2, 16, 8, 1)
-DELTA_FFT_GEOM(256, 16, 2, 16, 16, 1)
-DELTA_FFT_GEOM(512, 16, 3, 8, 8, 8)
-DELTA_FFT_GEOM(1024, 16, 3, 16, 8, 8)
-DELTA_FFT_GEOM(2048, 16, 3, 16, 16, 8)
+DELTA_FFT_GEOM(32, 0, 8, 2, 8, 4, 1)
+DELTA_FFT_GEOM(64, 0, 8, 2, 8, 8, 1)
+DELTA_FFT_GEOM(128, 0, 16, 2, 16, 8, 1)
+DELTA_FFT_GEOM(256, 0, 16, 2, 16, 16, 1)
+DELTA_FFT_GEOM(512, 0, 16, 3, 8, 8, 8)
+DELTA_FFT_GEOM(1024, 0, 16, 3, 16, 8, 8)
+DELTA_FFT_GEOM(2048, 0, 16, 3, 16, 16, 8)
+DELTA_FFT_GEOM(256, 1, 8, 3, 8, 8, 4)
 #undef DELTA_FFT_GEOM
 
 DELTA_HD int fft_pad(int i) { return i + (i >> 4); }
@@ -143,9 +147,9 @@ DELTA_HD float2 fft_ld_tw(const float2 *p) {
 }
 
 // One pass.  LAST: results stay in registers (natural order, see header); otherwise they go to `buf`.
-template <int N, int R, int S, bool LAST, bool INV, class Map>
+template <class G, int R, int S, bool LAST, bool INV, class Map>
 DELTA_HD void fft_pass(float2 *v, const Map &m, const float2 *tp, int tid) {
-  using G = FftGeom<N>;
+  constexpr int N = G::N;
   constexpr int NB = G::E / R, CNT = N / (R * S);
 #pragma unroll
   for (int i = 0; i < NB; ++i) {
@@ -171,9 +175,8 @@ DELTA_HD void fft_pass(float2 *v, const Map &m, const float2 *tp, int tid) {
   }
 }
 
-template <int N, class Map>
+template <class G, class Map>
 DELTA_HD void fft_readback(float2 *v, const Map &m, int tid) {
-  using G = FftGeom<N>;
 #pragma unroll
   for (int u = 0; u < G::E; ++u) v[u] = m(tid + G::T * u);
 }
@@ -189,51 +192,51 @@ __device__ __forceinline__ void fft_group_sync() {
 // v[u] <-> x[tid + T*u] in, X[tid + T*u] out (unnormalised).  The slots behind `m` are shared memory owned
 // by the group; other threads of the group may still be reading them when the call returns, so the group
 // must pass another fft_group_sync before it writes them again.
-template <int N, bool INV, class Map>
-__device__ __forceinline__ void fft_inplace(float2 *v, const Map &m, const float2 *__restrict__ tp, int tid) {
-  using G = FftGeom<N>;
-  fft_pass<N, G::R0, 1, false, INV>(v, m, tp, tid);
+template <class G, bool INV, class Map>
+__device__ __forceinline__ void fft_inplace_g(float2 *v, const Map &m, const float2 *__restrict__ tp, int tid) {
+  fft_pass<G, G::R0, 1, false, INV>(v, m, tp, tid);
   fft_group_sync<G::T>();
-  fft_readback<N>(v, m, tid);
+  fft_readback<G>(v, m, tid);
   if constexpr (G::NP == 2) {
-    fft_pass<N, G::R1, G::R0, true, INV>(v, m, tp, tid);
+    fft_pass<G, G::R1, G::R0, true, INV>(v, m, tp, tid);
   } else {
     fft_group_sync<G::T>();
-    fft_pass<N, G::R1, G::R0, false, INV>(v, m, tp + G::OFF1, tid);
+    fft_pass<G, G::R1, G::R0, false, INV>(v, m, tp + G::OFF1, tid);
     fft_group_sync<G::T>();
-    fft_readback<N>(v, m, tid);
-    fft_pass<N, G::R2, G::R0 * G::R1, true, INV>(v, m, tp, tid);
+    fft_readback<G>(v, m, tid);
+    fft_pass<G, G::R2, G::R0 * G::R1, true, INV>(v, m, tp, tid);
   }
+}
+template <int N, bool INV, class Map>
+__device__ __forceinline__ void fft_inplace(float2 *v, const Map &m, const float2 *__restrict__ tp, int tid) {
+  fft_inplace_g<FftGeom<N, 0>, INV>(v, m, tp, tid);
 }
 #endif
 
 // Host: the per-pass twiddle tables of FftGeom<N> (forward sign), float64 -> float32.
 // `out` must hold fft_table_size(N) entries.  Returns the entry count, 0 for an unsupported N.
-inline void fft_radices(int N, int *np, int *r) {
+inline void fft_radices(int N, int V, int *np, int *r) {
   *np = 0;
   r[0] = r[1] = r[2] = 1;
-#define DELTA_FFT_CASE(N_) \
-  case N_: *np = FftGeom<N_>::NP; r[0] = FftGeom<N_>::R0; r[1] = FftGeom<N_>::R1; r[2] = FftGeom<N_>::R2; break;
-  switch (N) {
-    DELTA_FFT_CASE(32) DELTA_FFT_CASE(64) DELTA_FFT_CASE(128) DELTA_FFT_CASE(256)
-    DELTA_FFT_CASE(512) DELTA_FFT_CASE(1024) DELTA_FFT_CASE(2048)
-    default: break;
-  }
+#define DELTA_FFT_CASE(N_, V_) \
+  if (N == N_ && V == V_) { *np = FftGeom<N_, V_>::NP; r[0] = FftGeom<N_, V_>::R0; r[1] = FftGeom<N_, V_>::R1; r[2] = FftGeom<N_, V_>::R2; }
+  DELTA_FFT_CASE(32, 0) DELTA_FFT_CASE(64, 0) DELTA_FFT_CASE(128, 0) DELTA_FFT_CASE(256, 0)
+  DELTA_FFT_CASE(512, 0) DELTA_FFT_CASE(1024, 0) DELTA_FFT_CASE(2048, 0) DELTA_FFT_CASE(256, 1)
 #undef DELTA_FFT_CASE
 }
 
-inline int fft_table_size(int N) {
+inline int fft_table_size(int N, int V = 0) {
   int np, r[3];
-  fft_radices(N, &np, r);
+  fft_radices(N, V, &np, r);
   if (np == 0) return 0;
   int n = (r[0] - 1) * (N / r[0]);
   if (np == 3) n += (r[1] - 1) * (N / (r[0] * r[1]));
   return n;
 }
 
-inline int fft_twiddle_table(int N, float2 *out) {
+inline int fft_twiddle_table(int N, float2 *out, int V = 0) {
   int np, r[3];
-  fft_radices(N, &np, r);
+  fft_radices(N, V, &np, r);
   if (np == 0) return 0;
   int o = 0, S = 1;
   for (int p = 0; p + 1 < np; ++p) {

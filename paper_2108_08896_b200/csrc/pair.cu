@@ -27,14 +27,13 @@ struct PairConsts {
 template <int L>
 struct PairCfg {
   static constexpr int N = L / 2, F = N + 1;
-  using G = FftGeom<N>;
+  using G = FftGeom<N, pair_fft_variant(N)>;
   static constexpr int T = G::T, E = G::E;
   static constexpr int PB = pair_block(L);
   static constexpr int THREADS = PB * T;
-#ifndef DELTA_PAIR_WARPS
-#define DELTA_PAIR_WARPS 32  // resident warps per SM the register budget is sized for
-#endif
-  static constexpr int MIN_CTAS = (DELTA_PAIR_WARPS * 32) / THREADS > 0 ? (DELTA_PAIR_WARPS * 32) / THREADS : 1;
+  // resident warps per SM the register budget is sized for: 48 (40 registers) with 8 points per thread, else 32 (64)
+  static constexpr int WARPS = E <= 8 ? 48 : 32;
+  static constexpr int MIN_CTAS = (WARPS * 32) / THREADS > 0 ? (WARPS * 32) / THREADS : 1;
   static constexpr size_t TILE_BYTES = (size_t)F * PB * sizeof(float2);
   static constexpr size_t EXCH_BYTES = (size_t)PB * G::BUF * sizeof(float2);
   static constexpr size_t BUF_BYTES = ((TILE_BYTES > EXCH_BYTES ? TILE_BYTES : EXCH_BYTES) + 15) & ~(size_t)15;
@@ -169,47 +168,74 @@ pair_kernel(const float2 *__restrict__ S, const float *__restrict__ Srsq, const 
   const int pl = tid / T, gt = tid % T;
   const int64_t p = p0 + pl;
   const bool valid = p < lay.P;
-  const ushort2 ij = ij_s[pl];
-  const bool gap = (G || A || Pw) && valid;
-  const float *ri = Srsq + (int64_t)ij.x * Cfg::FP, *rj = rowj + pl * Cfg::FP;
   const float2 wg = __ldg(tw + gt);  // e^{-2 pi i gt / L}
-  const int64_t o = p * F;
 
-  // ---- pass 1: G, A, P of the thread's bins -----------------------------------------------------------------
-  // The loads of a batch of UB bins (S from the tile, 1/sqrt(S_ii) from global memory, 1/sqrt(S_jj) from the staged
-  // row) are issued together; nothing else is live in registers yet, so their latencies overlap.
-  const int pg = pl ^ gt;
-  if (gap) {
-    auto emit = [&](float2 s, float gi, float gj, int f) {
-      const float mag = sqrt_approx(fmaf(s.x, s.x, s.y * s.y));
-      if (GAPALL || Pw) Pw[o + f] = mag;
-      if (GAPALL || G) G[o + f] = mag * gi * gj;
-      if (GAPALL || A) A[o + f] = atan2_poly(s.y, s.x);
+  // ---- pass 1: G, A, P ------------------------------------------------------------------------------------------
+  // The store path is what binds this kernel (without its stores it runs in half the time), so pass 1 has its own
+  // thread mapping: a thread owns 4 consecutive bins of one pair and stores float4; a warp covers 512 contiguous
+  // bytes of one row.  Rows have F = N + 1 floats (F mod 4 = 1), so element (p, f) is 16-byte aligned iff
+  // (p + f) mod 4 = 0: the groups of pair p start at f0 = (-p) mod 4; the f0 head and the 0..3 tail bins go scalar.
+  if ((G || A || Pw) && p0 < lay.P) {
+    auto value = [&](float2 s, float g2, float &mag, float &coh, float &ang) {
+      mag = sqrt_approx(fmaf(s.x, s.x, s.y * s.y));
+      coh = mag * g2;
+      ang = atan2_poly(s.y, s.x);
     };
-    constexpr int UB = E < 8 ? E : 8;
+    constexpr int NG = N / 4;  // group slots per pair
+    const bool vec4 = (((reinterpret_cast<uintptr_t>(G) | reinterpret_cast<uintptr_t>(A) | reinterpret_cast<uintptr_t>(Pw)) & 15) == 0);
+    if (vec4) {
+#pragma unroll 2
+      for (int item = tid; item < PB * NG; item += THREADS) {
+        const int ql = item / NG, g = item % NG;
+        const int64_t q = p0 + ql;
+        const int f0 = (int)((-q) & 3), ng = (F - f0) >> 2;
+        if (q >= lay.P || g >= ng) continue;
+        const int f = f0 + 4 * g;
+        const ushort2 qij = ij_s[ql];
+        const float *qi = Srsq + (int64_t)qij.x * Cfg::FP + f, *qj = rowj + ql * Cfg::FP + f;
+        float2 sv[4];
+        float g2[4];
 #pragma unroll
-    for (int ub = 0; ub < E; ub += UB) {
-      float2 sf[UB];
-      float gi[UB], gj[UB];
+        for (int k = 0; k < 4; ++k) {
+          sv[k] = tile[(f + k) * PB + ((ql ^ (f + k)) & (PB - 1))];
+          g2[k] = wantG ? __ldg(qi + k) * qj[k] : 0.f;
+        }
+        float m[4], c[4], an[4];
 #pragma unroll
-      for (int k = 0; k < UB; ++k) {
-        const int u = ub + k;
-        const int f = gt + T * u;  // gt < T and T is a power of two, so f = gt | T u
-        sf[k] = tile[f * PB + ((pg ^ (T * u)) & (PB - 1))];
-        gi[k] = wantG ? __ldg(ri + f) : 0.f;
-        gj[k] = wantG ? rj[f] : 0.f;
+        for (int k = 0; k < 4; ++k) value(sv[k], g2[k], m[k], c[k], an[k]);
+        const int64_t at = q * F + f;
+        if (GAPALL || Pw) *reinterpret_cast<float4 *>(Pw + at) = make_float4(m[0], m[1], m[2], m[3]);
+        if (GAPALL || G) *reinterpret_cast<float4 *>(G + at) = make_float4(c[0], c[1], c[2], c[3]);
+        if (GAPALL || A) *reinterpret_cast<float4 *>(A + at) = make_float4(an[0], an[1], an[2], an[3]);
       }
-#pragma unroll
-      for (int k = 0; k < UB; ++k) emit(sf[k], gi[k], gj[k], gt + T * (ub + k));
     }
-    if (gt == 0)  // the Nyquist bin
-      emit(tile[N * PB + ((pl ^ N) & (PB - 1))], wantG ? __ldg(ri + N) : 0.f, wantG ? rj[N] : 0.f, N);
+    // scalar bins: the edges of the vector path (at most 6 per pair), or everything if the arrays are not 16-byte aligned
+    const int per = vec4 ? 8 : F;
+    for (int item = tid; item < PB * per; item += THREADS) {
+      const int ql = item / per, e = item % per;
+      const int64_t q = p0 + ql;
+      if (q >= lay.P) continue;
+      int f = e;
+      if (vec4) {
+        const int f0 = (int)((-q) & 3), ng = (F - f0) >> 2;
+        f = e < f0 ? e : f0 + 4 * ng + (e - f0);
+        if (f >= F) continue;
+      }
+      const ushort2 qij = ij_s[ql];
+      const float g2 = wantG ? __ldg(Srsq + (int64_t)qij.x * Cfg::FP + f) * rowj[ql * Cfg::FP + f] : 0.f;
+      float m, c, an;
+      value(tile[f * PB + ((ql ^ f) & (PB - 1))], g2, m, c, an);
+      if (GAPALL || Pw) Pw[q * F + f] = m;
+      if (GAPALL || G) G[q * F + f] = c;
+      if (GAPALL || A) A[q * F + f] = an;
+    }
   }
   if (!wantR) return;
 
   // ---- pass 2: merge step of the inverse real transform (S read again from the tile; twice the merge of
   // irfft_merge, the factor 1/2 goes into the normalisation) ------------------------------------------------
   float2 v[E];
+  const int pg = pl ^ gt;
 #pragma unroll
   for (int u = 0; u < E; ++u) {
     const int f = gt + T * u;
@@ -223,13 +249,10 @@ pair_kernel(const float2 *__restrict__ S, const float *__restrict__ Srsq, const 
   __syncthreads();  // every S value is in registers: the tile becomes exchange space
 
   // ---- rho = irfft(S) / sqrt(R_ii[0] R_jj[0]) ----------------------------------------------------------------
-  fft_inplace<N, true>(v, FftPadMap{exch + pl * Geo::BUF}, ftab, gt);  // z[n] = (x[2n], x[2n+1]) * N, n = gt + T u
+  fft_inplace_g<Geo, true>(v, FftPadMap{exch + pl * Geo::BUF}, ftab, gt);  // z[n] = (x[2n], x[2n+1]) * N, n = gt + T u
   if (!valid) return;
-  int ki = pl, kj = pl;  // entries that hold the sums of this pair's channels
-  while (ki > 0 && ij_s[ki - 1].x == ij.x) --ki;
-  while (kj > 0 && ij_s[kj - 1].y == ij.y) --kj;
   // rho = x / sqrt(R_ii[0] R_jj[0]),  x = z/N,  R_cc[0] = (sum over all L bins of S_cc)/L
-  const float norm = rs[ki] * rs[PB + kj];  // 2 (L/N) x 1/2 (irfft_merge2)
+  const float norm = rs[pl] * rs[PB + pl];  // 2 (L/N) x 1/2 (irfft_merge2)
   float *Rp = R + p * lay.nlags;
   if (FULL) {
     // lag m = xi for xi <= L/2 and xi - L for xi >= L/2; row position q = m + L/2
@@ -239,6 +262,9 @@ pair_kernel(const float2 *__restrict__ S, const float *__restrict__ Srsq, const 
       const int n = gt + T * u;
       const float a = v[u].x * norm, b = v[u].y * norm;
       const int q = (u < E / 2) ? 2 * n + N : 2 * n - N;
+#ifdef DELTA_DBG_NOSTORE_R
+      if (lay.P < 0)
+#endif
       if (vec) {
         *reinterpret_cast<float2 *>(Rp + q) = make_float2(a, b);
       } else {
@@ -304,7 +330,7 @@ static int launch_pair_L(delta_plan *p, const float *d_S, const float *d_rsq, co
     if (rc) return rc;                                                                                              \
     LaunchCfg lc(dim3((unsigned)lay.Pblk), dim3(Cfg::THREADS), Cfg::SMEM, st, p->use_pdl);                          \
     DELTA_CUDA_CHECK(cudaLaunchKernelEx(&lc.cfg, pair_kernel<L, FULL_, GAPALL_>, reinterpret_cast<const float2 *>(d_S), \
-                                        d_rsq, rpart, nrp, rp_stride, rscale, p->d_tw(), p->d_ftab(), lay, pc, \
+                                        d_rsq, rpart, nrp, rp_stride, rscale, p->d_tw(), p->d_ftab2(), lay, pc, \
                                         d_G, d_A, d_P, d_R));                                                       \
   } while (0)
   const bool gapall = d_G && d_A && d_P;
