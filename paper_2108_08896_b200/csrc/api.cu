@@ -136,6 +136,8 @@ int delta_plan_create(const delta_config *cfg, delta_plan **out) {
   w.off_offs = take((size_t)l.C * sizeof(double));
   w.off_isum = take((size_t)l.C * sizeof(long long));
   w.off_chscale = take((size_t)l.C * sizeof(float));
+  w.off_chmax = take((size_t)l.C * sizeof(unsigned));
+  w.off_chcnt = take((size_t)l.C * sizeof(unsigned));
   w.off_X = take((size_t)l.F * l.x_elems_per_f * (p->contraction == DELTA_CONTRACT_TC ? 2 : 4));
   w.off_S = take((size_t)(l.Pblk > 0 ? l.Pblk : 1) * l.F * l.PB * sizeof(float2));
   w.off_auto = take((size_t)l.C * l.F * sizeof(float));

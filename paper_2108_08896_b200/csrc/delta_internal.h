@@ -49,7 +49,7 @@ struct Layout {
 };
 
 struct Workspace {
-  size_t off_tw, off_win, off_ftab, off_ftab2, off_pairs, off_offs, off_isum, off_chscale, off_X, off_S, off_auto, off_rsq, off_wpart, off_rsum, total;
+  size_t off_tw, off_win, off_ftab, off_ftab2, off_pairs, off_offs, off_isum, off_chscale, off_chmax, off_chcnt, off_X, off_S, off_auto, off_rsq, off_wpart, off_rsum, total;
 };
 
 }  // namespace delta
@@ -93,6 +93,8 @@ struct delta_plan {
   double *d_offs() const { return reinterpret_cast<double *>(ws + wsl.off_offs); }
   long long *d_isum() const { return reinterpret_cast<long long *>(ws + wsl.off_isum); }
   float *d_chscale() const { return reinterpret_cast<float *>(ws + wsl.off_chscale); }
+  unsigned *d_chmax() const { return reinterpret_cast<unsigned *>(ws + wsl.off_chmax); }  // zero between launches
+  unsigned *d_chcnt() const { return reinterpret_cast<unsigned *>(ws + wsl.off_chcnt); }  // zero between launches
   void *d_X() const { return ws + wsl.off_X; }
   float *d_S() const { return reinterpret_cast<float *>(ws + wsl.off_S); }
   float *d_auto() const { return reinterpret_cast<float *>(ws + wsl.off_auto); }

@@ -116,40 +116,79 @@ struct SampleLoader {
 };
 
 // per-channel power-of-two scale for the split-fp16 operands: |X| <= (L/2) max|y|  =>  scale * |X| <= 2^14.
-// One CTA of 1024 threads per channel; one pass over the chunk.
-__global__ void __launch_bounds__(1024)
+__device__ __forceinline__ float scale_from_max(float m, int L) {
+  const float bound = m * (0.5f * (float)L);  // sum_n w[n] |y| <= (L/2) max|y|
+  float sc = 1.f;
+  if (bound > 0.f && isfinite(bound)) {
+    int e;
+    frexpf(bound, &e);         // bound = mant * 2^e, mant in [0.5, 1)  =>  bound < 2^e
+    sc = ldexpf(1.f, 14 - e);  // scale * bound < 2^14
+  }
+  return sc;
+}
+
+// One pass over the chunk for chunks too long for the cluster variant of stft_kernel.  grid = (C, NS): every block
+// takes a slice of one channel (16-byte loads), the blocks of a channel combine their maxima with atomicMax on the
+// float bits (all values are >= 0) and the last one to arrive writes the scale and re-arms the two words.
+__global__ void __launch_bounds__(256)
 chscale_kernel(const void *__restrict__ x, int64_t ld, int in_dtype, int norm_mode, int n_first,
                const double *__restrict__ offs, const long long *__restrict__ isum, int T, int L,
-               float *__restrict__ chscale) {
-  const int c = blockIdx.x;
+               float *__restrict__ chscale, unsigned *__restrict__ chmax, unsigned *__restrict__ chcnt) {
+  const int c = blockIdx.x, NS = gridDim.y, tid = threadIdx.x;
   SampleLoader ldr;
   ldr.init(x, in_dtype, norm_mode, n_first, offs, isum, c);
   const int64_t row0 = (int64_t)c * ld;
-  const size_t esz = in_dtype == DELTA_I16 ? 2 : 4;
-  const bool pair_ok = ((row0 & 1) == 0) && ((reinterpret_cast<uintptr_t>(x) & (2 * esz - 1)) == 0);
+  const int per = (((T + NS - 1) / NS) + 7) & ~7;
+  const int s0 = blockIdx.y * per, s1 = min(T, s0 + per);
   float m = 0.f;
-  const int npairs = T >> 1;
-  for (int t = threadIdx.x; t < npairs; t += 1024) {
-    const float2 v = ldr.two(row0 + 2 * t, pair_ok);
-    m = fmaxf(m, fmaxf(fabsf(v.x), fabsf(v.y)));
-  }
-  if ((T & 1) && threadIdx.x == 0) m = fmaxf(m, fabsf(ldr(row0 + T - 1)));
-  for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
-  __shared__ float red[32];
-  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = m;
-  __syncthreads();
-  if (threadIdx.x < 32) {
-    m = red[threadIdx.x];
-    for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
-    if (threadIdx.x == 0) {
-      const float bound = m * (0.5f * (float)L);  // sum_n w[n] |y| <= (L/2) max|y|
-      float sc = 1.f;
-      if (bound > 0.f && isfinite(bound)) {
-        int e;
-        frexpf(bound, &e);         // bound = mant * 2^e, mant in [0.5, 1)  =>  bound < 2^e
-        sc = ldexpf(1.f, 14 - e);  // scale * bound < 2^14
+  if (in_dtype == DELTA_I16) {
+    const short *r = reinterpret_cast<const short *>(x) + row0;
+    int t = s0 + tid;
+    if ((reinterpret_cast<uintptr_t>(r + s0) & 15) == 0) {
+      const int nv = (s1 - s0) >> 3;
+#pragma unroll 4
+      for (int q = tid; q < nv; q += 256) {
+        const uint4 v = *reinterpret_cast<const uint4 *>(r + s0 + 8 * q);
+        const unsigned wv[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+          m = fmaxf(m, fabsf(ldr.conv_i16((short)(wv[k] & 0xffffu))));
+          m = fmaxf(m, fabsf(ldr.conv_i16((short)(wv[k] >> 16))));
+        }
       }
-      chscale[c] = sc;
+      t = s0 + 8 * nv + tid;
+    }
+    for (; t < s1; t += 256) m = fmaxf(m, fabsf(ldr.conv_i16(r[t])));
+  } else {
+    const float *r = reinterpret_cast<const float *>(x) + row0;
+    int t = s0 + tid;
+    if ((reinterpret_cast<uintptr_t>(r + s0) & 15) == 0) {
+      const int nv = (s1 - s0) >> 2;
+#pragma unroll 4
+      for (int q = tid; q < nv; q += 256) {
+        const float4 v = *reinterpret_cast<const float4 *>(r + s0 + 4 * q);
+        m = fmaxf(fmaxf(m, fabsf(ldr.conv_f32(v.x))), fabsf(ldr.conv_f32(v.y)));
+        m = fmaxf(fmaxf(m, fabsf(ldr.conv_f32(v.z))), fabsf(ldr.conv_f32(v.w)));
+      }
+      t = s0 + 4 * nv + tid;
+    }
+    for (; t < s1; t += 256) m = fmaxf(m, fabsf(ldr.conv_f32(r[t])));
+  }
+  for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
+  __shared__ float red[8];
+  if ((tid & 31) == 0) red[tid >> 5] = m;
+  __syncthreads();
+  if (tid == 0) {
+#pragma unroll
+    for (int w = 1; w < 8; ++w) m = fmaxf(m, red[w]);
+    if (!(m == m)) m = __int_as_float(0x7f800000);  // NaN input: treat as +inf (scale 1)
+    atomicMax(chmax + c, __float_as_uint(m));
+    __threadfence();
+    if (atomicAdd(chcnt + c, 1u) == (unsigned)(NS - 1)) {
+      __threadfence();
+      const float mm = __uint_as_float(atomicExch(chmax + c, 0u));
+      chcnt[c] = 0u;
+      chscale[c] = scale_from_max(mm, L);
     }
   }
 }
@@ -306,13 +345,7 @@ stft_kernel(const void *__restrict__ x, int64_t ld, int in_dtype, int norm_mode,
       float m = 0.f;
       const unsigned nb = cluster.num_blocks();
       for (unsigned r = 0; r < nb; ++r) m = fmaxf(m, *cluster.map_shared_rank(&cmax[tid], r));
-      const float bound = m * (0.5f * (float)L);
-      float sc = 1.f;
-      if (bound > 0.f && isfinite(bound)) {
-        int e;
-        frexpf(bound, &e);
-        sc = ldexpf(1.f, 14 - e);
-      }
+      const float sc = scale_from_max(m, L);
       csc[tid] = sc;
       if (kb == 0 && c0 + tid < lay.C) chscale[c0 + tid] = sc;
     }
@@ -437,8 +470,10 @@ static int launch_stft_L(delta_plan *p, const void *d_x, int64_t ld, void *d_X, 
   const Layout &lay = p->lay;
   if (p->contraction == DELTA_CONTRACT_TC) {
     if (lay.nkb <= 8) return launch_stft_LT<L, true, true>(p, d_x, ld, d_X, st);  // scale agreed inside the cluster
-    chscale_kernel<<<lay.C, 1024, 0, st>>>(d_x, ld, p->cfg.in_dtype, p->cfg.norm_mode, p->n_first, p->d_offs(), p->d_isum(),
-                                           lay.T, lay.L, p->d_chscale());
+    int ns = (8 * p->num_sms + lay.C - 1) / lay.C;  // about 8 blocks per SM
+    ns = ns < 1 ? 1 : (ns > 64 ? 64 : ns);
+    chscale_kernel<<<dim3(lay.C, ns), 256, 0, st>>>(d_x, ld, p->cfg.in_dtype, p->cfg.norm_mode, p->n_first, p->d_offs(),
+                                                    p->d_isum(), lay.T, lay.L, p->d_chscale(), p->d_chmax(), p->d_chcnt());
     p->launches++;
     DELTA_CUDA_CHECK(cudaGetLastError());
     return launch_stft_LT<L, true, false>(p, d_x, ld, d_X, st);
