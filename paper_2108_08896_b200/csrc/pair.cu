@@ -96,6 +96,18 @@ __device__ __forceinline__ ushort2 pair_of(int64_t p, int C) {
   return make_ushort2((unsigned short)i, (unsigned short)(p - start(i) + i + 1));
 }
 
+// Output stores: the results are written once and never read by this library, so they are marked streaming
+// (evict-first) to keep S and X, which the next kernels re-read, in L2.
+#ifdef DELTA_PLAIN_STORES
+#define ST4(p, v) (*reinterpret_cast<float4 *>(p) = (v))
+#define ST2(p, v) (*reinterpret_cast<float2 *>(p) = (v))
+#define ST1(p, v) (*(p) = (v))
+#else
+#define ST4(p, v) __stcs(reinterpret_cast<float4 *>(p), (v))
+#define ST2(p, v) __stcs(reinterpret_cast<float2 *>(p), (v))
+#define ST1(p, v) __stcs((p), (v))
+#endif
+
 }  // namespace
 
 // GAPALL: G, A and Pw are all requested (no per-element pointer tests)
@@ -204,9 +216,9 @@ pair_kernel(const float2 *__restrict__ S, const float *__restrict__ Srsq, const 
 #pragma unroll
         for (int k = 0; k < 4; ++k) value(sv[k], g2[k], m[k], c[k], an[k]);
         const int64_t at = q * F + f;
-        if (GAPALL || Pw) *reinterpret_cast<float4 *>(Pw + at) = make_float4(m[0], m[1], m[2], m[3]);
-        if (GAPALL || G) *reinterpret_cast<float4 *>(G + at) = make_float4(c[0], c[1], c[2], c[3]);
-        if (GAPALL || A) *reinterpret_cast<float4 *>(A + at) = make_float4(an[0], an[1], an[2], an[3]);
+        if (GAPALL || Pw) ST4(Pw + at, make_float4(m[0], m[1], m[2], m[3]));
+        if (GAPALL || G) ST4(G + at, make_float4(c[0], c[1], c[2], c[3]));
+        if (GAPALL || A) ST4(A + at, make_float4(an[0], an[1], an[2], an[3]));
       }
     }
     // scalar bins: the edges of the vector path (at most 6 per pair), or everything if the arrays are not 16-byte aligned
@@ -225,9 +237,9 @@ pair_kernel(const float2 *__restrict__ S, const float *__restrict__ Srsq, const 
       const float g2 = wantG ? __ldg(Srsq + (int64_t)qij.x * Cfg::FP + f) * rowj[ql * Cfg::FP + f] : 0.f;
       float m, c, an;
       value(tile[f * PB + ((ql ^ f) & (PB - 1))], g2, m, c, an);
-      if (GAPALL || Pw) Pw[q * F + f] = m;
-      if (GAPALL || G) G[q * F + f] = c;
-      if (GAPALL || A) A[q * F + f] = an;
+      if (GAPALL || Pw) ST1(Pw + q * F + f, m);
+      if (GAPALL || G) ST1(G + q * F + f, c);
+      if (GAPALL || A) ST1(A + q * F + f, an);
     }
   }
   if (!wantR) return;
@@ -266,12 +278,12 @@ pair_kernel(const float2 *__restrict__ S, const float *__restrict__ Srsq, const 
       if (lay.P < 0)
 #endif
       if (vec) {
-        *reinterpret_cast<float2 *>(Rp + q) = make_float2(a, b);
+        ST2(Rp + q, make_float2(a, b));
       } else {
-        Rp[q] = a;
-        Rp[q + 1] = b;
+        ST1(Rp + q, a);
+        ST1(Rp + q + 1, b);
       }
-      if (u == E / 2 && gt == 0) Rp[L] = a;  // xi = L/2 is lag -L/2 and lag +L/2
+      if (u == E / 2 && gt == 0) ST1(Rp + L, a);  // xi = L/2 is lag -L/2 and lag +L/2
     }
   } else {
     const int M = lay.M;

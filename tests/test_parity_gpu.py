@@ -312,3 +312,45 @@ def test_host_output_path_roundtrip():
     for n in range(3):
         ref = oracle_for(x[n], 128, 64, 64)
         compare({k: host[k][n].numpy() for k in host}, ref, o.all_pairs(12), f"host chunk {n}")
+
+
+def test_chunks_in_flight_two_plans_two_streams():
+    """bench.py keeps two independent chunks in flight (two plans = two workspaces, two streams).  Results must be
+    bit-identical to the same chunks analysed one after the other on one stream (P9: chunks are independent)."""
+    b = binding()
+    w = es.WORKLOADS["single"]
+    xs = [dev(es.turbulence(w.T, 700 + i)[:64]) for i in range(4)]
+    serial_plan = b.Plan(64, w.T, w.nfft, w.hop, w.max_lag)
+    serial = [{k: v.clone() for k, v in serial_plan.analyze_chunk(x).items()} for x in xs]
+    torch.cuda.synchronize()
+    plans = [b.Plan(64, w.T, w.nfft, w.hop, w.max_lag) for _ in range(2)]
+    streams = [torch.cuda.Stream() for _ in range(2)]
+    torch.cuda.synchronize()
+    outs = []
+    for rep in range(3):          # several rounds so that the kernels of the two streams really interleave
+        outs = []
+        for k, x in enumerate(xs):
+            with torch.cuda.stream(streams[k % 2]):
+                outs.append(plans[k % 2].analyze_chunk(x))
+    torch.cuda.synchronize()
+    for k in range(4):
+        for name in ("G", "A", "P", "R", "Sauto"):
+            assert torch.equal(outs[k][name], serial[k][name]), (k, name)
+
+
+def test_programmatic_dependent_launch_does_not_change_results(monkeypatch):
+    """The three kernels are chained by programmatic dependent launch; DELTA_NO_PDL=1 (read at plan creation)
+    launches them with plain stream order.  Same bits either way, also back to back on one stream."""
+    b = binding()
+    w = es.WORKLOADS["single"]
+    xs = [dev(es.turbulence(w.T, 800 + i)[:48]) for i in range(3)]
+    pdl = b.Plan(48, w.T, w.nfft, w.hop, w.max_lag)
+    monkeypatch.setenv("DELTA_NO_PDL", "1")
+    plain = b.Plan(48, w.T, w.nfft, w.hop, w.max_lag)
+    monkeypatch.delenv("DELTA_NO_PDL")
+    a = [pdl.analyze_chunk(x) for x in xs]        # no sync in between: chunk n+1 is launched while n runs
+    c = [plain.analyze_chunk(x) for x in xs]
+    torch.cuda.synchronize()
+    for k in range(3):
+        for name in ("G", "A", "P", "R", "Sauto"):
+            assert torch.equal(a[k][name], c[k][name]), (k, name)
