@@ -107,7 +107,7 @@ __device__ __forceinline__ void fence_before() { asm volatile("tcgen05.fence::be
 struct TcUnit {
   int row0;              // first channel of the 128-row A operand = channel of TMEM lane 0 (multiple of 8)
   int lane_lo, lane_hi;  // lanes [lane_lo, lane_hi) are owned by this unit (multiples of 32)
-  int col0, N;           // B operand rows = channels [col0, col0 + N), N in {32, 64, 96, 128}
+  int col0, N;           // B operand rows = channels [col0, col0 + N), N a multiple of 64 up to 256
   int tm;                // TMEM column of Re; Im follows at tm + N
 };
 struct TcParams {
@@ -373,9 +373,12 @@ bool tc_plan_tiles(int Cp, TcHostPlan *out) {
   U list[kTcMaxGroups * kTcMaxUnits];
   int n = 0;
   auto add_row_tile = [&](int r0, int lane_hi, int col_end) {
-    for (int c = 0; c < col_end; c += 128) {
+#ifndef DELTA_TC_MAX_N
+#define DELTA_TC_MAX_N 128  // widest accumulator unit (wider units were measured slower at config 2: their epilogue overlaps less)
+#endif
+    for (int c = 0, N = 0; c < col_end; c += N) {
       if (n >= kTcMaxGroups * kTcMaxUnits) return false;
-      const int N = (col_end - c) < 128 ? (col_end - c) : 128;
+      N = (col_end - c) < DELTA_TC_MAX_N ? (col_end - c) : DELTA_TC_MAX_N;
       int lane_lo = c > r0 ? ((c - r0) & ~31) : 0;  // lanes below have j < col0: nothing to keep
       list[n++] = {r0, lane_lo, lane_hi, c, N};
     }
