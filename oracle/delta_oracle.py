@@ -18,6 +18,7 @@ What it computes (citations are /root/reference/PAPER.md line numbers):
   * Eq. (1c): A_XY(w) = arctan(Im S_XY / Re S_XY)  (four-quadrant)         -> crossphase()
   * Eq. (1d), L102: R_XY = IFFT(S_XY)  (normalised, lags -M..M)                  -> crosscorr()
   * "(192 choose 2) = 18336 possible channel pair combinations" (L107)           -> all_pairs(), pair_index()
+  * optional band-pass pre-processing filter (L67, L231), reading R19              -> band_mask(), bandpass()
 
 Where the paper is silent the readings of DESIGN.md section 3 (R1..R16) apply; each function
 names the reading it uses.  Every convention that affects an output is pinned by
@@ -107,6 +108,20 @@ def stft(y: np.ndarray, L: int, H: int) -> np.ndarray:
     return X
 
 
+def band_mask(L: int, fs: float, lo_hz: float, hi_hz: float) -> np.ndarray:
+    """Pre-processing band-pass of PAPER.md L67 ("optional pre-processing filters"), L231 (the demo's 5-9 kHz pass
+    band), in reading R19: an ideal (brick-wall) mask on the bins of every segment's transform.  Bin f (frequency
+    f fs / L) is kept iff lo_hz <= f fs / L <= hi_hz, tested as lo_hz L <= f fs <= hi_hz L in float64.
+    Returns a boolean [L/2+1] array."""
+    f = np.arange(L // 2 + 1, dtype=np.float64)
+    return (np.float64(lo_hz) * L <= f * np.float64(fs)) & (f * np.float64(fs) <= np.float64(hi_hz) * L)
+
+
+def bandpass(X: np.ndarray, mask: np.ndarray) -> np.ndarray:
+    """X[c, k, f] with the bins outside the pass band set to zero (R19)."""
+    return np.where(mask[None, None, :], X, 0.0)
+
+
 def scale_factor(L: int, scaling: int = SCALE_WINPOW, fs: float = 1.0) -> float:
     """s^2 of step 6 (reading R6): WINPOW 1/sum w^2 (default), NONE 1, DENSITY 1/(fs sum w^2),
     SPECTRUM 1/(sum w)^2.  Two-sided values: no one-sided doubling (R7)."""
@@ -194,14 +209,17 @@ def crosscorr(S: np.ndarray, Sauto: np.ndarray, pairs: np.ndarray, L: int, M: in
 # ----------------------------------------------------------------------------------------------
 # the whole path for one chunk, in the paper's order (L107: normalise -> STFT -> Eqs. 1)
 def analyze_chunk(x, L, H, M, pairs=None, scaling=SCALE_WINPOW, fs=1.0,
-                  norm_mode=NORM_NONE, offs=None, want_S=False):
-    """Returns dict(G, A, P, R, Sauto[, S]) for one channel-by-time chunk x[C][T]."""
+                  norm_mode=NORM_NONE, offs=None, want_S=False, band=None):
+    """Returns dict(G, A, P, R, Sauto[, S]) for one channel-by-time chunk x[C][T].
+    band = (lo_hz, hi_hz): band-pass pre-processing (R19) between the transform and Eq. (1); needs fs."""
     x = np.asarray(x)
     C = x.shape[0]
     if pairs is None:
         pairs = all_pairs(C)
     y = normalise(x, offs, norm_mode)
     X = stft(y, L, H)
+    if band is not None:
+        X = bandpass(X, band_mask(L, fs, band[0], band[1]))
     s2 = scale_factor(L, scaling, fs)
     Sauto = auto_spectra(X, s2)
     S = cross_spectra(X, pairs, s2)

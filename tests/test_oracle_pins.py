@@ -406,3 +406,59 @@ def test_golden_oracle_regression():
     assert len(rows) > 20
     for name, p, q, val in rows:
         assert abs(r[name][int(p), int(q)] - float(val)) < 1e-12 * max(1.0, abs(float(val)))
+
+
+# ---------------------------------------------------------------------------- f1: band-pass pre-processing (R19)
+def test_P11_bandpass_kept_bins_of_the_papers_demo_band():
+    """the demo uses a 5-9 kHz pass band.  At BASELINE config 2 (nfft 512, fs 500 kHz) the bin
+    spacing is 976.5625 Hz, so the kept bins are 6..9 (5859.4 .. 8789.1 Hz): hand-computed, not from the oracle."""
+    m = o.band_mask(512, 500e3, 5e3, 9e3)
+    assert m.shape == (257,) and np.flatnonzero(m).tolist() == [6, 7, 8, 9]
+    assert o.band_mask(256, 500e3, 0.0, 250e3).all()                       # the whole band: nothing removed
+    assert np.flatnonzero(o.band_mask(256, 500e3, 0.0, 0.0)).tolist() == [0]   # DC only
+    # a band edge exactly on a bin keeps the bin (closed interval): bin 16 of 256 at fs = 512 Hz is 32 Hz
+    assert np.flatnonzero(o.band_mask(256, 512.0, 32.0, 34.0)).tolist() == [16, 17]
+
+
+def test_P12_bandpass_is_a_per_segment_circular_filter():
+    """Masking the bins of a segment's transform = filtering the windowed segment with the ideal circular filter.
+    So the band-passed cross-correlation must equal the brute-force circular correlation (P5's form) of the
+    FILTERED windowed segments, the filtered segments coming from numpy's rfft/irfft (independent library code),
+    and a tone outside the band must vanish from every output.  Catches: mask applied to the wrong side of the
+    spectrum, normalisation of rho taken from unfiltered autospectra, mask edges off by one."""
+    L, H, M, fs = 64, 32, 32, 6400.0       # bin spacing 100 Hz
+    lo, hi = 450.0, 1250.0                 # keeps bins 5..12
+    T = 400
+    t = np.arange(T)
+    rng = np.random.default_rng(12)
+    x = 0.05 * rng.standard_normal((3, T))
+    x += np.sin(2 * np.pi * 8 * t / L + np.array([[0.0], [0.4], [0.9]]))      # bin 8: in the band
+    x += 2.0 * np.sin(2 * np.pi * 20 * t / L + np.array([[0.1], [0.2], [0.3]]))  # bin 20: outside
+    K = o.n_segments(T, L, H)
+    w = o.hann_periodic(L)
+    s2 = o.scale_factor(L)
+    mask = o.band_mask(L, fs, lo, hi)
+    assert np.flatnonzero(mask).tolist() == list(range(5, 13))
+    r = o.analyze_chunk(x, L, H, M, fs=fs, band=(lo, hi))
+    full = o.analyze_chunk(x, L, H, M, fs=fs)
+    # in the band nothing changes, outside everything is exactly zero (G = 0 by R16, A = atan2(0, 0) = 0)
+    for k in ("G", "A", "P"):
+        assert np.array_equal(r[k][:, mask], full[k][:, mask])
+        assert np.all(r[k][:, ~mask] == 0.0)
+    assert np.all(r["Sauto"][:, ~mask] == 0.0) and np.array_equal(r["Sauto"][:, mask], full["Sauto"][:, mask])
+    assert full["P"][:, 20].min() > 1e-3           # the out-of-band tone was really there
+    # brute force in the time domain on filtered segments
+    def filt(seg):
+        Z = np.fft.rfft(seg)
+        Z[~mask] = 0.0
+        return np.fft.irfft(Z, L)
+    pairs = o.all_pairs(3)
+    yf = [[filt(w * x[c, k * H:k * H + L]) for k in range(K)] for c in range(3)]
+    def corr(i, j, m):
+        return s2 * sum(np.dot(np.roll(yf[i][k], -m), yf[j][k]) for k in range(K)) / K
+    r0 = [corr(c, c, 0) for c in range(3)]
+    for p, (i, j) in enumerate(pairs):
+        for q, m in enumerate(range(-M, M + 1)):
+            assert abs(r["R"][p, q] - corr(i, j, m) / np.sqrt(r0[i] * r0[j])) < 1e-12
+    # phases of the in-band tone survive: A_01 = -0.4, A_12 = -0.5 at bin 8 (x_i ahead of x_j => negative, R8)
+    assert abs(r["A"][0, 8] + 0.4) < 0.05 and abs(r["A"][2, 8] + 0.5) < 0.05
