@@ -38,7 +38,7 @@
 extern "C" {
 #endif
 
-#define DELTA_VERSION 100 /* 0.1.0 */
+#define DELTA_VERSION 101 /* 0.1.1: band-pass fields appended to delta_config */
 
 typedef enum {
   DELTA_OK = 0,
@@ -79,6 +79,12 @@ typedef struct {
   int32_t n_pairs;      /* 0 => all i < j in lexicographic order                                      */
   const int32_t *h_pairs; /* host [n_pairs][2] or NULL; explicit lists: DELTA_ERR_UNSUPPORTED for now */
   int32_t contraction;  /* DELTA_CONTRACT_*                                                           */
+  /* Optional band-pass pre-processing filter ("pre-processing filters", L231: the demo's 5-9 kHz pass
+   * band), reading R19: an ideal mask on the bins of every segment's transform; bin f is kept iff
+   * bp_lo_hz <= f fs / nfft <= bp_hi_hz.  Both 0 => no filter.  Needs fs > 0 and 0 <= bp_lo_hz <= bp_hi_hz, else
+   * DELTA_ERR_INVALID_ARG.  Outside the band S = 0, hence P = G = A = 0; rho is normalised with the filtered
+   * zero-lag autocorrelations. */
+  float   bp_lo_hz, bp_hi_hz;
 } delta_config;
 
 typedef struct {

@@ -26,6 +26,9 @@ static int validate(const delta_config *c) {
   if (c->contraction < DELTA_CONTRACT_AUTO || c->contraction > DELTA_CONTRACT_TC) return DELTA_ERR_INVALID_ARG;
   if (c->scaling == DELTA_SCALE_DENSITY && !(c->fs > 0.f)) return DELTA_ERR_INVALID_ARG;
   if (c->n_pairs < 0 || (c->n_pairs > 0 && !c->h_pairs)) return DELTA_ERR_INVALID_ARG;
+  if (c->bp_lo_hz != 0.f || c->bp_hi_hz != 0.f) {
+    if (!(c->fs > 0.f) || !(c->bp_lo_hz >= 0.f) || !(c->bp_hi_hz >= c->bp_lo_hz)) return DELTA_ERR_INVALID_ARG;
+  }
   const int L = c->nfft;
   if (L < 64 || L > 4096 || (L & (L - 1)) != 0) return DELTA_ERR_UNSUPPORTED;
   if (c->hop > L) return DELTA_ERR_UNSUPPORTED;
@@ -78,6 +81,19 @@ int delta_plan_create(const delta_config *cfg, delta_plan **out) {
   l.nkb = (l.K + kSegBlock - 1) / kSegBlock;
   l.F = l.L / 2 + 1;
   l.Fp = (l.F + 3) & ~3;
+  l.f_lo = 0;
+  l.f_hi = l.F - 1;
+  p->band_on = cfg->bp_lo_hz != 0.f || cfg->bp_hi_hz != 0.f;
+  if (p->band_on) {  // bin f is kept iff lo L <= f fs <= hi L (float64); the kept bins are one contiguous range
+    const double lo = (double)cfg->bp_lo_hz * l.L, hi = (double)cfg->bp_hi_hz * l.L, fs = (double)cfg->fs;
+    l.f_lo = l.F;
+    l.f_hi = -1;
+    for (int f = 0; f < l.F; ++f)
+      if (lo <= f * fs && f * fs <= hi) {
+        if (f < l.f_lo) l.f_lo = f;
+        l.f_hi = f;
+      }
+  }
   l.M = cfg->max_lag;
   l.nlags = 2 * l.M + 1;
   l.P = (int64_t)l.C * (l.C - 1) / 2;
@@ -332,8 +348,13 @@ int delta_analyze_chunk(delta_plan *p, const void *d_x, int64_t ld, float *d_G, 
   rc = contract(p, p->d_X(), pairs_wanted ? p->d_S() : nullptr, au, st);
   if (rc) return rc;
   if (ev) DELTA_CUDA_CHECK(cudaEventRecord(p->stage_ev[2], st));
-  // zero-lag autocorrelations for rho come from the windowed signal energy the STFT kernel left in wpart (Parseval)
-  if (pairs_wanted)
+  // zero-lag autocorrelations for rho come from the windowed signal energy the STFT kernel left in wpart (Parseval);
+  // with the band-pass filter on, from the filtered autospectra
+  if (pairs_wanted && p->band_on) {
+    rc = launch_auto_prep(p, au, p->d_rsq(), p->d_rsum(), st);
+    if (rc) return rc;
+    rc = launch_pair(p, p->d_S(), p->d_rsq(), p->d_rsum(), 1, 1, 1.f, d_G, d_A, d_P, d_R, st);
+  } else if (pairs_wanted)
     rc = launch_pair(p, p->d_S(), p->d_rsq(), p->d_wpart(), p->lay.nkb, p->lay.nkb, (float)p->lay.L * p->s2 / (float)p->lay.K,
                      d_G, d_A, d_P, d_R, st);
   if (rc) return rc;

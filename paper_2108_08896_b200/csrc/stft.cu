@@ -360,10 +360,11 @@ stft_kernel(const void *__restrict__ x, int64_t ld, int in_dtype, int norm_mode,
   auto store_bin = [&](int c, int pcl, int f, const float *re, const float *im) {
     const int64_t within = ((int64_t)kb * lay.Cp + c) * kSegBlock;
     const int64_t base = (int64_t)f * lay.x_elems_per_f + within;
+    const float keep = (f >= lay.f_lo && f <= lay.f_hi) ? 1.f : 0.f;  // band-pass mask (R19)
     if (TC) {
       // split fp16: v * scale = hi + lo (scale = the channel's power of two)
       __half *X = reinterpret_cast<__half *>(Xout);
-      const float sc = CLUSTER ? csc[pcl] : chscale[c];
+      const float sc = keep * (CLUSTER ? csc[pcl] : chscale[c]);
       __align__(16) __half2 hr[4], hi_[4], lr[4], li[4];
 #pragma unroll
       for (int q = 0; q < 4; ++q) {
@@ -380,10 +381,10 @@ stft_kernel(const void *__restrict__ x, int64_t ld, int in_dtype, int norm_mode,
       *reinterpret_cast<uint4 *>(X + base + 3 * plane) = *reinterpret_cast<const uint4 *>(li);
     } else {
       float *X = reinterpret_cast<float *>(Xout);
-      *reinterpret_cast<float4 *>(X + base) = make_float4(re[0], re[1], re[2], re[3]);
-      *reinterpret_cast<float4 *>(X + base + 4) = make_float4(re[4], re[5], re[6], re[7]);
-      *reinterpret_cast<float4 *>(X + base + plane) = make_float4(im[0], im[1], im[2], im[3]);
-      *reinterpret_cast<float4 *>(X + base + plane + 4) = make_float4(im[4], im[5], im[6], im[7]);
+      *reinterpret_cast<float4 *>(X + base) = make_float4(keep * re[0], keep * re[1], keep * re[2], keep * re[3]);
+      *reinterpret_cast<float4 *>(X + base + 4) = make_float4(keep * re[4], keep * re[5], keep * re[6], keep * re[7]);
+      *reinterpret_cast<float4 *>(X + base + plane) = make_float4(keep * im[0], keep * im[1], keep * im[2], keep * im[3]);
+      *reinterpret_cast<float4 *>(X + base + plane + 4) = make_float4(keep * im[4], keep * im[5], keep * im[6], keep * im[7]);
     }
   };
   constexpr int HB = N / 2 + 1;  // f = 0 .. N/2

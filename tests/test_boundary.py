@@ -27,7 +27,7 @@ def test_library_exports_every_declared_symbol():
     for name in ("delta_stft", "delta_cross_spectra", "delta_coherence", "delta_crossphase", "delta_crosspower",
                  "delta_crosscorr"):   # the six calls BASELINE.json's north_star names
         assert name in syms
-    assert b.LIB.delta_version() == 100
+    assert b.LIB.delta_version() == 101
     assert os.path.dirname(b.LIB_PATH).endswith("paper_2108_08896_b200")  # in-tree, not site-packages
 
 
@@ -115,3 +115,17 @@ def test_plan_needs_a_gpu_for_allocation():
         pytest.skip("GPU present")
     with pytest.raises(RuntimeError):
         b.Plan(8, 2048, 256, 128)
+
+
+def test_bandpass_config_validation():
+    """include/delta.h: both band edges 0 = off; otherwise fs > 0 and 0 <= lo <= hi."""
+    assert b.Plan(8, 2048, 256, 128, allocate=False, band=(5e3, 9e3)).sizes.F == 129
+    assert b.Plan(8, 2048, 256, 128, allocate=False, band=None).sizes.F == 129
+    for bad in [(9e3, 5e3), (-1.0, 5e3)]:
+        with pytest.raises(b.DeltaError) as e:
+            b.Plan(8, 2048, 256, 128, allocate=False, band=bad)
+        assert e.value.status == b.ERR_INVALID_ARG
+    with pytest.raises(b.DeltaError) as e:
+        b.Plan(8, 2048, 256, 128, allocate=False, band=(5e3, 9e3), fs=0.0)
+    assert e.value.status == b.ERR_INVALID_ARG
+    assert b.LIB.delta_version() >= 101

@@ -64,11 +64,12 @@ def mode(request):
     return b.CONTRACT_FP32 if request.param == "fp32" else b.CONTRACT_TC
 
 
-def gpu_analyze(x, L, H, M, in_dtype=None, norm_mode=0, n_first=0, contraction=0, scaling=0, fs=500e3, ld_pad=0):
+def gpu_analyze(x, L, H, M, in_dtype=None, norm_mode=0, n_first=0, contraction=0, scaling=0, fs=500e3, ld_pad=0, band=None):
     b = binding()
     C, T = x.shape
     in_dtype = (b.I16 if x.dtype == np.int16 else b.F32) if in_dtype is None else in_dtype
-    plan = b.Plan(C, T, L, H, M, in_dtype=in_dtype, norm_mode=norm_mode, contraction=contraction, scaling=scaling, fs=fs)
+    plan = b.Plan(C, T, L, H, M, in_dtype=in_dtype, norm_mode=norm_mode, contraction=contraction, scaling=scaling, fs=fs,
+                  band=band)
     if ld_pad:
         buf = torch.zeros((C, T + ld_pad), dtype=dev(x[:1, :1]).dtype, device="cuda")
         buf[:, :T] = dev(x)
@@ -82,8 +83,8 @@ def gpu_analyze(x, L, H, M, in_dtype=None, norm_mode=0, n_first=0, contraction=0
     return plan, {k: v.cpu().numpy() for k, v in out.items()}
 
 
-def oracle_for(x, L, H, M, pairs=None, norm_mode=0, offs=None, scaling=0, fs=500e3):
-    return o.analyze_chunk(x, L, H, M, pairs=pairs, norm_mode=norm_mode, offs=offs, scaling=scaling, fs=fs)
+def oracle_for(x, L, H, M, pairs=None, norm_mode=0, offs=None, scaling=0, fs=500e3, band=None):
+    return o.analyze_chunk(x, L, H, M, pairs=pairs, norm_mode=norm_mode, offs=offs, scaling=scaling, fs=fs, band=band)
 
 
 # ------------------------------------------------------------------------------------------
@@ -354,3 +355,25 @@ def test_programmatic_dependent_launch_does_not_change_results(monkeypatch):
     for k in range(3):
         for name in ("G", "A", "P", "R", "Sauto"):
             assert torch.equal(a[k][name], c[k][name]), (k, name)
+
+
+@pytest.mark.parametrize("band", [(5e3, 9e3), (15e3, 60e3), (0.0, 250e3)])
+def test_bandpass_preprocessing(band, mode):
+    """f1: band-pass pre-processing as a mask on the transform's bins (R19), here the demo's
+    5-9 kHz band of PAPER.md L231, a band around the 20 kHz mode, and the whole band (= no filter).  Outside the
+    band every output is exactly 0; rho is normalised with the filtered autospectra."""
+    w = es.WORKLOADS["single"]
+    x = es.single()[:40]
+    _, out = gpu_analyze(x, w.nfft, w.hop, w.max_lag, contraction=mode, band=band)
+    ref = oracle_for(x, w.nfft, w.hop, w.max_lag, band=band)
+    st = compare(out, ref, o.all_pairs(40), f"band {band}")
+    print(band, st)
+    mask = o.band_mask(w.nfft, 500e3, band[0], band[1])
+    for k in ("G", "A", "P"):
+        assert np.all(out[k][:, ~mask] == 0.0), k
+    assert np.all(out["Sauto"][:, ~mask] == 0.0)
+    if mask.all():   # the whole band must reproduce the unfiltered call (up to the source of R_cc[0]: Parseval)
+        _, plain = gpu_analyze(x, w.nfft, w.hop, w.max_lag, contraction=mode)
+        for k in ("G", "A", "P", "Sauto"):
+            assert np.array_equal(out[k], plain[k]), k
+        assert np.abs(out["R"] - plain["R"]).max() < 5e-6
