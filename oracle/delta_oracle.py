@@ -33,6 +33,8 @@ import numpy as np
 # enumerations mirrored (by value, not by import) from include/delta.h
 SCALE_WINPOW, SCALE_NONE, SCALE_DENSITY, SCALE_SPECTRUM = 0, 1, 2, 3
 NORM_NONE, NORM_SUBTRACT, NORM_RELATIVE = 0, 1, 2
+WIN_HANN, WIN_HAMMING, WIN_RECT, WIN_BLACKMAN = 0, 1, 2, 3
+DETREND_NONE, DETREND_CONSTANT = 0, 1
 
 
 # ----------------------------------------------------------------------------------------------
@@ -84,6 +86,22 @@ def hann_periodic(L: int) -> np.ndarray:
     return 0.5 - 0.5 * np.cos(2.0 * np.pi * n / L)
 
 
+def window(L: int, kind: int = WIN_HANN) -> np.ndarray:
+    """Periodic (DFT-even) windows, n = 0..L-1, x = 2 pi n / L  (the paper names none: R4 default Hann; the others are
+    the f1 variants of SURVEY.md section 8f):  Hann 0.5 - 0.5 cos x;  Hamming 0.54 - 0.46 cos x;  rectangular 1;
+    Blackman 0.42 - 0.5 cos x + 0.08 cos 2x."""
+    x = 2.0 * np.pi * np.arange(L, dtype=np.float64) / L
+    if kind == WIN_HANN:
+        return hann_periodic(L)
+    if kind == WIN_HAMMING:
+        return 0.54 - 0.46 * np.cos(x)
+    if kind == WIN_RECT:
+        return np.ones(L)
+    if kind == WIN_BLACKMAN:
+        return 0.42 - 0.5 * np.cos(x) + 0.08 * np.cos(2.0 * x)
+    raise ValueError("bad window")
+
+
 def dft_matrix(L: int, nbins: int) -> np.ndarray:
     """W[n, f] = exp(-2 pi i (n f mod L)/L), n < L, f < nbins; phase reduced in integers."""
     n = np.arange(L, dtype=np.int64)[:, None]
@@ -91,20 +109,23 @@ def dft_matrix(L: int, nbins: int) -> np.ndarray:
     return np.exp(-2j * np.pi * ((n * f) % L).astype(np.float64) / L)
 
 
-def stft(y: np.ndarray, L: int, H: int) -> np.ndarray:
+def stft(y: np.ndarray, L: int, H: int, win: int = WIN_HANN, detrend: int = DETREND_NONE) -> np.ndarray:
     """X[c, k, f] = sum_n w[n] y[c, kH + n] exp(-2 pi i f n / L),  f = 0..L/2, unscaled.
 
-    No detrend (R5), nperseg == nfft (R2), segments never leave the chunk (L107)."""
+    Default: no detrend (R5); nperseg == nfft (R2), segments never leave the chunk (L107).
+    detrend = CONSTANT (f1 variant): the mean of the L samples of a segment is subtracted before the window."""
     y = np.asarray(y, dtype=np.float64)
     C, T = y.shape
     K = n_segments(T, L, H)
     F = L // 2 + 1
-    w = hann_periodic(L)
+    w = window(L, win)
     W = dft_matrix(L, F)
     X = np.empty((C, K, F), dtype=np.complex128)
     for c in range(C):
-        seg = np.stack([y[c, k * H:k * H + L] for k in range(K)]) * w[None, :]
-        X[c] = seg @ W
+        seg = np.stack([y[c, k * H:k * H + L] for k in range(K)])
+        if detrend == DETREND_CONSTANT:
+            seg = seg - seg.mean(axis=1, keepdims=True)
+        X[c] = (seg * w[None, :]) @ W
     return X
 
 
@@ -122,10 +143,10 @@ def bandpass(X: np.ndarray, mask: np.ndarray) -> np.ndarray:
     return np.where(mask[None, None, :], X, 0.0)
 
 
-def scale_factor(L: int, scaling: int = SCALE_WINPOW, fs: float = 1.0) -> float:
+def scale_factor(L: int, scaling: int = SCALE_WINPOW, fs: float = 1.0, win: int = WIN_HANN) -> float:
     """s^2 of step 6 (reading R6): WINPOW 1/sum w^2 (default), NONE 1, DENSITY 1/(fs sum w^2),
     SPECTRUM 1/(sum w)^2.  Two-sided values: no one-sided doubling (R7)."""
-    w = hann_periodic(L)
+    w = window(L, win)
     if scaling == SCALE_WINPOW:
         return 1.0 / float(np.sum(w * w))
     if scaling == SCALE_NONE:
@@ -209,7 +230,7 @@ def crosscorr(S: np.ndarray, Sauto: np.ndarray, pairs: np.ndarray, L: int, M: in
 # ----------------------------------------------------------------------------------------------
 # the whole path for one chunk, in the paper's order (L107: normalise -> STFT -> Eqs. 1)
 def analyze_chunk(x, L, H, M, pairs=None, scaling=SCALE_WINPOW, fs=1.0,
-                  norm_mode=NORM_NONE, offs=None, want_S=False, band=None):
+                  norm_mode=NORM_NONE, offs=None, want_S=False, band=None, win=WIN_HANN, detrend=DETREND_NONE):
     """Returns dict(G, A, P, R, Sauto[, S]) for one channel-by-time chunk x[C][T].
     band = (lo_hz, hi_hz): band-pass pre-processing (R19) between the transform and Eq. (1); needs fs."""
     x = np.asarray(x)
@@ -217,10 +238,10 @@ def analyze_chunk(x, L, H, M, pairs=None, scaling=SCALE_WINPOW, fs=1.0,
     if pairs is None:
         pairs = all_pairs(C)
     y = normalise(x, offs, norm_mode)
-    X = stft(y, L, H)
+    X = stft(y, L, H, win, detrend)
     if band is not None:
         X = bandpass(X, band_mask(L, fs, band[0], band[1]))
-    s2 = scale_factor(L, scaling, fs)
+    s2 = scale_factor(L, scaling, fs, win)
     Sauto = auto_spectra(X, s2)
     S = cross_spectra(X, pairs, s2)
     out = dict(G=coherence(S, Sauto, pairs), A=crossphase(S), P=crosspower(S),

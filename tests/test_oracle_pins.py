@@ -462,3 +462,39 @@ def test_P12_bandpass_is_a_per_segment_circular_filter():
             assert abs(r["R"][p, q] - corr(i, j, m) / np.sqrt(r0[i] * r0[j])) < 1e-12
     # phases of the in-band tone survive: A_01 = -0.4, A_12 = -0.5 at bin 8 (x_i ahead of x_j => negative, R8)
     assert abs(r["A"][0, 8] + 0.4) < 0.05 and abs(r["A"][2, 8] + 0.5) < 0.05
+
+
+# ---------------------------------------------------------------------------- f1: other windows, constant detrend
+@pytest.mark.parametrize("kind,name", [(o.WIN_HANN, "hann"), (o.WIN_HAMMING, "hamming"), (o.WIN_RECT, "boxcar"),
+                                       (o.WIN_BLACKMAN, "blackman")])
+@pytest.mark.parametrize("detrend", [o.DETREND_NONE, o.DETREND_CONSTANT])
+def test_P13_windows_and_detrend_against_scipy(kind, name, detrend):
+    """The window variants equal scipy's periodic (fftbins) windows, and the whole estimator with a window and the
+    constant detrend equals scipy's Welch cross-spectral density (independent library code; scipy conjugates its
+    first argument, P6).  Closed form for the rectangular window: a bin-centred unit cosine has |X[q]| = L/2 and
+    nothing anywhere else.  Catches: symmetric instead of periodic window, mean taken over the chunk instead of the
+    segment, detrend after the window, s^2 taken from the wrong window."""
+    L, H = 128, 64
+    w = o.window(L, kind)
+    assert np.allclose(w, sps.get_window(name, L, fftbins=True), atol=1e-15)
+    x = _rand_chunk(3, 1500, 31) + np.array([[3.0], [-2.0], [0.5]])    # offsets make the detrend matter
+    X = o.stft(x, L, H, kind, detrend)
+    pairs = o.all_pairs(3)
+    s2 = o.scale_factor(L, o.SCALE_WINPOW, 1.0, kind)
+    assert abs(s2 - 1.0 / np.sum(w * w)) < 1e-15
+    S = o.cross_spectra(X, pairs, s2)
+    kw = dict(fs=1.0, window=name, nperseg=L, noverlap=L - H, nfft=L,
+              detrend="constant" if detrend == o.DETREND_CONSTANT else False, return_onesided=False, scaling="density")
+    for p, (i, j) in enumerate(pairs):
+        _, Pd = sps.csd(x[i], x[j], **kw)
+        assert np.allclose(np.conj(Pd[:L // 2 + 1]), S[p], rtol=1e-9, atol=1e-12)
+    if detrend == o.DETREND_CONSTANT:      # the DC bin of a detrended rectangular-window segment is exactly empty
+        Xr = o.stft(x, L, H, o.WIN_RECT, detrend)
+        assert np.abs(Xr[:, :, 0]).max() < 1e-10
+    if kind == o.WIN_RECT:
+        q = 9
+        t = np.arange(600)
+        Xc = o.stft(np.cos(2 * np.pi * q * t / L + 0.7)[None, :], L, H, kind, o.DETREND_NONE)
+        assert np.allclose(np.abs(Xc[0, :, q]), L / 2, atol=1e-9)
+        others = np.delete(np.abs(Xc[0]), q, axis=1)
+        assert others.max() < 1e-9
