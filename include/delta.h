@@ -38,7 +38,7 @@
 extern "C" {
 #endif
 
-#define DELTA_VERSION 101 /* 0.1.1: band-pass fields appended to delta_config */
+#define DELTA_VERSION 102 /* 0.1.2: band-pass, window variants and detrend appended to delta_config */
 
 typedef enum {
   DELTA_OK = 0,
@@ -51,7 +51,11 @@ typedef enum {
   DELTA_ERR_STATE = -6        /* e.g. norm_mode needs offsets and delta_set_offsets() was not called */
 } delta_status;
 
-enum { DELTA_WIN_HANN_PERIODIC = 0 };                /* w[n] = 1/2 - 1/2 cos(2 pi n/L)  (R4)          */
+/* periodic (DFT-even) windows, x = 2 pi n/L: Hann 1/2 - 1/2 cos x (R4, the default); the others are the f1 variants:
+ * Hamming 0.54 - 0.46 cos x, rectangular 1, Blackman 0.42 - 0.5 cos x + 0.08 cos 2x */
+enum { DELTA_WIN_HANN_PERIODIC = 0, DELTA_WIN_HAMMING_PERIODIC = 1, DELTA_WIN_RECT = 2, DELTA_WIN_BLACKMAN_PERIODIC = 3 };
+/* per-segment detrend before the window: none (R5, the default) or the mean of the segment's nfft samples */
+enum { DELTA_DETREND_NONE = 0, DELTA_DETREND_CONSTANT = 1 };
 enum { DELTA_SCALE_WINPOW = 0,                       /* s^2 = 1/sum w^2 (default; white noise of
                                                         variance v has E S_ii = v)                    */
        DELTA_SCALE_NONE = 1,                         /* s^2 = 1                                       */
@@ -70,7 +74,7 @@ typedef struct {
   int32_t n_samples;    /* T >= nfft, samples per channel per chunk                                   */
   int32_t nfft;         /* L, power of two in [64, 4096]; segment length == nfft (no zero padding)    */
   int32_t hop;          /* H in [1, L]; overlap = L - H                                               */
-  int32_t window;       /* DELTA_WIN_HANN_PERIODIC                                                    */
+  int32_t window;       /* DELTA_WIN_*                                                                */
   int32_t scaling;      /* DELTA_SCALE_*                                                              */
   float   fs;           /* sampling rate in Hz; only DELTA_SCALE_DENSITY uses it                      */
   int32_t in_dtype;     /* DELTA_F32 | DELTA_I16                                                      */
@@ -85,6 +89,7 @@ typedef struct {
    * DELTA_ERR_INVALID_ARG.  Outside the band S = 0, hence P = G = A = 0; rho is normalised with the filtered
    * zero-lag autocorrelations. */
   float   bp_lo_hz, bp_hi_hz;
+  int32_t detrend;      /* DELTA_DETREND_*                                                            */
 } delta_config;
 
 typedef struct {

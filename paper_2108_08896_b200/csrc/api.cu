@@ -19,7 +19,8 @@ static inline bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t
 static int validate(const delta_config *c) {
   if (!c) return DELTA_ERR_INVALID_ARG;
   if (c->n_channels < 1 || c->n_samples < 1 || c->nfft < 1 || c->hop < 1 || c->max_lag < 0) return DELTA_ERR_INVALID_ARG;
-  if (c->window != DELTA_WIN_HANN_PERIODIC) return DELTA_ERR_INVALID_ARG;
+  if (c->window < DELTA_WIN_HANN_PERIODIC || c->window > DELTA_WIN_BLACKMAN_PERIODIC) return DELTA_ERR_INVALID_ARG;
+  if (c->detrend < DELTA_DETREND_NONE || c->detrend > DELTA_DETREND_CONSTANT) return DELTA_ERR_INVALID_ARG;
   if (c->scaling < DELTA_SCALE_WINPOW || c->scaling > DELTA_SCALE_SPECTRUM) return DELTA_ERR_INVALID_ARG;
   if (c->in_dtype != DELTA_F32 && c->in_dtype != DELTA_I16) return DELTA_ERR_INVALID_ARG;
   if (c->norm_mode < DELTA_NORM_NONE || c->norm_mode > DELTA_NORM_RELATIVE) return DELTA_ERR_INVALID_ARG;
@@ -111,11 +112,20 @@ int delta_plan_create(const delta_config *cfg, delta_plan **out) {
   for (int n = 0; n < L; ++n) {
     const double ang = -2.0 * M_PI * (double)n / (double)L;
     p->h_tw[n] = make_float2((float)std::cos(ang), (float)std::sin(ang));
-    const double w = 0.5 - 0.5 * std::cos(2.0 * M_PI * (double)n / (double)L);
+    const double xw = 2.0 * M_PI * (double)n / (double)L;
+    double w;
+    switch (cfg->window) {
+      case DELTA_WIN_HAMMING_PERIODIC: w = 0.54 - 0.46 * std::cos(xw); break;
+      case DELTA_WIN_RECT: w = 1.0; break;
+      case DELTA_WIN_BLACKMAN_PERIODIC: w = 0.42 - 0.5 * std::cos(xw) + 0.08 * std::cos(2.0 * xw); break;
+      default: w = 0.5 - 0.5 * std::cos(xw); break;
+    }
     p->h_win[n] = (float)w;
     sw += w;
     sw2 += w * w;
   }
+  l.wsum = (float)(sw * (1.0 + 1e-6));  // all four windows are non-negative
+  l.detrend = cfg->detrend;
   p->h_ftab.resize((size_t)fft_table_size(l.N) + 1);
   fft_twiddle_table(l.N, p->h_ftab.data());
   p->h_ftab2.resize((size_t)fft_table_size(l.N, pair_fft_variant(l.N)) + 1);

@@ -39,6 +39,8 @@ struct Layout {
   // k = 8*kc + kk, c < Cp (rows C..Cp-1 are zero), kc < Kc = Kp/8, Kp = K rounded up to 16.
   int C, Cp, T, L, N, H, K, Kp, Kc, F, M, nlags;
   int Fp;   // row pitch of the rsq table: F rounded up to 4 floats (rows are 16-byte aligned bulk-copy sources)
+  float wsum;      // sum_n |w[n]|: |X| <= wsum max|y| bounds the split-fp16 operands
+  int detrend;     // DELTA_DETREND_*
   int f_lo, f_hi;  // pass band of the optional band-pass filter, in bins (0 .. F-1 when it is off)
   int nkb;  // segment blocks per channel = ceil(K / 8): one partial of the windowed signal energy each (wpart)
   // S (cross-spectra) is complex64 [Pblk][F][PB]: pairs in lexicographic order p = iC - i(i+1)/2 + (j-i-1),

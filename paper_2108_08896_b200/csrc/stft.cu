@@ -116,8 +116,8 @@ struct SampleLoader {
 };
 
 // per-channel power-of-two scale for the split-fp16 operands: |X| <= (L/2) max|y|  =>  scale * |X| <= 2^14.
-__device__ __forceinline__ float scale_from_max(float m, int L) {
-  const float bound = m * (0.5f * (float)L);  // sum_n w[n] |y| <= (L/2) max|y|
+__device__ __forceinline__ float scale_from_max(float m, float wsum) {
+  const float bound = m * wsum;  // |X| <= sum_n w[n] |y| <= wsum max|y|   (Hann: wsum = L/2)
   float sc = 1.f;
   if (bound > 0.f && isfinite(bound)) {
     int e;
@@ -132,7 +132,7 @@ __device__ __forceinline__ float scale_from_max(float m, int L) {
 // float bits (all values are >= 0) and the last one to arrive writes the scale and re-arms the two words.
 __global__ void __launch_bounds__(256)
 chscale_kernel(const void *__restrict__ x, int64_t ld, int in_dtype, int norm_mode, int n_first,
-               const double *__restrict__ offs, const long long *__restrict__ isum, int T, int L,
+               const double *__restrict__ offs, const long long *__restrict__ isum, int T, float wsum,
                float *__restrict__ chscale, unsigned *__restrict__ chmax, unsigned *__restrict__ chcnt) {
   const int c = blockIdx.x, NS = gridDim.y, tid = threadIdx.x;
   SampleLoader ldr;
@@ -188,7 +188,7 @@ chscale_kernel(const void *__restrict__ x, int64_t ld, int in_dtype, int norm_mo
       __threadfence();
       const float mm = __uint_as_float(atomicExch(chmax + c, 0u));
       chcnt[c] = 0u;
-      chscale[c] = scale_from_max(mm, L);
+      chscale[c] = scale_from_max(mm, wsum);
     }
   }
 }
@@ -209,6 +209,26 @@ struct StftCfg {
   static constexpr int SMEM_F2 = NFFT * G::BUF + CH * CHPAD;
 };
 
+// Sum of v over the T threads of a transform group (threads g*T .. g*T+T-1 of the CTA).  Groups wider than a warp go
+// through shared memory with CTA barriers, so for T > 32 EVERY thread of the CTA must call it.
+template <int T>
+__device__ __forceinline__ float group_sum(float v, float *wsums, int tid) {
+  constexpr int W = T < 32 ? T : 32;
+#pragma unroll
+  for (int o = W / 2; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o, W);
+  if (T > 32) {
+    __syncthreads();
+    if ((tid & 31) == 0) wsums[tid >> 5] = v;
+    __syncthreads();
+    constexpr int WPG = T / 32 > 0 ? T / 32 : 1;
+    const int w0 = (tid / T) * WPG;
+    v = 0.f;
+#pragma unroll
+    for (int w = 0; w < WPG; ++w) v += wsums[w0 + w];
+  }
+  return v;
+}
+
 // Real forward transform, split step: Z = FFT_N(z), z[n] = x[2n] + i x[2n+1]  ->
 //   X[f] = (Z[f] + conj Z[N-f])/2 - (i/2) e^{-2 pi i f/L} (Z[f] - conj Z[N-f]),  f = 0..N, Z[N] = Z[0].
 __device__ __forceinline__ float2 rfft_split(float2 zf, float2 zr, float2 w) {
@@ -224,7 +244,7 @@ __device__ __forceinline__ float2 rfft_split(float2 zf, float2 zr, float2 w) {
 // grid = (ceil(K/8), ceil(C/CH)).  Phase 1: one group of T threads per (channel, segment) transform.
 // Phase 2: one thread per (channel, bin) gathers the 8 segments of the CTA and writes one 16-byte
 // (fp16) or 32-byte (fp32) piece per operand plane of the frequency-major X layout.
-template <int L, bool TC, bool CLUSTER>
+template <int L, bool TC, bool CLUSTER, bool DETREND>
 __global__ void __launch_bounds__(StftCfg<L>::THREADS, 1024 / StftCfg<L>::THREADS)
 stft_kernel(const void *__restrict__ x, int64_t ld, int in_dtype, int norm_mode, int n_first,
             const double *__restrict__ offs, const long long *__restrict__ isum, const float2 *__restrict__ tw,
@@ -236,6 +256,7 @@ stft_kernel(const void *__restrict__ x, int64_t ld, int in_dtype, int norm_mode,
   extern __shared__ __align__(16) unsigned char smem_raw[];
   float2 *zb = reinterpret_cast<float2 *>(smem_raw);
   __shared__ float wred[Cfg::THREADS / 32];  // per-warp energy of the windowed samples
+  __shared__ float gsum[Cfg::THREADS / 32];  // per-warp sample sums (detrend, transforms wider than a warp)
   __shared__ float wmax[Cfg::THREADS / 32];  // per-warp max |y|
   __shared__ float cmax[CH];                 // per-channel max |y| over this CTA's segments (read by the cluster)
   __shared__ float csc[CH];                  // per-channel fp16 scale
@@ -250,7 +271,7 @@ stft_kernel(const void *__restrict__ x, int64_t ld, int in_dtype, int norm_mode,
 
   {
     const int c = c0 + cl, k = kb * kSegBlock + kk;
-    float2 v[E];
+    float2 v[E], wv[E];
     float amax = 0.f;
     if (c < lay.C && k < lay.K) {
       SampleLoader ldr;
@@ -259,7 +280,7 @@ stft_kernel(const void *__restrict__ x, int64_t ld, int in_dtype, int norm_mode,
       const size_t esz = in_dtype == DELTA_I16 ? 2 : 4;
       const bool pair_ok = ((t0 & 1) == 0) && ((reinterpret_cast<uintptr_t>(x) & (2 * esz - 1)) == 0);
       // all loads of the segment are issued before the first use (one DRAM latency per thread, not E)
-      float2 smp[E], wv[E];
+      float2 smp[E];
       if (in_dtype == DELTA_I16) {
         const short *xs = reinterpret_cast<const short *>(x) + t0;
         short2 raw[E];
@@ -287,14 +308,35 @@ stft_kernel(const void *__restrict__ x, int64_t ld, int in_dtype, int norm_mode,
       }
 #pragma unroll
       for (int u = 0; u < E; ++u) wv[u] = __ldg(reinterpret_cast<const float2 *>(win) + gt + T * u);
+      if (!DETREND) {
 #pragma unroll
-      for (int u = 0; u < E; ++u) {
-        if (CLUSTER) amax = fmaxf(amax, fmaxf(fabsf(smp[u].x), fabsf(smp[u].y)));
-        v[u] = make_float2(smp[u].x * wv[u].x, smp[u].y * wv[u].y);
+        for (int u = 0; u < E; ++u) {
+          if (CLUSTER) amax = fmaxf(amax, fmaxf(fabsf(smp[u].x), fabsf(smp[u].y)));
+          v[u] = make_float2(smp[u].x * wv[u].x, smp[u].y * wv[u].y);
+        }
+      } else {
+#pragma unroll
+        for (int u = 0; u < E; ++u) v[u] = smp[u];
       }
     } else {
 #pragma unroll
-      for (int u = 0; u < E; ++u) v[u] = make_float2(0.f, 0.f);
+      for (int u = 0; u < E; ++u) {
+        v[u] = make_float2(0.f, 0.f);
+        if (DETREND) wv[u] = make_float2(0.f, 0.f);
+      }
+    }
+    if (DETREND) {  // subtract the mean of the segment's L samples (f1 variant), then the window;
+      float sm = 0.f;  // every thread of the CTA takes part (group_sum may use CTA barriers)
+#pragma unroll
+      for (int u = 0; u < E; ++u) sm += v[u].x + v[u].y;
+      sm = group_sum<T>(sm, gsum, tid);
+      const float mean = sm * (1.f / (float)L);
+#pragma unroll
+      for (int u = 0; u < E; ++u) {
+        v[u] = make_float2(v[u].x - mean, v[u].y - mean);
+        if (CLUSTER) amax = fmaxf(amax, fmaxf(fabsf(v[u].x), fabsf(v[u].y)));
+        v[u] = make_float2(v[u].x * wv[u].x, v[u].y * wv[u].y);
+      }
     }
     {  // energy of the windowed segment (zero-lag autocorrelation of Eq. 1d by Parseval), fixed summation order
       float ss = 0.f;
@@ -345,7 +387,7 @@ stft_kernel(const void *__restrict__ x, int64_t ld, int in_dtype, int norm_mode,
       float m = 0.f;
       const unsigned nb = cluster.num_blocks();
       for (unsigned r = 0; r < nb; ++r) m = fmaxf(m, *cluster.map_shared_rank(&cmax[tid], r));
-      const float sc = scale_from_max(m, L);
+      const float sc = scale_from_max(m, lay.wsum);
       csc[tid] = sc;
       if (kb == 0 && c0 + tid < lay.C) chscale[c0 + tid] = sc;
     }
@@ -449,21 +491,27 @@ int launch_offsets(delta_plan *p, const void *d_x, int64_t ld, int n_first, cuda
   return DELTA_OK;
 }
 
-template <int L, bool TC, bool CLUSTER>
-static int launch_stft_LT(delta_plan *p, const void *d_x, int64_t ld, void *d_X, cudaStream_t st) {
+template <int L, bool TC, bool CLUSTER, bool DETREND>
+static int launch_stft_LTD(delta_plan *p, const void *d_x, int64_t ld, void *d_X, cudaStream_t st) {
   using Cfg = StftCfg<L>;
   const Layout &lay = p->lay;
   const size_t smem = (size_t)Cfg::SMEM_F2 * sizeof(float2);
-  int rc = opt_in_smem(stft_kernel<L, TC, CLUSTER>, smem);
+  int rc = opt_in_smem(stft_kernel<L, TC, CLUSTER, DETREND>, smem);
   if (rc) return rc;
   // the segment blocks of one channel group are one cluster
   LaunchCfg lc(dim3(lay.nkb, (lay.C + Cfg::CH - 1) / Cfg::CH), dim3(Cfg::THREADS), smem, st, p->use_pdl, CLUSTER ? lay.nkb : 0);
-  DELTA_CUDA_CHECK(cudaLaunchKernelEx(&lc.cfg, stft_kernel<L, TC, CLUSTER>, d_x, ld, p->cfg.in_dtype, p->cfg.norm_mode, p->n_first,
+  DELTA_CUDA_CHECK(cudaLaunchKernelEx(&lc.cfg, stft_kernel<L, TC, CLUSTER, DETREND>, d_x, ld, p->cfg.in_dtype, p->cfg.norm_mode, p->n_first,
                                       (const double *)p->d_offs(), (const long long *)p->d_isum(), p->d_tw(), p->d_win(),
                                       p->d_ftab(), lay, d_X, p->d_chscale(), p->d_wpart()));
   p->launches++;
   DELTA_CUDA_CHECK(cudaGetLastError());
   return DELTA_OK;
+}
+
+template <int L, bool TC, bool CLUSTER>
+static int launch_stft_LT(delta_plan *p, const void *d_x, int64_t ld, void *d_X, cudaStream_t st) {
+  return p->lay.detrend == DELTA_DETREND_CONSTANT ? launch_stft_LTD<L, TC, CLUSTER, true>(p, d_x, ld, d_X, st)
+                                                  : launch_stft_LTD<L, TC, CLUSTER, false>(p, d_x, ld, d_X, st);
 }
 
 template <int L>
@@ -474,7 +522,9 @@ static int launch_stft_L(delta_plan *p, const void *d_x, int64_t ld, void *d_X, 
     int ns = (8 * p->num_sms + lay.C - 1) / lay.C;  // about 8 blocks per SM
     ns = ns < 1 ? 1 : (ns > 64 ? 64 : ns);
     chscale_kernel<<<dim3(lay.C, ns), 256, 0, st>>>(d_x, ld, p->cfg.in_dtype, p->cfg.norm_mode, p->n_first, p->d_offs(),
-                                                    p->d_isum(), lay.T, lay.L, p->d_chscale(), p->d_chmax(), p->d_chcnt());
+                                                    p->d_isum(), lay.T,
+                                                    lay.wsum * (lay.detrend ? 2.f : 1.f),  // |y - mean| <= 2 max|y|
+                                                    p->d_chscale(), p->d_chmax(), p->d_chcnt());
     p->launches++;
     DELTA_CUDA_CHECK(cudaGetLastError());
     return launch_stft_LT<L, true, false>(p, d_x, ld, d_X, st);

@@ -27,7 +27,7 @@ def test_library_exports_every_declared_symbol():
     for name in ("delta_stft", "delta_cross_spectra", "delta_coherence", "delta_crossphase", "delta_crosspower",
                  "delta_crosscorr"):   # the six calls BASELINE.json's north_star names
         assert name in syms
-    assert b.LIB.delta_version() == 101
+    assert b.LIB.delta_version() == 102
     assert os.path.dirname(b.LIB_PATH).endswith("paper_2108_08896_b200")  # in-tree, not site-packages
 
 
@@ -59,7 +59,7 @@ def create(cfg):
     (dict(hop=0), b.ERR_INVALID_ARG),
     (dict(n_channels=0), b.ERR_INVALID_ARG),
     (dict(n_channels=5000), b.ERR_UNSUPPORTED),
-    (dict(window=3), b.ERR_INVALID_ARG),
+    (dict(window=9), b.ERR_INVALID_ARG),
     (dict(scaling=9), b.ERR_INVALID_ARG),
     (dict(scaling=2, fs=0.0), b.ERR_INVALID_ARG),
     (dict(in_dtype=7), b.ERR_INVALID_ARG),
@@ -129,3 +129,12 @@ def test_bandpass_config_validation():
         b.Plan(8, 2048, 256, 128, allocate=False, band=(5e3, 9e3), fs=0.0)
     assert e.value.status == b.ERR_INVALID_ARG
     assert b.LIB.delta_version() >= 101
+
+
+def test_window_and_detrend_validation():
+    for w in (0, 1, 2, 3):
+        assert b.Plan(8, 2048, 256, 128, allocate=False, window=w, detrend=1).sizes.K == 15
+    for kw in (dict(window=4), dict(window=-1), dict(detrend=2), dict(detrend=-1)):
+        with pytest.raises(b.DeltaError) as e:
+            b.Plan(8, 2048, 256, 128, allocate=False, **kw)
+        assert e.value.status == b.ERR_INVALID_ARG

@@ -64,12 +64,13 @@ def mode(request):
     return b.CONTRACT_FP32 if request.param == "fp32" else b.CONTRACT_TC
 
 
-def gpu_analyze(x, L, H, M, in_dtype=None, norm_mode=0, n_first=0, contraction=0, scaling=0, fs=500e3, ld_pad=0, band=None):
+def gpu_analyze(x, L, H, M, in_dtype=None, norm_mode=0, n_first=0, contraction=0, scaling=0, fs=500e3, ld_pad=0, band=None,
+                window=0, detrend=0):
     b = binding()
     C, T = x.shape
     in_dtype = (b.I16 if x.dtype == np.int16 else b.F32) if in_dtype is None else in_dtype
     plan = b.Plan(C, T, L, H, M, in_dtype=in_dtype, norm_mode=norm_mode, contraction=contraction, scaling=scaling, fs=fs,
-                  band=band)
+                  band=band, window=window, detrend=detrend)
     if ld_pad:
         buf = torch.zeros((C, T + ld_pad), dtype=dev(x[:1, :1]).dtype, device="cuda")
         buf[:, :T] = dev(x)
@@ -83,8 +84,9 @@ def gpu_analyze(x, L, H, M, in_dtype=None, norm_mode=0, n_first=0, contraction=0
     return plan, {k: v.cpu().numpy() for k, v in out.items()}
 
 
-def oracle_for(x, L, H, M, pairs=None, norm_mode=0, offs=None, scaling=0, fs=500e3, band=None):
-    return o.analyze_chunk(x, L, H, M, pairs=pairs, norm_mode=norm_mode, offs=offs, scaling=scaling, fs=fs, band=band)
+def oracle_for(x, L, H, M, pairs=None, norm_mode=0, offs=None, scaling=0, fs=500e3, band=None, win=0, detrend=0):
+    return o.analyze_chunk(x, L, H, M, pairs=pairs, norm_mode=norm_mode, offs=offs, scaling=scaling, fs=fs, band=band,
+                           win=win, detrend=detrend)
 
 
 # ------------------------------------------------------------------------------------------
@@ -377,3 +379,28 @@ def test_bandpass_preprocessing(band, mode):
         for k in ("G", "A", "P", "Sauto"):
             assert np.array_equal(out[k], plain[k]), k
         assert np.abs(out["R"] - plain["R"]).max() < 5e-6
+
+
+@pytest.mark.parametrize("window,detrend,L,H", [(1, 0, 512, 256), (2, 1, 512, 256), (3, 1, 256, 64), (0, 1, 2048, 1024),
+                                                (2, 0, 64, 32)])
+def test_window_variants_and_detrend(window, detrend, L, H, mode):
+    """f1: Hamming / rectangular / Blackman windows and the per-segment constant detrend, on
+    a signal with large per-channel offsets (so that a missing detrend or a wrong window shows).  L = 2048 uses
+    transforms wider than a warp (the detrend sum crosses warps), L = 64 the smallest."""
+    rng = np.random.default_rng(77)
+    C, T = 12, 9000
+    # white noise mixed over neighbouring channels (flat spectrum: the float32 dynamic-range question of R13 is
+    # config 2's business, not this test's) plus per-channel offsets
+    g = rng.standard_normal((C + 1, T))
+    x = (g[:C] + 0.7 * g[1:] + rng.uniform(-1, 1, size=(C, 1))).astype(np.float32)
+    M = L // 2
+    _, out = gpu_analyze(x, L, H, M, contraction=mode, window=window, detrend=detrend)
+    ref = oracle_for(x, L, H, M, win=window, detrend=detrend)
+    if window == 2 and detrend == 1:
+        # rectangular window + detrend: the DC bin is exactly empty (pin P13), so G and A are 0/0 there and the
+        # autospectrum is rounding residue on both sides; compare bins 1.. and bound the residue
+        assert np.abs(out["Sauto"][:, 0]).max() <= 1e-9 * out["Sauto"].max()
+        out = {k: (v if k == "R" else v[:, 1:]) for k, v in out.items()}
+        ref = {k: (v if k == "R" else v[:, 1:]) for k, v in ref.items()}
+    st = compare(out, ref, o.all_pairs(C), f"window {window} detrend {detrend} L {L}")
+    print(window, detrend, L, st)
