@@ -133,7 +133,7 @@ int delta_stft_unpack(delta_plan *plan, const void *d_X, float *d_out, void *str
 
 /* a2 + a3, Eq. (1a).  d_S: s_bytes of complex64 in the library's pair-block layout
  * [ceil(P/B)][F][B], B = s_block_pairs: lexicographic pair p is in block p / B, and inside row f of
- * the block in slot (p ^ f) mod B (use delta_cross_spectra_unpack to read it); d_Sauto: float [C][F]
+ * the block in slot (p ^ f ^ (f >> 2)) mod B (use delta_cross_spectra_unpack to read it); d_Sauto: float [C][F]
  * autospectra S_cc[f].  Either may be NULL. */
 int delta_cross_spectra(delta_plan *plan, const void *d_X, float *d_S, float *d_Sauto, void *stream);
 /* Test accessor: expands d_S to complex64 [P][F] (interleaved re, im), pairs lexicographic. */

@@ -99,7 +99,7 @@ int delta_plan_create(const delta_config *cfg, delta_plan **out) {
   l.nlags = 2 * l.M + 1;
   l.P = (int64_t)l.C * (l.C - 1) / 2;
   l.PB = pair_block(l.L);
-  l.pb_shift = l.PB == 16 ? 4 : (l.PB == 8 ? 3 : 2);
+  l.pb_shift = l.PB == 32 ? 5 : (l.PB == 16 ? 4 : (l.PB == 8 ? 3 : 2));
   l.Pblk = (l.P + l.PB - 1) / l.PB;
   // floats (2 parts) or halves (2 precisions x 2 parts) per frequency
   l.x_elems_per_f = (int64_t)(p->contraction == DELTA_CONTRACT_TC ? 4 : 2) * l.Kc * l.Cp * kSegBlock;

@@ -76,7 +76,7 @@ contract_fp32_kernel(const float *__restrict__ X, Layout lay, float scale, float
         if (S) {
           // lexicographic pair index, block-major, slot swizzled by bin (Layout in delta_internal.h)
           const int64_t p = (int64_t)i * C - ((int64_t)i * (i + 1)) / 2 + (j - i - 1);
-          S[((p >> lay.pb_shift) * lay.F + f) * lay.PB + ((p ^ f) & pb_mask)] =
+          S[((p >> lay.pb_shift) * lay.F + f) * lay.PB + ((p ^ s_swz(f)) & pb_mask)] =
               make_float2(acc_re[a][b] * scale, acc_im[a][b] * scale);
         }
       } else if (i == j) {

@@ -307,7 +307,7 @@ contract_tc_kernel(const __half *__restrict__ X, Layout lay, TcParams prm, float
     const int fstep = gridDim.x / prm.ngroups, gstep = gridDim.x % prm.ngroups;
     for (int item = blockIdx.x; item < nitems; item += gridDim.x, f += fstep + (g + gstep >= prm.ngroups), g = (g + gstep) % prm.ngroups) {
       const int nu = prm.nunits[g];
-      const int fx = f & pb_mask;
+      const int fx = s_swz(f) & pb_mask;
       float2 *Sf = S + (int64_t)f * lay.PB;
       for (int u = 0; u < nu; ++u) {
         const TcUnit un = prm.units[g][u];

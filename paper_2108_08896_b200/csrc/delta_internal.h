@@ -30,7 +30,10 @@ bool tc_plan_tiles(int Cp, TcHostPlan *out);
 #endif
 constexpr int pair_fft_variant(int N) { return (DELTA_PAIR_NARROW && N == 256) ? 1 : 0; }
 constexpr int pair_fft_points(int N) { return (N <= 64 || pair_fft_variant(N) == 1) ? 8 : 16; }  // E of that geometry
-constexpr int pair_block(int L) { return L <= 1024 ? 16 : (L == 2048 ? 8 : 4); }
+#ifndef DELTA_PB_SMALL
+#define DELTA_PB_SMALL 16
+#endif
+constexpr int pair_block(int L) { return L <= 512 ? DELTA_PB_SMALL : (L <= 1024 ? 16 : (L == 2048 ? 8 : 4)); }
 
 struct Layout {
   // X (STFT) buffer, frequency-major so that one bin's C x K matrix is one contiguous block:
@@ -44,12 +47,21 @@ struct Layout {
   int f_lo, f_hi;  // pass band of the optional band-pass filter, in bins (0 .. F-1 when it is off)
   int nkb;  // segment blocks per channel = ceil(K / 8): one partial of the windowed signal energy each (wpart)
   // S (cross-spectra) is complex64 [Pblk][F][PB]: pairs in lexicographic order p = iC - i(i+1)/2 + (j-i-1),
-  // block = p / PB, and inside row f of a block pair p sits in slot (p ^ f) & (PB-1).  One block is one
+  // block = p / PB, and inside row f of a block pair p sits in slot (p ^ s_swz(f)) & (PB-1), s_swz(f) = f ^ (f >> 2).
+  // One block is one
   // contiguous tile for the pair kernel; the XOR makes its column (fixed pair) reads bank-conflict free.
   int PB, pb_shift;
   int64_t P, Pblk;
   int64_t x_elems_per_f;  // elements (float or half) per frequency
 };
+
+// Row swizzle of the S layout.  It is XOR-linear (s_swz(a ^ b) = s_swz(a) ^ s_swz(b)), and makes the three column
+// access patterns of the pair kernel bank-conflict free: 4 consecutive bins per lane with lanes 4 bins apart (G/A/P pass),
+// bins gt + T u over lanes gt (merge), and at most 2-way for the mirrored bins N - f.
+#if defined(__CUDACC__)
+__host__ __device__
+#endif
+constexpr int s_swz(int f) { return f ^ (f >> 2); }
 
 struct Workspace {
   size_t off_tw, off_win, off_ftab, off_ftab2, off_pairs, off_offs, off_isum, off_chscale, off_chmax, off_chcnt, off_X, off_S, off_auto, off_rsq, off_wpart, off_rsum, total;

@@ -124,7 +124,7 @@ pair_kernel(const float2 *__restrict__ S, const float *__restrict__ Srsq, const 
   constexpr int N = Cfg::N, F = Cfg::F, T = Cfg::T, E = Cfg::E, PB = Cfg::PB;
   constexpr int THREADS = Cfg::THREADS;
   extern __shared__ __align__(128) unsigned char smem_raw[];
-  float2 *tile = reinterpret_cast<float2 *>(smem_raw);                     // [F][PB], slot = (pl ^ f) & (PB-1)
+  float2 *tile = reinterpret_cast<float2 *>(smem_raw);                     // [F][PB], slot = (pl ^ s_swz(f)) & (PB-1)
   float2 *exch = reinterpret_cast<float2 *>(smem_raw);                     // [PB][BUF] once the tile is dead
   float *rowj = reinterpret_cast<float *>(smem_raw + Cfg::BUF_BYTES);      // [PB][FP]: 1/sqrt(S_jj[f]) of pair pl's j
   float *rs = reinterpret_cast<float *>(smem_raw + Cfg::BUF_BYTES + Cfg::ROWS_BYTES);  // [2][PB]: 1/sqrt(L R_cc[0]) of i, j
@@ -209,7 +209,7 @@ pair_kernel(const float2 *__restrict__ S, const float *__restrict__ Srsq, const 
         float g2[4];
 #pragma unroll
         for (int k = 0; k < 4; ++k) {
-          sv[k] = tile[(f + k) * PB + ((ql ^ (f + k)) & (PB - 1))];
+          sv[k] = tile[(f + k) * PB + ((ql ^ s_swz(f + k)) & (PB - 1))];
           g2[k] = wantG ? __ldg(qi + k) * qj[k] : 0.f;
         }
         float m[4], c[4], an[4];
@@ -236,7 +236,7 @@ pair_kernel(const float2 *__restrict__ S, const float *__restrict__ Srsq, const 
       const ushort2 qij = ij_s[ql];
       const float g2 = wantG ? __ldg(Srsq + (int64_t)qij.x * Cfg::FP + f) * rowj[ql * Cfg::FP + f] : 0.f;
       float m, c, an;
-      value(tile[f * PB + ((ql ^ f) & (PB - 1))], g2, m, c, an);
+      value(tile[f * PB + ((ql ^ s_swz(f)) & (PB - 1))], g2, m, c, an);
       if (GAPALL || Pw) ST1(Pw + q * F + f, m);
       if (GAPALL || G) ST1(G + q * F + f, c);
       if (GAPALL || A) ST1(A + q * F + f, an);
@@ -247,13 +247,13 @@ pair_kernel(const float2 *__restrict__ S, const float *__restrict__ Srsq, const 
   // ---- pass 2: merge step of the inverse real transform (S read again from the tile; twice the merge of
   // irfft_merge, the factor 1/2 goes into the normalisation) ------------------------------------------------
   float2 v[E];
-  const int pg = pl ^ gt;
+  const int pg = pl ^ s_swz(gt);
 #pragma unroll
   for (int u = 0; u < E; ++u) {
     const int f = gt + T * u;
     const int fr = N - f;
-    float2 sf = tile[f * PB + ((pg ^ (T * u)) & (PB - 1))];
-    float2 sr = tile[fr * PB + ((pl ^ fr) & (PB - 1))];
+    float2 sf = tile[f * PB + ((pg ^ s_swz(T * u)) & (PB - 1))];  // s_swz(gt | T u) = s_swz(gt) ^ s_swz(T u)
+    float2 sr = tile[fr * PB + ((pl ^ s_swz(fr)) & (PB - 1))];
     if (u == 0 && gt == 0) { sf.y = 0.f; sr.y = 0.f; }  // Im S[0], Im S[N] do not enter the real transform
     const float2 w = cmul(wg, pc.wstep[u]);               // e^{-2 pi i f / L}; the inverse uses its conjugate
     v[u] = irfft_merge2(sf, sr, make_float2(w.x, -w.y));
@@ -322,7 +322,7 @@ __global__ void __launch_bounds__(256) s_unpack_kernel(const float2 *__restrict_
   for (int64_t idx = (int64_t)blockIdx.x * 256 + threadIdx.x; idx < total; idx += (int64_t)gridDim.x * 256) {
     const int f = (int)(idx % lay.F);
     const int64_t p = idx / lay.F;
-    out[idx] = S[((p >> lay.pb_shift) * lay.F + f) * lay.PB + ((p ^ f) & (lay.PB - 1))];
+    out[idx] = S[((p >> lay.pb_shift) * lay.F + f) * lay.PB + ((p ^ s_swz(f)) & (lay.PB - 1))];
   }
 }
 
