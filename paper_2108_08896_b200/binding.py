@@ -219,10 +219,12 @@ class Plan:
         _check(LIB.delta_crosscorr(self._h, S.data_ptr(), Sauto.data_ptr(), R.data_ptr(), _stream()), "delta_crosscorr")
         return R
 
-    def analyze_chunk(self, x, out=None):
+    def analyze_chunk(self, x, out=None, stream=None):
+        """stream: a torch.cuda.Stream (default: torch's current stream)."""
         out = self.empty_outputs() if out is None else out
         _check(LIB.delta_analyze_chunk(self._h, x.data_ptr(), x.stride(0), _ptr(out.get("G")), _ptr(out.get("A")),
-                                       _ptr(out.get("P")), _ptr(out.get("R")), _ptr(out.get("Sauto")), _stream()),
+                                       _ptr(out.get("P")), _ptr(out.get("R")), _ptr(out.get("Sauto")),
+                                       _stream() if stream is None else stream.cuda_stream),
                "delta_analyze_chunk")
         return out
 
