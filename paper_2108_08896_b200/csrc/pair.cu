@@ -196,11 +196,16 @@ pair_kernel(const float2 *__restrict__ S, const float *__restrict__ Srsq, const 
     constexpr int NG = N / 4;  // group slots per pair
     const bool vec4 = (((reinterpret_cast<uintptr_t>(G) | reinterpret_cast<uintptr_t>(A) | reinterpret_cast<uintptr_t>(Pw)) & 15) == 0);
     if (vec4) {
-#pragma unroll 2
-      for (int item = tid; item < PB * NG; item += THREADS) {
-        const int ql = item / NG, g = item % NG;
+      // R pairs are in flight per iteration; a thread keeps its group g and its pair slot qa, so with R a multiple of 4
+      // the bins f, the tile rows and the alignment shift f0 do not depend on the iteration (p0 is a multiple of 4)
+      constexpr int R = THREADS / NG, NIT = PB / R;
+      static_assert(R >= 1 && (R & (R - 1)) == 0 && PB % R == 0, "pairs per iteration");
+      const int g = tid % NG, qa = tid / NG;
+#pragma unroll
+      for (int it = 0; it < NIT; ++it) {
+        const int ql = (it * R) ^ qa;  // = it R + qa (qa < R, R a power of two)
         const int64_t q = p0 + ql;
-        const int f0 = (int)((-q) & 3), ng = (F - f0) >> 2;
+        const int f0 = (-(qa + ((it * R) & 3))) & 3, ng = (F - f0) >> 2;
         if (q >= lay.P || g >= ng) continue;
         const int f = f0 + 4 * g;
         const ushort2 qij = ij_s[ql];
@@ -209,7 +214,7 @@ pair_kernel(const float2 *__restrict__ S, const float *__restrict__ Srsq, const 
         float g2[4];
 #pragma unroll
         for (int k = 0; k < 4; ++k) {
-          sv[k] = tile[(f + k) * PB + ((ql ^ s_swz(f + k)) & (PB - 1))];
+          sv[k] = tile[(f + k) * PB + (((qa ^ s_swz(f + k)) ^ (it * R)) & (PB - 1))];
           g2[k] = wantG ? __ldg(qi + k) * qj[k] : 0.f;
         }
         float m[4], c[4], an[4];
