@@ -227,6 +227,17 @@ def crosscorr(S: np.ndarray, Sauto: np.ndarray, pairs: np.ndarray, L: int, M: in
     return rho
 
 
+# f2 variant: shot-level accumulation.  The expectation E[.] of Eq. (1a), taken
+# over the segments of SEVERAL chunks instead of one: since every chunk has the same K, that is the plain mean of the
+# per-chunk spectra.  Coherence, phase and correlation are then formed from the accumulated spectra (R10).
+def accumulate(spectra: list) -> np.ndarray:
+    """Mean over chunks of per-chunk cross- or auto-spectra (all of one shape)."""
+    acc = np.zeros_like(spectra[0])
+    for sp in spectra:
+        acc = acc + sp
+    return acc / len(spectra)
+
+
 # ----------------------------------------------------------------------------------------------
 # the whole path for one chunk, in the paper's order (L107: normalise -> STFT -> Eqs. 1)
 def analyze_chunk(x, L, H, M, pairs=None, scaling=SCALE_WINPOW, fs=1.0,

@@ -498,3 +498,24 @@ def test_P13_windows_and_detrend_against_scipy(kind, name, detrend):
         assert np.allclose(np.abs(Xc[0, :, q]), L / 2, atol=1e-9)
         others = np.delete(np.abs(Xc[0]), q, axis=1)
         assert others.max() < 1e-9
+
+
+# ---------------------------------------------------------------------------- f2: accumulation over chunks
+def test_P14_accumulation_over_chunks_is_the_mean_over_all_segments():
+    """Accumulating per-chunk spectra = Eq. (1a) with E[.] over the segments of all the chunks: compare with the
+    cross-spectrum computed in one go from the stacked segments.  And the point of it: for independent noise the
+    coherence floor drops like 1/sqrt(number of chunks) (P8's law with K -> n K)."""
+    L, H, T, n = 64, 32, 640, 6
+    rng = np.random.default_rng(14)
+    chunks = [rng.standard_normal((3, T)) for _ in range(n)]
+    pairs = o.all_pairs(3)
+    s2 = o.scale_factor(L)
+    Xs = [o.stft(c, L, H) for c in chunks]
+    S_acc = o.accumulate([o.cross_spectra(X, pairs, s2) for X in Xs])
+    Sa_acc = o.accumulate([o.auto_spectra(X, s2) for X in Xs])
+    X_all = np.concatenate(Xs, axis=1)                      # all segments of all chunks
+    assert np.allclose(S_acc, o.cross_spectra(X_all, pairs, s2), rtol=1e-12, atol=1e-14)
+    assert np.allclose(Sa_acc, o.auto_spectra(X_all, s2), rtol=1e-12, atol=1e-14)
+    G1 = o.coherence(o.cross_spectra(Xs[0], pairs, s2), o.auto_spectra(Xs[0], s2), pairs)
+    Gn = o.coherence(S_acc, Sa_acc, pairs)
+    assert 0.30 < Gn[:, 2:-2].mean() / G1[:, 2:-2].mean() < 0.55      # 1/sqrt(6) = 0.41
