@@ -38,7 +38,7 @@
 extern "C" {
 #endif
 
-#define DELTA_VERSION 102 /* 0.1.2: band-pass, window variants and detrend appended to delta_config */
+#define DELTA_VERSION 103 /* 0.1.3: band-pass, window variants, detrend in delta_config; delta_accumulate */
 
 typedef enum {
   DELTA_OK = 0,
@@ -148,6 +148,15 @@ int delta_crosspower(delta_plan *plan, const float *d_S, float *d_P, void *strea
 /* a5, Eq. (1d): d_R float [P][2M+1], lags -M..M increasing, normalised by sqrt(R_ii[0] R_jj[0]),
  * circular in the lag (R12).  0 where the denominator is 0. */
 int delta_crosscorr(delta_plan *plan, const float *d_S, const float *d_Sauto, float *d_R, void *stream);
+
+/* f2 (shot-level accumulation): the expectation of Eq. (1a), over the segments of several chunks.
+ * d_S_acc = w_acc d_S_acc + w_new d_S (s_bytes each, the library's layout) and the same for the autospectra
+ * (float [C][F]); either pair of pointers may be NULL.  w_acc = 0 initialises (the old contents are not read).
+ * Every chunk has the same number of segments, so n calls with (n-1)/n, 1/n weights -- or weights 1 and any common
+ * factor: G, A and rho do not depend on it -- give the average over all segments.  The staged calls
+ * (delta_coherence, ...) then work on the accumulated spectra. */
+int delta_accumulate(delta_plan *plan, float *d_S_acc, float *d_Sauto_acc, const float *d_S, const float *d_Sauto,
+                     float w_acc, float w_new, void *stream);
 
 /* The whole path a0..a5 for one chunk resident in device memory, using the plan's workspace for
  * X and S.  Any output pointer may be NULL (that quantity is then not computed / stored).

@@ -40,7 +40,7 @@ class DeltaSizes(C.Structure):
 EXPORTS = ["delta_plan_create", "delta_plan_destroy", "delta_plan_sizes", "delta_plan_set_workspace",
            "delta_set_offsets", "delta_get_offsets", "delta_stft", "delta_stft_unpack", "delta_cross_spectra",
            "delta_cross_spectra_unpack", "delta_debug_set_trace",
-           "delta_coherence", "delta_crossphase", "delta_crosspower", "delta_crosscorr", "delta_analyze_chunk",
+           "delta_coherence", "delta_crossphase", "delta_crosspower", "delta_crosscorr", "delta_accumulate", "delta_analyze_chunk",
            "delta_analyze_shot_host", "delta_plan_set_stage_events", "delta_last_launch_count", "delta_strerror", "delta_last_cuda_error",
            "delta_version"]
 
@@ -66,6 +66,7 @@ def _load() -> C.CDLL:
     lib.delta_crossphase.argtypes = [vp, vp, vp, vp]
     lib.delta_crosspower.argtypes = [vp, vp, vp, vp]
     lib.delta_crosscorr.argtypes = [vp, vp, vp, vp, vp]
+    lib.delta_accumulate.argtypes = [vp, vp, vp, vp, vp, C.c_float, C.c_float, vp]
     lib.delta_analyze_chunk.argtypes = [vp, vp, i64, vp, vp, vp, vp, vp, vp]
     lib.delta_analyze_shot_host.argtypes = [vp, vp, i32, vp, i32, i32, vp, vp, vp, vp, vp, i64, i64, i64,
                                             vp, vp, vp, vp, vp, vp]
@@ -218,6 +219,10 @@ class Plan:
         R = torch.empty((self.sizes.P, self.sizes.n_lags), dtype=torch.float32, device=self.device) if R is None else R
         _check(LIB.delta_crosscorr(self._h, S.data_ptr(), Sauto.data_ptr(), R.data_ptr(), _stream()), "delta_crosscorr")
         return R
+
+    def accumulate(self, S_acc, Sauto_acc, S, Sauto, w_acc, w_new):
+        _check(LIB.delta_accumulate(self._h, _ptr(S_acc), _ptr(Sauto_acc), _ptr(S), _ptr(Sauto), w_acc, w_new, _stream()),
+               "delta_accumulate")
 
     def analyze_chunk(self, x, out=None, stream=None):
         """stream: a torch.cuda.Stream (default: torch's current stream)."""

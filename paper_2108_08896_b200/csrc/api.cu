@@ -340,6 +340,23 @@ int delta_crosscorr(delta_plan *p, const float *d_S, const float *d_Sauto, float
   return pair_stage(p, d_S, d_Sauto, nullptr, nullptr, nullptr, d_R, stream, true);
 }
 
+int delta_accumulate(delta_plan *p, float *d_S_acc, float *d_Sauto_acc, const float *d_S, const float *d_Sauto, float w_acc,
+                     float w_new, void *stream) {
+  int rc = need_ws(p);
+  if (rc) return rc;
+  if ((d_S_acc == nullptr) != (d_S == nullptr) || (d_Sauto_acc == nullptr) != (d_Sauto == nullptr)) return DELTA_ERR_INVALID_ARG;
+  if (!d_S_acc && !d_Sauto_acc) return DELTA_ERR_INVALID_ARG;
+  if ((d_S_acc && (!aligned16(d_S_acc) || !aligned16(d_S)))) return DELTA_ERR_ALIGNMENT;
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+  const Layout &l = p->lay;
+  if (d_S_acc) {
+    rc = launch_axpby(p, d_S_acc, d_S, (int64_t)(l.Pblk > 0 ? l.Pblk : 1) * l.F * l.PB * 2, w_acc, w_new, st);
+    if (rc) return rc;
+  }
+  if (d_Sauto_acc) rc = launch_axpby(p, d_Sauto_acc, d_Sauto, (int64_t)l.C * l.F, w_acc, w_new, st);
+  return rc;
+}
+
 int delta_analyze_chunk(delta_plan *p, const void *d_x, int64_t ld, float *d_G, float *d_A, float *d_P, float *d_R,
                         float *d_Sauto, void *stream) {
   int rc = need_ws(p);

@@ -205,6 +205,7 @@ int launch_auto_prep(delta_plan *p, const float *d_auto, float *d_rsq, float *d_
 // rpart/nrp/rp_stride/rscale: sum over all L bins of S_cc = rscale * sum_{k<nrp} rpart[c * rp_stride + k]
 int launch_pair(delta_plan *p, const float *d_S, const float *d_rsq, const float *rpart, int nrp, int rp_stride, float rscale,
                 float *d_G, float *d_A, float *d_P, float *d_R, cudaStream_t st);
+int launch_axpby(delta_plan *p, float *acc, const float *x, int64_t n, float wa, float wn, cudaStream_t st);
 int launch_s_unpack(delta_plan *p, const float *d_S, float *d_out, cudaStream_t st);
 
 }  // namespace delta

@@ -321,6 +321,31 @@ __global__ void __launch_bounds__(32) auto_prep_kernel(const float *__restrict__
   if (lane == 0) rsum[c] = sum;
 }
 
+// acc = wa acc + wn x (f2: accumulation of spectra over chunks); wa == 0 does not read acc
+__global__ void __launch_bounds__(256) axpby_kernel(float *__restrict__ acc, const float *__restrict__ x, int64_t n, float wa,
+                                                    float wn, int vec) {
+  const int64_t stride = (int64_t)gridDim.x * 256;
+  if (vec) {
+    const int64_t n4 = n >> 2;
+    float4 *a4 = reinterpret_cast<float4 *>(acc);
+    const float4 *x4 = reinterpret_cast<const float4 *>(x);
+    for (int64_t i = (int64_t)blockIdx.x * 256 + threadIdx.x; i < n4; i += stride) {
+      const float4 v = x4[i];
+      float4 o = make_float4(wn * v.x, wn * v.y, wn * v.z, wn * v.w);
+      if (wa != 0.f) {
+        const float4 a = a4[i];
+        o = make_float4(fmaf(wa, a.x, o.x), fmaf(wa, a.y, o.y), fmaf(wa, a.z, o.z), fmaf(wa, a.w, o.w));
+      }
+      a4[i] = o;
+    }
+    for (int64_t i = (n4 << 2) + (int64_t)blockIdx.x * 256 + threadIdx.x; i < n; i += stride)
+      acc[i] = (wa != 0.f ? wa * acc[i] : 0.f) + wn * x[i];
+  } else {
+    for (int64_t i = (int64_t)blockIdx.x * 256 + threadIdx.x; i < n; i += stride)
+      acc[i] = (wa != 0.f ? wa * acc[i] : 0.f) + wn * x[i];
+  }
+}
+
 // test accessor: S layout -> complex64 [P][F], lexicographic pairs
 __global__ void __launch_bounds__(256) s_unpack_kernel(const float2 *__restrict__ S, Layout lay, float2 *__restrict__ out) {
   const int64_t total = lay.P * lay.F;
@@ -370,6 +395,17 @@ int launch_pair(delta_plan *p, const float *d_S, const float *d_rsq, const float
 
 int launch_auto_prep(delta_plan *p, const float *d_auto, float *d_rsq, float *d_rsum, cudaStream_t st) {
   auto_prep_kernel<<<(unsigned)p->lay.C, 32, 0, st>>>(d_auto, d_rsq, d_rsum, p->lay.F, p->lay.Fp);
+  p->launches++;
+  DELTA_CUDA_CHECK(cudaGetLastError());
+  return DELTA_OK;
+}
+
+int launch_axpby(delta_plan *p, float *acc, const float *x, int64_t n, float wa, float wn, cudaStream_t st) {
+  if (n <= 0) return DELTA_OK;
+  const int vec = ((reinterpret_cast<uintptr_t>(acc) | reinterpret_cast<uintptr_t>(x)) & 15) == 0;
+  const int64_t want = ((vec ? n / 4 : n) + 255) / 256;
+  const int64_t cap = (int64_t)p->num_sms * 16;
+  axpby_kernel<<<(unsigned)(want < 1 ? 1 : (want < cap ? want : cap)), 256, 0, st>>>(acc, x, n, wa, wn, vec);
   p->launches++;
   DELTA_CUDA_CHECK(cudaGetLastError());
   return DELTA_OK;

@@ -404,3 +404,34 @@ def test_window_variants_and_detrend(window, detrend, L, H, mode):
         ref = {k: (v if k == "R" else v[:, 1:]) for k, v in ref.items()}
     st = compare(out, ref, o.all_pairs(C), f"window {window} detrend {detrend} L {L}")
     print(window, detrend, L, st)
+
+
+def test_accumulation_over_chunks(mode):
+    """f2: the expectation of Eq. (1a) over the segments of several chunks: per-chunk spectra
+    accumulated with delta_accumulate, then the staged coherence / phase / power / correlation calls on the sum,
+    against the oracle's accumulated estimate."""
+    b = binding()
+    w = es.WORKLOADS["single"]
+    C, n = 32, 5
+    chunks = [es.turbulence(w.T, 900 + i)[:C] for i in range(n)]
+    plan = b.Plan(C, w.T, w.nfft, w.hop, w.max_lag, contraction=mode)
+    S_acc, Sa_acc = plan.empty_S(), torch.empty((C, plan.sizes.F), dtype=torch.float32, device="cuda")
+    S_acc.fill_(float("nan"))          # w_acc = 0 must not read the old contents
+    Sa_acc.fill_(float("nan"))
+    for k, x in enumerate(chunks):
+        X = plan.stft(dev(x))
+        S, Sa = plan.cross_spectra(X)
+        plan.accumulate(S_acc, Sa_acc, S, Sa, 0.0 if k == 0 else 1.0, 1.0 / n)   # running sum of S / n = the mean
+    out = dict(G=plan.coherence(S_acc, Sa_acc), A=plan.crossphase(S_acc), P=plan.crosspower(S_acc),
+               R=plan.crosscorr(S_acc, Sa_acc), Sauto=Sa_acc)
+    torch.cuda.synchronize()
+    out = {k: v.cpu().numpy() for k, v in out.items()}
+    pairs = o.all_pairs(C)
+    s2 = o.scale_factor(w.nfft)
+    Xs = [o.stft(x, w.nfft, w.hop) for x in chunks]
+    S_o = o.accumulate([o.cross_spectra(X, pairs, s2) for X in Xs])
+    Sa_o = o.accumulate([o.auto_spectra(X, s2) for X in Xs])
+    ref = dict(G=o.coherence(S_o, Sa_o, pairs), A=o.crossphase(S_o), P=o.crosspower(S_o),
+               R=o.crosscorr(S_o, Sa_o, pairs, w.nfft, w.max_lag), Sauto=Sa_o)
+    st = compare(out, ref, pairs, "accumulated")
+    print(st)
