@@ -80,8 +80,11 @@ typedef struct {
   int32_t in_dtype;     /* DELTA_F32 | DELTA_I16                                                      */
   int32_t norm_mode;    /* DELTA_NORM_*; SUBTRACT and RELATIVE need delta_set_offsets() once per shot */
   int32_t max_lag;      /* M in [0, L/2]; cross-correlation lags -M..M                                */
-  int32_t n_pairs;      /* 0 => all i < j in lexicographic order                                      */
-  const int32_t *h_pairs; /* host [n_pairs][2] or NULL; explicit lists: DELTA_ERR_UNSUPPORTED for now */
+  int32_t n_pairs;      /* 0 => all i < j in lexicographic order ("channel pair combinations") */
+  const int32_t *h_pairs; /* host [n_pairs][2] or NULL: explicit pair list (f2), every entry 0 <= i < j < C (else
+                           * DELTA_ERR_INVALID_ARG), copied by delta_plan_create; the per-pair outputs then have
+                           * n_pairs rows in list order (S_ji = conj S_ij gives the swapped pair: G, P equal, A
+                           * negated, rho with the lags reversed); d_S still holds all pairs */
   int32_t contraction;  /* DELTA_CONTRACT_*                                                           */
   /* Optional band-pass pre-processing filter ("pre-processing filters", L231: the demo's 5-9 kHz pass
    * band), reading R19: an ideal mask on the bins of every segment's transform; bin f is kept iff
@@ -97,7 +100,7 @@ typedef struct {
   int32_t n_bins;          /* F = L/2 + 1 */
   int32_t n_lags;          /* 2M + 1 */
   int32_t contraction;     /* the mode the plan resolved DELTA_CONTRACT_AUTO to */
-  int64_t n_pairs;         /* P */
+  int64_t n_pairs;         /* P: rows of the per-pair outputs (all pairs, or the length of the explicit list) */
   int64_t workspace_bytes; /* minimum size for delta_plan_set_workspace() */
   int64_t x_bytes;         /* size of a d_X buffer  (delta_stft output, opaque layout) */
   int64_t s_bytes;         /* size of a d_S buffer (delta_cross_spectra output, opaque layout) */

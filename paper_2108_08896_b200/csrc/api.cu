@@ -36,7 +36,10 @@ static int validate(const delta_config *c) {
   if (c->n_samples < L) return DELTA_ERR_UNSUPPORTED;
   if (c->max_lag > L / 2) return DELTA_ERR_UNSUPPORTED;
   if (c->n_channels > 4096) return DELTA_ERR_UNSUPPORTED;
-  if (c->n_pairs > 0) return DELTA_ERR_UNSUPPORTED;  // explicit pair lists: not in this version
+  for (int k = 0; k < c->n_pairs; ++k) {  // explicit pair list (f2): 0 <= i < j < C
+    const int i = c->h_pairs[2 * k], j = c->h_pairs[2 * k + 1];
+    if (i < 0 || j <= i || j >= c->n_channels) return DELTA_ERR_INVALID_ARG;
+  }
   return DELTA_OK;
 }
 
@@ -101,6 +104,8 @@ int delta_plan_create(const delta_config *cfg, delta_plan **out) {
   l.PB = pair_block(l.L);
   l.pb_shift = l.PB == 32 ? 5 : (l.PB == 16 ? 4 : (l.PB == 8 ? 3 : 2));
   l.Pblk = (l.P + l.PB - 1) / l.PB;
+  l.Po = cfg->n_pairs > 0 ? cfg->n_pairs : l.P;
+  l.Poblk = (l.Po + l.PB - 1) / l.PB;
   // floats (2 parts) or halves (2 precisions x 2 parts) per frequency
   l.x_elems_per_f = (int64_t)(p->contraction == DELTA_CONTRACT_TC ? 4 : 2) * l.Kc * l.Cp * kSegBlock;
 
@@ -145,9 +150,8 @@ int delta_plan_create(const delta_config *cfg, delta_plan **out) {
     case DELTA_SCALE_DENSITY: p->s2 = (float)(1.0 / ((double)cfg->fs * sw2)); break;
     default: p->s2 = (float)(1.0 / (sw * sw)); break;
   }
-  p->h_pairs.reserve((size_t)l.P);
-  for (int i = 0; i < l.C; ++i)
-    for (int j = i + 1; j < l.C; ++j) p->h_pairs.push_back(make_ushort2((unsigned short)i, (unsigned short)j));
+  for (int k = 0; k < cfg->n_pairs; ++k)
+    p->h_pairs.push_back(make_ushort2((unsigned short)cfg->h_pairs[2 * k], (unsigned short)cfg->h_pairs[2 * k + 1]));
   memset(&p->tc, 0, sizeof(p->tc));
   if (p->contraction == DELTA_CONTRACT_TC && !tc_plan_tiles(l.Cp, &p->tc)) { delete p; return DELTA_ERR_UNSUPPORTED; }
 
@@ -158,7 +162,7 @@ int delta_plan_create(const delta_config *cfg, delta_plan **out) {
   w.off_win = take((size_t)L * sizeof(float));
   w.off_ftab = take(p->h_ftab.size() * sizeof(float2));
   w.off_ftab2 = take(p->h_ftab2.size() * sizeof(float2));
-  w.off_pairs = take((size_t)(l.P > 0 ? l.P : 1) * sizeof(ushort2));
+  w.off_pairs = take((p->h_pairs.size() + 1) * sizeof(ushort2));
   w.off_offs = take((size_t)l.C * sizeof(double));
   w.off_isum = take((size_t)l.C * sizeof(long long));
   w.off_chscale = take((size_t)l.C * sizeof(float));
@@ -194,7 +198,7 @@ int delta_plan_sizes(const delta_plan *p, delta_sizes *out) {
   out->n_bins = l.F;
   out->n_lags = l.nlags;
   out->contraction = p->contraction;
-  out->n_pairs = l.P;
+  out->n_pairs = l.Po;
   out->workspace_bytes = (int64_t)p->wsl.total;
   out->x_bytes = (int64_t)l.F * l.x_elems_per_f * (p->contraction == DELTA_CONTRACT_TC ? 2 : 4);
   out->s_bytes = (int64_t)(l.Pblk > 0 ? l.Pblk : 1) * l.F * l.PB * (int64_t)sizeof(float2);
@@ -217,8 +221,8 @@ int delta_plan_set_workspace(delta_plan *p, void *d_ws, size_t bytes, void *stre
   DELTA_CUDA_CHECK(cudaMemcpyAsync(p->ws + p->wsl.off_win, p->h_win.data(), (size_t)l.L * sizeof(float), cudaMemcpyHostToDevice, st));
   DELTA_CUDA_CHECK(cudaMemcpyAsync(p->ws + p->wsl.off_ftab, p->h_ftab.data(), p->h_ftab.size() * sizeof(float2), cudaMemcpyHostToDevice, st));
   DELTA_CUDA_CHECK(cudaMemcpyAsync(p->ws + p->wsl.off_ftab2, p->h_ftab2.data(), p->h_ftab2.size() * sizeof(float2), cudaMemcpyHostToDevice, st));
-  if (l.P > 0)
-    DELTA_CUDA_CHECK(cudaMemcpyAsync(p->ws + p->wsl.off_pairs, p->h_pairs.data(), (size_t)l.P * sizeof(ushort2), cudaMemcpyHostToDevice, st));
+  if (!p->h_pairs.empty())
+    DELTA_CUDA_CHECK(cudaMemcpyAsync(p->ws + p->wsl.off_pairs, p->h_pairs.data(), p->h_pairs.size() * sizeof(ushort2), cudaMemcpyHostToDevice, st));
   // zero rows C..Cp-1 of the workspace X once (kernels never write them)
   DELTA_CUDA_CHECK(cudaMemsetAsync(p->ws + p->wsl.off_X, 0, p->wsl.off_S - p->wsl.off_X, st));
   DELTA_CUDA_CHECK(cudaMemsetAsync(p->ws + p->wsl.off_offs, 0, p->wsl.off_X - p->wsl.off_offs, st));
@@ -371,7 +375,7 @@ int delta_analyze_chunk(delta_plan *p, const void *d_x, int64_t ld, float *d_G, 
   if (rc) return rc;
   if (ev) DELTA_CUDA_CHECK(cudaEventRecord(p->stage_ev[1], st));
   float *au = d_Sauto ? d_Sauto : p->d_auto();
-  const bool pairs_wanted = (d_G || d_A || d_P || d_R) && p->lay.P > 0;
+  const bool pairs_wanted = (d_G || d_A || d_P || d_R) && p->lay.Po > 0;
   rc = contract(p, p->d_X(), pairs_wanted ? p->d_S() : nullptr, au, st);
   if (rc) return rc;
   if (ev) DELTA_CUDA_CHECK(cudaEventRecord(p->stage_ev[2], st));
@@ -425,7 +429,7 @@ int delta_analyze_shot_host(delta_plan *p, const void *h_x, int32_t n_chunks, vo
   // still reading the slots) has finished
   DELTA_CUDA_CHECK(cudaEventRecord(p->ev_done[0], st));
   DELTA_CUDA_CHECK(cudaStreamWaitEvent(p->copy_stream, p->ev_done[0], 0));
-  const size_t gap_bytes = (size_t)l.P * l.F * sizeof(float), r_bytes = (size_t)l.P * l.nlags * sizeof(float);
+  const size_t gap_bytes = (size_t)l.Po * l.F * sizeof(float), r_bytes = (size_t)l.Po * l.nlags * sizeof(float);
   const size_t au_bytes = (size_t)l.C * l.F * sizeof(float);
   int total_launches = 0;
   for (int n = 0; n < n_chunks; ++n) {
@@ -447,10 +451,10 @@ int delta_analyze_shot_host(delta_plan *p, const void *h_x, int32_t n_chunks, vo
     if (rc) return rc;
     total_launches += p->launches;
     DELTA_CUDA_CHECK(cudaEventRecord(p->ev_consumed[s], st));
-    if (h_G) DELTA_CUDA_CHECK(cudaMemcpyAsync(h_G + (size_t)n * l.P * l.F, g, gap_bytes, cudaMemcpyDeviceToHost, st));
-    if (h_A) DELTA_CUDA_CHECK(cudaMemcpyAsync(h_A + (size_t)n * l.P * l.F, a, gap_bytes, cudaMemcpyDeviceToHost, st));
-    if (h_P) DELTA_CUDA_CHECK(cudaMemcpyAsync(h_P + (size_t)n * l.P * l.F, pw, gap_bytes, cudaMemcpyDeviceToHost, st));
-    if (h_R) DELTA_CUDA_CHECK(cudaMemcpyAsync(h_R + (size_t)n * l.P * l.nlags, r, r_bytes, cudaMemcpyDeviceToHost, st));
+    if (h_G) DELTA_CUDA_CHECK(cudaMemcpyAsync(h_G + (size_t)n * l.Po * l.F, g, gap_bytes, cudaMemcpyDeviceToHost, st));
+    if (h_A) DELTA_CUDA_CHECK(cudaMemcpyAsync(h_A + (size_t)n * l.Po * l.F, a, gap_bytes, cudaMemcpyDeviceToHost, st));
+    if (h_P) DELTA_CUDA_CHECK(cudaMemcpyAsync(h_P + (size_t)n * l.Po * l.F, pw, gap_bytes, cudaMemcpyDeviceToHost, st));
+    if (h_R) DELTA_CUDA_CHECK(cudaMemcpyAsync(h_R + (size_t)n * l.Po * l.nlags, r, r_bytes, cudaMemcpyDeviceToHost, st));
     if (h_Sauto) DELTA_CUDA_CHECK(cudaMemcpyAsync(h_Sauto + (size_t)n * l.C * l.F, au, au_bytes, cudaMemcpyDeviceToHost, st));
   }
   p->launches = total_launches;

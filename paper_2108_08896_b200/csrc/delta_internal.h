@@ -51,7 +51,8 @@ struct Layout {
   // One block is one
   // contiguous tile for the pair kernel; the XOR makes its column (fixed pair) reads bank-conflict free.
   int PB, pb_shift;
-  int64_t P, Pblk;
+  int64_t P, Pblk;    // all pairs i < j: the S layout
+  int64_t Po, Poblk;  // output rows: P, or the length of the explicit pair list (f2)
   int64_t x_elems_per_f;  // elements (float or half) per frequency
 };
 
@@ -81,7 +82,7 @@ struct delta_plan {
   float2 h_wstep[16];            // e^{-2 pi i T u / L}, u < E: bin f = gt + T u of a thread has twiddle tw[gt] * wstep[u]
   std::vector<float2> h_ftab;    // per-pass twiddles of the register FFT (fft_reg.cuh), N = L/2
   std::vector<float2> h_ftab2;   // the same for the pair kernel's geometry variant
-  std::vector<ushort2> h_pairs;  // (i, j) of pair p, lexicographic
+  std::vector<ushort2> h_pairs;  // the explicit pair list (empty: all pairs)
   delta::TcHostPlan tc;
   int num_sms = 148;
   // device state

@@ -39,7 +39,11 @@ struct PairCfg {
   static constexpr size_t BUF_BYTES = ((TILE_BYTES > EXCH_BYTES ? TILE_BYTES : EXCH_BYTES) + 15) & ~(size_t)15;
   static constexpr int FP = (F + 3) & ~3;                                   // pitch of the rsq table
   static constexpr size_t ROWS_BYTES = (size_t)PB * FP * sizeof(float);     // 1/sqrt(S_jj) row of every pair's j
-  static constexpr size_t SMEM = BUF_BYTES + ROWS_BYTES + 2 * PB * sizeof(float) + PB * sizeof(ushort2) + 16;
+  static constexpr size_t OFF_RS = BUF_BYTES + ROWS_BYTES;                    // float [2][PB]
+  static constexpr size_t OFF_IJ = OFF_RS + 2 * PB * sizeof(float);           // ushort2 [PB]
+  static constexpr size_t OFF_PG = OFF_IJ + PB * sizeof(ushort2);             // int [PB]: lexicographic index (pair lists)
+  static constexpr size_t OFF_BAR = (OFF_PG + PB * sizeof(int) + 7) & ~(size_t)7;
+  static constexpr size_t SMEM = OFF_BAR + 16;
   static_assert(THREADS % 32 == 0 && THREADS <= 1024, "block shape");
   static_assert(TILE_BYTES % 16 == 0, "bulk copy size");
   static_assert((T & (T - 1)) == 0 && (PB & (PB - 1)) == 0, "powers of two");
@@ -116,7 +120,7 @@ __device__ __forceinline__ ushort2 pair_of(int64_t p, int C) {
 template <int L, bool FULL, bool GAPALL>
 __global__ void __launch_bounds__(PairCfg<L>::THREADS, PairCfg<L>::MIN_CTAS)
 pair_kernel(const float2 *__restrict__ S, const float *__restrict__ Srsq, const float *__restrict__ rpart, int nrp,
-            int rp_stride, float rscale, const float2 *__restrict__ tw,
+            int rp_stride, float rscale, const ushort2 *__restrict__ list, const float2 *__restrict__ tw,
             const float2 *__restrict__ ftab, Layout lay, PairConsts pc, float *__restrict__ G_, float *__restrict__ A_,
             float *__restrict__ Pw_, float *__restrict__ R_) {
   using Cfg = PairCfg<L>;
@@ -127,9 +131,10 @@ pair_kernel(const float2 *__restrict__ S, const float *__restrict__ Srsq, const 
   float2 *tile = reinterpret_cast<float2 *>(smem_raw);                     // [F][PB], slot = (pl ^ s_swz(f)) & (PB-1)
   float2 *exch = reinterpret_cast<float2 *>(smem_raw);                     // [PB][BUF] once the tile is dead
   float *rowj = reinterpret_cast<float *>(smem_raw + Cfg::BUF_BYTES);      // [PB][FP]: 1/sqrt(S_jj[f]) of pair pl's j
-  float *rs = reinterpret_cast<float *>(smem_raw + Cfg::BUF_BYTES + Cfg::ROWS_BYTES);  // [2][PB]: 1/sqrt(L R_cc[0]) of i, j
-  ushort2 *ij_s = reinterpret_cast<ushort2 *>(rs + 2 * PB);                // [PB]
-  uint64_t *bar = reinterpret_cast<uint64_t *>(smem_raw + ((Cfg::BUF_BYTES + Cfg::ROWS_BYTES + 2 * PB * sizeof(float) + PB * sizeof(ushort2) + 7) & ~(size_t)7));
+  float *rs = reinterpret_cast<float *>(smem_raw + Cfg::OFF_RS);           // [2][PB]: 1/sqrt(L R_cc[0]) of i, j
+  ushort2 *ij_s = reinterpret_cast<ushort2 *>(smem_raw + Cfg::OFF_IJ);     // [PB]
+  int *pg_s = reinterpret_cast<int *>(smem_raw + Cfg::OFF_PG);             // [PB]
+  uint64_t *bar = reinterpret_cast<uint64_t *>(smem_raw + Cfg::OFF_BAR);
 
   float *const G = G_, *const A = A_, *const Pw = Pw_, *const R = R_;
   const bool wantG = G, wantR = R;
@@ -137,7 +142,14 @@ pair_kernel(const float2 *__restrict__ S, const float *__restrict__ Srsq, const 
   const int64_t p0 = (int64_t)blockIdx.x * PB;
 
   pdl_launch_dependents();
-  if (tid < PB) ij_s[tid] = (p0 + tid < lay.P) ? pair_of(p0 + tid, lay.C) : make_ushort2(0, 0);
+  if (tid < PB) {
+    // all pairs: (i, j) of lexicographic pair p0 + tid;  pair list (f2): entry p0 + tid of the list, whose S values sit
+    // at lexicographic index pg in the S layout
+    ushort2 ij = make_ushort2(0, 1);
+    if (p0 + tid < lay.Po) ij = list ? list[p0 + tid] : pair_of(p0 + tid, lay.C);
+    ij_s[tid] = ij;
+    pg_s[tid] = (int)ij.x * lay.C - ((int)ij.x * ((int)ij.x + 1)) / 2 + (int)ij.y - (int)ij.x - 1;
+  }
   if (tid == 0) {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(1));
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -146,10 +158,18 @@ pair_kernel(const float2 *__restrict__ S, const float *__restrict__ Srsq, const 
   __syncthreads();
   if (tid == 0) {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)),
-                 "r"((uint32_t)(Cfg::TILE_BYTES + (wantG ? Cfg::ROWS_BYTES : 0))) : "memory");
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(tile)),
-                 "l"(S + (int64_t)blockIdx.x * F * PB), "r"((uint32_t)Cfg::TILE_BYTES), "r"(smem_u32(bar))
-                 : "memory");
+                 "r"((uint32_t)((list ? 0 : Cfg::TILE_BYTES) + (wantG ? Cfg::ROWS_BYTES : 0))) : "memory");
+    if (!list)
+      asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(tile)),
+                   "l"(S + (int64_t)blockIdx.x * F * PB), "r"((uint32_t)Cfg::TILE_BYTES), "r"(smem_u32(bar))
+                   : "memory");
+  }
+  if (list) {  // gather the tile: slot sl of row f belongs to the CTA's pair pl = (sl ^ s_swz(f)) mod PB
+    for (int idx = tid; idx < F * PB; idx += THREADS) {
+      const int f = idx / PB, sw = s_swz(f);
+      const int pg = pg_s[((idx % PB) ^ sw) & (PB - 1)];
+      tile[idx] = __ldg(S + ((int64_t)(pg >> lay.pb_shift) * F + f) * PB + ((pg ^ sw) & (PB - 1)));
+    }
   }
   if (tid < PB && wantG) {  // this pair's 1/sqrt(S_jj) row; a lane's complete_tx may precede lane 0's expect_tx: the
                             // transaction count is signed and the phase cannot complete before lane 0's arrival
@@ -179,7 +199,7 @@ pair_kernel(const float2 *__restrict__ S, const float *__restrict__ Srsq, const 
 
   const int pl = tid / T, gt = tid % T;
   const int64_t p = p0 + pl;
-  const bool valid = p < lay.P;
+  const bool valid = p < lay.Po;
   const float2 wg = __ldg(tw + gt);  // e^{-2 pi i gt / L}
 
   // ---- pass 1: G, A, P ------------------------------------------------------------------------------------------
@@ -187,7 +207,7 @@ pair_kernel(const float2 *__restrict__ S, const float *__restrict__ Srsq, const 
   // thread mapping: a thread owns 4 consecutive bins of one pair and stores float4; a warp covers 512 contiguous
   // bytes of one row.  Rows have F = N + 1 floats (F mod 4 = 1), so element (p, f) is 16-byte aligned iff
   // (p + f) mod 4 = 0: the groups of pair p start at f0 = (-p) mod 4; the f0 head and the 0..3 tail bins go scalar.
-  if ((G || A || Pw) && p0 < lay.P) {
+  if ((G || A || Pw) && p0 < lay.Po) {
     auto value = [&](float2 s, float g2, float &mag, float &coh, float &ang) {
       mag = sqrt_approx(fmaf(s.x, s.x, s.y * s.y));
       coh = mag * g2;
@@ -206,7 +226,7 @@ pair_kernel(const float2 *__restrict__ S, const float *__restrict__ Srsq, const 
         const int ql = (it * R) ^ qa;  // = it R + qa (qa < R, R a power of two)
         const int64_t q = p0 + ql;
         const int f0 = (-(qa + ((it * R) & 3))) & 3, ng = (F - f0) >> 2;
-        if (q >= lay.P || g >= ng) continue;
+        if (q >= lay.Po || g >= ng) continue;
         const int f = f0 + 4 * g;
         const ushort2 qij = ij_s[ql];
         const float *qi = Srsq + (int64_t)qij.x * Cfg::FP + f, *qj = rowj + ql * Cfg::FP + f;
@@ -231,7 +251,7 @@ pair_kernel(const float2 *__restrict__ S, const float *__restrict__ Srsq, const 
     for (int item = tid; item < PB * per; item += THREADS) {
       const int ql = item / per, e = item % per;
       const int64_t q = p0 + ql;
-      if (q >= lay.P) continue;
+      if (q >= lay.Po) continue;
       int f = e;
       if (vec4) {
         const int f0 = (int)((-q) & 3), ng = (F - f0) >> 2;
@@ -280,7 +300,7 @@ pair_kernel(const float2 *__restrict__ S, const float *__restrict__ Srsq, const 
       const float a = v[u].x * norm, b = v[u].y * norm;
       const int q = (u < E / 2) ? 2 * n + N : 2 * n - N;
 #ifdef DELTA_DBG_NOSTORE_R
-      if (lay.P < 0)
+      if (lay.Po < 0)
 #endif
       if (vec) {
         ST2(Rp + q, make_float2(a, b));
@@ -362,7 +382,8 @@ static int launch_pair_L(delta_plan *p, const float *d_S, const float *d_rsq, co
                          float rscale, float *d_G, float *d_A, float *d_P, float *d_R, cudaStream_t st) {
   using Cfg = PairCfg<L>;
   const Layout &lay = p->lay;
-  if (lay.Pblk == 0 || lay.P == 0) return DELTA_OK;
+  if (lay.Poblk == 0 || lay.Po == 0) return DELTA_OK;
+  const ushort2 *list = p->cfg.n_pairs > 0 ? p->d_pairs() : nullptr;
   PairConsts pc;
   for (int u = 0; u < 16; ++u) pc.wstep[u] = p->h_wstep[u];
   const bool full = lay.M == L / 2;
@@ -370,9 +391,9 @@ static int launch_pair_L(delta_plan *p, const float *d_S, const float *d_rsq, co
   do {                                                                                                              \
     int rc = opt_in_smem(pair_kernel<L, FULL_, GAPALL_>, Cfg::SMEM);                                                \
     if (rc) return rc;                                                                                              \
-    LaunchCfg lc(dim3((unsigned)lay.Pblk), dim3(Cfg::THREADS), Cfg::SMEM, st, p->use_pdl);                          \
+    LaunchCfg lc(dim3((unsigned)lay.Poblk), dim3(Cfg::THREADS), Cfg::SMEM, st, p->use_pdl);                          \
     DELTA_CUDA_CHECK(cudaLaunchKernelEx(&lc.cfg, pair_kernel<L, FULL_, GAPALL_>, reinterpret_cast<const float2 *>(d_S), \
-                                        d_rsq, rpart, nrp, rp_stride, rscale, p->d_tw(), p->d_ftab2(), lay, pc, \
+                                        d_rsq, rpart, nrp, rp_stride, rscale, list, p->d_tw(), p->d_ftab2(), lay, pc, \
                                         d_G, d_A, d_P, d_R));                                                       \
   } while (0)
   const bool gapall = d_G && d_A && d_P;

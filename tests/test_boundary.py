@@ -80,9 +80,10 @@ def test_null_arguments():
     assert b.LIB.delta_plan_sizes(None, None) == b.ERR_INVALID_ARG
 
 
-def test_explicit_pair_list_is_reported_unsupported():
+def test_explicit_pair_list_through_the_raw_struct():
     arr = (C.c_int32 * 4)(0, 1, 0, 2)
-    assert create(mk(n_pairs=2, h_pairs=C.cast(arr, C.POINTER(C.c_int32)))) == b.ERR_UNSUPPORTED
+    assert create(mk(n_pairs=2, h_pairs=C.cast(arr, C.POINTER(C.c_int32)))) == b.OK
+    assert create(mk(n_pairs=2, h_pairs=None)) == b.ERR_INVALID_ARG
 
 
 @pytest.mark.parametrize("name,K,F,P,nl", [("tiny", 15, 129, 28, 257), ("single", 38, 257, 18336, 513),
@@ -137,4 +138,14 @@ def test_window_and_detrend_validation():
     for kw in (dict(window=4), dict(window=-1), dict(detrend=2), dict(detrend=-1)):
         with pytest.raises(b.DeltaError) as e:
             b.Plan(8, 2048, 256, 128, allocate=False, **kw)
+        assert e.value.status == b.ERR_INVALID_ARG
+
+
+def test_explicit_pair_list_validation():
+    """f2: explicit pair lists (e.g. one reference channel against all others); entries must satisfy 0 <= i < j < C."""
+    p = b.Plan(8, 2048, 256, 128, allocate=False, pairs=[(0, 3), (2, 7), (0, 1)])
+    assert p.sizes.P == 3
+    for bad in ([(3, 3)], [(4, 2)], [(0, 8)], [(-1, 2)]):
+        with pytest.raises(b.DeltaError) as e:
+            b.Plan(8, 2048, 256, 128, allocate=False, pairs=bad)
         assert e.value.status == b.ERR_INVALID_ARG

@@ -435,3 +435,33 @@ def test_accumulation_over_chunks(mode):
                R=o.crosscorr(S_o, Sa_o, pairs, w.nfft, w.max_lag), Sauto=Sa_o)
     st = compare(out, ref, pairs, "accumulated")
     print(st)
+
+
+@pytest.mark.parametrize("kind", ["reference_channel", "random_37"])
+def test_explicit_pair_lists(kind, mode):
+    """f2: outputs for an explicit pair list only -- one reference channel against all the
+    others (the usual ECEi view), and a random list whose length is not a multiple of the 16-pair tile."""
+    w = es.WORKLOADS["single"]
+    C = 48
+    x = es.single()[:C]
+    if kind == "reference_channel":
+        ref_ch = 17
+        pairs = np.array([(min(ref_ch, c), max(ref_ch, c)) for c in range(C) if c != ref_ch], dtype=np.int32)
+    else:
+        allp = o.all_pairs(C)
+        pairs = allp[np.random.default_rng(37).choice(len(allp), 37, replace=False)]
+    b = binding()
+    plan = b.Plan(C, w.T, w.nfft, w.hop, w.max_lag, contraction=mode, pairs=pairs)
+    assert plan.sizes.P == len(pairs)
+    out = plan.analyze_chunk(dev(x))
+    torch.cuda.synchronize()
+    out = {k: v.cpu().numpy() for k, v in out.items()}
+    assert out["G"].shape == (len(pairs), w.F) and out["R"].shape == (len(pairs), 2 * w.max_lag + 1)
+    ref = oracle_for(x, w.nfft, w.hop, w.max_lag, pairs=pairs)
+    st = compare(out, ref, pairs, kind)
+    print(kind, st)
+    # the rows must equal the same pairs' rows of the all-pairs call, bit for bit (same S, same arithmetic)
+    _, full = gpu_analyze(x, w.nfft, w.hop, w.max_lag, contraction=mode)
+    idx = np.array([o.pair_index(int(i), int(j), C) for i, j in pairs])
+    for k in ("G", "A", "P", "R"):
+        assert np.array_equal(out[k], full[k][idx]), k
