@@ -181,7 +181,10 @@ contract_tc_kernel(const __half *__restrict__ X, Layout lay, TcParams prm, float
     const int fstep = gridDim.x / prm.ngroups, gstep = gridDim.x % prm.ngroups;
     for (int item = blockIdx.x; item < nitems; item += gridDim.x) {
       const __half *Xf = X + (int64_t)f * lay.x_elems_per_f;
-      for (int ks = 0; ks < prm.ksteps; ++ks, ++kidx) {
+      // mode 2 (the K steps of a bin do not fit in the ring): every unit streams the bin's operands again (L2 hits)
+      const int reps = prm.unit_major == 2 ? prm.nunits[g] : 1;
+      for (int kk = 0; kk < reps * prm.ksteps; ++kk, ++kidx) {
+        const int ks = kk % prm.ksteps;
         if (pass) mbar_wait(empty_bar + s, (pass - 1) & 1u);
         if (elect_one()) {
           mbar_expect_tx(full_bar + s, prm.stage_bytes);
@@ -246,7 +249,27 @@ contract_tc_kernel(const __half *__restrict__ X, Layout lay, TcParams prm, float
     const int gstep = gridDim.x % prm.ngroups;
     for (int item = blockIdx.x; item < nitems; item += gridDim.x) {
       const int nu = prm.nunits[g];
-      if (prm.unit_major) {
+      if (prm.unit_major == 2) {
+        // unit after unit, each with its own pass over the K steps: the epilogue of unit u overlaps the MMAs of unit u+1
+        uint32_t s = s0, pass = pass0;
+        for (int u = 0; u < nu; ++u) {
+          const TcUnit un = prm.units[g][u];
+          const uint32_t ao16 = (uint32_t)(un.row0 / 8) * 8u, bo16 = (uint32_t)(un.col0 / 8) * 8u;
+          const uint32_t id = make_idesc(un.N, 0), idn = make_idesc(un.N, 1);
+          const uint32_t d_re = tmem_base + (uint32_t)un.tm, d_im = d_re + (uint32_t)un.N;
+          wait_unit_free(u);
+          for (int ks = 0; ks < prm.ksteps; ++ks) {
+            mbar_wait(full_bar + s, pass & 1u);
+            fence_after();
+            issue(ao16, bo16, id, idn, d_re, d_im, s, ks > 0 ? 1u : 0u);
+            if (elect_one()) mma_commit(empty_bar + s);
+            __syncwarp();
+            if (++s == (uint32_t)prm.nstage) { s = 0; ++pass; }
+          }
+          unit_done(u);
+        }
+        s0 = s; pass0 = pass;
+      } else if (prm.unit_major) {
         for (int u = 0; u < nu; ++u) {
           const TcUnit un = prm.units[g][u];
           const uint32_t ao16 = (uint32_t)(un.row0 / 8) * 8u, bo16 = (uint32_t)(un.col0 / 8) * 8u;
@@ -431,7 +454,12 @@ int launch_contract_tc(delta_plan *p, const void *d_X, float *d_S, float *d_auto
   if (nstage > DELTA_TC_MAX_STAGES) nstage = DELTA_TC_MAX_STAGES;
   if (nstage < 2) return DELTA_ERR_UNSUPPORTED;
   prm.nstage = nstage;
-  prm.unit_major = (2 * prm.ksteps <= nstage) ? 1 : 0;
+#ifndef DELTA_TC_STREAM_UNITS
+#define DELTA_TC_STREAM_UNITS 1
+#endif
+  // 1: all K steps of a bin stay in the ring and are shared by its units;  2: every unit streams them again;
+  // 0: K-step-major (all units advance together; their epilogues cannot overlap the MMAs)
+  prm.unit_major = (2 * prm.ksteps <= nstage) ? 1 : (DELTA_TC_STREAM_UNITS ? 2 : 0);
   size_t smem = (size_t)nstage * prm.stage_bytes + fixed;
   if (smem < 120 * 1024) smem = 120 * 1024;  // one CTA per SM: each CTA allocates all 512 TMEM columns
   const int nitems = lay.F * prm.ngroups;
