@@ -227,6 +227,18 @@ def crosscorr(S: np.ndarray, Sauto: np.ndarray, pairs: np.ndarray, L: int, M: in
     return rho
 
 
+# f2 variant: per-segment-normalised coherence.  Eq. (1b), forms the coherence from
+# the segment-AVERAGED spectra (reading R10).  The variant used in the field for phase locking normalises every segment
+# first: X[c, k, f] -> X / |X| (0 where X = 0), so that S_ij[f] = s2 (1/K) sum_k exp(i (phi_i - phi_j)) is a mean of unit
+# phasors, S_cc = s2, and Eq. (1b) gives |mean phasor|: 1 for a phase difference that is the same in every segment, whatever
+# the amplitudes do; about sqrt(pi / 4K) for independent segments.
+def unit_phasors(X: np.ndarray) -> np.ndarray:
+    mag = np.abs(X)
+    out = np.zeros_like(X)
+    np.divide(X, mag, out=out, where=mag > 0)
+    return out
+
+
 # f2 variant: shot-level accumulation.  The expectation E[.] of Eq. (1a), taken
 # over the segments of SEVERAL chunks instead of one: since every chunk has the same K, that is the plain mean of the
 # per-chunk spectra.  Coherence, phase and correlation are then formed from the accumulated spectra (R10).
@@ -241,7 +253,8 @@ def accumulate(spectra: list) -> np.ndarray:
 # ----------------------------------------------------------------------------------------------
 # the whole path for one chunk, in the paper's order (L107: normalise -> STFT -> Eqs. 1)
 def analyze_chunk(x, L, H, M, pairs=None, scaling=SCALE_WINPOW, fs=1.0,
-                  norm_mode=NORM_NONE, offs=None, want_S=False, band=None, win=WIN_HANN, detrend=DETREND_NONE):
+                  norm_mode=NORM_NONE, offs=None, want_S=False, band=None, win=WIN_HANN, detrend=DETREND_NONE,
+                  phase_lock=False):
     """Returns dict(G, A, P, R, Sauto[, S]) for one channel-by-time chunk x[C][T].
     band = (lo_hz, hi_hz): band-pass pre-processing (R19) between the transform and Eq. (1); needs fs."""
     x = np.asarray(x)
@@ -252,6 +265,8 @@ def analyze_chunk(x, L, H, M, pairs=None, scaling=SCALE_WINPOW, fs=1.0,
     X = stft(y, L, H, win, detrend)
     if band is not None:
         X = bandpass(X, band_mask(L, fs, band[0], band[1]))
+    if phase_lock:
+        X = unit_phasors(X)
     s2 = scale_factor(L, scaling, fs, win)
     Sauto = auto_spectra(X, s2)
     S = cross_spectra(X, pairs, s2)

@@ -519,3 +519,28 @@ def test_P14_accumulation_over_chunks_is_the_mean_over_all_segments():
     G1 = o.coherence(o.cross_spectra(Xs[0], pairs, s2), o.auto_spectra(Xs[0], s2), pairs)
     Gn = o.coherence(S_acc, Sa_acc, pairs)
     assert 0.30 < Gn[:, 2:-2].mean() / G1[:, 2:-2].mean() < 0.55      # 1/sqrt(6) = 0.41
+
+
+# ---------------------------------------------------------------------------- f2: per-segment-normalised coherence
+def test_P15_phase_lock_estimator():
+    """Unit phasors per segment: (1) two tones with a fixed phase difference but amplitudes that jump from segment to
+    segment (one channel's amplitude independent of the other's): the ordinary coherence is well below 1, the
+    phase-lock value is 1 and the cross-phase is the injected one; (2) autospectra are exactly s2 everywhere;
+    (3) independent white noise without overlap: the mean of |mean of K random unit phasors| is the Rayleigh mean
+    sqrt(pi / (4 K)) (closed form), e.g. 0.221 for K = 16."""
+    L, H, q = 64, 64, 9                       # no overlap: segments are independent
+    K = 16
+    T = K * L
+    rng = np.random.default_rng(15)
+    a1 = np.repeat(rng.uniform(0.2, 3.0, K), L)
+    a2 = np.repeat(rng.uniform(0.2, 3.0, K), L)
+    t = np.arange(T)
+    x = np.stack([a1 * np.cos(2 * np.pi * q * t / L + 0.9), a2 * np.cos(2 * np.pi * q * t / L + 0.2)])
+    plain = o.analyze_chunk(x, L, H, L // 2)
+    lock = o.analyze_chunk(x, L, H, L // 2, phase_lock=True)
+    assert plain["G"][0, q] < 0.93
+    assert abs(lock["G"][0, q] - 1.0) < 1e-12 and abs(lock["A"][0, q] - 0.7) < 1e-9
+    assert np.allclose(lock["Sauto"], o.scale_factor(L), rtol=1e-12)
+    n = rng.standard_normal((24, T))
+    g = o.analyze_chunk(n, L, H, L // 2, phase_lock=True)["G"][:, 1:-1]
+    assert abs(g.mean() - np.sqrt(np.pi / (4 * K))) < 0.01
