@@ -38,7 +38,7 @@
 extern "C" {
 #endif
 
-#define DELTA_VERSION 103 /* 0.1.3: band-pass, window variants, detrend in delta_config; delta_accumulate */
+#define DELTA_VERSION 104 /* 0.1.4: band-pass, windows, detrend, estimator in delta_config; delta_accumulate; pair lists */
 
 typedef enum {
   DELTA_OK = 0,
@@ -54,6 +54,9 @@ typedef enum {
 /* periodic (DFT-even) windows, x = 2 pi n/L: Hann 1/2 - 1/2 cos x (R4, the default); the others are the f1 variants:
  * Hamming 0.54 - 0.46 cos x, rectangular 1, Blackman 0.42 - 0.5 cos x + 0.08 cos 2x */
 enum { DELTA_WIN_HANN_PERIODIC = 0, DELTA_WIN_HAMMING_PERIODIC = 1, DELTA_WIN_RECT = 2, DELTA_WIN_BLACKMAN_PERIODIC = 3 };
+/* Eq. (1b) estimator: from the segment-averaged spectra (R10, the default), or the per-segment-normalised variant (f2):
+ * every X[c,k,f] is replaced by X/|X| before Eq. (1a), so S is a mean of unit phasors, S_cc = s^2, G = |mean phasor| */
+enum { DELTA_EST_AVERAGED = 0, DELTA_EST_PHASE_LOCK = 1 };
 /* per-segment detrend before the window: none (R5, the default) or the mean of the segment's nfft samples */
 enum { DELTA_DETREND_NONE = 0, DELTA_DETREND_CONSTANT = 1 };
 enum { DELTA_SCALE_WINPOW = 0,                       /* s^2 = 1/sum w^2 (default; white noise of
@@ -93,6 +96,7 @@ typedef struct {
    * zero-lag autocorrelations. */
   float   bp_lo_hz, bp_hi_hz;
   int32_t detrend;      /* DELTA_DETREND_*                                                            */
+  int32_t estimator;    /* DELTA_EST_*                                                                */
 } delta_config;
 
 typedef struct {

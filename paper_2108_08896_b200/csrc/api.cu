@@ -21,6 +21,7 @@ static int validate(const delta_config *c) {
   if (c->n_channels < 1 || c->n_samples < 1 || c->nfft < 1 || c->hop < 1 || c->max_lag < 0) return DELTA_ERR_INVALID_ARG;
   if (c->window < DELTA_WIN_HANN_PERIODIC || c->window > DELTA_WIN_BLACKMAN_PERIODIC) return DELTA_ERR_INVALID_ARG;
   if (c->detrend < DELTA_DETREND_NONE || c->detrend > DELTA_DETREND_CONSTANT) return DELTA_ERR_INVALID_ARG;
+  if (c->estimator < DELTA_EST_AVERAGED || c->estimator > DELTA_EST_PHASE_LOCK) return DELTA_ERR_INVALID_ARG;
   if (c->scaling < DELTA_SCALE_WINPOW || c->scaling > DELTA_SCALE_SPECTRUM) return DELTA_ERR_INVALID_ARG;
   if (c->in_dtype != DELTA_F32 && c->in_dtype != DELTA_I16) return DELTA_ERR_INVALID_ARG;
   if (c->norm_mode < DELTA_NORM_NONE || c->norm_mode > DELTA_NORM_RELATIVE) return DELTA_ERR_INVALID_ARG;
@@ -87,8 +88,10 @@ int delta_plan_create(const delta_config *cfg, delta_plan **out) {
   l.Fp = (l.F + 3) & ~3;
   l.f_lo = 0;
   l.f_hi = l.F - 1;
-  p->band_on = cfg->bp_lo_hz != 0.f || cfg->bp_hi_hz != 0.f;
-  if (p->band_on) {  // bin f is kept iff lo L <= f fs <= hi L (float64); the kept bins are one contiguous range
+  l.estimator = cfg->estimator;
+  const bool band = cfg->bp_lo_hz != 0.f || cfg->bp_hi_hz != 0.f;
+  p->band_on = band || cfg->estimator == DELTA_EST_PHASE_LOCK;
+  if (band) {  // bin f is kept iff lo L <= f fs <= hi L (float64); the kept bins are one contiguous range
     const double lo = (double)cfg->bp_lo_hz * l.L, hi = (double)cfg->bp_hi_hz * l.L, fs = (double)cfg->fs;
     l.f_lo = l.F;
     l.f_hi = -1;

@@ -44,6 +44,7 @@ struct Layout {
   int Fp;   // row pitch of the rsq table: F rounded up to 4 floats (rows are 16-byte aligned bulk-copy sources)
   float wsum;      // sum_n |w[n]|: |X| <= wsum max|y| bounds the split-fp16 operands
   int detrend;     // DELTA_DETREND_*
+  int estimator;   // DELTA_EST_*
   int f_lo, f_hi;  // pass band of the optional band-pass filter, in bins (0 .. F-1 when it is off)
   int nkb;  // segment blocks per channel = ceil(K / 8): one partial of the windowed signal energy each (wpart)
   // S (cross-spectra) is complex64 [Pblk][F][PB]: pairs in lexicographic order p = iC - i(i+1)/2 + (j-i-1),
@@ -93,7 +94,8 @@ struct delta_plan {
   int n_first = 0;
   int launches = 0;
   long long *d_trace = nullptr;  // debug: clock stamps of the tensor-core contraction (delta_debug_set_trace)
-  bool band_on = false;  // band-pass filter active: rho is normalised from the (filtered) autospectra
+  bool band_on = false;  // band-pass filter or phase-lock estimator: rho is normalised from the autospectra, not from
+                         // the windowed signal energy (Parseval does not apply to the modified spectra)
   bool use_pdl = true;  // programmatic dependent launch between the hot-path kernels (DELTA_NO_PDL=1 switches it off)
   bool stage_events_on = false;
   cudaEvent_t stage_ev[4] = {nullptr, nullptr, nullptr, nullptr};

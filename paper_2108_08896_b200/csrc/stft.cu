@@ -378,6 +378,7 @@ stft_kernel(const void *__restrict__ x, int64_t ld, int in_dtype, int norm_mode,
 #pragma unroll
     for (int w = 0; w < WPC; ++w) e += wred[tid * WPC + w];
     wpart[(int64_t)(c0 + tid) * lay.nkb + kb] = e;
+    if (TC && !CLUSTER && kb == 0 && lay.estimator == DELTA_EST_PHASE_LOCK) chscale[c0 + tid] = 8192.f;  // unit phasors
   }
   if (CLUSTER) {
     // per-channel power-of-two scale: sum_n w[n] |y| <= (L/2) max|y|  =>  scale * |X| < 2^14 (same rule as chscale_kernel)
@@ -389,7 +390,7 @@ stft_kernel(const void *__restrict__ x, int64_t ld, int in_dtype, int norm_mode,
       for (unsigned r = 0; r < nb; ++r) m = fmaxf(m, *cluster.map_shared_rank(&cmax[tid], r));
       const float sc = scale_from_max(m, lay.wsum);
       csc[tid] = sc;
-      if (kb == 0 && c0 + tid < lay.C) chscale[c0 + tid] = sc;
+      if (kb == 0 && c0 + tid < lay.C) chscale[c0 + tid] = lay.estimator == DELTA_EST_PHASE_LOCK ? 8192.f : sc;
     }
     cluster.barrier_arrive();  // remote reads of cmax are done; waited for just before the CTA exits
     __syncthreads();           // csc is visible to the CTA
@@ -403,10 +404,23 @@ stft_kernel(const void *__restrict__ x, int64_t ld, int in_dtype, int norm_mode,
     const int64_t within = ((int64_t)kb * lay.Cp + c) * kSegBlock;
     const int64_t base = (int64_t)f * lay.x_elems_per_f + within;
     const float keep = (f >= lay.f_lo && f <= lay.f_hi) ? 1.f : 0.f;  // band-pass mask (R19)
+    const bool plv = lay.estimator == DELTA_EST_PHASE_LOCK;
+    float nre[kSegBlock], nim[kSegBlock];
+    if (plv) {  // per-segment-normalised estimator (f2): X -> X / |X|, 0 where X = 0
+#pragma unroll
+      for (int q = 0; q < kSegBlock; ++q) {
+        const float m2 = fmaf(re[q], re[q], im[q] * im[q]);
+        const float r = m2 > 0.f ? rsqrtf(m2) : 0.f;
+        nre[q] = re[q] * r;
+        nim[q] = im[q] * r;
+      }
+      re = nre;
+      im = nim;
+    }
     if (TC) {
-      // split fp16: v * scale = hi + lo (scale = the channel's power of two)
+      // split fp16: v * scale = hi + lo (scale = the channel's power of two; 2^13 for unit phasors)
       __half *X = reinterpret_cast<__half *>(Xout);
-      const float sc = keep * (CLUSTER ? csc[pcl] : chscale[c]);
+      const float sc = keep * (plv ? 8192.f : (CLUSTER ? csc[pcl] : chscale[c]));
       __align__(16) __half2 hr[4], hi_[4], lr[4], li[4];
 #pragma unroll
       for (int q = 0; q < 4; ++q) {
@@ -519,6 +533,7 @@ static int launch_stft_L(delta_plan *p, const void *d_x, int64_t ld, void *d_X, 
   const Layout &lay = p->lay;
   if (p->contraction == DELTA_CONTRACT_TC) {
     if (lay.nkb <= 8) return launch_stft_LT<L, true, true>(p, d_x, ld, d_X, st);  // scale agreed inside the cluster
+    if (lay.estimator == DELTA_EST_PHASE_LOCK) return launch_stft_LT<L, true, false>(p, d_x, ld, d_X, st);  // fixed scale
     int ns = (8 * p->num_sms + lay.C - 1) / lay.C;  // about 8 blocks per SM
     ns = ns < 1 ? 1 : (ns > 64 ? 64 : ns);
     chscale_kernel<<<dim3(lay.C, ns), 256, 0, st>>>(d_x, ld, p->cfg.in_dtype, p->cfg.norm_mode, p->n_first, p->d_offs(),

@@ -29,7 +29,7 @@ def dev(x):
     return torch.from_numpy(np.ascontiguousarray(x)).cuda()
 
 
-def compare(out, ref, pairs, label=""):
+def compare(out, ref, pairs, label="", p_abs_tol=1e-5):
     """out: dict of numpy float32 arrays for `pairs`; ref: oracle dict for the same pairs."""
     G, A, P, R, Sa = (np.asarray(out[k], dtype=np.float64) for k in ("G", "A", "P", "R", "Sauto"))
     for k in ("G", "A", "P", "R", "Sauto"):
@@ -50,7 +50,7 @@ def compare(out, ref, pairs, label=""):
     stats["A_gated"] = float(np.max(np.where(gate, dA, 0.0)))
     stats["R_abs"] = float(np.max(np.abs(R - ref["R"])))
     assert stats["P_rel_gated"] <= TOL_P_REL, f"{label}: cross-power rel err (G>0.1) {stats['P_rel_gated']:.3g}"
-    assert stats["P_abs_norm"] <= 1e-5, f"{label}: cross-power abs err / sqrt(SiiSjj) {stats['P_abs_norm']:.3g}"
+    assert stats["P_abs_norm"] <= p_abs_tol, f"{label}: cross-power abs err / sqrt(SiiSjj) {stats['P_abs_norm']:.3g}"
     assert stats["G_abs"] <= TOL_G, f"{label}: coherence abs err {stats['G_abs']:.3g}"
     assert stats["A_gated"] <= TOL_A, f"{label}: cross-phase err (G>0.1) {stats['A_gated']:.3g}"
     assert stats["R_abs"] <= TOL_R, f"{label}: cross-correlation abs err {stats['R_abs']:.3g}"
@@ -465,3 +465,22 @@ def test_explicit_pair_lists(kind, mode):
     idx = np.array([o.pair_index(int(i), int(j), C) for i, j in pairs])
     for k in ("G", "A", "P", "R"):
         assert np.array_equal(out[k], full[k][idx]), k
+
+
+@pytest.mark.parametrize("C,T,L,H", [(40, 10_000, 512, 256), (12, 40_000, 256, 128)])
+def test_phase_lock_estimator(C, T, L, H, mode):
+    """f2: per-segment-normalised coherence (unit phasors per segment).  The second case has
+    more than 8 segment blocks, i.e. the STFT variant without the cluster."""
+    x = es.turbulence(T, 61)[:C]
+    b = binding()
+    plan = b.Plan(C, T, L, H, L // 2, contraction=mode, estimator=1)
+    out = plan.analyze_chunk(dev(x))
+    torch.cuda.synchronize()
+    out = {k: v.cpu().numpy() for k, v in out.items()}
+    ref = o.analyze_chunk(x, L, H, L // 2, phase_lock=True)
+    # With unit phasors |dP| / sqrt(S_ii S_jj) IS the coherence error (S_cc = s^2), and every bin counts alike however
+    # little power it holds: the float32 transform's error relative to a weak bin (1e-7 x the spectrum's dynamic range)
+    # shows undiminished.  north_star's bound for the coherence is 1e-4; R13's tighter 1e-5 is relaxed to 5e-5 here.
+    st = compare(out, ref, o.all_pairs(C), "phase lock", p_abs_tol=5e-5)
+    print(st)
+    assert np.abs(out["Sauto"] / o.scale_factor(L) - 1).max() < 1e-5     # unit phasors: S_cc = s^2 in every bin
