@@ -484,3 +484,24 @@ def test_phase_lock_estimator(C, T, L, H, mode):
     st = compare(out, ref, o.all_pairs(C), "phase lock", p_abs_tol=5e-5)
     print(st)
     assert np.abs(out["Sauto"] / o.scale_factor(L) - 1).max() < 1e-5     # unit phasors: S_cc = s^2 in every bin
+
+
+def test_three_views_576_channels(mode):
+    """f3: the diagnostic has three 24 x 8 views: 576 channels, 165,600 pairs,
+    nfft 512.  Three independent config-2 arrays with a common component; checked on sampled channels."""
+    w = es.WORKLOADS["single"]
+    a, b2, c = (es.turbulence(w.T, s) for s in (71, 72, 73))
+    x = np.concatenate([a, 0.4 * a + 0.9 * b2, 0.4 * a + 0.9 * c]).astype(np.float32)
+    C = x.shape[0]
+    assert C == 576
+    _, out = gpu_analyze(x, w.nfft, w.hop, w.max_lag, contraction=mode)
+    P = C * (C - 1) // 2
+    assert out["G"].shape == (P, w.F) and P == 165_600
+    ch, loc, glob = _sampled_pairs(C, 10, 7)
+    ref = oracle_for(x[ch], w.nfft, w.hop, w.max_lag)
+    idx = np.array([o.pair_index(int(i), int(j), C) for i, j in glob])
+    sub = {k: out[k][idx] for k in ("G", "A", "P", "R")}
+    sub["Sauto"] = out["Sauto"][ch]
+    st = compare(sub, ref, loc, "576 channels")
+    print(st)
+    assert np.isfinite(out["G"]).all() and out["G"].max() <= 1 + 1e-4 and np.abs(out["R"]).max() <= 1 + 1e-4
