@@ -109,20 +109,24 @@ def dft_matrix(L: int, nbins: int) -> np.ndarray:
     return np.exp(-2j * np.pi * ((n * f) % L).astype(np.float64) / L)
 
 
-def stft(y: np.ndarray, L: int, H: int, win: int = WIN_HANN, detrend: int = DETREND_NONE) -> np.ndarray:
+def stft(y: np.ndarray, L: int, H: int, win: int = WIN_HANN, detrend: int = DETREND_NONE,
+         nperseg: int | None = None) -> np.ndarray:
     """X[c, k, f] = sum_n w[n] y[c, kH + n] exp(-2 pi i f n / L),  f = 0..L/2, unscaled.
 
     Default: no detrend (R5); nperseg == nfft (R2), segments never leave the chunk (L107).
-    detrend = CONSTANT (f1 variant): the mean of the L samples of a segment is subtracted before the window."""
+    detrend = CONSTANT (f1 variant): the mean of the samples of a segment is subtracted before the window.
+    nperseg = Ls < L (f2 variant, R22): segments of Ls samples (window of length Ls), zero-padded to the transform
+    length L, so that the circular correlation of Eq. (1d) is the LINEAR one for lags |m| <= L - Ls."""
     y = np.asarray(y, dtype=np.float64)
     C, T = y.shape
-    K = n_segments(T, L, H)
+    Ls = L if nperseg is None else nperseg
+    K = n_segments(T, Ls, H)
     F = L // 2 + 1
-    w = window(L, win)
-    W = dft_matrix(L, F)
+    w = window(Ls, win)
+    W = dft_matrix(L, F)[:Ls]          # the padded samples are zero: only the first Ls rows of the DFT matrix act
     X = np.empty((C, K, F), dtype=np.complex128)
     for c in range(C):
-        seg = np.stack([y[c, k * H:k * H + L] for k in range(K)])
+        seg = np.stack([y[c, k * H:k * H + Ls] for k in range(K)])
         if detrend == DETREND_CONSTANT:
             seg = seg - seg.mean(axis=1, keepdims=True)
         X[c] = (seg * w[None, :]) @ W
@@ -143,10 +147,11 @@ def bandpass(X: np.ndarray, mask: np.ndarray) -> np.ndarray:
     return np.where(mask[None, None, :], X, 0.0)
 
 
-def scale_factor(L: int, scaling: int = SCALE_WINPOW, fs: float = 1.0, win: int = WIN_HANN) -> float:
+def scale_factor(L: int, scaling: int = SCALE_WINPOW, fs: float = 1.0, win: int = WIN_HANN,
+                 nperseg: int | None = None) -> float:
     """s^2 of step 6 (reading R6): WINPOW 1/sum w^2 (default), NONE 1, DENSITY 1/(fs sum w^2),
     SPECTRUM 1/(sum w)^2.  Two-sided values: no one-sided doubling (R7)."""
-    w = window(L, win)
+    w = window(L if nperseg is None else nperseg, win)
     if scaling == SCALE_WINPOW:
         return 1.0 / float(np.sum(w * w))
     if scaling == SCALE_NONE:
@@ -254,7 +259,7 @@ def accumulate(spectra: list) -> np.ndarray:
 # the whole path for one chunk, in the paper's order (L107: normalise -> STFT -> Eqs. 1)
 def analyze_chunk(x, L, H, M, pairs=None, scaling=SCALE_WINPOW, fs=1.0,
                   norm_mode=NORM_NONE, offs=None, want_S=False, band=None, win=WIN_HANN, detrend=DETREND_NONE,
-                  phase_lock=False):
+                  phase_lock=False, nperseg=None):
     """Returns dict(G, A, P, R, Sauto[, S]) for one channel-by-time chunk x[C][T].
     band = (lo_hz, hi_hz): band-pass pre-processing (R19) between the transform and Eq. (1); needs fs."""
     x = np.asarray(x)
@@ -262,12 +267,12 @@ def analyze_chunk(x, L, H, M, pairs=None, scaling=SCALE_WINPOW, fs=1.0,
     if pairs is None:
         pairs = all_pairs(C)
     y = normalise(x, offs, norm_mode)
-    X = stft(y, L, H, win, detrend)
+    X = stft(y, L, H, win, detrend, nperseg)
     if band is not None:
         X = bandpass(X, band_mask(L, fs, band[0], band[1]))
     if phase_lock:
         X = unit_phasors(X)
-    s2 = scale_factor(L, scaling, fs, win)
+    s2 = scale_factor(L, scaling, fs, win, nperseg)
     Sauto = auto_spectra(X, s2)
     S = cross_spectra(X, pairs, s2)
     out = dict(G=coherence(S, Sauto, pairs), A=crossphase(S), P=crosspower(S),

@@ -544,3 +544,44 @@ def test_P15_phase_lock_estimator():
     n = rng.standard_normal((24, T))
     g = o.analyze_chunk(n, L, H, L // 2, phase_lock=True)["G"][:, 1:-1]
     assert abs(g.mean() - np.sqrt(np.pi / (4 * K))) < 0.01
+
+
+# ---------------------------------------------------------------------------- f2: zero-padded segments (R22)
+def test_P16_zero_padded_segments_give_the_linear_correlation():
+    """nperseg = L/2 samples zero-padded to L: (1) equals scipy's Welch CSD with nperseg < nfft; (2) the correlation
+    of Eq. (1d) is then the LINEAR (no wrap-around) windowed correlation for every lag |m| <= L - nperseg: brute force
+    over plain sums; (3) a copy delayed by d = 40 samples (more than half the un-padded transform) is found at m = -40."""
+    L, Ls, H = 128, 64, 32
+    x = _rand_chunk(3, 1200, 16)
+    X = o.stft(x, L, H, nperseg=Ls)
+    K = o.n_segments(1200, Ls, H)
+    assert X.shape == (3, K, L // 2 + 1)
+    pairs = o.all_pairs(3)
+    s2 = o.scale_factor(L, nperseg=Ls)
+    w = o.hann_periodic(Ls)
+    assert abs(s2 - 1.0 / np.sum(w * w)) < 1e-15
+    S = o.cross_spectra(X, pairs, s2)
+    kw = dict(fs=1.0, window="hann", nperseg=Ls, noverlap=Ls - H, nfft=L, detrend=False, return_onesided=False,
+              scaling="density")
+    for p, (i, j) in enumerate(pairs):
+        _, Pd = sps.csd(x[i], x[j], **kw)
+        assert np.allclose(np.conj(Pd[:L // 2 + 1]), S[p], rtol=1e-9, atol=1e-12)
+    M = L - Ls
+    r = o.analyze_chunk(x, L, H, M, nperseg=Ls)
+    def lin(i, j, m):     # sum_n yh_i[n + m] yh_j[n], indices outside 0..Ls-1 contribute nothing
+        acc = 0.0
+        for k in range(K):
+            yi, yj = w * x[i, k * H:k * H + Ls], w * x[j, k * H:k * H + Ls]
+            for n in range(Ls):
+                if 0 <= n + m < Ls:
+                    acc += yi[n + m] * yj[n]
+        return s2 * acc / K
+    r0 = [lin(c, c, 0) for c in range(3)]
+    for p, (i, j) in enumerate(pairs):
+        for q, m in enumerate(range(-M, M + 1)):
+            assert abs(r["R"][p, q] - lin(i, j, m) / np.sqrt(r0[i] * r0[j])) < 1e-12
+    d = 40                                            # a delay beyond L/2 of the un-padded transform (32)
+    base = np.random.default_rng(3).standard_normal(3000 + d)
+    xx = np.stack([base[d:], base[:3000]])            # x_1[t] = x_0[t - d]
+    padded = o.analyze_chunk(xx, 128, 32, 64, nperseg=64)["R"][0]
+    assert np.argmax(padded) - 64 == -d               # found at its true lag, no wrap-around image
