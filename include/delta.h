@@ -38,7 +38,7 @@
 extern "C" {
 #endif
 
-#define DELTA_VERSION 104 /* 0.1.4: band-pass, windows, detrend, estimator in delta_config; delta_accumulate; pair lists */
+#define DELTA_VERSION 105 /* 0.1.5: band-pass, windows, detrend, estimator, nperseg in delta_config; delta_accumulate; pair lists */
 
 typedef enum {
   DELTA_OK = 0,
@@ -97,6 +97,9 @@ typedef struct {
   float   bp_lo_hz, bp_hi_hz;
   int32_t detrend;      /* DELTA_DETREND_*                                                            */
   int32_t estimator;    /* DELTA_EST_*                                                                */
+  int32_t nperseg;      /* 0 => nfft.  Otherwise segments of nperseg <= nfft samples (window of that length),
+                         * zero-padded to nfft (f2, R22): the correlation of Eq. (1d) is then the linear one for
+                         * |lag| <= nfft - nperseg.  Needs hop <= nperseg <= n_samples; K = (T - nperseg)/hop + 1 */
 } delta_config;
 
 typedef struct {

@@ -28,7 +28,7 @@ class DeltaConfig(C.Structure):
                 ("window", C.c_int32), ("scaling", C.c_int32), ("fs", C.c_float), ("in_dtype", C.c_int32),
                 ("norm_mode", C.c_int32), ("max_lag", C.c_int32), ("n_pairs", C.c_int32),
                 ("h_pairs", C.POINTER(C.c_int32)), ("contraction", C.c_int32),
-                ("bp_lo_hz", C.c_float), ("bp_hi_hz", C.c_float), ("detrend", C.c_int32), ("estimator", C.c_int32)]
+                ("bp_lo_hz", C.c_float), ("bp_hi_hz", C.c_float), ("detrend", C.c_int32), ("estimator", C.c_int32), ("nperseg", C.c_int32)]
 
 
 class DeltaSizes(C.Structure):
@@ -123,7 +123,7 @@ class Plan:
 
     def __init__(self, n_channels, n_samples, nfft, hop, max_lag=None, in_dtype=F32, norm_mode=NORM_NONE,
                  scaling=SCALE_WINPOW, fs=500e3, contraction=CONTRACT_AUTO, window=WIN_HANN_PERIODIC,
-                 device=None, allocate=True, band=None, detrend=0, pairs=None, estimator=0):
+                 device=None, allocate=True, band=None, detrend=0, pairs=None, estimator=0, nperseg=0):
         """band = (lo_hz, hi_hz): optional band-pass pre-processing (include/delta.h), None = off."""
         lo_hz, hi_hz = (0.0, 0.0) if band is None else band
         n_list, p_list = 0, None
@@ -132,7 +132,7 @@ class Plan:
             self._pairs = np.ascontiguousarray(np.asarray(pairs, dtype=np.int32).reshape(-1, 2))
             n_list, p_list = self._pairs.shape[0], self._pairs.ctypes.data_as(C.POINTER(C.c_int32))
         self.cfg = DeltaConfig(n_channels, n_samples, nfft, hop, window, scaling, fs, in_dtype, norm_mode,
-                               nfft // 2 if max_lag is None else max_lag, n_list, p_list, contraction, lo_hz, hi_hz, detrend, estimator)
+                               nfft // 2 if max_lag is None else max_lag, n_list, p_list, contraction, lo_hz, hi_hz, detrend, estimator, nperseg)
         self._h = C.c_void_p()
         _check(LIB.delta_plan_create(C.byref(self.cfg), C.byref(self._h)), "delta_plan_create")
         sz = DeltaSizes()

@@ -33,8 +33,10 @@ static int validate(const delta_config *c) {
   }
   const int L = c->nfft;
   if (L < 64 || L > 4096 || (L & (L - 1)) != 0) return DELTA_ERR_UNSUPPORTED;
-  if (c->hop > L) return DELTA_ERR_UNSUPPORTED;
-  if (c->n_samples < L) return DELTA_ERR_UNSUPPORTED;
+  if (c->nperseg < 0 || c->nperseg > L) return DELTA_ERR_INVALID_ARG;
+  const int Ls = c->nperseg > 0 ? c->nperseg : L;
+  if (c->hop > Ls) return DELTA_ERR_UNSUPPORTED;
+  if (c->n_samples < Ls) return DELTA_ERR_UNSUPPORTED;
   if (c->max_lag > L / 2) return DELTA_ERR_UNSUPPORTED;
   if (c->n_channels > 4096) return DELTA_ERR_UNSUPPORTED;
   for (int k = 0; k < c->n_pairs; ++k) {  // explicit pair list (f2): 0 <= i < j < C
@@ -80,7 +82,8 @@ int delta_plan_create(const delta_config *cfg, delta_plan **out) {
   l.L = cfg->nfft;
   l.N = l.L / 2;
   l.H = cfg->hop;
-  l.K = (l.T - l.L) / l.H + 1;
+  l.Ls = cfg->nperseg > 0 ? cfg->nperseg : l.L;
+  l.K = (l.T - l.Ls) / l.H + 1;
   l.Kp = (int)align_up((size_t)l.K, 16);
   l.Kc = l.Kp / kSegBlock;
   l.nkb = (l.K + kSegBlock - 1) / kSegBlock;
@@ -120,7 +123,7 @@ int delta_plan_create(const delta_config *cfg, delta_plan **out) {
   for (int n = 0; n < L; ++n) {
     const double ang = -2.0 * M_PI * (double)n / (double)L;
     p->h_tw[n] = make_float2((float)std::cos(ang), (float)std::sin(ang));
-    const double xw = 2.0 * M_PI * (double)n / (double)L;
+    const double xw = 2.0 * M_PI * (double)n / (double)l.Ls;  // the window spans the segment; zero over the padding
     double w;
     switch (cfg->window) {
       case DELTA_WIN_HAMMING_PERIODIC: w = 0.54 - 0.46 * std::cos(xw); break;
@@ -128,6 +131,7 @@ int delta_plan_create(const delta_config *cfg, delta_plan **out) {
       case DELTA_WIN_BLACKMAN_PERIODIC: w = 0.42 - 0.5 * std::cos(xw) + 0.08 * std::cos(2.0 * xw); break;
       default: w = 0.5 - 0.5 * std::cos(xw); break;
     }
+    if (n >= l.Ls) w = 0.0;
     p->h_win[n] = (float)w;
     sw += w;
     sw2 += w * w;

@@ -41,6 +41,7 @@ struct Layout {
   //   TC   mode : __half X[f][prec][part][kc][c][8]           prec 0 = hi, 1 = lo (split fp16)
   // k = 8*kc + kk, c < Cp (rows C..Cp-1 are zero), kc < Kc = Kp/8, Kp = K rounded up to 16.
   int C, Cp, T, L, N, H, K, Kp, Kc, F, M, nlags;
+  int Ls;   // samples per segment (nperseg <= L; the rest of the transform's input is zero)
   int Fp;   // row pitch of the rsq table: F rounded up to 4 floats (rows are 16-byte aligned bulk-copy sources)
   float wsum;      // sum_n |w[n]|: |X| <= wsum max|y| bounds the split-fp16 operands
   int detrend;     // DELTA_DETREND_*

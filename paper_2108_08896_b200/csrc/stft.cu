@@ -279,17 +279,27 @@ stft_kernel(const void *__restrict__ x, int64_t ld, int in_dtype, int norm_mode,
       const int64_t t0 = (int64_t)c * ld + (int64_t)k * lay.H;
       const size_t esz = in_dtype == DELTA_I16 ? 2 : 4;
       const bool pair_ok = ((t0 & 1) == 0) && ((reinterpret_cast<uintptr_t>(x) & (2 * esz - 1)) == 0);
-      // all loads of the segment are issued before the first use (one DRAM latency per thread, not E)
+      // all loads of the segment are issued before the first use (one DRAM latency per thread, not E);
+      // samples beyond the segment length Ls <= L (zero-padded transforms, R22) are not read
+      const int nfull = lay.Ls >> 1;
+      const bool odd = lay.Ls & 1;
       float2 smp[E];
       if (in_dtype == DELTA_I16) {
         const short *xs = reinterpret_cast<const short *>(x) + t0;
         short2 raw[E];
         if (pair_ok) {
 #pragma unroll
-          for (int u = 0; u < E; ++u) raw[u] = *reinterpret_cast<const short2 *>(xs + 2 * (gt + T * u));
+          for (int u = 0; u < E; ++u) {
+            const int n = gt + T * u;
+            raw[u] = n < nfull ? *reinterpret_cast<const short2 *>(xs + 2 * n)
+                               : make_short2((n == nfull && odd) ? xs[2 * n] : (short)0, 0);
+          }
         } else {
 #pragma unroll
-          for (int u = 0; u < E; ++u) raw[u] = make_short2(xs[2 * (gt + T * u)], xs[2 * (gt + T * u) + 1]);
+          for (int u = 0; u < E; ++u) {
+            const int n = gt + T * u;
+            raw[u] = n < nfull ? make_short2(xs[2 * n], xs[2 * n + 1]) : make_short2((n == nfull && odd) ? xs[2 * n] : (short)0, 0);
+          }
         }
 #pragma unroll
         for (int u = 0; u < E; ++u) smp[u] = make_float2(ldr.conv_i16(raw[u].x), ldr.conv_i16(raw[u].y));
@@ -298,13 +308,27 @@ stft_kernel(const void *__restrict__ x, int64_t ld, int in_dtype, int norm_mode,
         float2 raw[E];
         if (pair_ok) {
 #pragma unroll
-          for (int u = 0; u < E; ++u) raw[u] = *reinterpret_cast<const float2 *>(xf + 2 * (gt + T * u));
+          for (int u = 0; u < E; ++u) {
+            const int n = gt + T * u;
+            raw[u] = n < nfull ? *reinterpret_cast<const float2 *>(xf + 2 * n)
+                               : make_float2((n == nfull && odd) ? xf[2 * n] : 0.f, 0.f);
+          }
         } else {
 #pragma unroll
-          for (int u = 0; u < E; ++u) raw[u] = make_float2(xf[2 * (gt + T * u)], xf[2 * (gt + T * u) + 1]);
+          for (int u = 0; u < E; ++u) {
+            const int n = gt + T * u;
+            raw[u] = n < nfull ? make_float2(xf[2 * n], xf[2 * n + 1]) : make_float2((n == nfull && odd) ? xf[2 * n] : 0.f, 0.f);
+          }
         }
 #pragma unroll
         for (int u = 0; u < E; ++u) smp[u] = make_float2(ldr.conv_f32(raw[u].x), ldr.conv_f32(raw[u].y));
+      }
+      if (lay.Ls < L) {  // the padding is zero whatever the normalisation made of the unread samples
+#pragma unroll
+        for (int u = 0; u < E; ++u) {
+          const int n = gt + T * u;
+          if (n >= nfull) smp[u] = make_float2((n == nfull && odd) ? smp[u].x : 0.f, 0.f);
+        }
       }
 #pragma unroll
       for (int u = 0; u < E; ++u) wv[u] = __ldg(reinterpret_cast<const float2 *>(win) + gt + T * u);
@@ -330,7 +354,7 @@ stft_kernel(const void *__restrict__ x, int64_t ld, int in_dtype, int norm_mode,
 #pragma unroll
       for (int u = 0; u < E; ++u) sm += v[u].x + v[u].y;
       sm = group_sum<T>(sm, gsum, tid);
-      const float mean = sm * (1.f / (float)L);
+      const float mean = sm / (float)lay.Ls;
 #pragma unroll
       for (int u = 0; u < E; ++u) {
         v[u] = make_float2(v[u].x - mean, v[u].y - mean);

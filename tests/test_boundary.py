@@ -27,7 +27,7 @@ def test_library_exports_every_declared_symbol():
     for name in ("delta_stft", "delta_cross_spectra", "delta_coherence", "delta_crossphase", "delta_crosspower",
                  "delta_crosscorr"):   # the six calls BASELINE.json's north_star names
         assert name in syms
-    assert b.LIB.delta_version() == 104
+    assert b.LIB.delta_version() == 105
     assert os.path.dirname(b.LIB_PATH).endswith("paper_2108_08896_b200")  # in-tree, not site-packages
 
 
@@ -149,3 +149,15 @@ def test_explicit_pair_list_validation():
         with pytest.raises(b.DeltaError) as e:
             b.Plan(8, 2048, 256, 128, allocate=False, pairs=bad)
         assert e.value.status == b.ERR_INVALID_ARG
+
+
+def test_nperseg_validation():
+    assert b.Plan(8, 2048, 256, 64, allocate=False, nperseg=128).sizes.K == (2048 - 128) // 64 + 1
+    assert b.Plan(8, 2048, 256, 128, allocate=False, nperseg=0).sizes.K == 15
+    for kw, st in ((dict(nperseg=300), b.ERR_INVALID_ARG), (dict(nperseg=-1), b.ERR_INVALID_ARG),
+                   (dict(nperseg=100, hop=128), b.ERR_UNSUPPORTED)):
+        args = dict(hop=128)
+        args.update(kw)
+        with pytest.raises(b.DeltaError) as e:
+            b.Plan(8, 2048, 256, allocate=False, **args)
+        assert e.value.status == st

@@ -505,3 +505,31 @@ def test_three_views_576_channels(mode):
     st = compare(sub, ref, loc, "576 channels")
     print(st)
     assert np.isfinite(out["G"]).all() and out["G"].max() <= 1 + 1e-4 and np.abs(out["R"]).max() <= 1 + 1e-4
+
+
+@pytest.mark.parametrize("L,Ls,H,detrend,dtype", [(512, 256, 128, 0, "f32"), (1024, 300, 100, 1, "f32"), (256, 129, 64, 0, "i16")])
+def test_zero_padded_segments(L, Ls, H, detrend, dtype, mode):
+    """f2: segments of nperseg < nfft samples zero-padded to the transform length (the
+    linear cross-correlation).  Cases: half-length segments; an odd-ish length that is no multiple of anything, with
+    detrend; an odd length with int16 counts and offset normalisation (the padding must stay zero)."""
+    C, T = 20, 10_000
+    b = binding()
+    if dtype == "i16":
+        counts, _ = es.streamed(n_chunks=1)
+        x = counts[0][:C]
+        offs = o.offsets(x[:, :5000])
+        plan = b.Plan(C, T, L, H, L // 2, contraction=mode, nperseg=Ls, detrend=detrend, in_dtype=b.I16, norm_mode=b.NORM_RELATIVE)
+        xd = dev(x)
+        plan.set_offsets(xd, 5000)
+        ref = o.analyze_chunk(x, L, H, L // 2, nperseg=Ls, detrend=detrend, norm_mode=o.NORM_RELATIVE, offs=offs)
+    else:
+        x = es.turbulence(T, 91)[:C]
+        plan = b.Plan(C, T, L, H, L // 2, contraction=mode, nperseg=Ls, detrend=detrend)
+        xd = dev(x)
+        ref = o.analyze_chunk(x, L, H, L // 2, nperseg=Ls, detrend=detrend)
+    assert plan.sizes.K == (T - Ls) // H + 1
+    out = plan.analyze_chunk(xd)
+    torch.cuda.synchronize()
+    out = {k: v.cpu().numpy() for k, v in out.items()}
+    st = compare(out, ref, o.all_pairs(C), f"nperseg {Ls} of {L}")
+    print(st)
