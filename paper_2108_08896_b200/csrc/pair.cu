@@ -122,7 +122,7 @@ __global__ void __launch_bounds__(PairCfg<L>::THREADS, PairCfg<L>::MIN_CTAS)
 pair_kernel(const float2 *__restrict__ S, const float *__restrict__ Srsq, const float *__restrict__ rpart, int nrp,
             int rp_stride, float rscale, const ushort2 *__restrict__ list, const float2 *__restrict__ tw,
             const float2 *__restrict__ ftab, Layout lay, PairConsts pc, float *__restrict__ G_, float *__restrict__ A_,
-            float *__restrict__ Pw_, float *__restrict__ R_) {
+            float *__restrict__ Pw_, float *__restrict__ R_, long long *trace) {
   using Cfg = PairCfg<L>;
   using Geo = typename Cfg::G;
   constexpr int N = Cfg::N, F = Cfg::F, T = Cfg::T, E = Cfg::E, PB = Cfg::PB;
@@ -141,6 +141,15 @@ pair_kernel(const float2 *__restrict__ S, const float *__restrict__ Srsq, const 
   const int tid = threadIdx.x;
   const int64_t p0 = (int64_t)blockIdx.x * PB;
 
+  // debug: globaltimer stamps of the CTA's phases (delta_debug_set_trace): trace[8192 + 8 blockIdx + k]
+  auto stamp = [&](int k) {
+    if (trace && tid == 0) {
+      long long g;
+      asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g));
+      trace[8192 + 8 * (int64_t)blockIdx.x + k] = g;
+    }
+  };
+  stamp(0);
   pdl_launch_dependents();
   if (tid < PB) {
     // all pairs: (i, j) of lexicographic pair p0 + tid;  pair list (f2): entry p0 + tid of the list, whose S values sit
@@ -155,6 +164,7 @@ pair_kernel(const float2 *__restrict__ S, const float *__restrict__ Srsq, const 
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   pdl_wait();  // S, rsq and the energy partials come from the preceding kernels; the outputs may still be read by a consumer
+  stamp(1);
   __syncthreads();
   if (tid == 0) {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)),
@@ -197,6 +207,7 @@ pair_kernel(const float2 *__restrict__ S, const float *__restrict__ Srsq, const 
                    : "=r"(ok) : "r"(smem_u32(bar)), "r"(0) : "memory");
   }
 
+  stamp(2);  // tile landed
   const int pl = tid / T, gt = tid % T;
   const int64_t p = p0 + pl;
   const bool valid = p < lay.Po;
@@ -221,29 +232,83 @@ pair_kernel(const float2 *__restrict__ S, const float *__restrict__ Srsq, const 
       constexpr int R = THREADS / NG, NIT = PB / R;
       static_assert(R >= 1 && (R & (R - 1)) == 0 && PB % R == 0, "pairs per iteration");
       const int g = tid % NG, qa = tid / NG;
+      if constexpr (R % 4 == 0) {
+        // Everything but the pair is the same in every iteration, so the bins, the four tile addresses (the pair offset
+        // it R only flips slot bits: one XOR) and the base pointers are hoisted.  The G/A/P pass is bound by the
+        // load/store unit's wavefronts, so the two 1/sqrt rows are read as aligned float4 (two loads cover the four
+        // bins f0 + 4g .. + 3 of a group that starts f0 floats past a 16-byte boundary; f0 is warp-uniform), and the
+        // row of channel i, shared by consecutive lexicographic pairs, is re-read only when i changes.
+        const int f0 = (-qa) & 3, ng = (F - f0) >> 2, f = f0 + 4 * g;
+        if (g < ng) {
+          int tb[4];
 #pragma unroll
-      for (int it = 0; it < NIT; ++it) {
-        const int ql = (it * R) ^ qa;  // = it R + qa (qa < R, R a power of two)
-        const int64_t q = p0 + ql;
-        const int f0 = (-(qa + ((it * R) & 3))) & 3, ng = (F - f0) >> 2;
-        if (q >= lay.Po || g >= ng) continue;
-        const int f = f0 + 4 * g;
-        const ushort2 qij = ij_s[ql];
-        const float *qi = Srsq + (int64_t)qij.x * Cfg::FP + f, *qj = rowj + ql * Cfg::FP + f;
-        float2 sv[4];
-        float g2[4];
+          for (int k = 0; k < 4; ++k) tb[k] = (f + k) * PB + ((qa ^ s_swz(f + k)) & (PB - 1));
+          const int64_t at0 = (p0 + qa) * F + f;
+          float *Pw0 = Pw ? Pw + at0 : nullptr, *G0 = G ? G + at0 : nullptr, *A0 = A ? A + at0 : nullptr;
+          auto quad = [&](const float4 a, const float4 bq, float *r) {  // elements f0 .. f0 + 3 of (a, bq)
+            switch (f0) {
+              case 0: r[0] = a.x; r[1] = a.y; r[2] = a.z; r[3] = a.w; break;
+              case 1: r[0] = a.y; r[1] = a.z; r[2] = a.w; r[3] = bq.x; break;
+              case 2: r[0] = a.z; r[1] = a.w; r[2] = bq.x; r[3] = bq.y; break;
+              default: r[0] = a.w; r[1] = bq.x; r[2] = bq.y; r[3] = bq.z; break;
+            }
+          };
+          int icur = -1;
+          float gi[4] = {0.f, 0.f, 0.f, 0.f};
 #pragma unroll
-        for (int k = 0; k < 4; ++k) {
-          sv[k] = tile[(f + k) * PB + (((qa ^ s_swz(f + k)) ^ (it * R)) & (PB - 1))];
-          g2[k] = wantG ? __ldg(qi + k) * qj[k] : 0.f;
+          for (int it = 0; it < NIT; ++it) {
+            const int ql = it * R + qa;
+            if (p0 + ql >= lay.Po) continue;
+            float g2[4] = {0.f, 0.f, 0.f, 0.f};
+            if (wantG) {
+              const int i = ij_s[ql].x;
+              if (i != icur) {  // warp-uniform
+                const float4 *src = reinterpret_cast<const float4 *>(Srsq + (int64_t)i * Cfg::FP + 4 * g);
+                quad(__ldg(src), __ldg(src + 1), gi);
+                icur = i;
+              }
+              const float4 *rowq = reinterpret_cast<const float4 *>(rowj + ql * Cfg::FP + 4 * g);
+              float gj[4];
+              quad(rowq[0], rowq[1], gj);
+#pragma unroll
+              for (int k = 0; k < 4; ++k) g2[k] = gi[k] * gj[k];
+            }
+            float2 sv[4];
+#pragma unroll
+            for (int k = 0; k < 4; ++k) sv[k] = tile[tb[k] ^ (it * R)];
+            float m[4], c[4], an[4];
+#pragma unroll
+            for (int k = 0; k < 4; ++k) value(sv[k], g2[k], m[k], c[k], an[k]);
+            if (GAPALL || Pw) ST4(Pw0 + it * R * F, make_float4(m[0], m[1], m[2], m[3]));
+            if (GAPALL || G) ST4(G0 + it * R * F, make_float4(c[0], c[1], c[2], c[3]));
+            if (GAPALL || A) ST4(A0 + it * R * F, make_float4(an[0], an[1], an[2], an[3]));
+          }
         }
-        float m[4], c[4], an[4];
+      } else {
 #pragma unroll
-        for (int k = 0; k < 4; ++k) value(sv[k], g2[k], m[k], c[k], an[k]);
-        const int64_t at = q * F + f;
-        if (GAPALL || Pw) ST4(Pw + at, make_float4(m[0], m[1], m[2], m[3]));
-        if (GAPALL || G) ST4(G + at, make_float4(c[0], c[1], c[2], c[3]));
-        if (GAPALL || A) ST4(A + at, make_float4(an[0], an[1], an[2], an[3]));
+        for (int it = 0; it < NIT; ++it) {
+          const int ql = (it * R) ^ qa;  // = it R + qa (qa < R, R a power of two)
+          const int64_t q = p0 + ql;
+          const int f0 = (-(qa + ((it * R) & 3))) & 3, ng = (F - f0) >> 2;
+          if (q >= lay.Po || g >= ng) continue;
+          const int f = f0 + 4 * g;
+          const ushort2 qij = ij_s[ql];
+          const float *qi = Srsq + (int64_t)qij.x * Cfg::FP + f, *qj = rowj + ql * Cfg::FP + f;
+          float2 sv[4];
+          float g2[4];
+#pragma unroll
+          for (int k = 0; k < 4; ++k) {
+            sv[k] = tile[(f + k) * PB + (((qa ^ s_swz(f + k)) ^ (it * R)) & (PB - 1))];
+            g2[k] = wantG ? __ldg(qi + k) * qj[k] : 0.f;
+          }
+          float m[4], c[4], an[4];
+#pragma unroll
+          for (int k = 0; k < 4; ++k) value(sv[k], g2[k], m[k], c[k], an[k]);
+          const int64_t at = q * F + f;
+          if (GAPALL || Pw) ST4(Pw + at, make_float4(m[0], m[1], m[2], m[3]));
+          if (GAPALL || G) ST4(G + at, make_float4(c[0], c[1], c[2], c[3]));
+          if (GAPALL || A) ST4(A + at, make_float4(an[0], an[1], an[2], an[3]));
+        }
       }
     }
     // scalar bins: the edges of the vector path (at most 6 per pair), or everything if the arrays are not 16-byte aligned
@@ -267,6 +332,7 @@ pair_kernel(const float2 *__restrict__ S, const float *__restrict__ Srsq, const 
       if (GAPALL || A) ST1(A + q * F + f, an);
     }
   }
+  stamp(3);  // pass 1 done (thread 0's share)
   if (!wantR) return;
 
   // ---- pass 2: merge step of the inverse real transform (S read again from the tile; twice the merge of
@@ -283,10 +349,12 @@ pair_kernel(const float2 *__restrict__ S, const float *__restrict__ Srsq, const 
     const float2 w = cmul(wg, pc.wstep[u]);               // e^{-2 pi i f / L}; the inverse uses its conjugate
     v[u] = irfft_merge2(sf, sr, make_float2(w.x, -w.y));
   }
+  stamp(4);
   __syncthreads();  // every S value is in registers: the tile becomes exchange space
 
   // ---- rho = irfft(S) / sqrt(R_ii[0] R_jj[0]) ----------------------------------------------------------------
   fft_inplace_g<Geo, true>(v, FftPadMap{exch + pl * Geo::BUF}, ftab, gt);  // z[n] = (x[2n], x[2n+1]) * N, n = gt + T u
+  stamp(5);  // FFT done
   if (!valid) return;
   // rho = x / sqrt(R_ii[0] R_jj[0]),  x = z/N,  R_cc[0] = (sum over all L bins of S_cc)/L
   const float norm = rs[pl] * rs[PB + pl];  // 2 (L/N) x 1/2 (irfft_merge2)
@@ -324,6 +392,7 @@ pair_kernel(const float2 *__restrict__ S, const float *__restrict__ Srsq, const 
       }
     }
   }
+  stamp(6);
 }
 
 // rsq[c][f] = 1/sqrt(S_cc[f]) (0 where S_cc[f] <= 0, reading R16) and
@@ -394,7 +463,7 @@ static int launch_pair_L(delta_plan *p, const float *d_S, const float *d_rsq, co
     LaunchCfg lc(dim3((unsigned)lay.Poblk), dim3(Cfg::THREADS), Cfg::SMEM, st, p->use_pdl);                          \
     DELTA_CUDA_CHECK(cudaLaunchKernelEx(&lc.cfg, pair_kernel<L, FULL_, GAPALL_>, reinterpret_cast<const float2 *>(d_S), \
                                         d_rsq, rpart, nrp, rp_stride, rscale, list, p->d_tw(), p->d_ftab2(), lay, pc, \
-                                        d_G, d_A, d_P, d_R));                                                       \
+                                        d_G, d_A, d_P, d_R, p->d_trace));                                                       \
   } while (0)
   const bool gapall = d_G && d_A && d_P;
   if (full && gapall) DELTA_PAIR_LAUNCH(true, true);
