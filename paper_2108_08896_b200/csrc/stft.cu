@@ -249,7 +249,7 @@ __global__ void __launch_bounds__(StftCfg<L>::THREADS, 1024 / StftCfg<L>::THREAD
 stft_kernel(const void *__restrict__ x, int64_t ld, int in_dtype, int norm_mode, int n_first,
             const double *__restrict__ offs, const long long *__restrict__ isum, const float2 *__restrict__ tw,
             const float *__restrict__ win, const float2 *__restrict__ ftab, Layout lay, void *__restrict__ Xout,
-            float *__restrict__ chscale, float *__restrict__ wpart) {
+            float *__restrict__ chscale, float *__restrict__ wpart, long long *trace) {
   using Cfg = StftCfg<L>;
   using G = typename Cfg::G;
   constexpr int N = Cfg::N, T = Cfg::T, E = G::E, CH = Cfg::CH;
@@ -261,8 +261,37 @@ stft_kernel(const void *__restrict__ x, int64_t ld, int in_dtype, int norm_mode,
   __shared__ float cmax[CH];                 // per-channel max |y| over this CTA's segments (read by the cluster)
   __shared__ float csc[CH];                  // per-channel fp16 scale
 
+  // debug: globaltimer stamps of the CTA's phases (delta_debug_set_trace): trace[32768 + 8 cta + k]
+  auto stamp = [&](int k) {
+    if (trace && threadIdx.x == 0) {
+      long long gtm;
+      asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(gtm));
+      trace[32768 + 8 * ((int64_t)blockIdx.y * gridDim.x + blockIdx.x) + k] = gtm;
+    }
+  };
+  stamp(0);
   pdl_launch_dependents();
+#ifndef DELTA_STFT_NO_PREFETCH
+  {
+    // L2 prefetch of the CTA's samples, one request per 128-byte line.  It is a hint without a data dependence, so it
+    // is issued before pdl_wait (while the predecessor drains) and with far more lines in flight than demand loads get:
+    // the loads after the wait then find the chunk in L2 instead of paying the DRAM latency with 16 loads per thread.
+    const size_t esz = in_dtype == DELTA_I16 ? 2 : 4;
+    const int64_t s0 = (int64_t)blockIdx.x * kSegBlock * lay.H;
+    const int64_t cnt = min((int64_t)(kSegBlock - 1) * lay.H + lay.Ls, (int64_t)lay.T - s0);
+    const int nl = (int)((cnt * (int64_t)esz + 127) / 128) + 1;
+    for (int i = threadIdx.x; i < CH * nl; i += Cfg::THREADS) {
+      const int ch = blockIdx.y * CH + i / nl;
+      if (ch < lay.C) {
+        const char *a = reinterpret_cast<const char *>(x) + ((int64_t)ch * ld + s0) * esz + (int64_t)(i % nl) * 128;
+        const char *end = reinterpret_cast<const char *>(x) + ((int64_t)ch * ld + s0 + cnt) * esz;
+        if (a < end) asm volatile("prefetch.global.L2 [%0];" ::"l"(a));
+      }
+    }
+  }
+#endif
   pdl_wait();  // the chunk may come from the caller's previous kernel; X, wpart and chscale are read by ours
+  stamp(1);
 
   const int tid = threadIdx.x, g = tid / T, gt = tid % T;
   const int cl = g / kSegBlock, kk = g % kSegBlock;
@@ -362,6 +391,8 @@ stft_kernel(const void *__restrict__ x, int64_t ld, int in_dtype, int norm_mode,
         v[u] = make_float2(v[u].x * wv[u].x, v[u].y * wv[u].y);
       }
     }
+    if (v[0].x == 123.456f) stamp(7);  // keep v live
+    stamp(6);  // samples in registers
     {  // energy of the windowed segment (zero-lag autocorrelation of Eq. 1d by Parseval), fixed summation order
       float ss = 0.f;
 #pragma unroll
@@ -390,6 +421,7 @@ stft_kernel(const void *__restrict__ x, int64_t ld, int in_dtype, int norm_mode,
       }
       cg::this_cluster().barrier_arrive();
     }
+    stamp(2);  // samples loaded, windowed, energy and max reduced
     fft_inplace<N, false>(v, FftPadMap{buf}, ftab, gt);
     fft_group_sync<T>();  // every read-back of the group is done before Z overwrites the buffer
 #pragma unroll
@@ -420,6 +452,7 @@ stft_kernel(const void *__restrict__ x, int64_t ld, int in_dtype, int norm_mode,
     __syncthreads();           // csc is visible to the CTA
   }
 
+  stamp(3);  // FFT done, scale agreed
   // Phase 2.  Bins f and N - f come from the same pair Z[f], Z[N-f]:  with e = (Z[f] + conj Z[N-f])/2,
   // d = (Z[f] - conj Z[N-f])/2 and (a, b) = e^{-2 pi i f/L} d:  X[f] = (e.x + b, e.y - a),  X[N-f] = (e.x - b, -e.y - a).
   // One thread does both for the 8 segments of the CTA; bin N/2 (its own partner) is done once.
@@ -490,7 +523,9 @@ stft_kernel(const void *__restrict__ x, int64_t ld, int in_dtype, int norm_mode,
     store_bin(c, pcl, f, re, im);
     if (2 * f != N) store_bin(c, pcl, N - f, re2, im2);
   }
+  stamp(4);  // write-out issued
   if (CLUSTER) cg::this_cluster().barrier_wait();  // no CTA exits while its cmax may still be read
+  stamp(5);
 }
 
 // test accessor: X layout -> complex64 [C][K][F]
@@ -540,7 +575,7 @@ static int launch_stft_LTD(delta_plan *p, const void *d_x, int64_t ld, void *d_X
   LaunchCfg lc(dim3(lay.nkb, (lay.C + Cfg::CH - 1) / Cfg::CH), dim3(Cfg::THREADS), smem, st, p->use_pdl, CLUSTER ? lay.nkb : 0);
   DELTA_CUDA_CHECK(cudaLaunchKernelEx(&lc.cfg, stft_kernel<L, TC, CLUSTER, DETREND>, d_x, ld, p->cfg.in_dtype, p->cfg.norm_mode, p->n_first,
                                       (const double *)p->d_offs(), (const long long *)p->d_isum(), p->d_tw(), p->d_win(),
-                                      p->d_ftab(), lay, d_X, p->d_chscale(), p->d_wpart()));
+                                      p->d_ftab(), lay, d_X, p->d_chscale(), p->d_wpart(), p->d_trace));
   p->launches++;
   DELTA_CUDA_CHECK(cudaGetLastError());
   return DELTA_OK;
