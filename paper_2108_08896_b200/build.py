@@ -40,17 +40,39 @@ def is_stale() -> bool:
 def build(force: bool = False, verbose: bool = False) -> str:
     if not force and not is_stale():
         return LIB
-    cmd = [nvcc_path(), *ARCH, "-O3", "-std=c++17", "-lineinfo", "-shared", "-Xcompiler", "-fPIC",
-           "-I", os.path.join(ROOT, "include"), "-I", CSRC, "-o", LIB, *sources()]
-    cmd[1:1] = os.environ.get("DELTA_NVCC_FLAGS", "").split()  # tuning experiments only (e.g. -DDELTA_PAIR_WARPS=32)
+    nvcc = nvcc_path()
+    objdir = os.path.join(PKG, "build")
+    os.makedirs(objdir, exist_ok=True)
+    common = [*ARCH, "-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC", "-I", os.path.join(ROOT, "include"), "-I", CSRC]
+    common[0:0] = os.environ.get("DELTA_NVCC_FLAGS", "").split()  # tuning experiments only (e.g. -DDELTA_PAIR_TILE_SPLIT=4)
     if verbose:
-        cmd.insert(1, "-Xptxas=-v")
-        print(" ".join(cmd))
-    res = subprocess.run(cmd, capture_output=True, text=True)
+        common.insert(0, "-Xptxas=-v")
+
+    def compile_one(src: str):
+        obj = os.path.join(objdir, os.path.basename(src)[:-3] + ".o")
+        cmd = [nvcc, *common, "-c", src, "-o", obj]
+        res = subprocess.run(cmd, capture_output=True, text=True)
+        return obj, cmd, res
+
+    # one nvcc per translation unit, in parallel (the kernels are independent; the launchers are plain host functions)
+    from concurrent.futures import ThreadPoolExecutor
+    with ThreadPoolExecutor(max_workers=len(sources())) as pool:
+        results = list(pool.map(compile_one, sources()))
+    failed = False
+    for obj, cmd, res in results:
+        if verbose:
+            print(" ".join(cmd))
+        if verbose or res.returncode != 0:
+            sys.stderr.write(res.stdout + res.stderr)
+        failed |= res.returncode != 0
+    if failed:
+        raise RuntimeError("nvcc failed building libdelta_b200.so")
+    link = [nvcc, *ARCH, "-shared", "-o", LIB, *[obj for obj, _, _ in results]]
+    res = subprocess.run(link, capture_output=True, text=True)
     if verbose or res.returncode != 0:
         sys.stderr.write(res.stdout + res.stderr)
     if res.returncode != 0:
-        raise RuntimeError("nvcc failed building libdelta_b200.so")
+        raise RuntimeError("nvcc failed linking libdelta_b200.so")
     return LIB
 
 
