@@ -533,3 +533,29 @@ def test_zero_padded_segments(L, Ls, H, detrend, dtype, mode):
     out = {k: v.cpu().numpy() for k, v in out.items()}
     st = compare(out, ref, o.all_pairs(C), f"nperseg {Ls} of {L}")
     print(st)
+
+
+def test_all_variants_together(mode):
+    """The f1/f2 options are independent switches; everything at once must still match the oracle: int16 counts with
+    offset normalisation, Blackman window, detrend, zero-padded segments, band-pass, phase-lock estimator, an explicit
+    pair list, a short lag window."""
+    b = binding()
+    C, T, L, Ls, H, M = 24, 10_000, 512, 320, 160, 100
+    counts, _ = es.streamed(n_chunks=1)
+    x = counts[0][:C]
+    offs = o.offsets(x[:, :5000])
+    allp = o.all_pairs(C)
+    pairs = allp[np.random.default_rng(5).choice(len(allp), 45, replace=False)]
+    band = (8e3, 120e3)
+    plan = b.Plan(C, T, L, H, M, contraction=mode, in_dtype=b.I16, norm_mode=b.NORM_RELATIVE, window=3, detrend=1,
+                  nperseg=Ls, band=band, estimator=1, pairs=pairs)
+    xd = dev(x)
+    plan.set_offsets(xd, 5000)
+    out = plan.analyze_chunk(xd)
+    torch.cuda.synchronize()
+    out = {k: v.cpu().numpy() for k, v in out.items()}
+    ref = o.analyze_chunk(x, L, H, M, pairs=pairs, fs=500e3, norm_mode=o.NORM_RELATIVE, offs=offs, band=band,
+                          win=o.WIN_BLACKMAN, detrend=o.DETREND_CONSTANT, phase_lock=True, nperseg=Ls)
+    assert out["R"].shape == (45, 2 * M + 1)
+    st = compare(out, ref, pairs, "all variants", p_abs_tol=5e-5)
+    print(st)
