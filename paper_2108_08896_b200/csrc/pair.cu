@@ -32,7 +32,10 @@ struct PairCfg {
   static constexpr int PB = pair_block(L);
   static constexpr int THREADS = PB * T;
   // resident warps per SM the register budget is sized for: 48 (40 registers) with 8 points per thread, else 32 (64)
-  static constexpr int WARPS = E <= 8 ? 48 : 32;
+#ifndef DELTA_PAIR_WARPS
+#define DELTA_PAIR_WARPS 32
+#endif
+  static constexpr int WARPS = E <= 8 ? 48 : DELTA_PAIR_WARPS;
   static constexpr int MIN_CTAS = (WARPS * 32) / THREADS > 0 ? (WARPS * 32) / THREADS : 1;
   static constexpr size_t TILE_BYTES = (size_t)F * PB * sizeof(float2);
   static constexpr size_t EXCH_BYTES = (size_t)PB * G::BUF * sizeof(float2);
