@@ -3,7 +3,7 @@
  * for NVIDIA B200 (sm_100a).
  *
  * What the library computes, per streamed channel-by-time chunk (citations are line numbers of
- * the paper text, /root/reference/PAPER.md; DESIGN.md section 3 lists the readings R1..R16 taken
+ * the paper text, /root/reference/PAPER.md; DESIGN.md section 3 lists the readings R1..R22 taken
  * where the paper is silent or garbled):
  *
  *   normalisation   y_c[t] = (x_c[t] - o_c)/o_c               "After normalizing each chunk" L107, L89
@@ -13,7 +13,9 @@
  *   Eq. (1b) L97    G_ij[f]  = |S_ij[f]| / sqrt(S_ii[f] S_jj[f])             coherence
  *   Eq. (1c) L100   A_ij[f]  = atan2(Im S_ij[f], Re S_ij[f])                 cross-phase
  *   Eq. (1d) L102   rho_ij[m] = IFFT_L(S_ij)[m] / sqrt(R_ii[0] R_jj[0])      cross-correlation, m = -M..M
- *   for all C(C-1)/2 channel pairs i < j, lexicographic ("18336 ... channel pair combinations" L107).
+ *   for all C(C-1)/2 channel pairs i < j, lexicographic ("18336 ... channel pair combinations" L107), or for an
+ *   explicit pair list.  Variants next to the path (delta_config): band-pass filter, other windows, detrend,
+ *   zero-padded segments, per-segment-normalised coherence; delta_accumulate averages spectra over chunks.
  *
  * Conventions
  *   - Pointers named d_* are DEVICE pointers, h_* are HOST pointers; all are owned by the caller.
@@ -26,7 +28,8 @@
  *   - There is no CPU fallback: without a CUDA device every compute call returns DELTA_ERR_CUDA.
  *
  * Symbols: C channels, T samples per chunk, L = nfft, H = hop, K = (T-L)/H + 1 segments (no
- * padding, tail dropped), F = L/2+1 one-sided bins, P = C(C-1)/2 pairs, M = max_lag.
+ * padding, tail dropped; (T - nperseg)/H + 1 with zero-padded segments), F = L/2+1 one-sided bins,
+ * P = C(C-1)/2 pairs (or the length of the pair list), M = max_lag.
  */
 #ifndef DELTA_B200_H
 #define DELTA_B200_H
@@ -43,8 +46,8 @@ extern "C" {
 typedef enum {
   DELTA_OK = 0,
   DELTA_ERR_INVALID_ARG = -1, /* NULL pointer, non-positive size, unknown enum value               */
-  DELTA_ERR_UNSUPPORTED = -2, /* nfft not a power of two in [64,4096], T < L, hop not in [1,L],
-                                 max_lag > L/2, explicit pair list (not in this version), C > 4096  */
+  DELTA_ERR_UNSUPPORTED = -2, /* nfft not a power of two in [64,4096], T < segment length, hop larger
+                                 than the segment, max_lag > L/2, C > 4096                         */
   DELTA_ERR_ALIGNMENT = -3,   /* a device pointer is not 16-byte aligned                            */
   DELTA_ERR_NO_WORKSPACE = -4,/* compute call before delta_plan_set_workspace(), or it is too small */
   DELTA_ERR_CUDA = -5,        /* a CUDA runtime call failed; see delta_last_cuda_error()            */
@@ -57,7 +60,7 @@ enum { DELTA_WIN_HANN_PERIODIC = 0, DELTA_WIN_HAMMING_PERIODIC = 1, DELTA_WIN_RE
 /* Eq. (1b) estimator: from the segment-averaged spectra (R10, the default), or the per-segment-normalised variant (f2):
  * every X[c,k,f] is replaced by X/|X| before Eq. (1a), so S is a mean of unit phasors, S_cc = s^2, G = |mean phasor| */
 enum { DELTA_EST_AVERAGED = 0, DELTA_EST_PHASE_LOCK = 1 };
-/* per-segment detrend before the window: none (R5, the default) or the mean of the segment's nfft samples */
+/* per-segment detrend before the window: none (R5, the default) or the mean of the segment's samples */
 enum { DELTA_DETREND_NONE = 0, DELTA_DETREND_CONSTANT = 1 };
 enum { DELTA_SCALE_WINPOW = 0,                       /* s^2 = 1/sum w^2 (default; white noise of
                                                         variance v has E S_ii = v)                    */
