@@ -161,3 +161,39 @@ def test_nperseg_validation():
         with pytest.raises(b.DeltaError) as e:
             b.Plan(8, 2048, 256, allocate=False, **args)
         assert e.value.status == st
+
+
+def test_header_is_plain_c_and_links(tmp_path):
+    """The boundary is a C ABI: include/delta.h must compile as C99 (no C++ or CUDA types in the signatures) and a
+    plain C program must link against the shared library and create / destroy a plan without a GPU."""
+    import shutil
+    import subprocess
+    gcc = shutil.which("gcc")
+    if gcc is None:
+        pytest.skip("no gcc")
+    src = tmp_path / "use_delta.c"
+    src.write_text('''
+#include <stdio.h>
+#include <string.h>
+#include "delta.h"
+int main(void) {
+  delta_config c;
+  memset(&c, 0, sizeof c);
+  c.n_channels = 192; c.n_samples = 10000; c.nfft = 512; c.hop = 256; c.max_lag = 256; c.fs = 500e3f;
+  delta_plan *p = NULL;
+  delta_sizes s;
+  if (delta_plan_create(&c, &p) != DELTA_OK || delta_plan_sizes(p, &s) != DELTA_OK) return 1;
+  printf("%d %d %lld %d\\n", s.n_segments, s.n_bins, (long long)s.n_pairs, delta_version());
+  c.nfft = 500;
+  delta_plan *q = NULL;
+  if (delta_plan_create(&c, &q) != DELTA_ERR_UNSUPPORTED || q != NULL) return 2;
+  return delta_plan_destroy(p) == DELTA_OK ? 0 : 3;
+}
+''')
+    exe = tmp_path / "use_delta"
+    libdir = os.path.dirname(b.LIB_PATH)
+    subprocess.run([gcc, "-std=c99", "-Wall", "-Wextra", "-pedantic", "-Werror", "-I", os.path.join(ROOT, "include"),
+                    str(src), "-o", str(exe), "-L", libdir, "-ldelta_b200", f"-Wl,-rpath,{libdir}"], check=True)
+    out = subprocess.run([str(exe)], capture_output=True, text=True)
+    assert out.returncode == 0, out
+    assert out.stdout.split()[:3] == ["38", "257", "18336"]
