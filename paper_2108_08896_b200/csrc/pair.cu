@@ -203,11 +203,15 @@ pair_kernel(const float2 *__restrict__ S, const float *__restrict__ Srsq, const 
   }
   __syncthreads();
 
-  {  // the tile has landed?
+  {  // the tile has landed?  (bounded: a faulted copy must trap, not hang the GPU)
     uint32_t ok = 0;
-    while (!ok)
+    long long t0 = 0;
+    for (uint32_t spins = 0; !ok; ++spins) {
       asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
                    : "=r"(ok) : "r"(smem_u32(bar)), "r"(0) : "memory");
+      if (spins == 64) t0 = clock64();
+      if (spins > 64 && (spins & 1023) == 0 && clock64() - t0 > 4000000000LL) __trap();
+    }
   }
 
   stamp(2);  // tile landed
