@@ -51,7 +51,8 @@ typedef enum {
   DELTA_ERR_ALIGNMENT = -3,   /* a device pointer is not 16-byte aligned                            */
   DELTA_ERR_NO_WORKSPACE = -4,/* compute call before delta_plan_set_workspace(), or it is too small */
   DELTA_ERR_CUDA = -5,        /* a CUDA runtime call failed; see delta_last_cuda_error()            */
-  DELTA_ERR_STATE = -6        /* e.g. norm_mode needs offsets and delta_set_offsets() was not called */
+  DELTA_ERR_STATE = -6,       /* e.g. norm_mode needs offsets and delta_set_offsets() was not called */
+  DELTA_ERR_NO_MEMORY = -7    /* host allocation of the plan failed                                 */
 } delta_status;
 
 /* periodic (DFT-even) windows, x = 2 pi n/L: Hann 1/2 - 1/2 cos x (R4, the default); the others are the f1 variants:
@@ -78,7 +79,7 @@ enum { DELTA_CONTRACT_AUTO = 0,                      /* library picks (tensor co
 typedef struct {
   int32_t n_channels;   /* C >= 1                                                                     */
   int32_t n_samples;    /* T >= nfft, samples per channel per chunk                                   */
-  int32_t nfft;         /* L, power of two in [64, 4096]; segment length == nfft (no zero padding)    */
+  int32_t nfft;         /* L, transform length, power of two in [64, 4096]; segment length: see nperseg  */
   int32_t hop;          /* H in [1, L]; overlap = L - H                                               */
   int32_t window;       /* DELTA_WIN_*                                                                */
   int32_t scaling;      /* DELTA_SCALE_*                                                              */
@@ -197,10 +198,6 @@ int delta_analyze_shot_host(delta_plan *plan, const void *h_x, int32_t n_chunks,
  * stage, events[1] after it, events[2] after the contraction and events[3] after the pair stage, on
  * the launching stream (so the caller can time each stage with cudaEventElapsedTime). */
 int delta_plan_set_stage_events(delta_plan *plan, void *const *events);
-
-/* Debug hook.  d_trace: device buffer of 3*512 int64 (or NULL to switch off).  While set, CTA 0 of the
- * tensor-core contraction writes SM clock stamps of its producer / MMA / epilogue roles into it. */
-int delta_debug_set_trace(delta_plan *plan, void *d_trace);
 
 /* Number of kernels the last delta_analyze_chunk() on this plan launched (for bench accounting). */
 int delta_last_launch_count(const delta_plan *plan);

@@ -15,7 +15,7 @@ from . import build as _build
 
 # ---- enums (include/delta.h) --------------------------------------------------------------
 OK = 0
-ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_ALIGNMENT, ERR_NO_WORKSPACE, ERR_CUDA, ERR_STATE = -1, -2, -3, -4, -5, -6
+ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_ALIGNMENT, ERR_NO_WORKSPACE, ERR_CUDA, ERR_STATE, ERR_NO_MEMORY = -1, -2, -3, -4, -5, -6, -7
 WIN_HANN_PERIODIC = 0
 SCALE_WINPOW, SCALE_NONE, SCALE_DENSITY, SCALE_SPECTRUM = 0, 1, 2, 3
 F32, I16 = 0, 1
@@ -39,7 +39,7 @@ class DeltaSizes(C.Structure):
 
 EXPORTS = ["delta_plan_create", "delta_plan_destroy", "delta_plan_sizes", "delta_plan_set_workspace",
            "delta_set_offsets", "delta_get_offsets", "delta_stft", "delta_stft_unpack", "delta_cross_spectra",
-           "delta_cross_spectra_unpack", "delta_debug_set_trace",
+           "delta_cross_spectra_unpack",
            "delta_coherence", "delta_crossphase", "delta_crosspower", "delta_crosscorr", "delta_accumulate", "delta_analyze_chunk",
            "delta_analyze_shot_host", "delta_plan_set_stage_events", "delta_last_launch_count", "delta_strerror", "delta_last_cuda_error",
            "delta_version"]
@@ -61,7 +61,7 @@ def _load() -> C.CDLL:
     lib.delta_stft_unpack.argtypes = [vp, vp, vp, vp]
     lib.delta_cross_spectra.argtypes = [vp, vp, vp, vp, vp]
     lib.delta_cross_spectra_unpack.argtypes = [vp, vp, vp, vp]
-    lib.delta_debug_set_trace.argtypes = [vp, vp]
+    lib.delta_internal_set_trace.argtypes = [vp, vp]   # development hook, not part of the C ABI
     lib.delta_coherence.argtypes = [vp, vp, vp, vp, vp]
     lib.delta_crossphase.argtypes = [vp, vp, vp, vp]
     lib.delta_crosspower.argtypes = [vp, vp, vp, vp]
@@ -202,8 +202,8 @@ class Plan:
                "delta_cross_spectra_unpack")
         return torch.view_as_complex(out)
 
-    def set_trace(self, buf):
-        _check(LIB.delta_debug_set_trace(self._h, None if buf is None else buf.data_ptr()), "delta_debug_set_trace")
+    def _set_trace(self, buf):
+        _check(LIB.delta_internal_set_trace(self._h, None if buf is None else buf.data_ptr()), "delta_internal_set_trace")
 
     def coherence(self, S, Sauto, G=None):
         G = torch.empty((self.sizes.P, self.sizes.F), dtype=torch.float32, device=self.device) if G is None else G

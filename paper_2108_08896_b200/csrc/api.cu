@@ -46,6 +46,12 @@ static int validate(const delta_config *c) {
   return DELTA_OK;
 }
 
+// bytes of an X buffer: the operand planes, then (tensor-core mode) the C per-channel scales
+static size_t x_buffer_bytes(const delta_plan *p) {
+  const size_t planes = (size_t)p->lay.x_scale_off;
+  return p->contraction == DELTA_CONTRACT_TC ? align_up(planes + (size_t)p->lay.C * sizeof(float), 16) : planes;
+}
+
 static bool tc_supported(const delta_config *c) {
   // two pipeline stages of 128*Cp bytes must fit in shared memory, and the tile plan must exist
   size_t Cp = align_up((size_t)c->n_channels, 64);
@@ -68,7 +74,7 @@ int delta_plan_create(const delta_config *cfg, delta_plan **out) {
   if (rc) return rc;
   if (cfg->contraction == DELTA_CONTRACT_TC && !tc_supported(cfg)) return DELTA_ERR_UNSUPPORTED;
   delta_plan *p = new (std::nothrow) delta_plan();
-  if (!p) return DELTA_ERR_INVALID_ARG;
+  if (!p) return DELTA_ERR_NO_MEMORY;
   p->cfg = *cfg;
   p->use_pdl = std::getenv("DELTA_NO_PDL") == nullptr;
   p->cfg.h_pairs = nullptr;
@@ -114,6 +120,8 @@ int delta_plan_create(const delta_config *cfg, delta_plan **out) {
   l.Poblk = (l.Po + l.PB - 1) / l.PB;
   // floats (2 parts) or halves (2 precisions x 2 parts) per frequency
   l.x_elems_per_f = (int64_t)(p->contraction == DELTA_CONTRACT_TC ? 4 : 2) * l.Kc * l.Cp * kSegBlock;
+  // TC mode: the C per-channel fp16 scales follow the operand planes inside the X buffer (a multiple of 16 bytes in)
+  l.x_scale_off = (int64_t)l.F * l.x_elems_per_f * (p->contraction == DELTA_CONTRACT_TC ? 2 : 4);
 
   // host tables in float64, rounded once
   const int L = l.L;
@@ -140,8 +148,6 @@ int delta_plan_create(const delta_config *cfg, delta_plan **out) {
   l.detrend = cfg->detrend;
   p->h_ftab.resize((size_t)fft_table_size(l.N) + 1);
   fft_twiddle_table(l.N, p->h_ftab.data());
-  p->h_ftab2.resize((size_t)fft_table_size(l.N, pair_fft_variant(l.N)) + 1);
-  fft_twiddle_table(l.N, p->h_ftab2.data(), pair_fft_variant(l.N));
   {
     const int E = pair_fft_points(l.N);  // E of the pair kernel's FFT geometry
     const int Tg = l.N / E;
@@ -168,19 +174,17 @@ int delta_plan_create(const delta_config *cfg, delta_plan **out) {
   w.off_tw = take((size_t)L * sizeof(float2));
   w.off_win = take((size_t)L * sizeof(float));
   w.off_ftab = take(p->h_ftab.size() * sizeof(float2));
-  w.off_ftab2 = take(p->h_ftab2.size() * sizeof(float2));
   w.off_pairs = take((p->h_pairs.size() + 1) * sizeof(ushort2));
   w.off_offs = take((size_t)l.C * sizeof(double));
   w.off_isum = take((size_t)l.C * sizeof(long long));
-  w.off_chscale = take((size_t)l.C * sizeof(float));
   w.off_chmax = take((size_t)l.C * sizeof(unsigned));
   w.off_chcnt = take((size_t)l.C * sizeof(unsigned));
-  w.off_X = take((size_t)l.F * l.x_elems_per_f * (p->contraction == DELTA_CONTRACT_TC ? 2 : 4));
+  w.off_X = take(x_buffer_bytes(p));
   w.off_S = take((size_t)(l.Pblk > 0 ? l.Pblk : 1) * l.F * l.PB * sizeof(float2));
   w.off_auto = take((size_t)l.C * l.F * sizeof(float));
-  w.off_rsq = take((size_t)l.C * l.Fp * sizeof(float));
+  w.off_rsq = take((size_t)4 * l.C * l.Fp * sizeof(float));  // four shifted copies (store_rsq4)
   w.off_wpart = take((size_t)l.C * l.nkb * sizeof(float));
-  w.off_rsum = take((size_t)l.C * sizeof(float));
+  w.off_rnorm = take((size_t)l.C * sizeof(float));
   w.total = o;
   *out = p;
   return DELTA_OK;
@@ -207,7 +211,7 @@ int delta_plan_sizes(const delta_plan *p, delta_sizes *out) {
   out->contraction = p->contraction;
   out->n_pairs = l.Po;
   out->workspace_bytes = (int64_t)p->wsl.total;
-  out->x_bytes = (int64_t)l.F * l.x_elems_per_f * (p->contraction == DELTA_CONTRACT_TC ? 2 : 4);
+  out->x_bytes = (int64_t)x_buffer_bytes(p);
   out->s_bytes = (int64_t)(l.Pblk > 0 ? l.Pblk : 1) * l.F * l.PB * (int64_t)sizeof(float2);
   out->s_block_pairs = l.PB;
   return DELTA_OK;
@@ -227,7 +231,6 @@ int delta_plan_set_workspace(delta_plan *p, void *d_ws, size_t bytes, void *stre
   DELTA_CUDA_CHECK(cudaMemcpyAsync(p->ws + p->wsl.off_tw, p->h_tw.data(), (size_t)l.L * sizeof(float2), cudaMemcpyHostToDevice, st));
   DELTA_CUDA_CHECK(cudaMemcpyAsync(p->ws + p->wsl.off_win, p->h_win.data(), (size_t)l.L * sizeof(float), cudaMemcpyHostToDevice, st));
   DELTA_CUDA_CHECK(cudaMemcpyAsync(p->ws + p->wsl.off_ftab, p->h_ftab.data(), p->h_ftab.size() * sizeof(float2), cudaMemcpyHostToDevice, st));
-  DELTA_CUDA_CHECK(cudaMemcpyAsync(p->ws + p->wsl.off_ftab2, p->h_ftab2.data(), p->h_ftab2.size() * sizeof(float2), cudaMemcpyHostToDevice, st));
   if (!p->h_pairs.empty())
     DELTA_CUDA_CHECK(cudaMemcpyAsync(p->ws + p->wsl.off_pairs, p->h_pairs.data(), p->h_pairs.size() * sizeof(ushort2), cudaMemcpyHostToDevice, st));
   // zero rows C..Cp-1 of the workspace X once (kernels never write them)
@@ -277,10 +280,9 @@ int delta_stft(delta_plan *p, const void *d_x, int64_t ld, void *d_X, void *stre
   if (rc) return rc;
   if (!aligned16(d_X)) return DELTA_ERR_ALIGNMENT;
   cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
-  if (p->lay.Cp != p->lay.C && d_X != p->d_X()) {
-    delta_sizes sz;
-    delta_plan_sizes(p, &sz);
-    DELTA_CUDA_CHECK(cudaMemsetAsync(d_X, 0, (size_t)sz.x_bytes, st));
+  if (d_X != p->d_X()) {  // the padding of the layout is read by the contraction: zero it in a caller's buffer
+    rc = launch_stft_pad_zero(p, d_X, st);
+    if (rc) return rc;
   }
   return launch_stft(p, d_x, ld, d_X, st);
 }
@@ -292,7 +294,10 @@ int delta_cross_spectra_unpack(delta_plan *p, const float *d_S, float *d_out, vo
   return launch_s_unpack(p, d_S, d_out, reinterpret_cast<cudaStream_t>(stream));
 }
 
-int delta_debug_set_trace(delta_plan *p, void *d_trace) {
+// Development hook, not part of the C ABI (not declared in include/delta.h): while d_trace (>= 8192 int64) is set, CTA 0 of
+// the tensor-core contraction writes SM clock stamps of its producer / MMA / epilogue roles and every CTA its start and
+// end time (contract_tc.cu).
+int delta_internal_set_trace(delta_plan *p, void *d_trace) {
   if (!p) return DELTA_ERR_INVALID_ARG;
   p->d_trace = reinterpret_cast<long long *>(d_trace);
   return DELTA_OK;
@@ -305,9 +310,12 @@ int delta_stft_unpack(delta_plan *p, const void *d_X, float *d_out, void *stream
   return launch_stft_unpack(p, d_X, d_out, reinterpret_cast<cudaStream_t>(stream));
 }
 
-static int contract(delta_plan *p, const void *d_X, float *d_S, float *d_auto, cudaStream_t st) {
-  return p->contraction == DELTA_CONTRACT_TC ? launch_contract_tc(p, d_X, d_S, d_auto, p->d_rsq(), st)
-                                             : launch_contract_fp32(p, d_X, d_S, d_auto, p->d_rsq(), st);
+// d_rsq / d_rnorm: the plan's tables for the pair stage of the fused call; null for the staged delta_cross_spectra,
+// which is a function of its arguments only
+static int contract(delta_plan *p, const void *d_X, float *d_S, float *d_auto, float *d_rsq, float *d_rnorm, cudaStream_t st) {
+  const float rscale = (float)p->lay.L * p->s2 / (float)p->lay.K;  // sum over all L bins of S_cc = rscale * sum_k wpart[c][k]
+  return p->contraction == DELTA_CONTRACT_TC ? launch_contract_tc(p, d_X, d_S, d_auto, d_rsq, d_rnorm, rscale, st)
+                                             : launch_contract_fp32(p, d_X, d_S, d_auto, d_rsq, d_rnorm, rscale, st);
 }
 
 int delta_cross_spectra(delta_plan *p, const void *d_X, float *d_S, float *d_Sauto, void *stream) {
@@ -316,7 +324,7 @@ int delta_cross_spectra(delta_plan *p, const void *d_X, float *d_S, float *d_Sau
   if (!d_X) return DELTA_ERR_INVALID_ARG;
   if (!aligned16(d_X) || (d_S && !aligned16(d_S))) return DELTA_ERR_ALIGNMENT;
   if (!d_S && !d_Sauto) return DELTA_OK;
-  return contract(p, d_X, d_S, d_Sauto, reinterpret_cast<cudaStream_t>(stream));
+  return contract(p, d_X, d_S, d_Sauto, nullptr, nullptr, reinterpret_cast<cudaStream_t>(stream));
 }
 
 static int pair_stage(delta_plan *p, const float *d_S, const float *d_Sauto, float *G, float *A, float *P, float *R,
@@ -327,11 +335,11 @@ static int pair_stage(delta_plan *p, const float *d_S, const float *d_Sauto, flo
   if (!G && !A && !P && !R) return DELTA_ERR_INVALID_ARG;
   if (!aligned16(d_S)) return DELTA_ERR_ALIGNMENT;
   cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
-  if (need_auto) {  // coherence and rho need 1/sqrt(S_cc[f]) of the caller's autospectra
-    rc = launch_auto_prep(p, d_Sauto, p->d_rsq(), p->d_rsum(), st);
+  if (need_auto) {  // coherence and rho need 1/sqrt(S_cc[f]) and 1/sqrt(R_cc[0]) of the caller's autospectra (plan scratch)
+    rc = launch_auto_prep(p, d_Sauto, p->d_rsq(), p->d_rnorm(), st);
     if (rc) return rc;
   }
-  return launch_pair(p, d_S, p->d_rsq(), p->d_rsum(), 1, 1, 1.f, G, A, P, R, st);
+  return launch_pair(p, d_S, p->d_rsq(), p->d_rnorm(), G, A, P, R, st);
 }
 
 int delta_coherence(delta_plan *p, const float *d_S, const float *d_Sauto, float *d_G, void *stream) {
@@ -383,18 +391,16 @@ int delta_analyze_chunk(delta_plan *p, const void *d_x, int64_t ld, float *d_G, 
   if (ev) DELTA_CUDA_CHECK(cudaEventRecord(p->stage_ev[1], st));
   float *au = d_Sauto ? d_Sauto : p->d_auto();
   const bool pairs_wanted = (d_G || d_A || d_P || d_R) && p->lay.Po > 0;
-  rc = contract(p, p->d_X(), pairs_wanted ? p->d_S() : nullptr, au, st);
+  rc = contract(p, p->d_X(), pairs_wanted ? p->d_S() : nullptr, au, p->d_rsq(), (pairs_wanted && !p->band_on) ? p->d_rnorm() : nullptr, st);
   if (rc) return rc;
   if (ev) DELTA_CUDA_CHECK(cudaEventRecord(p->stage_ev[2], st));
   // zero-lag autocorrelations for rho come from the windowed signal energy the STFT kernel left in wpart (Parseval);
   // with the band-pass filter on, from the filtered autospectra
   if (pairs_wanted && p->band_on) {
-    rc = launch_auto_prep(p, au, p->d_rsq(), p->d_rsum(), st);
+    rc = launch_auto_prep(p, au, p->d_rsq(), p->d_rnorm(), st);
     if (rc) return rc;
-    rc = launch_pair(p, p->d_S(), p->d_rsq(), p->d_rsum(), 1, 1, 1.f, d_G, d_A, d_P, d_R, st);
-  } else if (pairs_wanted)
-    rc = launch_pair(p, p->d_S(), p->d_rsq(), p->d_wpart(), p->lay.nkb, p->lay.nkb, (float)p->lay.L * p->s2 / (float)p->lay.K,
-                     d_G, d_A, d_P, d_R, st);
+  }
+  if (pairs_wanted) rc = launch_pair(p, p->d_S(), p->d_rsq(), p->d_rnorm(), d_G, d_A, d_P, d_R, st);
   if (rc) return rc;
   if (ev) DELTA_CUDA_CHECK(cudaEventRecord(p->stage_ev[3], st));
   return rc;
@@ -479,6 +485,7 @@ const char *delta_strerror(int status) {
     case DELTA_ERR_NO_WORKSPACE: return "workspace missing or too small";
     case DELTA_ERR_CUDA: return "CUDA runtime error (see delta_last_cuda_error)";
     case DELTA_ERR_STATE: return "call sequence error (offsets not set)";
+    case DELTA_ERR_NO_MEMORY: return "host memory allocation failed";
     default: return "unknown status";
   }
 }

@@ -9,11 +9,21 @@ namespace delta {
 // S_ij = scale * sum_k (a_i + i b_i)(a_j - i b_j) = scale * [ (a_i a_j + b_i b_j) + i (b_i a_j - a_i b_j) ]
 __global__ void __launch_bounds__(kThreads)
 contract_fp32_kernel(const float *__restrict__ X, Layout lay, float scale, float2 *__restrict__ S,
-                     float *__restrict__ Sauto, float *__restrict__ Srsq) {
+                     float *__restrict__ Sauto, float *__restrict__ Srsq, const float *__restrict__ wpart, float rscale,
+                     float *__restrict__ rnorm) {
   constexpr int KT = 32;  // segments per shared-memory stage
   __shared__ __align__(16) float As[2][KT][kPairTile];
   __shared__ __align__(16) float Bs[2][KT][kPairTile];
   const int f = blockIdx.y;
+  if (rnorm && blockIdx.x == 0 && blockIdx.y == 0) {
+    // 1/sqrt(L R_cc[0]) for the normalisation of rho, from the windowed signal energy (Parseval, pin P4): fixed order
+    for (int c = threadIdx.x; c < lay.C; c += kThreads) {
+      float sum = 0.f;
+      for (int k = 0; k < lay.nkb; ++k) sum += wpart[(int64_t)c * lay.nkb + k];
+      sum *= rscale;
+      rnorm[c] = sum > 0.f ? rsqrtf(sum) : 0.f;
+    }
+  }
   int bi = 0, rem = blockIdx.x;
   const int nb = (lay.C + kPairTile - 1) / kPairTile;
   while (rem >= nb - bi) { rem -= nb - bi; ++bi; }
@@ -82,18 +92,20 @@ contract_fp32_kernel(const float *__restrict__ X, Layout lay, float scale, float
       } else if (i == j) {
         const float v = acc_re[a][b] * scale;
         if (Sauto) Sauto[(int64_t)i * lay.F + f] = v;
-        if (Srsq) Srsq[(int64_t)i * lay.Fp + f] = v > 0.f ? rsqrtf(v) : 0.f;
+        if (Srsq) store_rsq4(Srsq, lay, i, f, v > 0.f ? rsqrtf(v) : 0.f);
       }
     }
   }
 }
 
-int launch_contract_fp32(delta_plan *p, const void *d_X, float *d_S, float *d_auto, float *d_rsq, cudaStream_t st) {
+int launch_contract_fp32(delta_plan *p, const void *d_X, float *d_S, float *d_auto, float *d_rsq, float *d_rnorm, float rscale,
+                         cudaStream_t st) {
   const Layout &lay = p->lay;
   const int nb = (lay.C + kPairTile - 1) / kPairTile;
   dim3 grid(nb * (nb + 1) / 2, lay.F);
   contract_fp32_kernel<<<grid, kThreads, 0, st>>>(reinterpret_cast<const float *>(d_X), lay, p->s2 / (float)lay.K,
-                                                  reinterpret_cast<float2 *>(d_S), d_auto, d_rsq);
+                                                  reinterpret_cast<float2 *>(d_S), d_auto, d_rsq, (const float *)p->d_wpart(), rscale,
+                                                  d_rnorm);
   p->launches++;
   DELTA_CUDA_CHECK(cudaGetLastError());
   return DELTA_OK;

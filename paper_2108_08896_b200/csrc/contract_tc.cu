@@ -94,6 +94,12 @@ __device__ __forceinline__ void tmem_ld16(uint32_t taddr, float *v) {
 #pragma unroll
   for (int q = 0; q < 16; ++q) v[q] = __uint_as_float(r[q]);
 }
+// predicated 8-byte global store (no branch: see the epilogue)
+__device__ __forceinline__ void st_pred_f2(float2 *p, float a, float b, bool pred) {
+  asm volatile("{\n\t.reg .pred q;\n\tsetp.ne.b32 q, %3, 0;\n\t@q st.global.v2.f32 [%0], {%1, %2};\n\t}" ::"l"(p), "f"(a), "f"(b),
+               "r"((int)pred)
+               : "memory");
+}
 __device__ __forceinline__ bool elect_one() {
   uint32_t pred;
   asm volatile("{\n\t.reg .pred p;\n\telect.sync _|p, 0xffffffff;\n\tselp.u32 %0, 1, 0, p;\n\t}" : "=r"(pred));
@@ -128,8 +134,9 @@ struct TcParams {
 
 template <bool TRACE>
 __global__ void __launch_bounds__(kTcThreads, 1)
-contract_tc_kernel(const __half *__restrict__ X, Layout lay, TcParams prm, float scale, const float *__restrict__ chscale,
-                   float2 *__restrict__ S, float *__restrict__ Sauto, float *__restrict__ Srsq, long long *trace) {
+contract_tc_kernel(const __half *__restrict__ X, Layout lay, TcParams prm, float scale, float2 *__restrict__ S,
+                   float *__restrict__ Sauto, float *__restrict__ Srsq, const float *__restrict__ wpart, float rscale,
+                   float *__restrict__ rnorm, long long *trace) {
   extern __shared__ __align__(1024) unsigned char smem_raw[];
   unsigned char *stages = smem_raw;
   // itab[c] = {rowbase(c) = c C - c(c+1)/2 - c - 1 (int bits), 1/chscale[c]}: pair index p(i, j) = rowbase(i) + j
@@ -162,7 +169,18 @@ contract_tc_kernel(const __half *__restrict__ X, Layout lay, TcParams prm, float
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
   }
   pdl_launch_dependents();
-  pdl_wait();  // X and chscale come from the STFT kernel; S, Sauto, Srsq of the previous chunk are still being read
+  pdl_wait();  // X (with its scales) comes from the STFT kernel; S, Sauto, Srsq of the previous chunk are still being read
+  // the per-channel fp16 scales travel with the operands: C floats behind the planes of the X buffer
+  const float *chscale = reinterpret_cast<const float *>(reinterpret_cast<const char *>(X) + lay.x_scale_off);
+  if (rnorm && blockIdx.x == gridDim.x - 1) {
+    // 1/sqrt(L R_cc[0]) for the normalisation of rho, from the windowed signal energy (Parseval, pin P4): fixed order
+    for (int c = tid; c < lay.C; c += kTcThreads) {
+      float sum = 0.f;
+      for (int k = 0; k < lay.nkb; ++k) sum += wpart[(int64_t)c * lay.nkb + k];
+      sum *= rscale;
+      rnorm[c] = sum > 0.f ? rsqrtf(sum) : 0.f;
+    }
+  }
   for (int c = tid; c < lay.Cp; c += kTcThreads)
     itab[c] = make_float2(__int_as_float(c * lay.C - (c * (c + 1)) / 2 - c - 1), (c < lay.C) ? 1.f / chscale[c] : 0.f);
   fence_before();
@@ -352,13 +370,18 @@ contract_tc_kernel(const __half *__restrict__ X, Layout lay, TcParams prm, float
             tmem_ld16(tmem_base + lane_addr + (uint32_t)(un.tm + un.N + c0), im);
             asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
             if (S) {
+              // All 16 table reads, then all 16 addresses, then 16 predicated stores: the stores are inline PTX so
+              // that the compiler cannot turn the predicate into a branch around each element (it did, and every
+              // element then waited for its own shared-memory read: 2,000 cycles per 16 columns).
+              float2 t[16];
+#pragma unroll
+              for (int e = 0; e < 16; ++e) t[e] = itab[ibase + e];  // {rowbase(i) as int bits, 1/scale_i}
 #pragma unroll
               for (int e = 0; e < 16; ++e) {
-                const float2 t = itab[ibase + e];          // {rowbase(i) as int bits, 1/scale_i}
-                const int p = __float_as_int(t.x) + j;     // lexicographic pair index of (i, j)
-                const float sc = sj * t.y;
+                const int p = __float_as_int(t[e].x) + j;  // lexicographic pair index of (i, j)
+                const float sc = sj * t[e].y;
                 const int off = (p >> lay.pb_shift) * blk_stride + ((p ^ fx) & pb_mask);
-                if (ibase + e < j && jok) Sf[off] = make_float2(re[e] * sc, im[e] * sc);
+                st_pred_f2(Sf + off, re[e] * sc, im[e] * sc, (ibase + e < j) && jok);
               }
             }
             if (ibase + 15 >= jw0) {  // this chunk crosses the diagonal: autospectrum of channel j
@@ -368,7 +391,7 @@ contract_tc_kernel(const __half *__restrict__ X, Layout lay, TcParams prm, float
               if (j >= ibase && j < ibase + 16 && jok) {
                 a *= sj * itab[j].y;
                 if (Sauto) Sauto[(int64_t)j * F + f] = a;
-                if (Srsq) Srsq[(int64_t)j * lay.Fp + f] = a > 0.f ? rsqrtf(a) : 0.f;
+                if (Srsq) store_rsq4(Srsq, lay, j, f, a > 0.f ? rsqrtf(a) : 0.f);
               }
             }
           }
@@ -429,7 +452,8 @@ bool tc_plan_tiles(int Cp, TcHostPlan *out) {
   return true;
 }
 
-int launch_contract_tc(delta_plan *p, const void *d_X, float *d_S, float *d_auto, float *d_rsq, cudaStream_t st) {
+int launch_contract_tc(delta_plan *p, const void *d_X, float *d_S, float *d_auto, float *d_rsq, float *d_rnorm, float rscale,
+                       cudaStream_t st) {
   const Layout &lay = p->lay;
   TcParams prm;
   memset(&prm, 0, sizeof(prm));
@@ -470,14 +494,15 @@ int launch_contract_tc(delta_plan *p, const void *d_X, float *d_S, float *d_auto
     if (rc) return rc;
     LaunchCfg lc(dim3(grid), dim3(kTcThreads), smem, st, p->use_pdl);
     DELTA_CUDA_CHECK(cudaLaunchKernelEx(&lc.cfg, contract_tc_kernel<true>, reinterpret_cast<const __half *>(d_X), lay, prm, scale,
-                                        (const float *)p->d_chscale(), reinterpret_cast<float2 *>(d_S), d_auto, d_rsq, p->d_trace));
+                                        reinterpret_cast<float2 *>(d_S), d_auto, d_rsq, (const float *)p->d_wpart(), rscale,
+                                        d_rnorm, p->d_trace));
   } else {
     int rc = opt_in_smem(contract_tc_kernel<false>, smem);
     if (rc) return rc;
     LaunchCfg lc(dim3(grid), dim3(kTcThreads), smem, st, p->use_pdl);
     DELTA_CUDA_CHECK(cudaLaunchKernelEx(&lc.cfg, contract_tc_kernel<false>, reinterpret_cast<const __half *>(d_X), lay, prm, scale,
-                                        (const float *)p->d_chscale(), reinterpret_cast<float2 *>(d_S), d_auto, d_rsq,
-                                        (long long *)nullptr));
+                                        reinterpret_cast<float2 *>(d_S), d_auto, d_rsq, (const float *)p->d_wpart(), rscale,
+                                        d_rnorm, (long long *)nullptr));
   }
   p->launches++;
   DELTA_CUDA_CHECK(cudaGetLastError());

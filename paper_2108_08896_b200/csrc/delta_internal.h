@@ -23,17 +23,10 @@ struct TcHostPlan {
 };
 bool tc_plan_tiles(int Cp, TcHostPlan *out);
 
-// pairs per block of the S layout = pairs per CTA of the pair kernel (its S tile must fit shared memory)
-// FFT geometry variant of the pair kernel (fft_reg.cuh): narrow (8 points per thread, one warp per pair) where it exists
-#ifndef DELTA_PAIR_NARROW
-#define DELTA_PAIR_NARROW 0  // measured on B200: 35.6 us (narrow, 48 warps/SM) against 34.3 us (wide, 32 warps/SM) at config 2
-#endif
-constexpr int pair_fft_variant(int N) { return (DELTA_PAIR_NARROW && N == 256) ? 1 : 0; }
-constexpr int pair_fft_points(int N) { return (N <= 64 || pair_fft_variant(N) == 1) ? 8 : 16; }  // E of that geometry
-#ifndef DELTA_PB_SMALL
-#define DELTA_PB_SMALL 16
-#endif
-constexpr int pair_block(int L) { return L <= 512 ? DELTA_PB_SMALL : (L <= 1024 ? 16 : (L == 2048 ? 8 : 4)); }
+// pairs per block of the S layout = pairs per tile of the pair kernel (two tiles and the exchange buffers must fit
+// shared memory).  8 or 32 pairs per tile instead of 16 were measured slower at nfft 512 (round 1).
+constexpr int pair_block(int L) { return L <= 1024 ? 16 : (L == 2048 ? 8 : 4); }
+constexpr int pair_fft_points(int N) { return N <= 64 ? 8 : 16; }  // E of FftGeom<N> (fft_reg.cuh)
 
 struct Layout {
   // X (STFT) buffer, frequency-major so that one bin's C x K matrix is one contiguous block:
@@ -42,7 +35,8 @@ struct Layout {
   // k = 8*kc + kk, c < Cp (rows C..Cp-1 are zero), kc < Kc = Kp/8, Kp = K rounded up to 16.
   int C, Cp, T, L, N, H, K, Kp, Kc, F, M, nlags;
   int Ls;   // samples per segment (nperseg <= L; the rest of the transform's input is zero)
-  int Fp;   // row pitch of the rsq table: F rounded up to 4 floats (rows are 16-byte aligned bulk-copy sources)
+  int Fp;   // row pitch of the rsq table: F rounded up to 4 floats
+  int64_t x_scale_off;  // TC mode: byte offset of the C per-channel fp16 scales (float) behind the operand planes of an X buffer
   float wsum;      // sum_n |w[n]|: |X| <= wsum max|y| bounds the split-fp16 operands
   int detrend;     // DELTA_DETREND_*
   int estimator;   // DELTA_EST_*
@@ -67,8 +61,19 @@ __host__ __device__
 constexpr int s_swz(int f) { return f ^ (f >> 2); }
 
 struct Workspace {
-  size_t off_tw, off_win, off_ftab, off_ftab2, off_pairs, off_offs, off_isum, off_chscale, off_chmax, off_chcnt, off_X, off_S, off_auto, off_rsq, off_wpart, off_rsum, total;
+  size_t off_tw, off_win, off_ftab, off_pairs, off_offs, off_isum, off_chmax, off_chcnt, off_X, off_S, off_auto, off_rsq, off_wpart, off_rnorm, total;
 };
+
+// The table of 1/sqrt(S_cc[f]) is kept as four shifted copies, float rsq4[4][C][Fp]: copy s holds bin f at index f - s
+// (f >= s).  The float4 groups of an output row start at bin f0 = (-p) mod 4 (pair.cu), and copy f0 makes the matching
+// float4 reads of the table 16-byte aligned.  Copy 0 is the plain table.
+#if defined(__CUDACC__)
+__device__ __forceinline__ void store_rsq4(float *rsq4, const Layout &lay, int c, int f, float v) {
+#pragma unroll
+  for (int s = 0; s < 4; ++s)
+    if (f >= s) rsq4[((int64_t)s * lay.C + c) * lay.Fp + (f - s)] = v;
+}
+#endif
 
 }  // namespace delta
 
@@ -83,7 +88,6 @@ struct delta_plan {
   std::vector<float> h_win;      // periodic Hann
   float2 h_wstep[16];            // e^{-2 pi i T u / L}, u < E: bin f = gt + T u of a thread has twiddle tw[gt] * wstep[u]
   std::vector<float2> h_ftab;    // per-pass twiddles of the register FFT (fft_reg.cuh), N = L/2
-  std::vector<float2> h_ftab2;   // the same for the pair kernel's geometry variant
   std::vector<ushort2> h_pairs;  // the explicit pair list (empty: all pairs)
   delta::TcHostPlan tc;
   int num_sms = 148;
@@ -108,11 +112,9 @@ struct delta_plan {
   const float2 *d_tw() const { return reinterpret_cast<const float2 *>(ws + wsl.off_tw); }
   const float *d_win() const { return reinterpret_cast<const float *>(ws + wsl.off_win); }
   const float2 *d_ftab() const { return reinterpret_cast<const float2 *>(ws + wsl.off_ftab); }
-  const float2 *d_ftab2() const { return reinterpret_cast<const float2 *>(ws + wsl.off_ftab2); }
   const ushort2 *d_pairs() const { return reinterpret_cast<const ushort2 *>(ws + wsl.off_pairs); }
   double *d_offs() const { return reinterpret_cast<double *>(ws + wsl.off_offs); }
   long long *d_isum() const { return reinterpret_cast<long long *>(ws + wsl.off_isum); }
-  float *d_chscale() const { return reinterpret_cast<float *>(ws + wsl.off_chscale); }
   unsigned *d_chmax() const { return reinterpret_cast<unsigned *>(ws + wsl.off_chmax); }  // zero between launches
   unsigned *d_chcnt() const { return reinterpret_cast<unsigned *>(ws + wsl.off_chcnt); }  // zero between launches
   void *d_X() const { return ws + wsl.off_X; }
@@ -122,8 +124,9 @@ struct delta_plan {
   // wpart[c][kb] = sum over the 8 segments of block kb of sum_n (w[n] y_c[kH+n])^2  (written by stft_kernel);
   // by Parseval  sum over all L bins of S_cc = L s^2/K * sum_kb wpart[c][kb] = L R_cc[0]   (pin P4)
   float *d_wpart() const { return reinterpret_cast<float *>(ws + wsl.off_wpart); }
-  // rsum[c] = sum over all L bins of caller-supplied autospectra (staged calls; auto_prep_kernel)
-  float *d_rsum() const { return reinterpret_cast<float *>(ws + wsl.off_rsum); }
+  // rnorm[c] = 1/sqrt(sum over all L bins of S_cc) = 1/sqrt(L R_cc[0]): from wpart (contraction kernels, fused call) or
+  // from caller-supplied autospectra (auto_prep_kernel, staged calls)
+  float *d_rnorm() const { return reinterpret_cast<float *>(ws + wsl.off_rnorm); }
 };
 
 namespace delta {
@@ -201,14 +204,17 @@ static inline int opt_in_smem(Kern kern, size_t bytes) {
 // launchers (each returns a delta_status and counts its launches into plan->launches)
 int launch_offsets(delta_plan *p, const void *d_x, int64_t ld, int n_first, cudaStream_t st);
 int launch_stft(delta_plan *p, const void *d_x, int64_t ld, void *d_X, cudaStream_t st);
+int launch_stft_pad_zero(delta_plan *p, void *d_X, cudaStream_t st);  // zero padding of a caller-supplied X buffer
 int launch_stft_unpack(delta_plan *p, const void *d_X, float *d_out, cudaStream_t st);
-// both contractions write S (may be null), the autospectra and 1/sqrt(autospectra) (either may be null)
-int launch_contract_fp32(delta_plan *p, const void *d_X, float *d_S, float *d_auto, float *d_rsq, cudaStream_t st);
-int launch_contract_tc(delta_plan *p, const void *d_X, float *d_S, float *d_auto, float *d_rsq, cudaStream_t st);
-int launch_auto_prep(delta_plan *p, const float *d_auto, float *d_rsq, float *d_rsum, cudaStream_t st);
-// rpart/nrp/rp_stride/rscale: sum over all L bins of S_cc = rscale * sum_{k<nrp} rpart[c * rp_stride + k]
-int launch_pair(delta_plan *p, const float *d_S, const float *d_rsq, const float *rpart, int nrp, int rp_stride, float rscale,
-                float *d_G, float *d_A, float *d_P, float *d_R, cudaStream_t st);
+// Both contractions write S (may be null), the autospectra and the rsq4 table (either may be null), and, if d_rnorm is
+// not null, rnorm[c] = 1/sqrt(rscale * sum_k wpart[c][k]) from the STFT kernel's energy partials.
+int launch_contract_fp32(delta_plan *p, const void *d_X, float *d_S, float *d_auto, float *d_rsq, float *d_rnorm, float rscale,
+                         cudaStream_t st);
+int launch_contract_tc(delta_plan *p, const void *d_X, float *d_S, float *d_auto, float *d_rsq, float *d_rnorm, float rscale,
+                       cudaStream_t st);
+int launch_auto_prep(delta_plan *p, const float *d_auto, float *d_rsq, float *d_rnorm, cudaStream_t st);
+int launch_pair(delta_plan *p, const float *d_S, const float *d_rsq, const float *d_rnorm, float *d_G, float *d_A, float *d_P,
+                float *d_R, cudaStream_t st);
 int launch_axpby(delta_plan *p, float *acc, const float *x, int64_t n, float wa, float wn, cudaStream_t st);
 int launch_s_unpack(delta_plan *p, const float *d_S, float *d_out, cudaStream_t st);
 

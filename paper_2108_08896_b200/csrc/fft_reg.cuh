@@ -133,24 +133,34 @@ DELTA_FFT_GEOM(256, 1, 8, 3, 8, 8, 4)
 #undef DELTA_FFT_GEOM
 
 DELTA_HD int fft_pad(int i) { return i + (i >> 4); }
+// Exchange maps.  An element index always splits into a thread-dependent part e_t and a compile-time part e_c that occupy
+// disjoint bits (e = e_t + e_c = e_t | e_c); a map turns e_t into a handle once (`pre`) and then addresses element
+// e_t + e_c from the handle and e_c (`at`), so that the compile-time part folds into an immediate.
 struct FftPadMap {
-  float2 *buf;  // FftGeom<N>::BUF entries
-  DELTA_HD float2 &operator()(int e) const { return buf[fft_pad(e)]; }
+  float2 *buf;  // FftGeom<N>::BUF entries, private to the group
+  typedef int Handle;
+  DELTA_HD Handle pre(int e_t) const { return e_t; }
+  DELTA_HD float2 &at(Handle h, int e_c) const { return buf[fft_pad(h + e_c)]; }
 };
 
 DELTA_HD float2 fft_ld_tw(const float2 *p) {
 #ifdef __CUDA_ARCH__
-  return __ldg(p);
+  return *p;  // shared memory or global memory; the callers keep the tables in shared memory
 #else
   return *p;
 #endif
 }
 
-// One pass.  LAST: results stay in registers (natural order, see header); otherwise they go to `buf`.
+// One pass.  LAST: results stay in registers (natural order, see header); otherwise they go through the map.
+// Butterfly b = tid + T i: with S | T the thread part of its output index is  (tid mod S) + S R (tid / S)  and the
+// compile-time part  R T i + S k.
 template <class G, int R, int S, bool LAST, bool INV, class Map>
 DELTA_HD void fft_pass(float2 *v, const Map &m, const float2 *tp, int tid) {
   constexpr int N = G::N;
   constexpr int NB = G::E / R, CNT = N / (R * S);
+  static_assert(LAST || G::T % S == 0, "the stride of a pass must divide the group size");
+  const int r_t = tid / S;
+  const typename Map::Handle h = m.pre((tid & (S - 1)) + S * R * r_t);
 #pragma unroll
   for (int i = 0; i < NB; ++i) {
     float2 a[R];
@@ -161,8 +171,7 @@ DELTA_HD void fft_pass(float2 *v, const Map &m, const float2 *tp, int tid) {
 #pragma unroll
       for (int k = 0; k < R; ++k) v[i + NB * k] = a[k];
     } else {
-      const int b = tid + G::T * i;
-      const int q = b & (S - 1), r = b / S;
+      const int r = r_t + (G::T / S) * i;
 #pragma unroll
       for (int k = 1; k < R; ++k) {
         float2 w = fft_ld_tw(tp + (k - 1) * CNT + r);
@@ -170,15 +179,16 @@ DELTA_HD void fft_pass(float2 *v, const Map &m, const float2 *tp, int tid) {
         a[k] = cmul(a[k], w);
       }
 #pragma unroll
-      for (int k = 0; k < R; ++k) m(q + S * (R * r + k)) = a[k];
+      for (int k = 0; k < R; ++k) m.at(h, R * G::T * i + S * k) = a[k];
     }
   }
 }
 
 template <class G, class Map>
 DELTA_HD void fft_readback(float2 *v, const Map &m, int tid) {
+  const typename Map::Handle h = m.pre(tid);
 #pragma unroll
-  for (int u = 0; u < G::E; ++u) v[u] = m(tid + G::T * u);
+  for (int u = 0; u < G::E; ++u) v[u] = m.at(h, G::T * u);
 }
 
 #ifdef __CUDACC__
@@ -188,28 +198,40 @@ template <int T>
 __device__ __forceinline__ void fft_group_sync() {
   if (T <= 32) __syncwarp(); else __syncthreads();
 }
+template <int T>
+struct FftCtaSync {
+  static __device__ __forceinline__ void sync() { fft_group_sync<T>(); }
+};
+// The same for a kernel whose CTA also holds warps that do not take part (a producer warp): groups wider than a warp
+// meet at named barrier ID with NT participating threads (all the transform threads of the CTA).
+template <int T, int ID, int NT>
+struct FftNamedSync {
+  static __device__ __forceinline__ void sync() {
+    if (T <= 32) __syncwarp(); else asm volatile("bar.sync %0, %1;" ::"n"(ID), "n"(NT) : "memory");
+  }
+};
 
 // v[u] <-> x[tid + T*u] in, X[tid + T*u] out (unnormalised).  The slots behind `m` are shared memory owned
 // by the group; other threads of the group may still be reading them when the call returns, so the group
-// must pass another fft_group_sync before it writes them again.
-template <class G, bool INV, class Map>
+// must pass another Sync::sync() before it writes them again.
+template <class G, bool INV, class Sync, class Map>
 __device__ __forceinline__ void fft_inplace_g(float2 *v, const Map &m, const float2 *__restrict__ tp, int tid) {
   fft_pass<G, G::R0, 1, false, INV>(v, m, tp, tid);
-  fft_group_sync<G::T>();
+  Sync::sync();
   fft_readback<G>(v, m, tid);
   if constexpr (G::NP == 2) {
     fft_pass<G, G::R1, G::R0, true, INV>(v, m, tp, tid);
   } else {
-    fft_group_sync<G::T>();
+    Sync::sync();
     fft_pass<G, G::R1, G::R0, false, INV>(v, m, tp + G::OFF1, tid);
-    fft_group_sync<G::T>();
+    Sync::sync();
     fft_readback<G>(v, m, tid);
     fft_pass<G, G::R2, G::R0 * G::R1, true, INV>(v, m, tp, tid);
   }
 }
 template <int N, bool INV, class Map>
 __device__ __forceinline__ void fft_inplace(float2 *v, const Map &m, const float2 *__restrict__ tp, int tid) {
-  fft_inplace_g<FftGeom<N, 0>, INV>(v, m, tp, tid);
+  fft_inplace_g<FftGeom<N, 0>, INV, FftCtaSync<FftGeom<N, 0>::T>>(v, m, tp, tid);
 }
 #endif
 

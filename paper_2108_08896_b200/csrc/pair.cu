@@ -4,13 +4,16 @@
 //   auto_prep_kernel  1/sqrt(S_cc[f]) from caller-supplied autospectra (staged calls only)
 //   s_unpack_kernel   test accessor: S layout -> complex64 [P][F]
 //
-// One CTA owns one block of PB consecutive (lexicographic) pairs, i.e. one contiguous [F][PB] tile of S and one
-// contiguous run of rows in each output array.  The tile arrives with a single cp.async.bulk copy.  Every pair
-// has a group of T = N/E threads; thread gt of the group owns the bins f = gt + T u (u < E), which is exactly the
-// register layout the inverse FFT of fft_reg.cuh starts from.  Each S value is therefore read from shared memory
-// once for G, A, P (stored straight away, 16 lanes = 64 contiguous bytes per row) and for the merge step of the
-// inverse real transform; the transform exchanges through a private padded buffer that aliases the (by then
-// dead) tile, ends in registers in natural order, and rho is stored from registers as float2.
+// pair_kernel is persistent: a CTA walks over blocks of PB consecutive (lexicographic) pairs.  One block is one
+// contiguous [F][PB] tile of S and one contiguous run of rows in each output array.  A producer warp brings tile n+1
+// into the second stage of a two-stage ring with one cp.async.bulk copy (and works out the pairs' channels and their
+// rho normalisation) while the compute warps work on tile n; the only CTA-wide synchronisation is the ring's full /
+// empty mbarrier pair.  Every pair has a group of T = N/E threads (for L <= 1024 inside one warp, so warps run free of
+// each other and their store-bound and arithmetic-bound phases overlap on the SM):
+//   pass 1  a thread owns 4 consecutive bins per step: |S| (cross-power), |S|/sqrt(S_ii S_jj), atan2; float4 stores
+//   pass 2  thread gt owns bins f = gt + T u (u < E), the register layout the inverse FFT of fft_reg.cuh starts from:
+//           merge step of the inverse real transform, register FFT through a private padded exchange buffer,
+//           rho stored from registers as float2.
 #include "delta_internal.h"
 #include "fft_reg.cuh"
 
@@ -24,32 +27,65 @@ struct PairConsts {
   float2 wstep[16];  // e^{-2 pi i T u / L}
 };
 
+constexpr size_t kSmemPerSm = 227 * 1024;
+
 template <int L>
 struct PairCfg {
   static constexpr int N = L / 2, F = N + 1;
-  using G = FftGeom<N, pair_fft_variant(N)>;
+  using G = FftGeom<N, 0>;
   static constexpr int T = G::T, E = G::E;
   static constexpr int PB = pair_block(L);
-  static constexpr int THREADS = PB * T;
-  // resident warps per SM the register budget is sized for: 48 (40 registers) with 8 points per thread, else 32 (64)
-#ifndef DELTA_PAIR_WARPS
-#define DELTA_PAIR_WARPS 32
-#endif
-  static constexpr int WARPS = E <= 8 ? 48 : DELTA_PAIR_WARPS;
-  static constexpr int MIN_CTAS = (WARPS * 32) / THREADS > 0 ? (WARPS * 32) / THREADS : 1;
+  static constexpr int FP = (F + 3) & ~3;  // pitch of the rsq table
+  static constexpr int TTHREADS = PB * T;  // threads of a team: one group of T per pair of a tile
+  static constexpr int TW = TTHREADS / 32; // warps of a team
+  // The inverse transform of a pair exchanges through the pair's own (by then dead) column of the tile where the tile has
+  // 16 pairs per row (FftTileMap); the narrower tiles of the long transforms use private padded buffers, and their
+  // 1/sqrt(S_jj) rows come from global memory instead of the slot.
+  static constexpr bool IN_TILE = PB == 16;
+  static constexpr bool ROWS = IN_TILE;
   static constexpr size_t TILE_BYTES = (size_t)F * PB * sizeof(float2);
-  static constexpr size_t EXCH_BYTES = (size_t)PB * G::BUF * sizeof(float2);
-  static constexpr size_t BUF_BYTES = ((TILE_BYTES > EXCH_BYTES ? TILE_BYTES : EXCH_BYTES) + 15) & ~(size_t)15;
-  static constexpr int FP = (F + 3) & ~3;                                   // pitch of the rsq table
-  static constexpr size_t ROWS_BYTES = (size_t)PB * FP * sizeof(float);     // 1/sqrt(S_jj) row of every pair's j
-  static constexpr size_t OFF_RS = BUF_BYTES + ROWS_BYTES;                    // float [2][PB]
-  static constexpr size_t OFF_IJ = OFF_RS + 2 * PB * sizeof(float);           // ushort2 [PB]
-  static constexpr size_t OFF_PG = OFF_IJ + PB * sizeof(ushort2);             // int [PB]: lexicographic index (pair lists)
-  static constexpr size_t OFF_BAR = (OFF_PG + PB * sizeof(int) + 7) & ~(size_t)7;
-  static constexpr size_t SMEM = OFF_BAR + 16;
-  static_assert(THREADS % 32 == 0 && THREADS <= 1024, "block shape");
-  static_assert(TILE_BYTES % 16 == 0, "bulk copy size");
-  static_assert((T & (T - 1)) == 0 && (PB & (PB - 1)) == 0, "powers of two");
+  // per slot, behind the tile: [rows: float [PB][FP]]  ij ushort2[PB], pg int[PB] (lexicographic index), rs float[2][PB]
+  static constexpr size_t OFF_ROWS = TILE_BYTES;
+  static constexpr size_t ROW_BYTES = (size_t)FP * sizeof(float);
+  static constexpr size_t OFF_IJ = OFF_ROWS + (ROWS ? PB * ROW_BYTES : 0), OFF_PG = OFF_IJ + PB * 4, OFF_RS = OFF_PG + PB * 4;
+  static constexpr size_t SLOT_BYTES = (OFF_RS + 2 * PB * 4 + 127) & ~(size_t)127;
+  static constexpr size_t FTAB_BYTES = (((size_t)(G::TABLE > 0 ? G::TABLE : 1) * sizeof(float2)) + 15) & ~(size_t)15;
+  static constexpr size_t EXCH_BYTES = IN_TILE ? 0 : (size_t)PB * G::BUF * sizeof(float2);  // per team
+  // One CTA per SM: NTEAM teams work on NTEAM tiles while a producer warp fills the remaining slot(s) of the ring.
+  static constexpr size_t FIXED = FTAB_BYTES + 256;
+  static constexpr int MAX_TEAMS = 768 / TTHREADS < 8 ? (768 / TTHREADS < 1 ? 1 : 768 / TTHREADS) : 8;  // 24 warps: 80 registers each
+  static constexpr int FIT = (int)((kSmemPerSm - FIXED - EXCH_BYTES) / SLOT_BYTES);  // slots if there is one team
+  static constexpr int NTEAM = IN_TILE ? (FIT - 1 < 1 ? 1 : (FIT - 1 > MAX_TEAMS ? MAX_TEAMS : FIT - 1)) : 1;
+  static constexpr int NSLOT = IN_TILE ? (FIT > NTEAM + 2 ? NTEAM + 2 : FIT) : 2;
+  static constexpr int CTHREADS = NTEAM * TTHREADS;
+  static constexpr int THREADS = CTHREADS + 32;  // + the producer warp
+  static constexpr size_t OFF_EXCH = NSLOT * SLOT_BYTES;
+  static constexpr size_t OFF_FTAB = (OFF_EXCH + NTEAM * EXCH_BYTES + 15) & ~(size_t)15;  // the transform's twiddle tables
+  static constexpr size_t OFF_BAR = (OFF_FTAB + FTAB_BYTES + 7) & ~(size_t)7;              // full[NSLOT], empty[NSLOT]
+  static constexpr size_t SMEM = OFF_BAR + 2 * NSLOT * 8;
+  static_assert(TTHREADS % 32 == 0 && THREADS <= 1024 && NTEAM >= 1, "block shape");
+  static_assert(TILE_BYTES % 16 == 0 && ROW_BYTES % 16 == 0 && PB % 4 == 0 && 2 * PB <= 32, "tile shape");
+  static_assert((T & (T - 1)) == 0 && (PB & (PB - 1)) == 0 && E % 4 == 0, "powers of two");
+  static_assert(NSLOT >= 2 && NSLOT > NTEAM - 1 && SMEM <= kSmemPerSm, "shared memory");
+};
+
+// Exchange map of the register FFT onto a pair's own column of a 16-pairs-per-row tile (float2 slots, 128 bytes per row,
+// pair pl in slot (pl ^ s_swz(row)) & 15 of a row).  Element e = 16 a + b goes to row 16 a + phi(b ^ a ^ 4 (a & 3)),
+// phi(x) = x ^ (x >> 2): its slot is then (pl ^ b ^ a) & 15, which makes the transposing writes (a = thread) and the
+// read-back (b = thread) of every geometry bank-conflict free (brute-force checked).  Everything is linear over XOR,
+// so the compile-time part of an index folds into one immediate: one LOP3 per access.
+__host__ __device__ constexpr uint32_t tile_phi(uint32_t x) { return (x ^ (x >> 2)) & 15u; }
+__host__ __device__ constexpr uint32_t tile_lin(uint32_t e) {  // byte offset of element e in the column of pair 0
+  return ((e >> 4) << 11) | (tile_phi((e & 15u) ^ ((e >> 4) & 15u) ^ (((e >> 4) & 3u) << 2)) << 7) | ((((e & 15u) ^ (e >> 4)) & 15u) << 3);
+}
+struct FftTileMap {
+  unsigned char *tile;
+  uint32_t plx;  // pl << 3
+  typedef uint32_t Handle;
+  __device__ __forceinline__ Handle pre(int e_t) const { return tile_lin((uint32_t)e_t) ^ plx; }
+  __device__ __forceinline__ float2 &at(Handle h, int e_c) const {
+    return *reinterpret_cast<float2 *>(tile + (h ^ tile_lin((uint32_t)e_c)));
+  }
 };
 
 // atan2 from a degree-13 odd minimax polynomial on [0, 1] (max error 3.2e-7 rad), octant folding
@@ -105,316 +141,299 @@ __device__ __forceinline__ ushort2 pair_of(int64_t p, int C) {
 
 // Output stores: the results are written once and never read by this library, so they are marked streaming
 // (evict-first) to keep S and X, which the next kernels re-read, in L2.
-#ifdef DELTA_PLAIN_STORES
-#define ST4(p, v) (*reinterpret_cast<float4 *>(p) = (v))
-#define ST2(p, v) (*reinterpret_cast<float2 *>(p) = (v))
-#define ST1(p, v) (*(p) = (v))
-#else
 #define ST4(p, v) __stcs(reinterpret_cast<float4 *>(p), (v))
 #define ST2(p, v) __stcs(reinterpret_cast<float2 *>(p), (v))
 #define ST1(p, v) __stcs((p), (v))
-#endif
+
+__device__ __forceinline__ void mbar_init(uint64_t *b, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(b)), "r"(count));
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t *b) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(b)) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *b, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(b)), "r"(bytes) : "memory");
+}
+// Bounded wait: a faulted copy or a pipeline bug must trap after ~2 s, not hang the GPU.
+__device__ __forceinline__ void mbar_wait(uint64_t *b, uint32_t parity) {
+  const uint32_t addr = smem_u32(b);
+  long long t0 = 0;
+  for (uint32_t spins = 0;; ++spins) {
+    uint32_t ok;
+    asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                 : "=r"(ok) : "r"(addr), "r"(parity) : "memory");
+    if (ok) return;
+    if (spins == 64) t0 = clock64();
+    if (spins > 64 && (spins & 1023) == 0 && clock64() - t0 > 4000000000LL) __trap();
+  }
+}
+__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t bytes, uint64_t *bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)),
+               "l"(src), "r"(bytes), "r"(smem_u32(bar))
+               : "memory");
+}
 
 }  // namespace
 
 // GAPALL: G, A and Pw are all requested (no per-element pointer tests)
 // FULL: max_lag == L/2 (every lag of the circular correlation is stored; the two end points are the same sample)
-// Zero-lag autocorrelations (R12): sum over all L bins of S_cc = rscale * sum_{k<nrp} rpart[c rp_stride + k].
+// rnorm[c] = 1/sqrt(sum over all L bins of S_cc) = 1/sqrt(L R_cc[0]) (0 where that sum is 0; reading R16).
+// Srsq: the four shifted copies of 1/sqrt(S_cc[f]) (store_rsq4 in delta_internal.h).
 template <int L, bool FULL, bool GAPALL>
-__global__ void __launch_bounds__(PairCfg<L>::THREADS, PairCfg<L>::MIN_CTAS)
-pair_kernel(const float2 *__restrict__ S, const float *__restrict__ Srsq, const float *__restrict__ rpart, int nrp,
-            int rp_stride, float rscale, const ushort2 *__restrict__ list, const float2 *__restrict__ tw,
-            const float2 *__restrict__ ftab, Layout lay, PairConsts pc, float *__restrict__ G_, float *__restrict__ A_,
-            float *__restrict__ Pw_, float *__restrict__ R_, long long *trace) {
+__global__ void __launch_bounds__(PairCfg<L>::THREADS, 1)
+pair_kernel(const float2 *__restrict__ S, const float *__restrict__ Srsq, const float *__restrict__ rnorm,
+            const ushort2 *__restrict__ list, const float2 *__restrict__ tw, const float2 *__restrict__ ftab, Layout lay,
+            PairConsts pc, float *__restrict__ G_, float *__restrict__ A_, float *__restrict__ Pw_, float *__restrict__ R_) {
   using Cfg = PairCfg<L>;
   using Geo = typename Cfg::G;
-  constexpr int N = Cfg::N, F = Cfg::F, T = Cfg::T, E = Cfg::E, PB = Cfg::PB;
-  constexpr int THREADS = Cfg::THREADS;
+  constexpr int N = Cfg::N, F = Cfg::F, T = Cfg::T, E = Cfg::E, PB = Cfg::PB, NSLOT = Cfg::NSLOT, NTEAM = Cfg::NTEAM;
   extern __shared__ __align__(128) unsigned char smem_raw[];
-  float2 *tile = reinterpret_cast<float2 *>(smem_raw);                     // [F][PB], slot = (pl ^ s_swz(f)) & (PB-1)
-  float2 *exch = reinterpret_cast<float2 *>(smem_raw);                     // [PB][BUF] once the tile is dead
-  float *rowj = reinterpret_cast<float *>(smem_raw + Cfg::BUF_BYTES);      // [PB][FP]: 1/sqrt(S_jj[f]) of pair pl's j
-  float *rs = reinterpret_cast<float *>(smem_raw + Cfg::OFF_RS);           // [2][PB]: 1/sqrt(L R_cc[0]) of i, j
-  ushort2 *ij_s = reinterpret_cast<ushort2 *>(smem_raw + Cfg::OFF_IJ);     // [PB]
-  int *pg_s = reinterpret_cast<int *>(smem_raw + Cfg::OFF_PG);             // [PB]
-  uint64_t *bar = reinterpret_cast<uint64_t *>(smem_raw + Cfg::OFF_BAR);
+  float2 *ftab_s = reinterpret_cast<float2 *>(smem_raw + Cfg::OFF_FTAB);
+  uint64_t *full = reinterpret_cast<uint64_t *>(smem_raw + Cfg::OFF_BAR), *empty = full + NSLOT;
 
   float *const G = G_, *const A = A_, *const Pw = Pw_, *const R = R_;
-  const bool wantG = G, wantR = R;
+  const bool wantG = G != nullptr, wantGAP = G || A || Pw;
   const int tid = threadIdx.x;
-  const int64_t p0 = (int64_t)blockIdx.x * PB;
+  // the CTA's tiles: blockIdx.x + n gridDim.x, n = 0 .. ncta-1; tile n goes through slot n mod NSLOT and is worked on
+  // by team n mod NTEAM
+  const int ntiles = (int)lay.Poblk;
+  const int ncta = ((int)blockIdx.x < ntiles) ? (ntiles - 1 - (int)blockIdx.x) / (int)gridDim.x + 1 : 0;
 
-  // debug: globaltimer stamps of the CTA's phases (delta_debug_set_trace): trace[8192 + 8 blockIdx + k]
-  auto stamp = [&](int k) {
-    if (trace && tid == 0) {
-      long long g;
-      asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g));
-      trace[8192 + 8 * (int64_t)blockIdx.x + k] = g;
-    }
-  };
-  stamp(0);
   pdl_launch_dependents();
-  if (tid < PB) {
-    // all pairs: (i, j) of lexicographic pair p0 + tid;  pair list (f2): entry p0 + tid of the list, whose S values sit
-    // at lexicographic index pg in the S layout
-    ushort2 ij = make_ushort2(0, 1);
-    if (p0 + tid < lay.Po) ij = list ? list[p0 + tid] : pair_of(p0 + tid, lay.C);
-    ij_s[tid] = ij;
-    pg_s[tid] = (int)ij.x * lay.C - ((int)ij.x * ((int)ij.x + 1)) / 2 + (int)ij.y - (int)ij.x - 1;
-  }
   if (tid == 0) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(1));
+    for (int s = 0; s < NSLOT; ++s) {
+      mbar_init(full + s, 1);
+      mbar_init(empty + s, Cfg::TW);
+    }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
-  pdl_wait();  // S, rsq and the energy partials come from the preceding kernels; the outputs may still be read by a consumer
-  stamp(1);
+  for (int i = tid; i < Geo::TABLE; i += Cfg::THREADS) ftab_s[i] = __ldg(ftab + i);  // a constant table of the plan
   __syncthreads();
-  if (tid == 0) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)),
-                 "r"((uint32_t)((list ? 0 : Cfg::TILE_BYTES) + (wantG ? Cfg::ROWS_BYTES : 0))) : "memory");
-    if (!list)
-      asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(tile)),
-                   "l"(S + (int64_t)blockIdx.x * F * PB), "r"((uint32_t)Cfg::TILE_BYTES), "r"(smem_u32(bar))
-                   : "memory");
-  }
-  if (list) {  // gather the tile: slot sl of row f belongs to the CTA's pair pl = (sl ^ s_swz(f)) mod PB
-    for (int idx = tid; idx < F * PB; idx += THREADS) {
-      const int f = idx / PB, sw = s_swz(f);
-      const int pg = pg_s[((idx % PB) ^ sw) & (PB - 1)];
-      tile[idx] = __ldg(S + ((int64_t)(pg >> lay.pb_shift) * F + f) * PB + ((pg ^ sw) & (PB - 1)));
-    }
-  }
-  if (tid < PB && wantG) {  // this pair's 1/sqrt(S_jj) row; a lane's complete_tx may precede lane 0's expect_tx: the
-                            // transaction count is signed and the phase cannot complete before lane 0's arrival
-    const ushort2 ij = ij_s[tid];
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(rowj + tid * Cfg::FP)),
-                 "l"(Srsq + (int64_t)ij.y * Cfg::FP), "r"((uint32_t)(Cfg::FP * sizeof(float))), "r"(smem_u32(bar))
-                 : "memory");
-  }
-
-  // rs[role][pl] = 1/sqrt(sum over all L bins of S_cc) = 1/sqrt(L R_cc[0]),  c = i (role 0) or j (role 1) of pair pl
-  if (R && tid < 2 * PB) {
-    const ushort2 ij = ij_s[tid % PB];
-    const float *a = rpart + (int64_t)(tid / PB ? ij.y : ij.x) * rp_stride;
-    float sum = 0.f;
-    for (int k = 0; k < nrp; ++k) sum += __ldg(a + k);
-    sum *= rscale;
-    rs[tid] = sum > 0.f ? rsqrtf(sum) : 0.f;
-  }
-  __syncthreads();
-
-  {  // the tile has landed?  (bounded: a faulted copy must trap, not hang the GPU)
-    uint32_t ok = 0;
-    long long t0 = 0;
-    for (uint32_t spins = 0; !ok; ++spins) {
-      asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
-                   : "=r"(ok) : "r"(smem_u32(bar)), "r"(0) : "memory");
-      if (spins == 64) t0 = clock64();
-      if (spins > 64 && (spins & 1023) == 0 && clock64() - t0 > 4000000000LL) __trap();
-    }
-  }
-
-  stamp(2);  // tile landed
-  const int pl = tid / T, gt = tid % T;
-  const int64_t p = p0 + pl;
-  const bool valid = p < lay.Po;
-  const float2 wg = __ldg(tw + gt);  // e^{-2 pi i gt / L}
-
-  // ---- pass 1: G, A, P ------------------------------------------------------------------------------------------
-  // The store path is what binds this kernel (without its stores it runs in half the time), so pass 1 has its own
-  // thread mapping: a thread owns 4 consecutive bins of one pair and stores float4; a warp covers 512 contiguous
-  // bytes of one row.  Rows have F = N + 1 floats (F mod 4 = 1), so element (p, f) is 16-byte aligned iff
-  // (p + f) mod 4 = 0: the groups of pair p start at f0 = (-p) mod 4; the f0 head and the 0..3 tail bins go scalar.
-  if ((G || A || Pw) && p0 < lay.Po) {
-    auto value = [&](float2 s, float g2, float &mag, float &coh, float &ang) {
-      mag = sqrt_approx(fmaf(s.x, s.x, s.y * s.y));
-      coh = mag * g2;
-      ang = atan2_poly(s.y, s.x);
+  pdl_wait();  // S, rsq and rnorm come from the preceding kernels; the outputs may still be read by a consumer
+  if (tid >= Cfg::CTHREADS) {
+    // ===== producer warp: fills slot n mod NSLOT with tile n of this CTA: the pairs' channels, the rho normalisation
+    // and the bulk copies.  The tables of tile n + 1 are worked out (global loads and all) before the wait for its slot.
+    const int lane = tid - Cfg::CTHREADS, pl = lane % PB;
+    const bool rows = Cfg::ROWS && wantG;
+    ushort2 ij = make_ushort2(0, 1);
+    float rs = 0.f;
+    auto tables = [&](int n) {
+      const int64_t p = ((int64_t)blockIdx.x + (int64_t)n * gridDim.x) * PB + pl;
+      // all pairs: (i, j) of lexicographic pair p;  pair list (f2): entry p of the list, whose S values sit at
+      // lexicographic index pg in the S layout
+      ij = make_ushort2(0, 1);
+      if (p < lay.Po) ij = list ? list[p] : pair_of(p, lay.C);
+      if (R) rs = __ldg(rnorm + (lane < PB ? ij.x : ij.y));
     };
-    constexpr int NG = N / 4;  // group slots per pair
-    const bool vec4 = (((reinterpret_cast<uintptr_t>(G) | reinterpret_cast<uintptr_t>(A) | reinterpret_cast<uintptr_t>(Pw)) & 15) == 0);
-    if (vec4) {
-      // R pairs are in flight per iteration; a thread keeps its group g and its pair slot qa, so with R a multiple of 4
-      // the bins f, the tile rows and the alignment shift f0 do not depend on the iteration (p0 is a multiple of 4)
-      constexpr int R = THREADS / NG, NIT = PB / R;
-      static_assert(R >= 1 && (R & (R - 1)) == 0 && PB % R == 0, "pairs per iteration");
-      const int g = tid % NG, qa = tid / NG;
-      if constexpr (R % 4 == 0) {
-        // Everything but the pair is the same in every iteration, so the bins, the four tile addresses (the pair offset
-        // it R only flips slot bits: one XOR) and the base pointers are hoisted.  The G/A/P pass is bound by the
-        // load/store unit's wavefronts, so the two 1/sqrt rows are read as aligned float4 (two loads cover the four
-        // bins f0 + 4g .. + 3 of a group that starts f0 floats past a 16-byte boundary; f0 is warp-uniform), and the
-        // row of channel i, shared by consecutive lexicographic pairs, is re-read only when i changes.
-        const int f0 = (-qa) & 3, ng = (F - f0) >> 2, f = f0 + 4 * g;
-        if (g < ng) {
-          int tb[4];
+    if (ncta > 0) tables(0);
+    for (int n = 0; n < ncta; ++n) {
+      const int tile = blockIdx.x + n * gridDim.x;
+      const int s = n % NSLOT;
+      unsigned char *st = smem_raw + (size_t)s * Cfg::SLOT_BYTES;
+      if (n >= NSLOT) mbar_wait(empty + s, (n / NSLOT - 1) & 1);
+      if (lane < PB) {
+        reinterpret_cast<ushort2 *>(st + Cfg::OFF_IJ)[lane] = ij;
+        reinterpret_cast<int *>(st + Cfg::OFF_PG)[lane] = (int)ij.x * lay.C - ((int)ij.x * ((int)ij.x + 1)) / 2 + (int)ij.y - (int)ij.x - 1;
+      }
+      if (R && lane < 2 * PB) reinterpret_cast<float *>(st + Cfg::OFF_RS)[lane] = rs;
+      __syncwarp();
+      if (lane == 0) {
+        const uint32_t bytes = (list ? 0u : (uint32_t)Cfg::TILE_BYTES) + (rows ? (uint32_t)(PB * Cfg::ROW_BYTES) : 0u);
+        if (bytes) mbar_expect_tx(full + s, bytes); else mbar_arrive(full + s);
+        if (!list) bulk_g2s(st, S + (int64_t)tile * F * PB, (uint32_t)Cfg::TILE_BYTES, full + s);  // else: the groups gather
+      }
+      __syncwarp();
+      // 1/sqrt(S_jj) row of every pair, from the copy of the table that is aligned for the pair's float4 groups
+      if (rows && lane < PB)
+        bulk_g2s(st + Cfg::OFF_ROWS + lane * Cfg::ROW_BYTES, Srsq + ((int64_t)((-pl) & 3) * lay.C + ij.y) * Cfg::FP,
+                 (uint32_t)Cfg::ROW_BYTES, full + s);
+      if (n + 1 < ncta) tables(n + 1);
+    }
+    return;
+  }
+  // ===== compute warps =====
+  const int team = tid / Cfg::TTHREADS, tt = tid % Cfg::TTHREADS;
+
+  using Sync = FftNamedSync<T, 1, Cfg::TTHREADS>;  // groups wider than a warp: NTEAM is 1 then
+  float2 *exch = reinterpret_cast<float2 *>(smem_raw + Cfg::OFF_EXCH);  // [PB][BUF] (narrow tiles only)
+  const int pl = tt / T, gt = tt % T;
+  float2 wg = __ldg(tw + gt);  // e^{-2 pi i gt / L}
+  // Output rows have F = N + 1 floats (F mod 4 = 1), so element (p, f) is 16-byte aligned iff (p + f) mod 4 = 0: the
+  // float4 groups of pair p start at f0 = (-p) mod 4 = (-pl) mod 4 (tiles start at multiples of 4); the f0 head bins and
+  // the tail bins go scalar.  Copy f0 of the rsq table holds bin f at index f - f0, so its float4 reads are aligned too.
+  const bool vec4 = (((reinterpret_cast<uintptr_t>(G) | reinterpret_cast<uintptr_t>(A) | reinterpret_cast<uintptr_t>(Pw)) & 15) == 0);
+  const int f0 = (-pl) & 3, ng = (F - f0) >> 2;
+  const float *rsq_f0 = Srsq + (int64_t)f0 * lay.C * Cfg::FP;
+  auto value = [&](float2 s, float g2, float &mag, float &coh, float &ang) {
+    mag = sqrt_approx(fmaf(s.x, s.x, s.y * s.y));
+    coh = mag * g2;
+    ang = atan2_poly(s.y, s.x);
+  };
+
+  for (int n = team; n < ncta; n += NTEAM) {
+    const int tile = blockIdx.x + n * gridDim.x;
+    const int s = n % NSLOT, use = n / NSLOT;
+    unsigned char *st = smem_raw + (size_t)s * Cfg::SLOT_BYTES;
+    float2 *tl = reinterpret_cast<float2 *>(st);  // [F][PB], slot = (pl ^ s_swz(f)) & (PB-1)
+    mbar_wait(full + s, use & 1);
+    const ushort2 ij = reinterpret_cast<const ushort2 *>(st + Cfg::OFF_IJ)[pl];
+    const int64_t p = (int64_t)tile * PB + pl;
+    const bool valid = p < lay.Po;
+    if (list) {  // gather this pair's column: slot (pl ^ s_swz(f)) of row f holds S[pg][f]
+      const int pg = reinterpret_cast<const int *>(st + Cfg::OFF_PG)[pl];
+      const float2 *src = S + (int64_t)(pg >> lay.pb_shift) * F * PB;
+      for (int f = gt; f < F; f += T) {
+        const int sw = s_swz(f);
+        tl[f * PB + ((pl ^ sw) & (PB - 1))] = __ldg(src + f * PB + ((pg ^ sw) & (PB - 1)));
+      }
+      Sync::sync();
+    }
+
+    // ---- pass 1: G, A, P ----------------------------------------------------------------------------------------
+    if (wantGAP && valid) {
+      const float *ri = rsq_f0 + (int64_t)ij.x * Cfg::FP;
+      if (vec4 && gt < ng) {
+        // Step q covers the bins f0 + 4 (gt + T q) .. + 3.  A step moves 4 T rows down the tile, which changes neither
+        // the slot (it depends on bits 0..5 of the row, and 4 T is a multiple of 64 or the only step) nor anything
+        // else but a constant offset: tile addresses, table rows and output pointers are set up once per tile.
+        // (The two shortest transforms have 4 T < 64: their slots are worked out per step.)
+        constexpr int NQ = E / 4;
+        constexpr bool HOIST = (4 * T) % 64 == 0;
+        const int fb = f0 + 4 * gt;
+        const float2 *tb[4];
 #pragma unroll
-          for (int k = 0; k < 4; ++k) tb[k] = (f + k) * PB + ((qa ^ s_swz(f + k)) & (PB - 1));
-          const int64_t at0 = (p0 + qa) * F + f;
-          float *Pw0 = Pw ? Pw + at0 : nullptr, *G0 = G ? G + at0 : nullptr, *A0 = A ? A + at0 : nullptr;
-          auto quad = [&](const float4 a, const float4 bq, float *r) {  // elements f0 .. f0 + 3 of (a, bq)
-            switch (f0) {
-              case 0: r[0] = a.x; r[1] = a.y; r[2] = a.z; r[3] = a.w; break;
-              case 1: r[0] = a.y; r[1] = a.z; r[2] = a.w; r[3] = bq.x; break;
-              case 2: r[0] = a.z; r[1] = a.w; r[2] = bq.x; r[3] = bq.y; break;
-              default: r[0] = a.w; r[1] = bq.x; r[2] = bq.y; r[3] = bq.z; break;
-            }
-          };
-          int icur = -1;
-          float gi[4] = {0.f, 0.f, 0.f, 0.f};
+        for (int k = 0; k < 4; ++k) tb[k] = tl + (fb + k) * PB + ((pl ^ s_swz(fb + k)) & (PB - 1));
+        const float4 *gi4 = reinterpret_cast<const float4 *>(ri) + gt;
+        const float4 *gj4 = Cfg::ROWS ? reinterpret_cast<const float4 *>(st + Cfg::OFF_ROWS + pl * Cfg::ROW_BYTES) + gt
+                                      : reinterpret_cast<const float4 *>(rsq_f0 + (int64_t)ij.y * Cfg::FP) + gt;
+        if (wantG) {  // the later steps' pieces of the row of channel i: into L1 now, so that only the first step can miss
 #pragma unroll
-          for (int it = 0; it < NIT; ++it) {
-            const int ql = it * R + qa;
-            if (p0 + ql >= lay.Po) continue;
-            float g2[4] = {0.f, 0.f, 0.f, 0.f};
-            if (wantG) {
-              const int i = ij_s[ql].x;
-              if (i != icur) {  // warp-uniform
-                const float4 *src = reinterpret_cast<const float4 *>(Srsq + (int64_t)i * Cfg::FP + 4 * g);
-                quad(__ldg(src), __ldg(src + 1), gi);
-                icur = i;
-              }
-              const float4 *rowq = reinterpret_cast<const float4 *>(rowj + ql * Cfg::FP + 4 * g);
-              float gj[4];
-              quad(rowq[0], rowq[1], gj);
-#pragma unroll
-              for (int k = 0; k < 4; ++k) g2[k] = gi[k] * gj[k];
-            }
-            float2 sv[4];
-#pragma unroll
-            for (int k = 0; k < 4; ++k) sv[k] = tile[tb[k] ^ (it * R)];
-            float m[4], c[4], an[4];
-#pragma unroll
-            for (int k = 0; k < 4; ++k) value(sv[k], g2[k], m[k], c[k], an[k]);
-            if (GAPALL || Pw) ST4(Pw0 + it * R * F, make_float4(m[0], m[1], m[2], m[3]));
-            if (GAPALL || G) ST4(G0 + it * R * F, make_float4(c[0], c[1], c[2], c[3]));
-            if (GAPALL || A) ST4(A0 + it * R * F, make_float4(an[0], an[1], an[2], an[3]));
-          }
+          for (int q = 1; q < NQ; ++q)
+            if (gt + T * q < ng) asm volatile("prefetch.global.L1 [%0];" ::"l"(gi4 + T * q));
         }
-      } else {
+        const int64_t at = p * F + fb;
+        float *Pw0 = Pw ? Pw + at : nullptr, *G0 = G ? G + at : nullptr, *A0 = A ? A + at : nullptr;
 #pragma unroll
-        for (int it = 0; it < NIT; ++it) {
-          const int ql = (it * R) ^ qa;  // = it R + qa (qa < R, R a power of two)
-          const int64_t q = p0 + ql;
-          const int f0 = (-(qa + ((it * R) & 3))) & 3, ng = (F - f0) >> 2;
-          if (q >= lay.Po || g >= ng) continue;
-          const int f = f0 + 4 * g;
-          const ushort2 qij = ij_s[ql];
-          const float *qi = Srsq + (int64_t)qij.x * Cfg::FP + f, *qj = rowj + ql * Cfg::FP + f;
+        for (int q = 0; q < NQ; ++q) {
+          if (gt + T * q >= ng) continue;
           float2 sv[4];
-          float g2[4];
 #pragma unroll
           for (int k = 0; k < 4; ++k) {
-            sv[k] = tile[(f + k) * PB + (((qa ^ s_swz(f + k)) ^ (it * R)) & (PB - 1))];
-            g2[k] = wantG ? __ldg(qi + k) * qj[k] : 0.f;
+            const int f = fb + k + 4 * T * q;
+            sv[k] = HOIST ? tb[k][q * 4 * T * PB] : tl[f * PB + ((pl ^ s_swz(f)) & (PB - 1))];
+          }
+          float g2[4] = {0.f, 0.f, 0.f, 0.f};
+          if (wantG) {
+            // the row of channel i comes through L1 (every pair of the tile reads the same one or two rows)
+            const float4 gi = __ldg(gi4 + T * q), gj = Cfg::ROWS ? gj4[T * q] : __ldg(gj4 + T * q);
+            g2[0] = gi.x * gj.x; g2[1] = gi.y * gj.y; g2[2] = gi.z * gj.z; g2[3] = gi.w * gj.w;
           }
           float m[4], c[4], an[4];
 #pragma unroll
           for (int k = 0; k < 4; ++k) value(sv[k], g2[k], m[k], c[k], an[k]);
-          const int64_t at = q * F + f;
-          if (GAPALL || Pw) ST4(Pw + at, make_float4(m[0], m[1], m[2], m[3]));
-          if (GAPALL || G) ST4(G + at, make_float4(c[0], c[1], c[2], c[3]));
-          if (GAPALL || A) ST4(A + at, make_float4(an[0], an[1], an[2], an[3]));
+          if (GAPALL || Pw) ST4(Pw0 + q * 4 * T, make_float4(m[0], m[1], m[2], m[3]));
+          if (GAPALL || G) ST4(G0 + q * 4 * T, make_float4(c[0], c[1], c[2], c[3]));
+          if (GAPALL || A) ST4(A0 + q * 4 * T, make_float4(an[0], an[1], an[2], an[3]));
+        }
+      }
+      // scalar bins: the edges of the vector path (the f0 head bins and the bins from f0 + 4 ng on: at most 5), or every
+      // bin if the arrays are not 16-byte aligned.  Copy 0 of the rsq table holds bin f at index f.
+      const int ntail = vec4 ? F - (f0 + 4 * ng) : F - f0;
+      for (int e = gt; e < f0 + ntail; e += T) {
+        const int f = e < f0 ? e : (vec4 ? f0 + 4 * ng : f0) + (e - f0);
+        const float g2 = wantG ? __ldg(Srsq + (int64_t)ij.x * Cfg::FP + f) * __ldg(Srsq + (int64_t)ij.y * Cfg::FP + f) : 0.f;
+        float m, c, an;
+        value(tl[f * PB + ((pl ^ s_swz(f)) & (PB - 1))], g2, m, c, an);
+        if (GAPALL || Pw) ST1(Pw + p * F + f, m);
+        if (GAPALL || G) ST1(G + p * F + f, c);
+        if (GAPALL || A) ST1(A + p * F + f, an);
+      }
+    }
+    if (!R) {  // the slot is free once every group of this warp has read it
+      __syncwarp();
+      if ((tid & 31) == 0) mbar_arrive(empty + s);
+      continue;
+    }
+
+    // ---- pass 2: merge step of the inverse real transform (S read again from the tile; twice the merge of
+    // irfft_merge, the factor 1/2 goes into the normalisation) ------------------------------------------------
+    float2 v[E];
+    // (the products wg * wstep[u] below are the same for every tile; the compiler would keep all E of them alive across
+    // the tile loop, in local memory: make wg opaque per tile instead)
+    asm volatile("" : "+f"(wg.x), "+f"(wg.y));
+    const int pg = pl ^ s_swz(gt);
+#pragma unroll
+    for (int u = 0; u < E; ++u) {
+      const int f = gt + T * u;
+      const int fr = N - f;
+      float2 sf = tl[f * PB + ((pg ^ s_swz(T * u)) & (PB - 1))];  // s_swz(gt | T u) = s_swz(gt) ^ s_swz(T u)
+      float2 sr = tl[fr * PB + ((pl ^ s_swz(fr)) & (PB - 1))];
+      if (u == 0 && gt == 0) { sf.y = 0.f; sr.y = 0.f; }  // Im S[0], Im S[N] do not enter the real transform
+      const float2 w = cmul(wg, pc.wstep[u]);               // e^{-2 pi i f / L}; the inverse uses its conjugate
+      v[u] = irfft_merge2(sf, sr, make_float2(w.x, -w.y));
+    }
+    const float norm = reinterpret_cast<const float *>(st + Cfg::OFF_RS)[pl] * reinterpret_cast<const float *>(st + Cfg::OFF_RS)[PB + pl];
+
+    // ---- rho = irfft(S) / sqrt(R_ii[0] R_jj[0]) ----------------------------------------------------------------
+    // x = z/N with z[n] = (x[2n], x[2n+1]) N, n = gt + T u; norm = 1/(L sqrt(R_ii[0] R_jj[0])) carries 2 (L/N) x 1/2.
+    Sync::sync();  // every S value of the group's pairs is in registers (and the last transform's read-back is done)
+    if constexpr (Cfg::IN_TILE) {
+      fft_inplace_g<Geo, true, Sync>(v, FftTileMap{st, (uint32_t)pl << 3}, ftab_s, gt);
+      Sync::sync();  // the group's read-back is done: the slot can be refilled
+      if ((tid & 31) == 0) mbar_arrive(empty + s);
+    } else {
+      if ((tid & 31) == 0) mbar_arrive(empty + s);  // T >= 64 here: Sync is a barrier over all compute warps
+      fft_inplace_g<Geo, true, Sync>(v, FftPadMap{exch + pl * Geo::BUF}, ftab_s, gt);
+    }
+    float *Rp = R + p * lay.nlags;
+    if (!valid) {
+    } else if (FULL) {
+      // lag m = xi for xi <= L/2 and xi - L for xi >= L/2; row position q = m + L/2
+      const bool vec = (reinterpret_cast<uintptr_t>(Rp) & 7) == 0;  // q is even: float2 stores iff the row is 8-byte aligned
+#pragma unroll
+      for (int u = 0; u < E; ++u) {
+        const int nn = gt + T * u;
+        const float a = v[u].x * norm, b = v[u].y * norm;
+        const int q = (u < E / 2) ? 2 * nn + N : 2 * nn - N;
+        if (vec) {
+          ST2(Rp + q, make_float2(a, b));
+        } else {
+          ST1(Rp + q, a);
+          ST1(Rp + q + 1, b);
+        }
+        if (u == E / 2 && gt == 0) ST1(Rp + L, a);  // xi = L/2 is lag -L/2 and lag +L/2
+      }
+    } else {
+      const int M = lay.M;
+#pragma unroll
+      for (int u = 0; u < E; ++u) {
+        const int nn = gt + T * u;
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+          const int xi = 2 * nn + h;
+          const float val = (h ? v[u].y : v[u].x) * norm;
+          if (xi <= M) Rp[xi + M] = val;
+          if (xi >= L - M) Rp[xi - L + M] = val;
         }
       }
     }
-    // scalar bins: the edges of the vector path (at most 6 per pair), or everything if the arrays are not 16-byte aligned
-    const int per = vec4 ? 8 : F;
-    for (int item = tid; item < PB * per; item += THREADS) {
-      const int ql = item / per, e = item % per;
-      const int64_t q = p0 + ql;
-      if (q >= lay.Po) continue;
-      int f = e;
-      if (vec4) {
-        const int f0 = (int)((-q) & 3), ng = (F - f0) >> 2;
-        f = e < f0 ? e : f0 + 4 * ng + (e - f0);
-        if (f >= F) continue;
-      }
-      const ushort2 qij = ij_s[ql];
-      const float g2 = wantG ? __ldg(Srsq + (int64_t)qij.x * Cfg::FP + f) * rowj[ql * Cfg::FP + f] : 0.f;
-      float m, c, an;
-      value(tile[f * PB + ((ql ^ s_swz(f)) & (PB - 1))], g2, m, c, an);
-      if (GAPALL || Pw) ST1(Pw + q * F + f, m);
-      if (GAPALL || G) ST1(G + q * F + f, c);
-      if (GAPALL || A) ST1(A + q * F + f, an);
-    }
   }
-  stamp(3);  // pass 1 done (thread 0's share)
-  if (!wantR) return;
-
-  // ---- pass 2: merge step of the inverse real transform (S read again from the tile; twice the merge of
-  // irfft_merge, the factor 1/2 goes into the normalisation) ------------------------------------------------
-  float2 v[E];
-  const int pg = pl ^ s_swz(gt);
-#pragma unroll
-  for (int u = 0; u < E; ++u) {
-    const int f = gt + T * u;
-    const int fr = N - f;
-    float2 sf = tile[f * PB + ((pg ^ s_swz(T * u)) & (PB - 1))];  // s_swz(gt | T u) = s_swz(gt) ^ s_swz(T u)
-    float2 sr = tile[fr * PB + ((pl ^ s_swz(fr)) & (PB - 1))];
-    if (u == 0 && gt == 0) { sf.y = 0.f; sr.y = 0.f; }  // Im S[0], Im S[N] do not enter the real transform
-    const float2 w = cmul(wg, pc.wstep[u]);               // e^{-2 pi i f / L}; the inverse uses its conjugate
-    v[u] = irfft_merge2(sf, sr, make_float2(w.x, -w.y));
-  }
-  stamp(4);
-  __syncthreads();  // every S value is in registers: the tile becomes exchange space
-
-  // ---- rho = irfft(S) / sqrt(R_ii[0] R_jj[0]) ----------------------------------------------------------------
-  fft_inplace_g<Geo, true>(v, FftPadMap{exch + pl * Geo::BUF}, ftab, gt);  // z[n] = (x[2n], x[2n+1]) * N, n = gt + T u
-  stamp(5);  // FFT done
-  if (!valid) return;
-  // rho = x / sqrt(R_ii[0] R_jj[0]),  x = z/N,  R_cc[0] = (sum over all L bins of S_cc)/L
-  const float norm = rs[pl] * rs[PB + pl];  // 2 (L/N) x 1/2 (irfft_merge2)
-  float *Rp = R + p * lay.nlags;
-  if (FULL) {
-    // lag m = xi for xi <= L/2 and xi - L for xi >= L/2; row position q = m + L/2
-    const bool vec = (reinterpret_cast<uintptr_t>(Rp) & 7) == 0;  // q is even: float2 stores iff the row is 8-byte aligned
-#pragma unroll
-    for (int u = 0; u < E; ++u) {
-      const int n = gt + T * u;
-      const float a = v[u].x * norm, b = v[u].y * norm;
-      const int q = (u < E / 2) ? 2 * n + N : 2 * n - N;
-#ifdef DELTA_DBG_NOSTORE_R
-      if (lay.Po < 0)
-#endif
-      if (vec) {
-        ST2(Rp + q, make_float2(a, b));
-      } else {
-        ST1(Rp + q, a);
-        ST1(Rp + q + 1, b);
-      }
-      if (u == E / 2 && gt == 0) ST1(Rp + L, a);  // xi = L/2 is lag -L/2 and lag +L/2
-    }
-  } else {
-    const int M = lay.M;
-#pragma unroll
-    for (int u = 0; u < E; ++u) {
-      const int n = gt + T * u;
-#pragma unroll
-      for (int h = 0; h < 2; ++h) {
-        const int xi = 2 * n + h;
-        const float val = (h ? v[u].y : v[u].x) * norm;
-        if (xi <= M) Rp[xi + M] = val;
-        if (xi >= L - M) Rp[xi - L + M] = val;
-      }
-    }
-  }
-  stamp(6);
 }
 
-// rsq[c][f] = 1/sqrt(S_cc[f]) (0 where S_cc[f] <= 0, reading R16) and
-// rsum[c] = S_cc[0] + 2 sum_{0<f<N} S_cc[f] + S_cc[N] = sum over all L bins = L R_cc[0].  One warp per channel.
-__global__ void __launch_bounds__(32) auto_prep_kernel(const float *__restrict__ Sauto, float *__restrict__ rsq,
-                                                       float *__restrict__ rsum, int F, int Fp) {
-  const int c = blockIdx.x, lane = threadIdx.x;
+// rsq4 = the four shifted copies of 1/sqrt(S_cc[f]) (0 where S_cc[f] <= 0, reading R16) and
+// rnorm[c] = 1/sqrt(S_cc[0] + 2 sum_{0<f<N} S_cc[f] + S_cc[N]) = 1/sqrt(sum over all L bins) = 1/sqrt(L R_cc[0]).
+// One warp per channel.
+__global__ void __launch_bounds__(32) auto_prep_kernel(const float *__restrict__ Sauto, float *__restrict__ rsq4,
+                                                       float *__restrict__ rnorm, Layout lay) {
+  const int c = blockIdx.x, lane = threadIdx.x, F = lay.F;
   float sum = 0.f;
   for (int f = lane; f < F; f += 32) {
     const float a = Sauto[(int64_t)c * F + f];
-    rsq[(int64_t)c * Fp + f] = a > 0.f ? rsqrtf(a) : 0.f;
+    store_rsq4(rsq4, lay, c, f, a > 0.f ? rsqrtf(a) : 0.f);
     sum = fmaf((f == 0 || f == F - 1) ? 1.f : 2.f, a, sum);
   }
   for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
-  if (lane == 0) rsum[c] = sum;
+  if (lane == 0) rnorm[c] = sum > 0.f ? rsqrtf(sum) : 0.f;
 }
 
 // acc = wa acc + wn x (f2: accumulation of spectra over chunks); wa == 0 does not read acc
@@ -454,8 +473,8 @@ __global__ void __launch_bounds__(256) s_unpack_kernel(const float2 *__restrict_
 
 // ------------------------------------------------------------------------------------------
 template <int L>
-static int launch_pair_L(delta_plan *p, const float *d_S, const float *d_rsq, const float *rpart, int nrp, int rp_stride,
-                         float rscale, float *d_G, float *d_A, float *d_P, float *d_R, cudaStream_t st) {
+static int launch_pair_L(delta_plan *p, const float *d_S, const float *d_rsq, const float *d_rnorm, float *d_G, float *d_A,
+                         float *d_P, float *d_R, cudaStream_t st) {
   using Cfg = PairCfg<L>;
   const Layout &lay = p->lay;
   if (lay.Poblk == 0 || lay.Po == 0) return DELTA_OK;
@@ -463,14 +482,16 @@ static int launch_pair_L(delta_plan *p, const float *d_S, const float *d_rsq, co
   PairConsts pc;
   for (int u = 0; u < 16; ++u) pc.wstep[u] = p->h_wstep[u];
   const bool full = lay.M == L / 2;
+  // persistent: one CTA per SM (or fewer if there are not that many tiles), NTEAM tiles in work on each
+  const int64_t want = (lay.Poblk + Cfg::NTEAM - 1) / Cfg::NTEAM;
+  const unsigned grid = (unsigned)(want < p->num_sms ? want : p->num_sms);
 #define DELTA_PAIR_LAUNCH(FULL_, GAPALL_)                                                                           \
   do {                                                                                                              \
     int rc = opt_in_smem(pair_kernel<L, FULL_, GAPALL_>, Cfg::SMEM);                                                \
     if (rc) return rc;                                                                                              \
-    LaunchCfg lc(dim3((unsigned)lay.Poblk), dim3(Cfg::THREADS), Cfg::SMEM, st, p->use_pdl);                          \
+    LaunchCfg lc(dim3(grid), dim3(Cfg::THREADS), Cfg::SMEM, st, p->use_pdl);                                        \
     DELTA_CUDA_CHECK(cudaLaunchKernelEx(&lc.cfg, pair_kernel<L, FULL_, GAPALL_>, reinterpret_cast<const float2 *>(d_S), \
-                                        d_rsq, rpart, nrp, rp_stride, rscale, list, p->d_tw(), p->d_ftab2(), lay, pc, \
-                                        d_G, d_A, d_P, d_R, p->d_trace));                                                       \
+                                        d_rsq, d_rnorm, list, p->d_tw(), p->d_ftab(), lay, pc, d_G, d_A, d_P, d_R)); \
   } while (0)
   const bool gapall = d_G && d_A && d_P;
   if (full && gapall) DELTA_PAIR_LAUNCH(true, true);
@@ -483,15 +504,15 @@ static int launch_pair_L(delta_plan *p, const float *d_S, const float *d_rsq, co
   return DELTA_OK;
 }
 
-int launch_pair(delta_plan *p, const float *d_S, const float *d_rsq, const float *rpart, int nrp, int rp_stride, float rscale,
-                float *d_G, float *d_A, float *d_P, float *d_R, cudaStream_t st) {
-#define CALL(LL) launch_pair_L<LL>(p, d_S, d_rsq, rpart, nrp, rp_stride, rscale, d_G, d_A, d_P, d_R, st)
+int launch_pair(delta_plan *p, const float *d_S, const float *d_rsq, const float *d_rnorm, float *d_G, float *d_A, float *d_P,
+                float *d_R, cudaStream_t st) {
+#define CALL(LL) launch_pair_L<LL>(p, d_S, d_rsq, d_rnorm, d_G, d_A, d_P, d_R, st)
   DELTA_SWITCH_L(p->lay.L, CALL)
 #undef CALL
 }
 
-int launch_auto_prep(delta_plan *p, const float *d_auto, float *d_rsq, float *d_rsum, cudaStream_t st) {
-  auto_prep_kernel<<<(unsigned)p->lay.C, 32, 0, st>>>(d_auto, d_rsq, d_rsum, p->lay.F, p->lay.Fp);
+int launch_auto_prep(delta_plan *p, const float *d_auto, float *d_rsq, float *d_rnorm, cudaStream_t st) {
+  auto_prep_kernel<<<(unsigned)p->lay.C, 32, 0, st>>>(d_auto, d_rsq, d_rnorm, p->lay);
   p->launches++;
   DELTA_CUDA_CHECK(cudaGetLastError());
   return DELTA_OK;

@@ -199,10 +199,7 @@ struct StftCfg {
   static constexpr int N = L / 2;
   using G = FftGeom<N>;
   static constexpr int T = G::T;
-#ifndef DELTA_STFT_CH
-#define DELTA_STFT_CH 2
-#endif
-  static constexpr int CH = (N <= 256) ? DELTA_STFT_CH : (N == 512 ? 2 : 1);  // channels per CTA
+  static constexpr int CH = N <= 512 ? 2 : 1;  // channels per CTA
   static constexpr int NFFT = CH * kSegBlock;                      // transforms per CTA
   static constexpr int THREADS = NFFT * T;
   static constexpr int CHPAD = CH > 1 ? 16 / CH : 0;                 // float2 skew between channels (bank spread)
@@ -249,7 +246,7 @@ __global__ void __launch_bounds__(StftCfg<L>::THREADS, 1024 / StftCfg<L>::THREAD
 stft_kernel(const void *__restrict__ x, int64_t ld, int in_dtype, int norm_mode, int n_first,
             const double *__restrict__ offs, const long long *__restrict__ isum, const float2 *__restrict__ tw,
             const float *__restrict__ win, const float2 *__restrict__ ftab, Layout lay, void *__restrict__ Xout,
-            float *__restrict__ chscale, float *__restrict__ wpart, long long *trace) {
+            float *__restrict__ wpart) {
   using Cfg = StftCfg<L>;
   using G = typename Cfg::G;
   constexpr int N = Cfg::N, T = Cfg::T, E = G::E, CH = Cfg::CH;
@@ -261,17 +258,9 @@ stft_kernel(const void *__restrict__ x, int64_t ld, int in_dtype, int norm_mode,
   __shared__ float cmax[CH];                 // per-channel max |y| over this CTA's segments (read by the cluster)
   __shared__ float csc[CH];                  // per-channel fp16 scale
 
-  // debug: globaltimer stamps of the CTA's phases (delta_debug_set_trace): trace[32768 + 8 cta + k]
-  auto stamp = [&](int k) {
-    if (trace && threadIdx.x == 0) {
-      long long gtm;
-      asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(gtm));
-      trace[32768 + 8 * ((int64_t)blockIdx.y * gridDim.x + blockIdx.x) + k] = gtm;
-    }
-  };
-  stamp(0);
+  // tensor-core mode: the per-channel fp16 scales travel with the operands (C floats behind the planes of the X buffer)
+  float *chscale = reinterpret_cast<float *>(reinterpret_cast<char *>(Xout) + lay.x_scale_off);
   pdl_launch_dependents();
-#ifndef DELTA_STFT_NO_PREFETCH
   {
     // L2 prefetch of the CTA's samples, one request per 128-byte line.  It is a hint without a data dependence, so it
     // is issued before pdl_wait (while the predecessor drains) and with far more lines in flight than demand loads get:
@@ -289,9 +278,7 @@ stft_kernel(const void *__restrict__ x, int64_t ld, int in_dtype, int norm_mode,
       }
     }
   }
-#endif
-  pdl_wait();  // the chunk may come from the caller's previous kernel; X, wpart and chscale are read by ours
-  stamp(1);
+  pdl_wait();  // the chunk may come from the caller's previous kernel; X, wpart and the scales are read by ours
 
   const int tid = threadIdx.x, g = tid / T, gt = tid % T;
   const int cl = g / kSegBlock, kk = g % kSegBlock;
@@ -391,8 +378,6 @@ stft_kernel(const void *__restrict__ x, int64_t ld, int in_dtype, int norm_mode,
         v[u] = make_float2(v[u].x * wv[u].x, v[u].y * wv[u].y);
       }
     }
-    if (v[0].x == 123.456f) stamp(7);  // keep v live
-    stamp(6);  // samples in registers
     {  // energy of the windowed segment (zero-lag autocorrelation of Eq. 1d by Parseval), fixed summation order
       float ss = 0.f;
 #pragma unroll
@@ -421,7 +406,6 @@ stft_kernel(const void *__restrict__ x, int64_t ld, int in_dtype, int norm_mode,
       }
       cg::this_cluster().barrier_arrive();
     }
-    stamp(2);  // samples loaded, windowed, energy and max reduced
     fft_inplace<N, false>(v, FftPadMap{buf}, ftab, gt);
     fft_group_sync<T>();  // every read-back of the group is done before Z overwrites the buffer
 #pragma unroll
@@ -452,7 +436,6 @@ stft_kernel(const void *__restrict__ x, int64_t ld, int in_dtype, int norm_mode,
     __syncthreads();           // csc is visible to the CTA
   }
 
-  stamp(3);  // FFT done, scale agreed
   // Phase 2.  Bins f and N - f come from the same pair Z[f], Z[N-f]:  with e = (Z[f] + conj Z[N-f])/2,
   // d = (Z[f] - conj Z[N-f])/2 and (a, b) = e^{-2 pi i f/L} d:  X[f] = (e.x + b, e.y - a),  X[N-f] = (e.x - b, -e.y - a).
   // One thread does both for the 8 segments of the CTA; bin N/2 (its own partner) is done once.
@@ -523,15 +506,13 @@ stft_kernel(const void *__restrict__ x, int64_t ld, int in_dtype, int norm_mode,
     store_bin(c, pcl, f, re, im);
     if (2 * f != N) store_bin(c, pcl, N - f, re2, im2);
   }
-  stamp(4);  // write-out issued
   if (CLUSTER) cg::this_cluster().barrier_wait();  // no CTA exits while its cmax may still be read
-  stamp(5);
 }
 
 // test accessor: X layout -> complex64 [C][K][F]
 __global__ void __launch_bounds__(256)
-stft_unpack_kernel(const void *__restrict__ Xin, Layout lay, int tc_mode, const float *__restrict__ chscale,
-                   float2 *__restrict__ out) {
+stft_unpack_kernel(const void *__restrict__ Xin, Layout lay, int tc_mode, float2 *__restrict__ out) {
+  const float *chscale = reinterpret_cast<const float *>(reinterpret_cast<const char *>(Xin) + lay.x_scale_off);
   const int64_t total = (int64_t)lay.C * lay.K * lay.F;
   for (int64_t idx = (int64_t)blockIdx.x * 256 + threadIdx.x; idx < total; idx += (int64_t)gridDim.x * 256) {
     const int f = (int)(idx % lay.F);
@@ -575,7 +556,7 @@ static int launch_stft_LTD(delta_plan *p, const void *d_x, int64_t ld, void *d_X
   LaunchCfg lc(dim3(lay.nkb, (lay.C + Cfg::CH - 1) / Cfg::CH), dim3(Cfg::THREADS), smem, st, p->use_pdl, CLUSTER ? lay.nkb : 0);
   DELTA_CUDA_CHECK(cudaLaunchKernelEx(&lc.cfg, stft_kernel<L, TC, CLUSTER, DETREND>, d_x, ld, p->cfg.in_dtype, p->cfg.norm_mode, p->n_first,
                                       (const double *)p->d_offs(), (const long long *)p->d_isum(), p->d_tw(), p->d_win(),
-                                      p->d_ftab(), lay, d_X, p->d_chscale(), p->d_wpart(), p->d_trace));
+                                      p->d_ftab(), lay, d_X, p->d_wpart()));
   p->launches++;
   DELTA_CUDA_CHECK(cudaGetLastError());
   return DELTA_OK;
@@ -598,7 +579,8 @@ static int launch_stft_L(delta_plan *p, const void *d_x, int64_t ld, void *d_X, 
     chscale_kernel<<<dim3(lay.C, ns), 256, 0, st>>>(d_x, ld, p->cfg.in_dtype, p->cfg.norm_mode, p->n_first, p->d_offs(),
                                                     p->d_isum(), lay.T,
                                                     lay.wsum * (lay.detrend ? 2.f : 1.f),  // |y - mean| <= 2 max|y|
-                                                    p->d_chscale(), p->d_chmax(), p->d_chcnt());
+                                                    reinterpret_cast<float *>(reinterpret_cast<char *>(d_X) + lay.x_scale_off),
+                                                    p->d_chmax(), p->d_chcnt());
     p->launches++;
     DELTA_CUDA_CHECK(cudaGetLastError());
     return launch_stft_LT<L, true, false>(p, d_x, ld, d_X, st);
@@ -612,12 +594,38 @@ int launch_stft(delta_plan *p, const void *d_x, int64_t ld, void *d_X, cudaStrea
 #undef CALL
 }
 
+// The padding of the X layout (rows C..Cp-1 of every [kc] block, and the blocks kc >= ceil(K/8)) is read by both
+// contractions and written by no kernel: the workspace X is zeroed once, a caller-supplied X here.  One thread per
+// 8-segment run (16 bytes of fp16 or 32 bytes of fp32).
+__global__ void __launch_bounds__(256) stft_pad_zero_kernel(void *__restrict__ Xout, Layout lay, int planes, int elem_bytes) {
+  const int64_t total = (int64_t)lay.F * planes * lay.Kc * lay.Cp;
+  for (int64_t idx = (int64_t)blockIdx.x * 256 + threadIdx.x; idx < total; idx += (int64_t)gridDim.x * 256) {
+    const int c = (int)(idx % lay.Cp);
+    const int kc = (int)((idx / lay.Cp) % lay.Kc);
+    if (c < lay.C && kc < lay.nkb) continue;
+    uint4 *q = reinterpret_cast<uint4 *>(reinterpret_cast<char *>(Xout) + idx * kSegBlock * elem_bytes);
+    q[0] = make_uint4(0u, 0u, 0u, 0u);
+    if (elem_bytes == 4) q[1] = make_uint4(0u, 0u, 0u, 0u);
+  }
+}
+
+int launch_stft_pad_zero(delta_plan *p, void *d_X, cudaStream_t st) {
+  const Layout &lay = p->lay;
+  if (lay.Cp == lay.C && lay.Kc == lay.nkb) return DELTA_OK;
+  const bool tc = p->contraction == DELTA_CONTRACT_TC;
+  const int64_t total = (int64_t)lay.F * (tc ? 4 : 2) * lay.Kc * lay.Cp;
+  const int64_t want = (total + 255) / 256;
+  stft_pad_zero_kernel<<<(unsigned)(want < 148 * 16 ? want : 148 * 16), 256, 0, st>>>(d_X, lay, tc ? 4 : 2, tc ? 2 : 4);
+  p->launches++;
+  DELTA_CUDA_CHECK(cudaGetLastError());
+  return DELTA_OK;
+}
+
 int launch_stft_unpack(delta_plan *p, const void *d_X, float *d_out, cudaStream_t st) {
   const int64_t total = (int64_t)p->lay.C * p->lay.K * p->lay.F;
   const int64_t want = (total + 255) / 256;
   const int blocks = (int)(want < 148 * 16 ? want : 148 * 16);
-  stft_unpack_kernel<<<blocks, 256, 0, st>>>(d_X, p->lay, p->contraction == DELTA_CONTRACT_TC, p->d_chscale(),
-                                             reinterpret_cast<float2 *>(d_out));
+  stft_unpack_kernel<<<blocks, 256, 0, st>>>(d_X, p->lay, p->contraction == DELTA_CONTRACT_TC, reinterpret_cast<float2 *>(d_out));
   p->launches++;
   DELTA_CUDA_CHECK(cudaGetLastError());
   return DELTA_OK;
