@@ -168,3 +168,40 @@ def make(name: str) -> np.ndarray:
     if name == "streamed":
         return streamed()[0]
     raise KeyError(name)
+
+
+# ------------------------------------------------------------------------------------------
+# High-dynamic-range stress inputs ("literal 1/f^2 stress case"): they attack the per-channel scale of
+# the split-fp16 operands of the tensor-core contraction, whose bins far below a channel's strongest component
+# have the fewest significant bits.
+def tone_over_floor(C: int, T: int, floor: float, seed: int, f_tone: float = 31.25e3, shared: float = 0.7) -> np.ndarray:
+    """Unit-amplitude tone (the same frequency in every channel, phase 0.2 c rad) over a white floor of standard
+    deviation `floor`; a fraction `shared` of the floor's amplitude is common to all channels, so that the floor bins
+    are coherent (G > 0.1) and their cross-power counts at the relative tolerance."""
+    rng = np.random.Generator(np.random.PCG64(seed))
+    t = np.arange(T, dtype=np.float64) / FS
+    common = rng.standard_normal(T)
+    x = np.empty((C, T))
+    for c in range(C):
+        own = rng.standard_normal(T)
+        x[c] = np.sin(2 * np.pi * f_tone * t + 0.2 * c) + floor * (shared * common + np.sqrt(1.0 - shared ** 2) * own)
+    return x.astype(np.float32)
+
+
+def power_law(C: int, T: int, seed: int, exponent: float = 2.0, shared: float = 0.7) -> np.ndarray:
+    """Gaussian noise with PSD ~ 1/f^exponent down to the lowest non-zero frequency of the record (no knee, DC
+    removed), unit variance; a common component of amplitude fraction `shared` makes all bins coherent."""
+    rng = np.random.Generator(np.random.PCG64(seed))
+    freqs = np.fft.rfftfreq(T, d=1.0 / FS)
+    colour = np.zeros_like(freqs)
+    colour[1:] = freqs[1:] ** (-exponent / 2.0)
+
+    def coloured():
+        g = np.fft.irfft(np.fft.rfft(rng.standard_normal(T)) * colour, n=T)
+        return g / g.std()
+
+    common = coloured()
+    x = np.empty((C, T))
+    for c in range(C):
+        x[c] = shared * common + np.sqrt(1.0 - shared ** 2) * coloured()
+    return x.astype(np.float32)

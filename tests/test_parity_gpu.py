@@ -239,24 +239,47 @@ def _sampled_pairs(C, n_ch, seed):
     return ch, loc, glob
 
 
+TOLS = dict(P_rel=TOL_P_REL, P_abs=1e-5, G=TOL_G, A=TOL_A, R=TOL_R)
+
+
+def _full_size_check(x, w_nfft, w_hop, w_max_lag, label, n_ch, seed):
+    """Both contraction modes at full size, EVERY output element of every pair compared in float64.
+
+    The oracle's direct DFT with its Python loop over pairs would take hours at these sizes, so all rows are checked
+    with tests/fastcheck.py (float64, numpy rfft / irfft / matmul) -- after that checker has itself been compared with
+    the oracle on a sample of channels of this very input (all pairs among them, first and last channel included)."""
+    import fastcheck as fc
+    b = binding()
+    C = x.shape[0]
+    ch, loc, glob = _sampled_pairs(C, n_ch, seed)
+    ref = oracle_for(x[ch], w_nfft, w_hop, w_max_lag)
+    fast = fc.analyze_sampled(x[ch], w_nfft, w_hop, w_max_lag)
+    for k in ("G", "P", "R", "Sauto"):
+        assert np.max(np.abs(fast[k] - ref[k])) <= 1e-9 * max(1.0, float(np.abs(ref[k]).max())), k
+    assert np.max(np.abs(np.angle(np.exp(1j * (fast["A"] - ref["A"]))))) <= 1e-8
+    outs = {}
+    for name, mode in (("fp32", b.CONTRACT_FP32), ("tc", b.CONTRACT_TC)):
+        _, out = gpu_analyze(x, w_nfft, w_hop, w_max_lag, contraction=mode)
+        P = C * (C - 1) // 2
+        assert out["G"].shape == (P, w_nfft // 2 + 1) and out["R"].shape == (P, 2 * w_max_lag + 1)
+        for k in ("G", "A", "P", "R", "Sauto"):
+            assert np.isfinite(out[k]).all(), (name, k)
+        # the sampled pairs against the oracle itself
+        idx = np.array([o.pair_index(int(i), int(j), C) for i, j in glob])
+        sub = {k: out[k][idx] for k in ("G", "A", "P", "R")}
+        sub["Sauto"] = out["Sauto"][ch]
+        compare(sub, ref, loc, f"{label} sampled {name}")
+        outs[name] = out
+    st = fc.check_all_pairs(x, w_nfft, w_hop, w_max_lag, outs, TOLS, label)
+    print(label, st)
+
+
 @pytest.mark.parametrize("name,n_ch", [("long", 12), ("wide", 10)])
-def test_full_size_configs_on_sampled_pairs(name, n_ch, mode):
-    """Configs 3 and 5 at BASELINE's full sizes; the oracle's direct DFT is run on a sample of
-    channels (all pairs among them, incl. first/last channel), compared element by element."""
+def test_full_size_configs_all_pairs(name, n_ch):
+    """Configs 3 and 5 at BASELINE's full sizes (checked in full): all 18,336 / 73,536 rows of
+    G, A, P, rho and the autospectra, both contraction modes."""
     w = es.WORKLOADS[name]
-    x = es.make(name)
-    _, out = gpu_analyze(x, w.nfft, w.hop, w.max_lag, contraction=mode)
-    assert out["G"].shape == (w.P, w.F) and out["R"].shape == (w.P, 2 * w.max_lag + 1)
-    ch, loc, glob = _sampled_pairs(w.C, n_ch, 42)
-    ref = oracle_for(x[ch], w.nfft, w.hop, w.max_lag)
-    idx = np.array([o.pair_index(int(i), int(j), w.C) for i, j in glob])
-    sub = {k: out[k][idx] for k in ("G", "A", "P", "R")}
-    sub["Sauto"] = out["Sauto"][ch]
-    st = compare(sub, ref, loc, name)
-    print(name, st)
-    # properties that hold at any size, on every output element
-    assert np.isfinite(out["G"]).all() and out["G"].min() >= 0 and out["G"].max() <= 1 + 1e-4
-    assert np.abs(out["R"]).max() <= 1 + 1e-4 and np.abs(out["A"]).max() <= np.pi + 1e-6
+    _full_size_check(es.make(name), w.nfft, w.hop, w.max_lag, name, n_ch, 42)
 
 
 def test_config4_streamed_shot():
@@ -486,25 +509,66 @@ def test_phase_lock_estimator(C, T, L, H, mode):
     assert np.abs(out["Sauto"] / o.scale_factor(L) - 1).max() < 1e-5     # unit phasors: S_cc = s^2 in every bin
 
 
-def test_three_views_576_channels(mode):
+def test_three_views_576_channels():
     """f3: the diagnostic has three 24 x 8 views: 576 channels, 165,600 pairs,
-    nfft 512.  Three independent config-2 arrays with a common component; checked on sampled channels."""
+    nfft 512.  Three independent config-2 arrays with a common component; every row checked, both modes."""
     w = es.WORKLOADS["single"]
     a, b2, c = (es.turbulence(w.T, s) for s in (71, 72, 73))
     x = np.concatenate([a, 0.4 * a + 0.9 * b2, 0.4 * a + 0.9 * c]).astype(np.float32)
-    C = x.shape[0]
-    assert C == 576
-    _, out = gpu_analyze(x, w.nfft, w.hop, w.max_lag, contraction=mode)
-    P = C * (C - 1) // 2
-    assert out["G"].shape == (P, w.F) and P == 165_600
-    ch, loc, glob = _sampled_pairs(C, 10, 7)
-    ref = oracle_for(x[ch], w.nfft, w.hop, w.max_lag)
-    idx = np.array([o.pair_index(int(i), int(j), C) for i, j in glob])
-    sub = {k: out[k][idx] for k in ("G", "A", "P", "R")}
-    sub["Sauto"] = out["Sauto"][ch]
-    st = compare(sub, ref, loc, "576 channels")
-    print(st)
-    assert np.isfinite(out["G"]).all() and out["G"].max() <= 1 + 1e-4 and np.abs(out["R"]).max() <= 1 + 1e-4
+    assert x.shape[0] == 576
+    _full_size_check(x, w.nfft, w.hop, w.max_lag, "576 channels", 10, 7)
+
+
+def test_staged_external_X_with_padding_not_zeroed():
+    """A caller-supplied X buffer whose padding (rows C..Cp-1, segment blocks beyond ceil(K/8)) holds NaN before
+    delta_stft: C = 192 and 128 have Cp == C and an odd number of segment blocks (K = 38: 5 of 6), the case where the
+    contraction reads a block no STFT CTA writes.  Staged results must equal the fused call bit for bit."""
+    b = binding()
+    w = es.WORKLOADS["single"]
+    for C in (192, 128):
+        for mode in (b.CONTRACT_TC, b.CONTRACT_FP32):
+            x = dev(es.single()[:C])
+            plan = b.Plan(C, w.T, w.nfft, w.hop, w.max_lag, contraction=mode)
+            fused = plan.analyze_chunk(x)
+            X = plan.empty_X()
+            X.view(torch.float16 if mode == b.CONTRACT_TC else torch.float32).fill_(float("nan"))
+            plan.stft(x, X)
+            S, Sa = plan.cross_spectra(X)
+            G, A, P, R = plan.coherence(S, Sa), plan.crossphase(S), plan.crosspower(S), plan.crosscorr(S, Sa)
+            torch.cuda.synchronize()
+            for name, t in (("G", G), ("A", A), ("P", P), ("Sauto", Sa)):
+                assert torch.isfinite(t).all(), (C, mode, name)
+                assert torch.equal(t, fused[name]), (C, mode, name)
+            assert torch.max(torch.abs(R - fused["R"])).item() < 5e-6
+
+
+def test_X_buffers_are_self_contained():
+    """delta_stft(x1 -> X1), delta_stft(x2 -> X2), then delta_cross_spectra(X1): the spectra of x1, whatever the plan
+    did in between (the per-channel fp16 scales of the tensor-core mode travel inside the X buffer)."""
+    b = binding()
+    w = es.WORKLOADS["single"]
+    C = 40
+    x1 = es.single()[:C]
+    x2 = (1000.0 * es.turbulence(w.T, 55)[:C]).astype(np.float32)   # very different amplitudes: different scales
+    for mode in (b.CONTRACT_TC, b.CONTRACT_FP32):
+        plan = b.Plan(C, w.T, w.nfft, w.hop, w.max_lag, contraction=mode)
+        X1 = plan.stft(dev(x1))
+        X2 = plan.stft(dev(x2))
+        S1, Sa1 = plan.cross_spectra(X1)
+        S2, Sa2 = plan.cross_spectra(X2)
+        torch.cuda.synchronize()
+        pairs = o.all_pairs(C)
+        s2 = o.scale_factor(w.nfft)
+        for x, S, Sa in ((x1, S1, Sa1), (x2, S2, Sa2)):
+            Xo = o.stft(x, w.nfft, w.hop)
+            So, Sao = o.cross_spectra(Xo, pairs, s2), o.auto_spectra(Xo, s2)
+            den = np.sqrt(Sao[pairs[:, 0]] * Sao[pairs[:, 1]])
+            assert np.max(np.abs(plan.cross_spectra_unpack(S).cpu().numpy() - So) / den) < 1e-5
+            assert np.max(np.abs(Sa.cpu().numpy() - Sao) / Sao) < 1e-4
+        # and the unpack accessor reads the scales from the buffer it is given
+        Xg = plan.stft_unpack(X1).cpu().numpy()
+        Xo = o.stft(x1, w.nfft, w.hop)
+        assert np.abs(Xg - Xo).max() <= 2e-6 * np.abs(Xo).max()
 
 
 @pytest.mark.parametrize("L,Ls,H,detrend,dtype", [(512, 256, 128, 0, "f32"), (1024, 300, 100, 1, "f32"), (256, 129, 64, 0, "i16")])
