@@ -1,12 +1,14 @@
 #!/usr/bin/env python
 """bench.py -- throughput of the all-channel-pairs spectral path (delta_analyze_chunk) on B200.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload single]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+                    [--workload single|long|streamed|wide|views3] [--scaling weak|strong]
 
 One "step" = one pass of the whole hot path (STFT -> cross-spectra -> coherence, cross-phase,
-cross-power, cross-correlation for all pairs) over one synthetic ECEi-shaped chunk (BASELINE.json
-configs[1]: 192 channels x 10,000 float32 samples, nfft 512, 50 % overlap, 18,336 pairs).
-Prints ONE JSON line (rank 0).  See DESIGN.md section 8 for what each number means.
+cross-power, cross-correlation for all pairs) over one synthetic ECEi-shaped chunk.  The default
+workload is BASELINE.json configs[1] (192 channels x 10,000 float32 samples, nfft 512, 50 %
+overlap, 18,336 pairs).  Prints ONE JSON line (rank 0).  See DESIGN.md section 8 for what each
+number means.
 """
 from __future__ import annotations
 
@@ -27,7 +29,16 @@ import ecei_synth as es  # noqa: E402
 
 METRIC = "channel_pair_spectra_per_s"
 UNIT = "pair-spectra/s"
-N_IN, N_OUT = 4, 6   # rotating input chunks / output buffer sets (6 x 94.4 MB > 126 MB L2)
+N_IN = 4            # rotating input chunks
+L2_BYTES = 126e6    # outputs rotate over enough buffer sets to exceed this
+REPEATS = 5         # the K-step timed region is repeated and the median reported (steps stays K)
+
+# the three-view workload: not a BASELINE config, so it lives here
+VIEWS3 = es.Workload("views3", 576, 10_000, 512, 256, 256, "f32")
+
+
+def workload(name):
+    return VIEWS3 if name == "views3" else es.WORKLOADS[name]
 
 
 def load_peaks():
@@ -110,6 +121,11 @@ def rank_chunk_seeds(rank: int, n: int = N_IN):
     return [2 + 100 * i + 1000 * rank for i in range(n)]
 
 
+def shot_chunks_of_rank(n_chunks: int, rank: int, world: int):
+    """Strong scaling of one shot (chunks are independent): chunk n goes to rank n mod world."""
+    return list(range(rank, n_chunks, world))
+
+
 def aggregate_value(pairs_per_step: int, steps: int, world: int, ms_max: float) -> float:
     """Whole-job throughput: units processed by all ranks / max-over-ranks time."""
     return world * pairs_per_step * steps / (ms_max * 1e-3)
@@ -125,14 +141,27 @@ def physical_gpu_index(local_rank: int) -> int:
     return local_rank
 
 
-def alg_bytes(w, in_esz=4):
+def alg_bytes(w):
     """Algorithmic bytes per chunk: read the chunk once, write every requested
     output once.  X, S and tables are implementation intermediates and are not counted."""
-    inp = w.C * w.T * in_esz
+    inp = w.C * w.T * (2 if w.dtype == "i16" else 4)
     gap = 3 * w.P * w.F * 4
     rho = w.P * (2 * w.max_lag + 1) * 4
     auto = w.C * w.F * 4
     return dict(input=inp, gap=gap, rho=rho, auto=auto, total=inp + gap + rho + auto)
+
+
+def host_chunks(w, rank, n):
+    """n float32 (or, for the streamed shot, int16) chunks [C][T] of the workload, seeded per rank."""
+    if w.name == "views3":
+        out = []
+        for s in rank_chunk_seeds(rank, n):
+            a, b2, c = (es.turbulence(w.T, s + k) for k in (0, 7, 13))
+            out.append(np.concatenate([a, 0.4 * a + 0.9 * b2, 0.4 * a + 0.9 * c]).astype(np.float32))
+        return out
+    if w.name == "wide":
+        return [es.wide(s, s + 50) for s in rank_chunk_seeds(rank, n)]
+    return [es.turbulence(w.T, s) for s in rank_chunk_seeds(rank, n)]
 
 
 def oracle_chunk(x, w):
@@ -148,20 +177,35 @@ def blas_threads():
         return os.cpu_count() or 1
 
 
-def cpu_baseline(w, budget_s=12.0):
-    """The oracle as it stands, timed on this box's host cores on whole chunks of the workload."""
-    xs = [es.turbulence(w.T, 9000 + i) for i in range(2)]
-    t0 = time.perf_counter()
-    n = 0
-    while True:
-        oracle_chunk(xs[n % 2], w)
-        n += 1
-        dt = time.perf_counter() - t0
-        if dt >= budget_s or n >= 64:
-            break
-    return {"value": w.P * n / dt, "unit": UNIT, "cores": blas_threads(), "kind": "oracle",
-            "sample": f"{n} whole chunk(s) of the '{w.name}' workload ({w.C}x{w.T} f32, all {w.P} pairs, G+A+P+rho), "
-                      f"float64 direct-DFT numpy oracle, {dt:.1f} s", "seconds": dt}
+def cpu_baseline(w, budget_s=10.0):
+    """Two CPU figures on this box's host cores, on a bounded sample of the workload (same generator, float32 input):
+    the oracle as it stands (float64, direct DFT) and -- labelled as such -- the same float64 pipeline with numpy's FFT
+    (BASELINE.md section 3).  Channel subsets keep each at ~10 s; the unit is still pair-spectra/s."""
+    from oracle import fft_baseline as fb
+    x_full = host_chunks(w, 0, 1)[0] if w.dtype == "f32" else es.turbulence(w.T, 9000)
+    # oracle: cost grows with pairs; time 16 channels, then as many as the budget allows
+    def timed(fn, x):
+        t0 = time.perf_counter()
+        fn(x)
+        return time.perf_counter() - t0
+    n0 = min(16, w.C)
+    t16 = timed(lambda x: oracle_chunk(x, w), x_full[:n0])
+    n_or = int(max(n0, min(w.C, n0 * np.sqrt(budget_s / max(t16, 1e-3)))))
+    t_or = timed(lambda x: oracle_chunk(x, w), x_full[:n_or]) if n_or > n0 else t16
+    P_or = n_or * (n_or - 1) // 2
+    n1 = min(48, w.C)
+    t48 = timed(lambda x: fb.analyze_chunk(x, w.nfft, w.hop, w.max_lag), x_full[:n1])
+    n_fb = int(max(n1, min(w.C, n1 * np.sqrt(budget_s / max(t48, 1e-3)))))
+    t_fb = timed(lambda x: fb.analyze_chunk(x, w.nfft, w.hop, w.max_lag), x_full[:n_fb]) if n_fb > n1 else t48
+    P_fb = n_fb * (n_fb - 1) // 2
+    cores = blas_threads()
+    return {"value": P_or / t_or, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"the first {n_or} channels ({P_or} pairs) of one '{w.name}' chunk ({w.T} samples, nfft {w.nfft}), "
+                      f"all four quantities, float64 direct-DFT numpy oracle, {t_or:.1f} s", "seconds": t_or,
+            "library_fft": {"value": P_fb / t_fb, "unit": UNIT, "cores": cores, "kind": "CPU, library FFT",
+                            "sample": f"the first {n_fb} channels ({P_fb} pairs) of the same chunk, float64 numpy rfft / "
+                                      f"matmul / ifft (oracle/fft_baseline.py, pinned to the oracle), {t_fb:.1f} s",
+                            "seconds": t_fb}}
 
 
 # --------------------------------------------------------------------------------------------
@@ -170,19 +214,16 @@ def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    w = es.WORKLOADS[args.workload]
-    x_full = es.turbulence(w.T, 2)
+    w = workload(args.workload)
+    x_full = host_chunks(w, 0, 1)[0]
     # bounded sample per step so that (W + K) steps end within a few minutes
+    n0 = min(32, w.C)
     t0 = time.perf_counter()
-    oracle_chunk(x_full[:48], w)
-    t48 = time.perf_counter() - t0
+    oracle_chunk(x_full[:n0], w)
+    t32 = time.perf_counter() - t0
     budget = 150.0
-    n_ch = w.C
     steps_total = args.steps + args.warmup
-    # oracle cost ~ a*C + b*C^2; take the pair term as dominant for the estimate (conservative)
-    est_full = t48 * (w.C / 48.0) ** 2
-    if est_full * steps_total > budget:
-        n_ch = int(max(8, min(w.C, 48.0 * np.sqrt(budget / steps_total / t48))))
+    n_ch = int(max(8, min(w.C, n0 * np.sqrt(budget / steps_total / max(t32, 1e-3)))))
     x = x_full[:n_ch]
     P = n_ch * (n_ch - 1) // 2
     for _ in range(args.warmup):
@@ -198,7 +239,7 @@ def run_reference(args):
             "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": w.name, "channels": w.C, "samples": w.T, "nfft": w.nfft, "hop": w.hop,
-                       "pairs": w.P, "max_lag": w.max_lag, "sample": sample},
+                       "segments": w.K, "pairs": w.P, "max_lag": w.max_lag, "sample": sample},
             "cpu_baseline": {"value": val, "unit": UNIT, "cores": blas_threads(), "kind": "oracle", "sample": sample},
             "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
@@ -221,38 +262,62 @@ def run_ours(args):
 
     from paper_2108_08896_b200 import binding as b
 
-    w = es.WORKLOADS[args.workload]
+    w = workload(args.workload)
+    streamed = w.name == "streamed"
+    strong = args.scaling == "strong"
+    if strong and not streamed:
+        raise SystemExit("--scaling strong splits the chunks of one shot over the ranks: use --workload streamed")
     peaks = load_peaks()
     contraction = {"auto": b.CONTRACT_AUTO, "fp32": b.CONTRACT_FP32, "tc": b.CONTRACT_TC}[args.contraction]
+    plan_kw = dict(contraction=contraction)
+    if streamed:
+        plan_kw.update(in_dtype=b.I16, norm_mode=b.NORM_RELATIVE)
     # chunks are independent, so `inflight` of them are kept in flight: one plan (= one workspace)
     # and one CUDA stream each; a plan is never used from two streams at once (include/delta.h)
-    plans = [b.Plan(w.C, w.T, w.nfft, w.hop, w.max_lag, contraction=contraction) for _ in range(max(1, args.inflight))]
+    plans = [b.Plan(w.C, w.T, w.nfft, w.hop, w.max_lag, **plan_kw) for _ in range(max(1, args.inflight))]
     streams = [torch.cuda.Stream() for _ in plans]
     plan = plans[0]
     s = plan.sizes
-    # inputs resident in HBM before the timed region; every rank works on its own chunks (weak scaling)
-    xs_host = [es.turbulence(w.T, seed) for seed in rank_chunk_seeds(rank)]
-    xs = [torch.from_numpy(x).cuda() for x in xs_host]
-    outs = [plan.empty_outputs() for _ in range(N_OUT)]
+    ab = alg_bytes(w)
     K, W = args.steps, args.warmup
+
+    # ---- inputs resident in HBM before the timed region ------------------------------------------
+    if streamed:
+        # one shot: 250 int16 chunks; weak scaling: every rank its own shot; strong: rank r takes chunks r, r + world, ...
+        counts, _ = es.streamed(seed=4 + (0 if strong else 1000 * rank), n_chunks=w.n_chunks)
+        mine = shot_chunks_of_rank(w.n_chunks, rank, world) if strong else list(range(w.n_chunks))
+        shot_dev = torch.from_numpy(counts).cuda()
+        xs = [shot_dev[n] for n in mine]
+        first = shot_dev[0]                                      # the offsets come from the first chunk of the shot (R1);
+        for p_ in plans:                                         # every rank recomputes them from chunk 0, no broadcast
+            p_.set_offsets(first, w.n_first)
+        xs_host = None
+    else:
+        xs_host = host_chunks(w, rank, N_IN)
+        xs = [torch.from_numpy(x).cuda() for x in xs_host]
+    out_bytes = ab["gap"] + ab["rho"] + ab["auto"]
+    n_out = max(2 * len(plans), int(np.ceil(4.5 * L2_BYTES / out_bytes)))
+    n_out = (n_out + len(plans) - 1) // len(plans) * len(plans)
+    outs = [plan.empty_outputs() for _ in range(n_out)]
+    n_in = len(xs)
 
     def barrier():
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
 
-    per_stream = max(1, N_OUT // len(plans))
+    per_stream = n_out // len(plans)
 
     def out_set(k):
         # every stream rotates over its own output sets (no two streams ever write the same buffers)
         i = k % len(plans)
-        return (i * per_stream + (k // len(plans)) % per_stream) % N_OUT
+        return i * per_stream + (k // len(plans)) % per_stream
 
-    def steps(n, first=0):
-        # step k runs on stream k % inflight; a buffer set is reused only after N_OUT further steps
-        for k in range(first, first + n):
+    def steps(n, first_k=0):
+        # step k runs on stream k % inflight; a buffer set is reused only after n_out further steps
+        for k in range(first_k, first_k + n):
             i = k % len(plans)
-            plans[i].analyze_chunk(xs[k % N_IN], outs[out_set(k)], stream=streams[i])
+            plans[i].analyze_chunk(xs[k % n_in], outs[out_set(k)], stream=streams[i])
 
     main = torch.cuda.current_stream()
 
@@ -268,32 +333,39 @@ def run_ours(args):
         e1.record(main)
         return e0, e1
 
-    steps(W)
+    steps(max(W, 3))
     torch.cuda.synchronize()
     launches_per_step = plan.last_launch_count
 
-    # ---- timed region: exactly K steps ----------------------------------------------------------
+    # ---- timed region: exactly K steps, repeated; the median of the repeats is reported --------
     sampler = ClockSampler(physical_gpu_index(local_rank))
     barrier()
     sampler.start()
-    t_cpu0 = time.perf_counter()
-    e0, e1 = timed(K)
-    t_cpu = time.perf_counter() - t_cpu0   # host time to enqueue the K steps (must stay below the device time)
-    barrier()
+    reps, t_cpu = [], []
+    for _ in range(REPEATS):
+        barrier()
+        t0 = time.perf_counter()
+        e0, e1 = timed(K)
+        t_cpu.append(time.perf_counter() - t0)   # host time to enqueue the K steps (must stay below the device time)
+        barrier()
+        reps.append(max_over_ranks(e0.elapsed_time(e1), world))
     clocks = sampler.stop()
-    ms = max_over_ranks(e0.elapsed_time(e1), world)
+    ms = float(np.median(reps))
 
     # the same K steps on ONE stream (no chunk overlap), for reference
-    barrier()
-    g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    g0.record()
-    for k in range(K):
-        plan.analyze_chunk(xs[k % N_IN], outs[k % N_OUT])
-    g1.record()
-    barrier()
-    ms_serial = max_over_ranks(g0.elapsed_time(g1), world)
+    serial = []
+    for _ in range(3):
+        barrier()
+        g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        g0.record()
+        for k in range(K):
+            plan.analyze_chunk(xs[k % n_in], outs[k % n_out])
+        g1.record()
+        barrier()
+        serial.append(max_over_ranks(g0.elapsed_time(g1), world))
+    ms_serial = float(np.median(serial))
 
-    # ---- per-stage durations (same K steps again, events recorded between the kernels) ----------
+    # ---- per-stage durations (same steps again, events recorded between the kernels) -------------
     Ks = min(K, 400)
     evs = [[torch.cuda.Event(enable_timing=True) for _ in range(4)] for _ in range(Ks)]
     for row in evs:
@@ -302,17 +374,16 @@ def run_ours(args):
     torch.cuda.synchronize()
     for k in range(Ks):
         plan.set_stage_events(evs[k])
-        plan.analyze_chunk(xs[k % N_IN], outs[k % N_OUT])
+        plan.analyze_chunk(xs[k % n_in], outs[k % n_out])
     plan.set_stage_events(None)
     torch.cuda.synchronize()
     stage_ms = np.array([[row[i].elapsed_time(row[i + 1]) for i in range(3)] for row in evs])
-    stage_mean = stage_ms.mean(axis=0)
-    ab = alg_bytes(w)
+    stage_mean = np.median(stage_ms, axis=0)
     tc = s.contraction == b.CONTRACT_TC
     flops_contract = 8.0 * (w.P + w.C) * w.F * w.K   # useful FP32-equivalent flops of Eq. (1a), Hermitian half
     alu_peak_tf = 148 * 128 * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
     stages = [
-        {"kernel": "stft_kernel" + ("+chscale_kernel" if tc else ""), "ms": float(stage_mean[0]), "bound": "hbm",
+        {"kernel": "stft_kernel" + ("+chscale_kernel" if tc and s.K > 64 else ""), "ms": float(stage_mean[0]), "bound": "hbm",
          "alg_bytes": ab["input"], "achieved": ab["input"] / (stage_mean[0] * 1e-3) / 1e9, "unit": "GB/s"},
         {"kernel": "contract_tc_kernel" if tc else "contract_fp32_kernel", "ms": float(stage_mean[1]),
          "bound": "tensor" if tc else "alu", "alg_flops": flops_contract,
@@ -329,11 +400,13 @@ def run_ours(args):
         peak, peak_src = alu_peak_tf, "148 SMs x 128 FP32 lanes x 2 flop x sm_max_mhz (DESIGN.md section 7)"
     else:
         peak, peak_src = peaks["bf16_tflops"], f"MEASURED_PEAKS.json bf16_tflops burst ({peaks['source']}); fp16 kind::f16"
+    # DRAM traffic of the dominant kernel per launch: from the committed ncu capture of this workload (dram bytes summed over
+    # consecutive steps with --cache-control none, profiles/r02_traffic.json.txt); null if there is none for it
     traffic = None
-    tpath = os.path.join(ROOT, "profiles", "ncu_traffic.json.txt")
+    tpath = os.path.join(ROOT, "profiles", "r02_traffic.json.txt")
     if os.path.exists(tpath):
         try:
-            traffic = json.load(open(tpath)).get(d["kernel"].split("+")[0])
+            traffic = json.load(open(tpath)).get(w.name, {}).get(d["kernel"].split("+")[0])
         except Exception:
             traffic = None
     roofline = {"kernel": d["kernel"], "bound": d["bound"], "achieved": d["achieved"], "peak": peak, "unit": d["unit"],
@@ -345,19 +418,34 @@ def run_ours(args):
                              "frac_of_8TBs": ab["total"] / (ms / K * 1e-3) / 1e9 / 8000.0}}
 
     # ---- end to end through the C ABI with HOST buffers (H2D + D2H inside the timed region) ------
-    n_e2e = max(1, min(K, 12))
-    h_x = torch.from_numpy(np.stack([xs_host[i % N_IN] for i in range(n_e2e)])).pin_memory()
-    host_out = dict(G=torch.empty((n_e2e, s.P, s.F)).pin_memory(), A=torch.empty((n_e2e, s.P, s.F)).pin_memory(),
-                    P=torch.empty((n_e2e, s.P, s.F)).pin_memory(), R=torch.empty((n_e2e, s.P, s.n_lags)).pin_memory(),
-                    Sauto=torch.empty((n_e2e, w.C, s.F)).pin_memory())
+    if streamed:
+        # the whole shot (this rank's chunks) from pinned host memory through delta_analyze_shot_host: H2D of chunk n+1 on
+        # the side stream under the kernels of chunk n; outputs stay on the device, the
+        # autospectra of every chunk are read back (the per-step result)
+        sel = counts[mine]
+        h_x = torch.from_numpy(np.ascontiguousarray(sel)).pin_memory()
+        n_e2e = h_x.shape[0]
+        host_out = dict(Sauto=torch.empty((n_e2e, w.C, s.F)).pin_memory())
+        d2h = ab["auto"]
+        call = ("delta_analyze_shot_host: the shot's int16 chunks from pinned host memory, H2D on the side stream, G/A/P/rho "
+                "left on the device (rotating sets), autospectra of every chunk copied back")
+    else:
+        n_e2e = max(1, min(K, 12 if out_bytes < 200e6 else 3))
+        h_x = torch.from_numpy(np.stack([xs_host[i % N_IN] for i in range(n_e2e)])).pin_memory()
+        host_out = dict(G=torch.empty((n_e2e, s.P, s.F)).pin_memory(), A=torch.empty((n_e2e, s.P, s.F)).pin_memory(),
+                        P=torch.empty((n_e2e, s.P, s.F)).pin_memory(), R=torch.empty((n_e2e, s.P, s.n_lags)).pin_memory(),
+                        Sauto=torch.empty((n_e2e, w.C, s.F)).pin_memory())
+        d2h = out_bytes
+        call = "delta_analyze_shot_host: pinned host chunks in, all five outputs copied back to pinned host memory"
     slots = torch.empty(plan.slot_bytes(), dtype=torch.uint8, device="cuda")
     dev_out = dict(G=torch.empty((2, s.P, s.F), device="cuda"), A=torch.empty((2, s.P, s.F), device="cuda"),
                    P=torch.empty((2, s.P, s.F), device="cuda"), R=torch.empty((2, s.P, s.n_lags), device="cuda"),
                    Sauto=torch.empty((2, w.C, s.F), device="cuda"))
 
     def e2e_once():
-        # D2H copies run on the launching stream right after each chunk, so one device output set suffices
-        plan.analyze_shot_host(h_x, slots, dev_out, strides=(0, 0, 0), host_out=host_out)
+        # two device output sets: the copy-back of chunk n runs on the library's copy stream under the kernels of chunk n + 1
+        plan.analyze_shot_host(h_x, slots, dev_out, strides=(s.P * s.F, s.P * s.n_lags, w.C * s.F), host_out=host_out,
+                               set_offsets=streamed, n_first=w.n_first, ring=2)
 
     e2e_once()
     barrier()
@@ -367,10 +455,8 @@ def run_ours(args):
     f1.record()
     barrier()
     e2e_ms = max_over_ranks(f0.elapsed_time(f1), world)
-    d2h = ab["gap"] + ab["rho"] + ab["auto"]
     e2e = {"value": aggregate_value(w.P, n_e2e, world, e2e_ms), "unit": UNIT, "h2d_bytes_per_step": ab["input"],
-           "d2h_bytes_per_step": d2h, "steps": n_e2e, "ms_per_step": e2e_ms / n_e2e,
-           "call": "delta_analyze_shot_host: pinned host chunks in, all five outputs copied back to pinned host memory"}
+           "d2h_bytes_per_step": d2h, "steps": n_e2e, "ms_per_step": e2e_ms / n_e2e, "call": call}
 
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
@@ -378,17 +464,20 @@ def run_ours(args):
 
     if rank == 0:
         value = aggregate_value(w.P, K, world, ms)
+        scaling = "strong" if strong else "weak"
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
-                "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                "ms_per_step": ms / K, "higher_is_better": True, "scaling": scaling, "vs_baseline": None,
                 "dtype": "f32", "data": "synthetic",
                 "config": {"workload": w.name, "channels": w.C, "samples": w.T, "nfft": w.nfft, "hop": w.hop,
-                           "segments": w.K, "pairs": w.P, "max_lag": w.max_lag, "outputs": "G,A,P,rho,autospectra",
+                           "segments": w.K, "pairs": w.P, "max_lag": w.max_lag, "input": w.dtype, "outputs": "G,A,P,rho,autospectra",
                            "contraction": "tcgen05 split-fp16" if tc else "fp32 fma",
-                           "l2_policy": f"inputs rotate over {N_IN} chunks, outputs over {N_OUT} buffer sets "
-                                        f"({N_OUT * (ab['gap'] + ab['rho']) / 1e6:.0f} MB > 126 MB L2)",
-                           "chunks_in_flight": len(plans),
-                           "parallelism": f"chunk-parallel replicas x{world}, no collective"},
-                "ms_per_step_one_stream": ms_serial / K, "host_enqueue_ms_per_step": 1e3 * t_cpu / K,
+                           "l2_policy": f"inputs rotate over {n_in} chunks, outputs over {n_out} buffer sets "
+                                        f"({n_out * out_bytes / 1e6:.0f} MB > 126 MB L2)",
+                           "chunks_in_flight": len(plans), "timed_region_repeats": REPEATS,
+                           "parallelism": (f"one shot's chunks dealt round-robin to {world} replicas, no collective" if strong
+                                           else f"chunk-parallel replicas x{world}, no collective")},
+                "ms_per_step_repeats": [r / K for r in reps],
+                "ms_per_step_one_stream": ms_serial / K, "host_enqueue_ms_per_step": 1e3 * float(np.median(t_cpu)) / K,
                 "samples_per_s": world * w.C * w.T * K / (ms * 1e-3),
                 "clocks": clocks, "e2e": e2e, "gpu_launches": launches_per_step * K, "roofline": roofline,
                 "cpu_baseline": cpu}
@@ -400,19 +489,23 @@ def run_ours(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=1000)
-    ap.add_argument("--warmup", type=int, default=100)
+    ap.add_argument("--steps", type=int, default=None)
+    ap.add_argument("--warmup", type=int, default=None)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="single", choices=["single"])
+    ap.add_argument("--workload", default="single", choices=["single", "long", "streamed", "wide", "views3"])
+    ap.add_argument("--scaling", default="weak", choices=["weak", "strong"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--contraction", default="auto", choices=["auto", "fp32", "tc"])
     ap.add_argument("--inflight", type=int, default=2, help="independent chunks kept in flight (plans x streams)")
     args = ap.parse_args()
     if args.impl == "reference":
-        if args.steps == 1000 and args.warmup == 100:   # defaults are sized for the GPU arm
-            args.steps, args.warmup = 20, 3
+        args.steps = 20 if args.steps is None else args.steps   # defaults sized per arm
+        args.warmup = 3 if args.warmup is None else args.warmup
         run_reference(args)
     else:
+        big = args.workload in ("long", "wide", "views3")
+        args.steps = (100 if big else 1000) if args.steps is None else args.steps
+        args.warmup = (10 if big else 100) if args.warmup is None else args.warmup
         run_ours(args)
 
 

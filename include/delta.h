@@ -41,7 +41,7 @@
 extern "C" {
 #endif
 
-#define DELTA_VERSION 105 /* 0.1.5: band-pass, windows, detrend, estimator, nperseg in delta_config; delta_accumulate; pair lists */
+#define DELTA_VERSION 200 /* 0.2.0: out_ring in delta_analyze_shot_host; scales inside X buffers; DELTA_ERR_NO_MEMORY */
 
 typedef enum {
   DELTA_OK = 0,
@@ -178,18 +178,22 @@ int delta_accumulate(delta_plan *plan, float *d_S_acc, float *d_Sauto_acc, const
 int delta_analyze_chunk(delta_plan *plan, const void *d_x, int64_t ld,
                         float *d_G, float *d_A, float *d_P, float *d_R, float *d_Sauto, void *stream);
 
-/* a6: a whole shot from HOST memory.  h_x: [n_chunks][C][T] of in_dtype (pinned memory for true
- * overlap), chunk n+1 is copied host->device on an internal side stream while chunk n is analysed on
- * `stream` (two device input slots taken from d_slots, >= 2*C*T*sizeof(in_dtype) bytes, 256-byte
- * aligned).  If set_offsets != 0 the offsets are taken from the first n_first samples of chunk 0.
- * Device outputs: chunk n goes to d_X + n*stride_X elements (stride may be 0 to overwrite; NULL
- * pointer = skip).  Host outputs (any may be NULL): if non-NULL, chunk n's result is copied
- * device->host to h_X + n*(its full size) after it is computed.  Returns after enqueuing; the
- * caller synchronises `stream`. */
+/* a6: a whole shot from HOST memory ("streamed as chunks of 10,000 samples"; ~500 MB/s stream, L201).
+ * h_x: [n_chunks][C][T] of in_dtype (pinned memory for true overlap).  Chunk n+1 is copied host->device on an
+ * internal side stream while chunk n is analysed on `stream` (two device input slots taken from d_slots,
+ * >= 2*C*T*sizeof(in_dtype) bytes, 256-byte aligned).  If set_offsets != 0 the offsets are taken from the first
+ * n_first samples of chunk 0.
+ * Device outputs (NULL pointer = that quantity is skipped): chunk n goes to output set  n mod out_ring  (out_ring = 0:
+ * every chunk its own set, n), set s starting s*stride_X elements into d_X (a stride of 0 makes all sets one).
+ * Host outputs (any may be NULL): chunk n's result is copied device->host to h_X + n*(its full size) on a second
+ * internal stream, under the kernels of the following chunks; an output set is not overwritten before its
+ * copy-back is over (out_ring <= 64 when host outputs are requested and sets are reused, else
+ * DELTA_ERR_UNSUPPORTED).  Returns after enqueuing; `stream` ends after the last copy-back, so the caller
+ * synchronises that one stream. */
 int delta_analyze_shot_host(delta_plan *plan, const void *h_x, int32_t n_chunks, void *d_slots,
                             int32_t set_offsets, int32_t n_first,
                             float *d_G, float *d_A, float *d_P, float *d_R, float *d_Sauto,
-                            int64_t stride_GAP, int64_t stride_R, int64_t stride_auto,
+                            int64_t stride_GAP, int64_t stride_R, int64_t stride_auto, int32_t out_ring,
                             float *h_G, float *h_A, float *h_P, float *h_R, float *h_Sauto,
                             void *stream);
 

@@ -68,7 +68,7 @@ def _load() -> C.CDLL:
     lib.delta_crosscorr.argtypes = [vp, vp, vp, vp, vp]
     lib.delta_accumulate.argtypes = [vp, vp, vp, vp, vp, C.c_float, C.c_float, vp]
     lib.delta_analyze_chunk.argtypes = [vp, vp, i64, vp, vp, vp, vp, vp, vp]
-    lib.delta_analyze_shot_host.argtypes = [vp, vp, i32, vp, i32, i32, vp, vp, vp, vp, vp, i64, i64, i64,
+    lib.delta_analyze_shot_host.argtypes = [vp, vp, i32, vp, i32, i32, vp, vp, vp, vp, vp, i64, i64, i64, i32,
                                             vp, vp, vp, vp, vp, vp]
     lib.delta_last_launch_count.argtypes = [vp]
     lib.delta_plan_set_stage_events.argtypes = [vp, C.POINTER(vp)]
@@ -238,15 +238,15 @@ class Plan:
                "delta_analyze_chunk")
         return out
 
-    def analyze_shot_host(self, h_x, slots, dev_out, strides=(0, 0, 0), host_out=None, set_offsets=False, n_first=0):
+    def analyze_shot_host(self, h_x, slots, dev_out, strides=(0, 0, 0), host_out=None, set_offsets=False, n_first=0, ring=0):
         """h_x: pinned host tensor [n_chunks][C][T]; slots: device uint8 buffer (2 input slots);
-        dev_out: dict of device tensors (chunk n at offset n*stride elements); host_out: dict of pinned
-        host tensors [n_chunks][...] or None."""
+        dev_out: dict of device tensors (chunk n in set n mod ring, or n if ring == 0, at set*stride elements);
+        host_out: dict of pinned host tensors [n_chunks][...] or None."""
         host_out = host_out or {}
         _check(LIB.delta_analyze_shot_host(
             self._h, h_x.data_ptr(), h_x.shape[0], slots.data_ptr(), int(set_offsets), n_first,
             _ptr(dev_out.get("G")), _ptr(dev_out.get("A")), _ptr(dev_out.get("P")), _ptr(dev_out.get("R")),
-            _ptr(dev_out.get("Sauto")), strides[0], strides[1], strides[2],
+            _ptr(dev_out.get("Sauto")), strides[0], strides[1], strides[2], ring,
             _ptr(host_out.get("G")), _ptr(host_out.get("A")), _ptr(host_out.get("P")), _ptr(host_out.get("R")),
             _ptr(host_out.get("Sauto")), _stream()), "delta_analyze_shot_host")
 

@@ -193,11 +193,14 @@ int delta_plan_create(const delta_config *cfg, delta_plan **out) {
 int delta_plan_destroy(delta_plan *p) {
   if (!p) return DELTA_ERR_INVALID_ARG;
   if (p->copy_stream) cudaStreamDestroy(p->copy_stream);
+  if (p->d2h_stream) cudaStreamDestroy(p->d2h_stream);
   for (int s = 0; s < 2; ++s) {
     if (p->ev_copied[s]) cudaEventDestroy(p->ev_copied[s]);
     if (p->ev_consumed[s]) cudaEventDestroy(p->ev_consumed[s]);
-    if (p->ev_done[s]) cudaEventDestroy(p->ev_done[s]);
   }
+  if (p->ev_start) cudaEventDestroy(p->ev_start);
+  for (cudaEvent_t e : p->ev_out) cudaEventDestroy(e);
+  for (cudaEvent_t e : p->ev_back) cudaEventDestroy(e);
   delete p;
   return DELTA_OK;
 }
@@ -418,11 +421,11 @@ int delta_plan_set_stage_events(delta_plan *p, void *const *events) {
 
 int delta_analyze_shot_host(delta_plan *p, const void *h_x, int32_t n_chunks, void *d_slots, int32_t set_offsets,
                             int32_t n_first, float *d_G, float *d_A, float *d_P, float *d_R, float *d_Sauto,
-                            int64_t stride_GAP, int64_t stride_R, int64_t stride_auto, float *h_G, float *h_A,
-                            float *h_P, float *h_R, float *h_Sauto, void *stream) {
+                            int64_t stride_GAP, int64_t stride_R, int64_t stride_auto, int32_t out_ring, float *h_G,
+                            float *h_A, float *h_P, float *h_R, float *h_Sauto, void *stream) {
   int rc = need_ws(p);
   if (rc) return rc;
-  if (!h_x || !d_slots || n_chunks < 1) return DELTA_ERR_INVALID_ARG;
+  if (!h_x || !d_slots || n_chunks < 1 || out_ring < 0) return DELTA_ERR_INVALID_ARG;
   if ((reinterpret_cast<uintptr_t>(d_slots) & 255u) != 0) return DELTA_ERR_ALIGNMENT;
   if ((h_G && !d_G) || (h_A && !d_A) || (h_P && !d_P) || (h_R && !d_R) || (h_Sauto && !d_Sauto)) return DELTA_ERR_INVALID_ARG;
   cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
@@ -430,18 +433,37 @@ int delta_analyze_shot_host(delta_plan *p, const void *h_x, int32_t n_chunks, vo
   const size_t esz = p->cfg.in_dtype == DELTA_I16 ? 2 : 4;
   const size_t chunk_bytes = (size_t)l.C * l.T * esz;
   const size_t slot_bytes = align_up(chunk_bytes, 256);
+  const bool any_host = h_G || h_A || h_P || h_R || h_Sauto;
+  // device output set of chunk n: n mod out_ring (out_ring = 0: every chunk its own set, n)
+  int nsets = out_ring > 0 ? (out_ring < n_chunks ? out_ring : n_chunks) : n_chunks;
+  // a zero stride of a requested output makes all sets one
+  if (((d_G || d_A || d_P) && stride_GAP == 0) || (d_R && stride_R == 0) || (d_Sauto && stride_auto == 0)) nsets = 1;
   if (!p->copy_stream) {
     DELTA_CUDA_CHECK(cudaStreamCreateWithFlags(&p->copy_stream, cudaStreamNonBlocking));
+    DELTA_CUDA_CHECK(cudaStreamCreateWithFlags(&p->d2h_stream, cudaStreamNonBlocking));
     for (int s = 0; s < 2; ++s) {
       DELTA_CUDA_CHECK(cudaEventCreateWithFlags(&p->ev_copied[s], cudaEventDisableTiming));
       DELTA_CUDA_CHECK(cudaEventCreateWithFlags(&p->ev_consumed[s], cudaEventDisableTiming));
-      DELTA_CUDA_CHECK(cudaEventCreateWithFlags(&p->ev_done[s], cudaEventDisableTiming));
     }
+    DELTA_CUDA_CHECK(cudaEventCreateWithFlags(&p->ev_start, cudaEventDisableTiming));
   }
-  // the copy stream must not start before work already queued on `stream` (e.g. a previous shot
-  // still reading the slots) has finished
-  DELTA_CUDA_CHECK(cudaEventRecord(p->ev_done[0], st));
-  DELTA_CUDA_CHECK(cudaStreamWaitEvent(p->copy_stream, p->ev_done[0], 0));
+  // one "computed" / "copied back" event pair per output set that is reused (bounded: sets beyond 64 are never reused
+  // before the shot ends unless the ring is shorter, and a ring is at most a handful of sets)
+  const bool reuse = any_host && nsets < n_chunks;
+  if (reuse && nsets > 64) return DELTA_ERR_UNSUPPORTED;
+  const int nev = any_host ? (reuse ? nsets : 1) : 0;
+  while ((int)p->ev_out.size() < nev) {
+    cudaEvent_t a = nullptr, b = nullptr;
+    DELTA_CUDA_CHECK(cudaEventCreateWithFlags(&a, cudaEventDisableTiming));
+    DELTA_CUDA_CHECK(cudaEventCreateWithFlags(&b, cudaEventDisableTiming));
+    p->ev_out.push_back(a);
+    p->ev_back.push_back(b);
+  }
+  // the copy streams must not start before work already queued on `stream` (e.g. a previous shot still reading the
+  // slots or the output sets) has finished
+  DELTA_CUDA_CHECK(cudaEventRecord(p->ev_start, st));
+  DELTA_CUDA_CHECK(cudaStreamWaitEvent(p->copy_stream, p->ev_start, 0));
+  if (any_host) DELTA_CUDA_CHECK(cudaStreamWaitEvent(p->d2h_stream, p->ev_start, 0));
   const size_t gap_bytes = (size_t)l.Po * l.F * sizeof(float), r_bytes = (size_t)l.Po * l.nlags * sizeof(float);
   const size_t au_bytes = (size_t)l.C * l.F * sizeof(float);
   int total_launches = 0;
@@ -457,18 +479,33 @@ int delta_analyze_shot_host(delta_plan *p, const void *h_x, int32_t n_chunks, vo
       rc = delta_set_offsets(p, slot, l.T, n_first, stream);
       if (rc) return rc;
     }
-    float *g = d_G ? d_G + (size_t)n * stride_GAP : nullptr, *a = d_A ? d_A + (size_t)n * stride_GAP : nullptr;
-    float *pw = d_P ? d_P + (size_t)n * stride_GAP : nullptr, *r = d_R ? d_R + (size_t)n * stride_R : nullptr;
-    float *au = d_Sauto ? d_Sauto + (size_t)n * stride_auto : nullptr;
+    const int set = n % nsets;
+    // the copy-back of the chunk that used this output set before must be over before the kernels overwrite it
+    if (reuse && n >= nsets) DELTA_CUDA_CHECK(cudaStreamWaitEvent(st, p->ev_back[set], 0));
+    float *g = d_G ? d_G + (size_t)set * stride_GAP : nullptr, *a = d_A ? d_A + (size_t)set * stride_GAP : nullptr;
+    float *pw = d_P ? d_P + (size_t)set * stride_GAP : nullptr, *r = d_R ? d_R + (size_t)set * stride_R : nullptr;
+    float *au = d_Sauto ? d_Sauto + (size_t)set * stride_auto : nullptr;
     rc = delta_analyze_chunk(p, slot, l.T, g, a, pw, r, au, stream);
     if (rc) return rc;
     total_launches += p->launches;
     DELTA_CUDA_CHECK(cudaEventRecord(p->ev_consumed[s], st));
-    if (h_G) DELTA_CUDA_CHECK(cudaMemcpyAsync(h_G + (size_t)n * l.Po * l.F, g, gap_bytes, cudaMemcpyDeviceToHost, st));
-    if (h_A) DELTA_CUDA_CHECK(cudaMemcpyAsync(h_A + (size_t)n * l.Po * l.F, a, gap_bytes, cudaMemcpyDeviceToHost, st));
-    if (h_P) DELTA_CUDA_CHECK(cudaMemcpyAsync(h_P + (size_t)n * l.Po * l.F, pw, gap_bytes, cudaMemcpyDeviceToHost, st));
-    if (h_R) DELTA_CUDA_CHECK(cudaMemcpyAsync(h_R + (size_t)n * l.Po * l.nlags, r, r_bytes, cudaMemcpyDeviceToHost, st));
-    if (h_Sauto) DELTA_CUDA_CHECK(cudaMemcpyAsync(h_Sauto + (size_t)n * l.C * l.F, au, au_bytes, cudaMemcpyDeviceToHost, st));
+    if (any_host) {
+      // device -> host on its own stream, so that it runs under the kernels (and the host -> device copy) of the next chunks
+      const int e = reuse ? set : 0;
+      DELTA_CUDA_CHECK(cudaEventRecord(p->ev_out[e], st));
+      DELTA_CUDA_CHECK(cudaStreamWaitEvent(p->d2h_stream, p->ev_out[e], 0));
+      cudaStream_t dh = p->d2h_stream;
+      if (h_G) DELTA_CUDA_CHECK(cudaMemcpyAsync(h_G + (size_t)n * l.Po * l.F, g, gap_bytes, cudaMemcpyDeviceToHost, dh));
+      if (h_A) DELTA_CUDA_CHECK(cudaMemcpyAsync(h_A + (size_t)n * l.Po * l.F, a, gap_bytes, cudaMemcpyDeviceToHost, dh));
+      if (h_P) DELTA_CUDA_CHECK(cudaMemcpyAsync(h_P + (size_t)n * l.Po * l.F, pw, gap_bytes, cudaMemcpyDeviceToHost, dh));
+      if (h_R) DELTA_CUDA_CHECK(cudaMemcpyAsync(h_R + (size_t)n * l.Po * l.nlags, r, r_bytes, cudaMemcpyDeviceToHost, dh));
+      if (h_Sauto) DELTA_CUDA_CHECK(cudaMemcpyAsync(h_Sauto + (size_t)n * l.C * l.F, au, au_bytes, cudaMemcpyDeviceToHost, dh));
+      DELTA_CUDA_CHECK(cudaEventRecord(p->ev_back[e], dh));
+    }
+  }
+  if (any_host) {  // `stream` ends after the last copy-back: the caller synchronises one stream
+    DELTA_CUDA_CHECK(cudaEventRecord(p->ev_back[0], p->d2h_stream));
+    DELTA_CUDA_CHECK(cudaStreamWaitEvent(st, p->ev_back[0], 0));
   }
   p->launches = total_launches;
   return DELTA_OK;

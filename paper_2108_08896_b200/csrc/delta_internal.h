@@ -104,10 +104,12 @@ struct delta_plan {
   bool use_pdl = true;  // programmatic dependent launch between the hot-path kernels (DELTA_NO_PDL=1 switches it off)
   bool stage_events_on = false;
   cudaEvent_t stage_ev[4] = {nullptr, nullptr, nullptr, nullptr};
-  cudaStream_t copy_stream = nullptr;
-  cudaEvent_t ev_copied[2] = {nullptr, nullptr};
-  cudaEvent_t ev_consumed[2] = {nullptr, nullptr};
-  cudaEvent_t ev_done[2] = {nullptr, nullptr};
+  // delta_analyze_shot_host: host -> device copies on copy_stream, device -> host copies on d2h_stream
+  cudaStream_t copy_stream = nullptr, d2h_stream = nullptr;
+  cudaEvent_t ev_copied[2] = {nullptr, nullptr};    // input slot s holds its chunk
+  cudaEvent_t ev_consumed[2] = {nullptr, nullptr};  // the kernels have read input slot s
+  cudaEvent_t ev_start = nullptr;
+  std::vector<cudaEvent_t> ev_out, ev_back;         // per output set: computed / copied back
 
   const float2 *d_tw() const { return reinterpret_cast<const float2 *>(ws + wsl.off_tw); }
   const float *d_win() const { return reinterpret_cast<const float *>(ws + wsl.off_win); }

@@ -585,3 +585,19 @@ def test_P16_zero_padded_segments_give_the_linear_correlation():
     xx = np.stack([base[d:], base[:3000]])            # x_1[t] = x_0[t - d]
     padded = o.analyze_chunk(xx, 128, 32, 64, nperseg=64)["R"][0]
     assert np.argmax(padded) - 64 == -d               # found at its true lag, no wrap-around image
+
+
+# ----------------------------------------------------------------------------------------------
+# oracle/fft_baseline.py is the "CPU, library FFT" arm of BASELINE.md section 3 and the float64 checker of the full-size
+# GPU tests.  It is not the oracle; it is pinned TO the oracle here (the library FFT itself is pin P6).
+@pytest.mark.parametrize("C,T,L,H,M", [(8, 2048, 256, 128, 128), (5, 3000, 128, 100, 40), (12, 10_000, 512, 256, 256)])
+def test_fft_baseline_equals_oracle(C, T, L, H, M):
+    from oracle import fft_baseline as fb
+    x = np.random.default_rng(C * 31 + L).standard_normal((C, T))
+    x[1] += 0.6 * x[0]
+    ref = o.analyze_chunk(x, L, H, M)
+    got = fb.analyze_chunk(x, L, H, M)
+    for k in ("G", "P", "R", "Sauto"):
+        assert got[k].shape == ref[k].shape, k
+        assert np.max(np.abs(got[k] - ref[k])) <= 1e-10 * max(1.0, float(np.abs(ref[k]).max())), k
+    assert np.max(np.abs(np.angle(np.exp(1j * (got["A"] - ref["A"]))))) <= 1e-8

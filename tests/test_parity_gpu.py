@@ -321,23 +321,32 @@ def test_config4_streamed_shot():
         assert torch.equal(alone[k], t[124]), k
 
 
-def test_host_output_path_roundtrip():
-    """delta_analyze_shot_host with host outputs (the e2e path bench.py times)."""
+@pytest.mark.parametrize("ring", [0, 2, 3])
+def test_host_output_path_roundtrip(ring):
+    """delta_analyze_shot_host with host outputs (the e2e path bench.py times): the device->host copies run on the
+    library's second copy stream under the kernels of the next chunks.  ring = 0 with zero strides: one device output
+    set, overwritten chunk after chunk (every overwrite must wait for the copy-back); ring = 2, 3: rotating sets."""
     b = binding()
-    x = np.random.default_rng(3).standard_normal((3, 12, 1024)).astype(np.float32)
+    n = 7
+    x = np.random.default_rng(3).standard_normal((n, 12, 1024)).astype(np.float32)
     plan = b.Plan(12, 1024, 128, 64, 64)
     s = plan.sizes
     h_x = torch.from_numpy(x).pin_memory()
     slots = torch.empty(plan.slot_bytes(), dtype=torch.uint8, device="cuda")
-    dev_out = plan.empty_outputs()
-    host = dict(G=torch.empty((3, s.P, s.F)).pin_memory(), A=torch.empty((3, s.P, s.F)).pin_memory(),
-                P=torch.empty((3, s.P, s.F)).pin_memory(), R=torch.empty((3, s.P, s.n_lags)).pin_memory(),
-                Sauto=torch.empty((3, 12, s.F)).pin_memory())
-    plan.analyze_shot_host(h_x, slots, dev_out, host_out=host)
+    sets = max(ring, 1)
+    dev_out = dict(G=torch.empty((sets, s.P, s.F), device="cuda"), A=torch.empty((sets, s.P, s.F), device="cuda"),
+                   P=torch.empty((sets, s.P, s.F), device="cuda"), R=torch.empty((sets, s.P, s.n_lags), device="cuda"),
+                   Sauto=torch.empty((sets, 12, s.F), device="cuda"))
+    strides = (s.P * s.F, s.P * s.n_lags, 12 * s.F) if ring else (0, 0, 0)
+    host = dict(G=torch.empty((n, s.P, s.F)).pin_memory(), A=torch.empty((n, s.P, s.F)).pin_memory(),
+                P=torch.empty((n, s.P, s.F)).pin_memory(), R=torch.empty((n, s.P, s.n_lags)).pin_memory(),
+                Sauto=torch.empty((n, 12, s.F)).pin_memory())
+    for rep in range(2):   # twice back to back: the second shot must wait for the first one's copies
+        plan.analyze_shot_host(h_x, slots, dev_out, strides=strides, host_out=host, ring=ring)
     torch.cuda.synchronize()
-    for n in range(3):
-        ref = oracle_for(x[n], 128, 64, 64)
-        compare({k: host[k][n].numpy() for k in host}, ref, o.all_pairs(12), f"host chunk {n}")
+    for k in range(n):
+        ref = oracle_for(x[k], 128, 64, 64)
+        compare({q: host[q][k].numpy() for q in host}, ref, o.all_pairs(12), f"host chunk {k}")
 
 
 def test_chunks_in_flight_two_plans_two_streams():
