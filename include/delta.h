@@ -46,7 +46,7 @@ extern "C" {
 typedef enum {
   DELTA_OK = 0,
   DELTA_ERR_INVALID_ARG = -1, /* NULL pointer, non-positive size, unknown enum value               */
-  DELTA_ERR_UNSUPPORTED = -2, /* nfft not a power of two in [64,4096], T < segment length, hop larger
+  DELTA_ERR_UNSUPPORTED = -2, /* nfft odd or outside [16,4096], T < segment length, hop larger
                                  than the segment, max_lag > L/2, C > 4096                         */
   DELTA_ERR_ALIGNMENT = -3,   /* a device pointer is not 16-byte aligned                            */
   DELTA_ERR_NO_WORKSPACE = -4,/* compute call before delta_plan_set_workspace(), or it is too small */
@@ -79,7 +79,8 @@ enum { DELTA_CONTRACT_AUTO = 0,                      /* library picks (tensor co
 typedef struct {
   int32_t n_channels;   /* C >= 1                                                                     */
   int32_t n_samples;    /* T >= nfft, samples per channel per chunk                                   */
-  int32_t nfft;         /* L, transform length, power of two in [64, 4096]; segment length: see nperseg  */
+  int32_t nfft;         /* L, transform length: even, 16..4096.  Powers of two from 64 up run on the register
+                         * FFT; any other even length on direct-DFT kernels (O(L^2), correct, not tuned)        */
   int32_t hop;          /* H in [1, L]; overlap = L - H                                               */
   int32_t window;       /* DELTA_WIN_*                                                                */
   int32_t scaling;      /* DELTA_SCALE_*                                                              */

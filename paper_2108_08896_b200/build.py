@@ -44,7 +44,6 @@ def build(force: bool = False, verbose: bool = False) -> str:
     objdir = os.path.join(PKG, "build")
     os.makedirs(objdir, exist_ok=True)
     common = [*ARCH, "-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC", "-I", os.path.join(ROOT, "include"), "-I", CSRC]
-    common[0:0] = os.environ.get("DELTA_NVCC_FLAGS", "").split()  # tuning experiments only (e.g. -DDELTA_PAIR_TILE_SPLIT=4)
     if verbose:
         common.insert(0, "-Xptxas=-v")
 

@@ -32,7 +32,7 @@ static int validate(const delta_config *c) {
     if (!(c->fs > 0.f) || !(c->bp_lo_hz >= 0.f) || !(c->bp_hi_hz >= c->bp_lo_hz)) return DELTA_ERR_INVALID_ARG;
   }
   const int L = c->nfft;
-  if (L < 64 || L > 4096 || (L & (L - 1)) != 0) return DELTA_ERR_UNSUPPORTED;
+  if (L < 16 || L > 4096 || (L & 1) != 0) return DELTA_ERR_UNSUPPORTED;  // even lengths; see has_fft_path()
   if (c->nperseg < 0 || c->nperseg > L) return DELTA_ERR_INVALID_ARG;
   const int Ls = c->nperseg > 0 ? c->nperseg : L;
   if (c->hop > Ls) return DELTA_ERR_UNSUPPORTED;

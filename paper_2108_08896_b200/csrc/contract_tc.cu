@@ -19,8 +19,9 @@
 // units cover the lower triangle; a lane (fixed j) then walks consecutive lexicographic pairs when the
 // epilogue fixes i and lets the 32 lanes of a warp store: S leaves the SM in 256-byte runs.
 //
-// Roles (one CTA per SM, persistent over (bin, group) items): warp 8 lane 0 = bulk-copy producer,
-// warp 9 lane 0 = MMA issuer, warps 0-7 = epilogue (TMEM -> registers -> scale -> S stores).  Every unit has
+// Roles (one CTA per SM, persistent over (bin, group) items): warps 0-15 = epilogue (4 TMEM lane quadrants x 4 column
+// slices: TMEM -> registers -> scale -> S stores), warp 16 = bulk-copy producer, warp 17 = MMA issuer (both loops are
+// warp-uniform, one elected lane issues).  Every unit has
 // its own TMEM region and full/empty mbarrier pair, so the epilogue of unit u overlaps the MMAs of the
 // following units (and, when all K steps of a bin fit in the operand ring, of the next bin: "unit-major").
 #include <cuda_fp16.h>
@@ -287,7 +288,7 @@ contract_tc_kernel(const __half *__restrict__ X, Layout lay, TcParams prm, float
           unit_done(u);
         }
         s0 = s; pass0 = pass;
-      } else if (prm.unit_major) {
+      } else {
         for (int u = 0; u < nu; ++u) {
           const TcUnit un = prm.units[g][u];
           const uint32_t ao16 = (uint32_t)(un.row0 / 8) * 8u, bo16 = (uint32_t)(un.col0 / 8) * 8u;
@@ -312,24 +313,6 @@ contract_tc_kernel(const __half *__restrict__ X, Layout lay, TcParams prm, float
           if (lane == 0) { TC_TRACE(1, tr); } ++tr;
           if (u == nu - 1) { s0 = s; pass0 = pass; }
         }
-      } else {
-        uint32_t s = s0, pass = pass0;
-        for (int ks = 0; ks < prm.ksteps; ++ks) {
-          mbar_wait(full_bar + s, pass & 1u);
-          fence_after();
-          for (int u = 0; u < nu; ++u) {
-            const TcUnit un = prm.units[g][u];
-            if (ks == 0) wait_unit_free(u);
-            issue((uint32_t)(un.row0 / 8) * 8u, (uint32_t)(un.col0 / 8) * 8u, make_idesc(un.N, 0), make_idesc(un.N, 1),
-                  tmem_base + (uint32_t)un.tm, tmem_base + (uint32_t)(un.tm + un.N), s, ks > 0 ? 1u : 0u);
-          }
-          if (elect_one()) mma_commit(empty_bar + s);
-          __syncwarp();
-          if (++s == (uint32_t)prm.nstage) { s = 0; ++pass; }
-        }
-        for (int u = 0; u < nu; ++u) unit_done(u);
-        if (lane == 0) { TC_TRACE(1, tr); } ++tr;
-        s0 = s; pass0 = pass;
       }
       g += gstep;
       if (g >= prm.ngroups) g -= prm.ngroups;
@@ -419,12 +402,10 @@ bool tc_plan_tiles(int Cp, TcHostPlan *out) {
   U list[kTcMaxGroups * kTcMaxUnits];
   int n = 0;
   auto add_row_tile = [&](int r0, int lane_hi, int col_end) {
-#ifndef DELTA_TC_MAX_N
-#define DELTA_TC_MAX_N 128  // widest accumulator unit (wider units were measured slower at config 2: their epilogue overlaps less)
-#endif
+    constexpr int kMaxN = 128;  // widest accumulator unit (wider units: less tensor time, but their epilogue overlaps less)
     for (int c = 0, N = 0; c < col_end; c += N) {
       if (n >= kTcMaxGroups * kTcMaxUnits) return false;
-      N = (col_end - c) < DELTA_TC_MAX_N ? (col_end - c) : DELTA_TC_MAX_N;
+      N = (col_end - c) < kMaxN ? (col_end - c) : kMaxN;
       int lane_lo = c > r0 ? ((c - r0) & ~31) : 0;  // lanes below have j < col0: nothing to keep
       list[n++] = {r0, lane_lo, lane_hi, c, N};
     }
@@ -472,18 +453,12 @@ int launch_contract_tc(delta_plan *p, const void *d_X, float *d_S, float *d_auto
   prm.kstep_elems = (int64_t)2 * lay.Cp * kSegBlock;
   const size_t fixed = (size_t)lay.Cp * sizeof(float2) + 64 * sizeof(uint64_t) + 64;
   int nstage = (int)((200 * 1024 - fixed) / prm.stage_bytes);
-#ifndef DELTA_TC_MAX_STAGES
-#define DELTA_TC_MAX_STAGES 8
-#endif
-  if (nstage > DELTA_TC_MAX_STAGES) nstage = DELTA_TC_MAX_STAGES;
+  if (nstage > 8) nstage = 8;
   if (nstage < 2) return DELTA_ERR_UNSUPPORTED;
   prm.nstage = nstage;
-#ifndef DELTA_TC_STREAM_UNITS
-#define DELTA_TC_STREAM_UNITS 1
-#endif
-  // 1: all K steps of a bin stay in the ring and are shared by its units;  2: every unit streams them again;
-  // 0: K-step-major (all units advance together; their epilogues cannot overlap the MMAs)
-  prm.unit_major = (2 * prm.ksteps <= nstage) ? 1 : (DELTA_TC_STREAM_UNITS ? 2 : 0);
+  // 1: all K steps of a bin stay in the ring and are shared by its units;  2: every unit streams them again
+  // (K-step-major order, all units advancing together, was measured slower: their epilogues cannot overlap the MMAs)
+  prm.unit_major = (2 * prm.ksteps <= nstage) ? 1 : 2;
   size_t smem = (size_t)nstage * prm.stage_bytes + fixed;
   if (smem < 120 * 1024) smem = 120 * 1024;  // one CTA per SM: each CTA allocates all 512 TMEM columns
   const int nitems = lay.F * prm.ngroups;

@@ -28,6 +28,10 @@ bool tc_plan_tiles(int Cp, TcHostPlan *out);
 constexpr int pair_block(int L) { return L <= 1024 ? 16 : (L == 2048 ? 8 : 4); }
 constexpr int pair_fft_points(int N) { return N <= 64 ? 8 : 16; }  // E of FftGeom<N> (fft_reg.cuh)
 
+// transform lengths served by the register FFT (fft_reg.cuh); every other even length in [16, 4096] takes the direct-DFT
+// kernels (stft_dft_kernel, pair_dft_kernel)
+constexpr bool has_fft_path(int L) { return (L & (L - 1)) == 0 && L >= 64 && L <= 4096; }
+
 struct Layout {
   // X (STFT) buffer, frequency-major so that one bin's C x K matrix is one contiguous block:
   //   FP32 mode : float  X[f][part][kc][c][8]                 part 0 = Re, 1 = Im

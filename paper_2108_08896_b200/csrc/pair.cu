@@ -504,8 +504,89 @@ static int launch_pair_L(delta_plan *p, const float *d_S, const float *d_rsq, co
   return DELTA_OK;
 }
 
+// ------------------------------------------------------------------------------------------
+// Transform lengths that are not powers of two: the per-pair quantities from the definitions,
+// with Eq. (1d) as the direct inverse sum  R[m] = (1/L) (S[0] + (-1)^m S[L/2] + 2 sum_{0<f<L/2} Re(S[f] e^{+2 pi i f m/L}))
+// over the Hermitian half spectrum (L even; Im S[0], Im S[L/2] ignored).  One CTA per tile of PB pairs; O(L^2) per pair.
+__global__ void __launch_bounds__(256)
+pair_dft_kernel(const float2 *__restrict__ S, const float *__restrict__ Srsq, const float *__restrict__ rnorm,
+                const ushort2 *__restrict__ list, const float2 *__restrict__ tw, Layout lay, float *__restrict__ G,
+                float *__restrict__ A, float *__restrict__ Pw, float *__restrict__ R) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  float2 *tl = reinterpret_cast<float2 *>(smem_raw);  // [F][PB], slot = (pl ^ s_swz(f)) & (PB-1)
+  __shared__ ushort2 ij_s[16];
+  __shared__ int pg_s[16];
+  const int tid = threadIdx.x, PB = lay.PB, F = lay.F, L = lay.L, Fp = lay.Fp;
+  const int64_t p0 = (int64_t)blockIdx.x * PB;
+  pdl_launch_dependents();
+  if (tid < PB) {
+    ushort2 ij = make_ushort2(0, 1);
+    if (p0 + tid < lay.Po) ij = list ? list[p0 + tid] : pair_of(p0 + tid, lay.C);
+    ij_s[tid] = ij;
+    pg_s[tid] = (int)ij.x * lay.C - ((int)ij.x * ((int)ij.x + 1)) / 2 + (int)ij.y - (int)ij.x - 1;
+  }
+  pdl_wait();
+  __syncthreads();
+  for (int idx = tid; idx < F * PB; idx += 256) {
+    const int f = idx / PB, sw = s_swz(f);
+    const int pg = pg_s[((idx % PB) ^ sw) & (PB - 1)];  // the pair whose slot this is
+    tl[idx] = __ldg(S + ((int64_t)(pg >> lay.pb_shift) * F + f) * PB + ((pg ^ sw) & (PB - 1)));
+  }
+  __syncthreads();
+  const int nv = (int)(lay.Po - p0 < PB ? lay.Po - p0 : PB);
+  if (G || A || Pw) {
+    for (int e = tid; e < nv * F; e += 256) {
+      const int pl = e / F, f = e - pl * F;
+      const ushort2 ij = ij_s[pl];
+      const float2 s = tl[f * PB + ((pl ^ s_swz(f)) & (PB - 1))];
+      const float mag = sqrt_approx(fmaf(s.x, s.x, s.y * s.y));
+      const int64_t at = (p0 + pl) * F + f;
+      if (Pw) Pw[at] = mag;
+      if (G) G[at] = mag * __ldg(Srsq + (int64_t)ij.x * Fp + f) * __ldg(Srsq + (int64_t)ij.y * Fp + f);
+      if (A) A[at] = atan2_poly(s.y, s.x);
+    }
+  }
+  if (R) {
+    const int nl = lay.nlags, M = lay.M, half = L / 2;
+    for (int e = tid; e < nv * nl; e += 256) {
+      const int pl = e / nl, q = e - pl * nl;
+      const int m = q - M, mm = m < 0 ? m + L : m;  // lag mod L
+      const int slot = pl, sgn = (m & 1) ? -1 : 1;
+      float acc = 0.f;
+      int idx = 0;  // f mm mod L
+      for (int f = 1; f < half; ++f) {
+        idx += mm;
+        if (idx >= L) idx -= L;
+        const float2 w = __ldg(tw + idx);  // e^{-2 pi i idx / L}: cos = w.x, sin = -w.y
+        const float2 s = tl[f * PB + ((slot ^ s_swz(f)) & (PB - 1))];
+        acc = fmaf(s.x, w.x, fmaf(s.y, w.y, acc));  // Re(S e^{+i theta}) = S.x cos - S.y sin
+      }
+      const float s0 = tl[(pl ^ s_swz(0)) & (PB - 1)].x, sh = tl[half * PB + ((pl ^ s_swz(half)) & (PB - 1))].x;
+      const ushort2 ij = ij_s[pl];
+      R[(p0 + pl) * nl + q] = (2.f * acc + s0 + (float)sgn * sh) * __ldg(rnorm + ij.x) * __ldg(rnorm + ij.y);
+    }
+  }
+}
+
+static int launch_pair_dft(delta_plan *p, const float *d_S, const float *d_rsq, const float *d_rnorm, float *d_G, float *d_A,
+                           float *d_P, float *d_R, cudaStream_t st) {
+  const Layout &lay = p->lay;
+  if (lay.Poblk == 0 || lay.Po == 0) return DELTA_OK;
+  const ushort2 *list = p->cfg.n_pairs > 0 ? p->d_pairs() : nullptr;
+  const size_t smem = (size_t)lay.F * lay.PB * sizeof(float2);
+  int rc = opt_in_smem(pair_dft_kernel, smem);
+  if (rc) return rc;
+  LaunchCfg lc(dim3((unsigned)lay.Poblk), dim3(256), smem, st, p->use_pdl);
+  DELTA_CUDA_CHECK(cudaLaunchKernelEx(&lc.cfg, pair_dft_kernel, reinterpret_cast<const float2 *>(d_S), d_rsq, d_rnorm, list,
+                                      p->d_tw(), lay, d_G, d_A, d_P, d_R));
+  p->launches++;
+  DELTA_CUDA_CHECK(cudaGetLastError());
+  return DELTA_OK;
+}
+
 int launch_pair(delta_plan *p, const float *d_S, const float *d_rsq, const float *d_rnorm, float *d_G, float *d_A, float *d_P,
                 float *d_R, cudaStream_t st) {
+  if (!has_fft_path(p->lay.L)) return launch_pair_dft(p, d_S, d_rsq, d_rnorm, d_G, d_A, d_P, d_R, st);
 #define CALL(LL) launch_pair_L<LL>(p, d_S, d_rsq, d_rnorm, d_G, d_A, d_P, d_R, st)
   DELTA_SWITCH_L(p->lay.L, CALL)
 #undef CALL

@@ -11,6 +11,7 @@
 
 #include "delta_internal.h"
 #include "fft_reg.cuh"
+#include "x_store.cuh"
 
 namespace cg = cooperative_groups;
 
@@ -439,49 +440,10 @@ stft_kernel(const void *__restrict__ x, int64_t ld, int in_dtype, int norm_mode,
   // Phase 2.  Bins f and N - f come from the same pair Z[f], Z[N-f]:  with e = (Z[f] + conj Z[N-f])/2,
   // d = (Z[f] - conj Z[N-f])/2 and (a, b) = e^{-2 pi i f/L} d:  X[f] = (e.x + b, e.y - a),  X[N-f] = (e.x - b, -e.y - a).
   // One thread does both for the 8 segments of the CTA; bin N/2 (its own partner) is done once.
-  const int64_t plane = (int64_t)lay.Kc * lay.Cp * kSegBlock;  // one [kc][c][8] block
   auto store_bin = [&](int c, int pcl, int f, const float *re, const float *im) {
-    const int64_t within = ((int64_t)kb * lay.Cp + c) * kSegBlock;
-    const int64_t base = (int64_t)f * lay.x_elems_per_f + within;
-    const float keep = (f >= lay.f_lo && f <= lay.f_hi) ? 1.f : 0.f;  // band-pass mask (R19)
-    const bool plv = lay.estimator == DELTA_EST_PHASE_LOCK;
-    float nre[kSegBlock], nim[kSegBlock];
-    if (plv) {  // per-segment-normalised estimator (f2): X -> X / |X|, 0 where X = 0
-#pragma unroll
-      for (int q = 0; q < kSegBlock; ++q) {
-        const float m2 = fmaf(re[q], re[q], im[q] * im[q]);
-        const float r = m2 > 0.f ? rsqrtf(m2) : 0.f;
-        nre[q] = re[q] * r;
-        nim[q] = im[q] * r;
-      }
-      re = nre;
-      im = nim;
-    }
-    if (TC) {
-      // split fp16: v * scale = hi + lo (scale = the channel's power of two; 2^13 for unit phasors)
-      __half *X = reinterpret_cast<__half *>(Xout);
-      const float sc = keep * (plv ? 8192.f : (CLUSTER ? csc[pcl] : chscale[c]));
-      __align__(16) __half2 hr[4], hi_[4], lr[4], li[4];
-#pragma unroll
-      for (int q = 0; q < 4; ++q) {
-        const float r0 = re[2 * q] * sc, r1 = re[2 * q + 1] * sc, i0 = im[2 * q] * sc, i1 = im[2 * q + 1] * sc;
-        hr[q] = __floats2half2_rn(r0, r1);
-        hi_[q] = __floats2half2_rn(i0, i1);
-        const float2 hrf = __half22float2(hr[q]), hif = __half22float2(hi_[q]);
-        lr[q] = __floats2half2_rn(r0 - hrf.x, r1 - hrf.y);
-        li[q] = __floats2half2_rn(i0 - hif.x, i1 - hif.y);
-      }
-      *reinterpret_cast<uint4 *>(X + base + 0 * plane) = *reinterpret_cast<const uint4 *>(hr);
-      *reinterpret_cast<uint4 *>(X + base + 1 * plane) = *reinterpret_cast<const uint4 *>(hi_);
-      *reinterpret_cast<uint4 *>(X + base + 2 * plane) = *reinterpret_cast<const uint4 *>(lr);
-      *reinterpret_cast<uint4 *>(X + base + 3 * plane) = *reinterpret_cast<const uint4 *>(li);
-    } else {
-      float *X = reinterpret_cast<float *>(Xout);
-      *reinterpret_cast<float4 *>(X + base) = make_float4(keep * re[0], keep * re[1], keep * re[2], keep * re[3]);
-      *reinterpret_cast<float4 *>(X + base + 4) = make_float4(keep * re[4], keep * re[5], keep * re[6], keep * re[7]);
-      *reinterpret_cast<float4 *>(X + base + plane) = make_float4(keep * im[0], keep * im[1], keep * im[2], keep * im[3]);
-      *reinterpret_cast<float4 *>(X + base + plane + 4) = make_float4(keep * im[4], keep * im[5], keep * im[6], keep * im[7]);
-    }
+    // split fp16 scale of the channel (2^13 for unit phasors); unused in FP32 mode
+    const float sc = !TC ? 1.f : (lay.estimator == DELTA_EST_PHASE_LOCK ? 8192.f : (CLUSTER ? csc[pcl] : chscale[c]));
+    store_x_bin<TC>(Xout, lay, kb, c, f, sc, re, im);
   };
   constexpr int HB = N / 2 + 1;  // f = 0 .. N/2
   for (int idx = tid; idx < CH * HB; idx += Cfg::THREADS) {
@@ -588,7 +550,112 @@ static int launch_stft_L(delta_plan *p, const void *d_x, int64_t ld, void *d_X, 
   return launch_stft_LT<L, false, false>(p, d_x, ld, d_X, st);
 }
 
+// ------------------------------------------------------------------------------------------
+// Transform lengths that are not powers of two (the paper fixes no segment length, L107): the
+// definition itself,  X[k, f] = sum_n w[n] y[kH + n] e^{-2 pi i f n / L},  as a direct sum over the windowed samples of a
+// segment block held in shared memory (the phase index f n mod L is advanced by additions).  O(L^2) per segment: a
+// correct, unhurried path for the odd case (a 500-point transform costs about 0.1 ms per 192-channel chunk); the
+// register FFT serves the powers of two.  grid = (ceil(K/8), C), 256 threads; shared memory: float [8][L].
+template <bool TC, bool DETREND>
+__global__ void __launch_bounds__(256)
+stft_dft_kernel(const void *__restrict__ x, int64_t ld, int in_dtype, int norm_mode, int n_first,
+                const double *__restrict__ offs, const long long *__restrict__ isum, const float2 *__restrict__ tw,
+                const float *__restrict__ win, Layout lay, void *__restrict__ Xout, float *__restrict__ wpart) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  float *seg = reinterpret_cast<float *>(smem_raw);  // [8][L]
+  __shared__ float red[8];
+  const float *chscale = reinterpret_cast<const float *>(reinterpret_cast<const char *>(Xout) + lay.x_scale_off);
+  pdl_launch_dependents();
+  pdl_wait();
+  const int tid = threadIdx.x, kb = blockIdx.x, c = blockIdx.y, L = lay.L;
+  SampleLoader ldr;
+  ldr.init(x, in_dtype, norm_mode, n_first, offs, isum, c);
+  for (int idx = tid; idx < kSegBlock * L; idx += 256) {
+    const int k8 = idx / L, n = idx - k8 * L, k = kb * kSegBlock + k8;
+    seg[idx] = (k < lay.K && n < lay.Ls) ? ldr((int64_t)c * ld + (int64_t)k * lay.H + n) : 0.f;
+  }
+  __syncthreads();
+  {  // warp k8 owns segment k8: optional detrend (mean of the Ls samples), window, energy of the windowed samples
+    const int k8 = tid >> 5, lane = tid & 31;
+    float *sk = seg + k8 * L;
+    float mean = 0.f;
+    if (DETREND) {
+      float sm = 0.f;
+      for (int n = lane; n < lay.Ls; n += 32) sm += sk[n];
+      for (int o = 16; o > 0; o >>= 1) sm += __shfl_xor_sync(0xffffffffu, sm, o);
+      mean = kb * kSegBlock + k8 < lay.K ? sm / (float)lay.Ls : 0.f;
+    }
+    float ss = 0.f;
+    for (int n = lane; n < L; n += 32) {
+      const float v = (sk[n] - mean) * __ldg(win + n);  // the window is zero beyond Ls
+      sk[n] = v;
+      ss = fmaf(v, v, ss);
+    }
+    for (int o = 16; o > 0; o >>= 1) ss += __shfl_xor_sync(0xffffffffu, ss, o);
+    if (lane == 0) red[k8] = ss;
+  }
+  __syncthreads();
+  if (tid == 0) {
+    float e = 0.f;
+    for (int w = 0; w < 8; ++w) e += red[w];
+    wpart[(int64_t)c * lay.nkb + kb] = e;
+  }
+  const float sc = !TC ? 1.f : (lay.estimator == DELTA_EST_PHASE_LOCK ? 8192.f : chscale[c]);
+  for (int f = tid; f < lay.F; f += 256) {
+    float re[kSegBlock], im[kSegBlock];
+#pragma unroll
+    for (int q = 0; q < kSegBlock; ++q) re[q] = im[q] = 0.f;
+    int idx = 0;  // f n mod L
+    for (int n = 0; n < L; ++n) {
+      const float2 w = __ldg(tw + idx);  // e^{-2 pi i (f n mod L) / L}
+#pragma unroll
+      for (int q = 0; q < kSegBlock; ++q) {
+        const float sv = seg[q * L + n];
+        re[q] = fmaf(sv, w.x, re[q]);
+        im[q] = fmaf(sv, w.y, im[q]);
+      }
+      idx += f;
+      if (idx >= L) idx -= L;
+    }
+    store_x_bin<TC>(Xout, lay, kb, c, f, sc, re, im);
+  }
+}
+
+static int launch_stft_dft(delta_plan *p, const void *d_x, int64_t ld, void *d_X, cudaStream_t st) {
+  const Layout &lay = p->lay;
+  const bool tc = p->contraction == DELTA_CONTRACT_TC, det = lay.detrend == DELTA_DETREND_CONSTANT;
+  if (tc && lay.estimator != DELTA_EST_PHASE_LOCK) {  // per-channel fp16 scales: one pass over the chunk
+    int ns = (8 * p->num_sms + lay.C - 1) / lay.C;
+    ns = ns < 1 ? 1 : (ns > 64 ? 64 : ns);
+    chscale_kernel<<<dim3(lay.C, ns), 256, 0, st>>>(d_x, ld, p->cfg.in_dtype, p->cfg.norm_mode, p->n_first, p->d_offs(),
+                                                    p->d_isum(), lay.T, lay.wsum * (det ? 2.f : 1.f),
+                                                    reinterpret_cast<float *>(reinterpret_cast<char *>(d_X) + lay.x_scale_off),
+                                                    p->d_chmax(), p->d_chcnt());
+    p->launches++;
+    DELTA_CUDA_CHECK(cudaGetLastError());
+  }
+  const size_t smem = (size_t)kSegBlock * lay.L * sizeof(float);
+  LaunchCfg lc(dim3(lay.nkb, lay.C), dim3(256), smem, st, p->use_pdl);
+#define DELTA_DFT_LAUNCH(TC_, DET_)                                                                                        \
+  do {                                                                                                                     \
+    int rc = opt_in_smem(stft_dft_kernel<TC_, DET_>, smem);                                                                \
+    if (rc) return rc;                                                                                                     \
+    DELTA_CUDA_CHECK(cudaLaunchKernelEx(&lc.cfg, stft_dft_kernel<TC_, DET_>, d_x, ld, p->cfg.in_dtype, p->cfg.norm_mode,   \
+                                        p->n_first, (const double *)p->d_offs(), (const long long *)p->d_isum(), p->d_tw(), \
+                                        p->d_win(), lay, d_X, p->d_wpart()));                                              \
+  } while (0)
+  if (tc && det) DELTA_DFT_LAUNCH(true, true);
+  else if (tc) DELTA_DFT_LAUNCH(true, false);
+  else if (det) DELTA_DFT_LAUNCH(false, true);
+  else DELTA_DFT_LAUNCH(false, false);
+#undef DELTA_DFT_LAUNCH
+  p->launches++;
+  DELTA_CUDA_CHECK(cudaGetLastError());
+  return DELTA_OK;
+}
+
 int launch_stft(delta_plan *p, const void *d_x, int64_t ld, void *d_X, cudaStream_t st) {
+  if (!has_fft_path(p->lay.L)) return launch_stft_dft(p, d_x, ld, d_X, st);
 #define CALL(LL) launch_stft_L<LL>(p, d_x, ld, d_X, st)
   DELTA_SWITCH_L(p->lay.L, CALL)
 #undef CALL

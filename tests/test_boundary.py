@@ -50,8 +50,8 @@ def create(cfg):
 
 @pytest.mark.parametrize("kw,status", [
     (dict(), b.OK),
-    (dict(nfft=500), b.ERR_UNSUPPORTED),          # not a power of two
-    (dict(nfft=32, hop=16, max_lag=8), b.ERR_UNSUPPORTED),
+    (dict(nfft=501, hop=250, max_lag=250), b.ERR_UNSUPPORTED),   # odd transform length
+    (dict(nfft=8, hop=4, max_lag=4), b.ERR_UNSUPPORTED),
     (dict(nfft=8192, hop=4096, n_samples=100_000), b.ERR_UNSUPPORTED),
     (dict(n_samples=300), b.ERR_UNSUPPORTED),     # T < L
     (dict(max_lag=257), b.ERR_UNSUPPORTED),       # M > L/2
@@ -184,7 +184,7 @@ int main(void) {
   delta_sizes s;
   if (delta_plan_create(&c, &p) != DELTA_OK || delta_plan_sizes(p, &s) != DELTA_OK) return 1;
   printf("%d %d %lld %d\\n", s.n_segments, s.n_bins, (long long)s.n_pairs, delta_version());
-  c.nfft = 500;
+  c.nfft = 501;
   delta_plan *q = NULL;
   if (delta_plan_create(&c, &q) != DELTA_ERR_UNSUPPORTED || q != NULL) return 2;
   return delta_plan_destroy(p) == DELTA_OK ? 0 : 3;
@@ -197,3 +197,10 @@ int main(void) {
     out = subprocess.run([str(exe)], capture_output=True, text=True)
     assert out.returncode == 0, out
     assert out.stdout.split()[:3] == ["38", "257", "18336"]
+
+
+def test_non_power_of_two_nfft_is_accepted():
+    """Even transform lengths that are not powers of two take the direct-DFT kernels (f1): the plan is created and
+    reports K, F as the definitions give them."""
+    p = b.Plan(192, 10_000, 500, 250, 250, allocate=False)
+    assert p.sizes.K == (10_000 - 500) // 250 + 1 and p.sizes.F == 251 and p.sizes.n_lags == 501

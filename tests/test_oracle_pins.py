@@ -601,3 +601,32 @@ def test_fft_baseline_equals_oracle(C, T, L, H, M):
         assert got[k].shape == ref[k].shape, k
         assert np.max(np.abs(got[k] - ref[k])) <= 1e-10 * max(1.0, float(np.abs(ref[k]).max())), k
     assert np.max(np.abs(np.angle(np.exp(1j * (got["A"] - ref["A"]))))) <= 1e-8
+
+
+# ----------------------------------------------------------------------------------------------
+# f1: transform lengths that are not powers of two.  The oracle is a direct DFT and takes any even L; what pins it
+# there is again independent library code (scipy's Welch CSD / coherence and numpy's irfft run at L = 500, 768, 1000).
+@pytest.mark.parametrize("L,H", [(500, 250), (768, 192), (1000, 400)])
+def test_non_power_of_two_lengths_against_scipy(L, H):
+    rng = np.random.default_rng(L)
+    T = 12 * L
+    x = rng.standard_normal((3, T))
+    x[1] = 0.8 * np.roll(x[0], 3) + 0.4 * x[1]
+    out = o.analyze_chunk(x, L, H, L // 2, want_S=True)
+    K = o.n_segments(T, L, H)
+    pairs = o.all_pairs(3)
+    for p, (i, j) in enumerate(pairs):
+        f, Pxy = sps.csd(x[i, :(K - 1) * H + L], x[j, :(K - 1) * H + L], fs=1.0, window=sps.get_window("hann", L, fftbins=True),
+                         nperseg=L, noverlap=L - H, nfft=L, detrend=False, return_onesided=False, scaling="spectrum")
+        w = o.hann_periodic(L)
+        s_spec = 1.0 / np.sum(w) ** 2
+        S_sc = np.conj(Pxy[:L // 2 + 1]) / s_spec * o.scale_factor(L)     # scipy: conj(X_i) X_j, 'spectrum' scaling
+        assert np.max(np.abs(out["S"][p] - S_sc)) <= 1e-10 * np.max(np.abs(S_sc))
+        _, Cxy = sps.coherence(x[i, :(K - 1) * H + L], x[j, :(K - 1) * H + L], window=sps.get_window("hann", L, fftbins=True),
+                               nperseg=L, noverlap=L - H, nfft=L, detrend=False)
+        assert np.max(np.abs(out["G"][p] ** 2 - Cxy)) <= 1e-10
+        # Eq. (1d): numpy's inverse real FFT of the half spectrum (Im of DC and Nyquist dropped, as irfft does)
+        R = np.fft.irfft(out["S"][p], n=L)
+        R0 = np.array([np.fft.irfft(out["Sauto"][c], n=L)[0] for c in (i, j)])
+        rho = np.concatenate([R[L - L // 2:], R[:L // 2 + 1]]) / np.sqrt(R0[0] * R0[1])
+        assert np.max(np.abs(out["R"][p] - rho)) <= 1e-12

@@ -632,3 +632,47 @@ def test_all_variants_together(mode):
     assert out["R"].shape == (45, 2 * M + 1)
     st = compare(out, ref, pairs, "all variants", p_abs_tol=5e-5)
     print(st)
+
+
+@pytest.mark.parametrize("C,T,L,H,M", [(24, 10_000, 500, 250, 250), (10, 9_000, 768, 192, 100), (6, 12_000, 1000, 400, 500),
+                                        (5, 1_000, 48, 24, 24), (7, 3_000, 250, 100, 60)])
+def test_non_power_of_two_nfft(C, T, L, H, M, mode):
+    """f1: even transform lengths that are not powers of two run on the direct-DFT kernels
+    (stft_dft_kernel, pair_dft_kernel), through the same contraction; north_star's tolerances, both modes."""
+    x = es.turbulence(T, 300 + L)[:C]
+    _, out = gpu_analyze(x, L, H, M, contraction=mode)
+    ref = oracle_for(x, L, H, M)
+    assert out["G"].shape == ref["G"].shape == (C * (C - 1) // 2, L // 2 + 1) and out["R"].shape == ref["R"].shape
+    st = compare(out, ref, o.all_pairs(C), f"nfft {L}")
+    print(L, st)
+
+
+def test_non_power_of_two_nfft_with_variants(mode):
+    """The direct-DFT path with the f1/f2 switches on: int16 counts with offset normalisation, Hamming window, detrend,
+    zero-padded segments, band-pass, an explicit pair list, a short lag window; and its staged calls."""
+    b = binding()
+    C, T, L, Ls, H, M = 16, 10_000, 600, 400, 200, 77
+    counts, _ = es.streamed(n_chunks=1)
+    x = counts[0][:C]
+    offs = o.offsets(x[:, :5000])
+    allp = o.all_pairs(C)
+    pairs = allp[np.random.default_rng(9).choice(len(allp), 21, replace=False)]
+    band = (4e3, 150e3)
+    plan = b.Plan(C, T, L, H, M, contraction=mode, in_dtype=b.I16, norm_mode=b.NORM_RELATIVE, window=1, detrend=1,
+                  nperseg=Ls, band=band, pairs=pairs)
+    xd = dev(x)
+    plan.set_offsets(xd, 5000)
+    out = plan.analyze_chunk(xd)
+    torch.cuda.synchronize()
+    out = {k: v.cpu().numpy() for k, v in out.items()}
+    ref = o.analyze_chunk(x, L, H, M, pairs=pairs, fs=500e3, norm_mode=o.NORM_RELATIVE, offs=offs, band=band,
+                          win=o.WIN_HAMMING, detrend=o.DETREND_CONSTANT, nperseg=Ls)
+    st = compare(out, ref, pairs, "nfft 600 with variants")
+    print(st)
+    # staged calls give the same G, A, P
+    X = plan.stft(xd)
+    S, Sa = plan.cross_spectra(X)
+    G, A, P = plan.coherence(S, Sa), plan.crossphase(S), plan.crosspower(S)
+    torch.cuda.synchronize()
+    for name, t in (("G", G), ("A", A), ("P", P)):
+        assert np.array_equal(t.cpu().numpy(), out[name]), name
