@@ -676,3 +676,34 @@ def test_non_power_of_two_nfft_with_variants(mode):
     torch.cuda.synchronize()
     for name, t in (("G", G), ("A", A), ("P", P)):
         assert np.array_equal(t.cpu().numpy(), out[name]), name
+
+
+def test_strong_scaling_split_gives_the_same_bits():
+    """f4: one shot's chunks dealt round-robin to replicas (bench.py --scaling strong), every replica with its own plan
+    and its own offsets from chunk 0.  On one GPU: two plans take the even and the odd chunks; every chunk's results are
+    bit-identical to the single-plan run over the whole shot."""
+    import bench
+    b = binding()
+    w = es.WORKLOADS["streamed"]
+    counts, _ = es.streamed(n_chunks=6)
+    counts = counts[:, :48]
+    C = counts.shape[1]
+    first = dev(counts[0])
+
+    def run(chunks):
+        plan = b.Plan(C, w.T, w.nfft, w.hop, w.max_lag, in_dtype=b.I16, norm_mode=b.NORM_RELATIVE)
+        plan.set_offsets(first, w.n_first)
+        res = {}
+        for n in chunks:
+            out = plan.analyze_chunk(dev(counts[n]))
+            res[n] = {k: v.clone() for k, v in out.items()}
+        torch.cuda.synchronize()
+        return res
+
+    whole = run(range(6))
+    for rank in range(2):
+        part = run(bench.shot_chunks_of_rank(6, rank, 2))
+        assert sorted(part) == list(range(rank, 6, 2))
+        for n, out in part.items():
+            for k in ("G", "A", "P", "R", "Sauto"):
+                assert torch.equal(out[k], whole[n][k]), (rank, n, k)
