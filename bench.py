@@ -183,28 +183,35 @@ def cpu_baseline(w, budget_s=10.0):
     (BASELINE.md section 3).  Channel subsets keep each at ~10 s; the unit is still pair-spectra/s."""
     from oracle import fft_baseline as fb
     x_full = host_chunks(w, 0, 1)[0] if w.dtype == "f32" else es.turbulence(w.T, 9000)
-    # oracle: cost grows with pairs; time 16 channels, then as many as the budget allows
+    # cost grows with the pairs: time a few channels first, then as many as the budget allows; if a whole chunk takes less
+    # than the budget, whole chunks are repeated until ~budget seconds of CPU work have been timed
     def timed(fn, x):
         t0 = time.perf_counter()
         fn(x)
         return time.perf_counter() - t0
-    n0 = min(16, w.C)
-    t16 = timed(lambda x: oracle_chunk(x, w), x_full[:n0])
-    n_or = int(max(n0, min(w.C, n0 * np.sqrt(budget_s / max(t16, 1e-3)))))
-    t_or = timed(lambda x: oracle_chunk(x, w), x_full[:n_or]) if n_or > n0 else t16
-    P_or = n_or * (n_or - 1) // 2
-    n1 = min(48, w.C)
-    t48 = timed(lambda x: fb.analyze_chunk(x, w.nfft, w.hop, w.max_lag), x_full[:n1])
-    n_fb = int(max(n1, min(w.C, n1 * np.sqrt(budget_s / max(t48, 1e-3)))))
-    t_fb = timed(lambda x: fb.analyze_chunk(x, w.nfft, w.hop, w.max_lag), x_full[:n_fb]) if n_fb > n1 else t48
-    P_fb = n_fb * (n_fb - 1) // 2
+
+    def sample(fn, n0):
+        t_small = timed(fn, x_full[:n0])
+        n = int(max(n0, min(w.C, n0 * np.sqrt(budget_s / max(t_small, 1e-3)))))
+        reps, t = 0, 0.0
+        while True:
+            t += timed(fn, x_full[:n])
+            reps += 1
+            if t >= budget_s or n < w.C or reps >= 64:
+                break
+        return n, reps, t
+
+    n_or, r_or, t_or = sample(lambda x: oracle_chunk(x, w), min(16, w.C))
+    P_or = r_or * (n_or * (n_or - 1) // 2)
+    n_fb, r_fb, t_fb = sample(lambda x: fb.analyze_chunk(x, w.nfft, w.hop, w.max_lag), min(48, w.C))
+    P_fb = r_fb * (n_fb * (n_fb - 1) // 2)
     cores = blas_threads()
     return {"value": P_or / t_or, "unit": UNIT, "cores": cores, "kind": "oracle",
-            "sample": f"the first {n_or} channels ({P_or} pairs) of one '{w.name}' chunk ({w.T} samples, nfft {w.nfft}), "
-                      f"all four quantities, float64 direct-DFT numpy oracle, {t_or:.1f} s", "seconds": t_or,
+            "sample": f"{r_or} x the first {n_or} channels ({n_or * (n_or - 1) // 2} pairs) of one '{w.name}' chunk ({w.T} samples, "
+                      f"nfft {w.nfft}), all four quantities, float64 direct-DFT numpy oracle, {t_or:.1f} s", "seconds": t_or,
             "library_fft": {"value": P_fb / t_fb, "unit": UNIT, "cores": cores, "kind": "CPU, library FFT",
-                            "sample": f"the first {n_fb} channels ({P_fb} pairs) of the same chunk, float64 numpy rfft / "
-                                      f"matmul / ifft (oracle/fft_baseline.py, pinned to the oracle), {t_fb:.1f} s",
+                            "sample": f"{r_fb} x the first {n_fb} channels ({n_fb * (n_fb - 1) // 2} pairs) of the same chunk, float64 numpy "
+                                      f"rfft / matmul / ifft (oracle/fft_baseline.py, pinned to the oracle), {t_fb:.1f} s",
                             "seconds": t_fb}}
 
 

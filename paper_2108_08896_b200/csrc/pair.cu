@@ -4,16 +4,16 @@
 //   auto_prep_kernel  1/sqrt(S_cc[f]) from caller-supplied autospectra (staged calls only)
 //   s_unpack_kernel   test accessor: S layout -> complex64 [P][F]
 //
-// pair_kernel is persistent: a CTA walks over blocks of PB consecutive (lexicographic) pairs.  One block is one
-// contiguous [F][PB] tile of S and one contiguous run of rows in each output array.  A producer warp brings tile n+1
-// into the second stage of a two-stage ring with one cp.async.bulk copy (and works out the pairs' channels and their
-// rho normalisation) while the compute warps work on tile n; the only CTA-wide synchronisation is the ring's full /
-// empty mbarrier pair.  Every pair has a group of T = N/E threads (for L <= 1024 inside one warp, so warps run free of
-// each other and their store-bound and arithmetic-bound phases overlap on the SM):
+// pair_kernel is persistent, one CTA per SM.  A tile = PB consecutive (lexicographic) pairs = one contiguous [F][PB] block
+// of S and one contiguous run of rows in each output array.  A producer warp keeps a ring of NSLOT tile slots full (one
+// cp.async.bulk copy per tile, one per 1/sqrt(S_jj) row, and the pairs' channels and rho normalisations) while NTEAM
+// teams of PB x T threads work on NTEAM tiles; the only CTA-wide synchronisation is the full / empty mbarrier pair of
+// each slot.  Every pair has a group of T = N/E threads (for L <= 1024 inside one warp, so warps run free of each other
+// and their store-bound and arithmetic-bound phases overlap on the SM):
 //   pass 1  a thread owns 4 consecutive bins per step: |S| (cross-power), |S|/sqrt(S_ii S_jj), atan2; float4 stores
 //   pass 2  thread gt owns bins f = gt + T u (u < E), the register layout the inverse FFT of fft_reg.cuh starts from:
-//           merge step of the inverse real transform, register FFT through a private padded exchange buffer,
-//           rho stored from registers as float2.
+//           merge step of the inverse real transform, register FFT exchanging through the pair's own column of the
+//           tile (private padded buffers for the long transforms), rho stored from registers as float2.
 #include "delta_internal.h"
 #include "fft_reg.cuh"
 
