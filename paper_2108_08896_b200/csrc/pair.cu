@@ -61,12 +61,19 @@ struct PairCfg {
   static constexpr int THREADS = CTHREADS + 32;  // + the producer warp
   static constexpr size_t OFF_EXCH = NSLOT * SLOT_BYTES;
   static constexpr size_t OFF_FTAB = (OFF_EXCH + NTEAM * EXCH_BYTES + 15) & ~(size_t)15;  // the transform's twiddle tables
-  static constexpr size_t OFF_BAR = (OFF_FTAB + FTAB_BYTES + 7) & ~(size_t)7;              // full[NSLOT], empty[NSLOT]
-  static constexpr size_t SMEM = OFF_BAR + 2 * NSLOT * 8;
+  // Tile n is announced on full[n mod 2 NSLOT]: two "full" barriers per slot, used in turn.  A parity wait is right only if
+  // the waiter is less than one phase ahead of the barrier, and with one barrier per slot a team could be: the copies of
+  // tiles n and n + 1 may land out of order, and the team done with n + 1 would then take the still pending phase of
+  // tile n for the completed phase of tile n + NSLOT.  With two barriers the phase in doubt belongs to tile n - NSLOT,
+  // which was consumed before the producer could issue tile n, and that was before the tile this team worked on last
+  // (n + NSLOT - NTEAM >= n).
+  static constexpr int NFULL = 2 * NSLOT;
+  static constexpr size_t OFF_BAR = (OFF_FTAB + FTAB_BYTES + 7) & ~(size_t)7;              // full[NFULL], empty[NSLOT]
+  static constexpr size_t SMEM = OFF_BAR + (NFULL + NSLOT) * 8;
   static_assert(TTHREADS % 32 == 0 && THREADS <= 1024 && NTEAM >= 1, "block shape");
   static_assert(TILE_BYTES % 16 == 0 && ROW_BYTES % 16 == 0 && PB % 4 == 0 && 2 * PB <= 32, "tile shape");
   static_assert((T & (T - 1)) == 0 && (PB & (PB - 1)) == 0 && E % 4 == 0, "powers of two");
-  static_assert(NSLOT >= 2 && NSLOT > NTEAM - 1 && SMEM <= kSmemPerSm, "shared memory");
+  static_assert(NSLOT >= 2 && NSLOT >= NTEAM && SMEM <= kSmemPerSm, "shared memory");
 };
 
 // Exchange map of the register FFT onto a pair's own column of a 16-pairs-per-row tile (float2 slots, 128 bytes per row,
@@ -189,7 +196,7 @@ pair_kernel(const float2 *__restrict__ S, const float *__restrict__ Srsq, const 
   constexpr int N = Cfg::N, F = Cfg::F, T = Cfg::T, E = Cfg::E, PB = Cfg::PB, NSLOT = Cfg::NSLOT, NTEAM = Cfg::NTEAM;
   extern __shared__ __align__(128) unsigned char smem_raw[];
   float2 *ftab_s = reinterpret_cast<float2 *>(smem_raw + Cfg::OFF_FTAB);
-  uint64_t *full = reinterpret_cast<uint64_t *>(smem_raw + Cfg::OFF_BAR), *empty = full + NSLOT;
+  uint64_t *full = reinterpret_cast<uint64_t *>(smem_raw + Cfg::OFF_BAR), *empty = full + Cfg::NFULL;
 
   float *const G = G_, *const A = A_, *const Pw = Pw_, *const R = R_;
   const bool wantG = G != nullptr, wantGAP = G || A || Pw;
@@ -201,10 +208,8 @@ pair_kernel(const float2 *__restrict__ S, const float *__restrict__ Srsq, const 
 
   pdl_launch_dependents();
   if (tid == 0) {
-    for (int s = 0; s < NSLOT; ++s) {
-      mbar_init(full + s, 1);
-      mbar_init(empty + s, Cfg::TW);
-    }
+    for (int s = 0; s < Cfg::NFULL; ++s) mbar_init(full + s, 1);
+    for (int s = 0; s < NSLOT; ++s) mbar_init(empty + s, Cfg::TW);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   for (int i = tid; i < Geo::TABLE; i += Cfg::THREADS) ftab_s[i] = __ldg(ftab + i);  // a constant table of the plan
@@ -229,6 +234,7 @@ pair_kernel(const float2 *__restrict__ S, const float *__restrict__ Srsq, const 
     for (int n = 0; n < ncta; ++n) {
       const int tile = blockIdx.x + n * gridDim.x;
       const int s = n % NSLOT;
+      uint64_t *fullb = full + n % Cfg::NFULL;
       unsigned char *st = smem_raw + (size_t)s * Cfg::SLOT_BYTES;
       if (n >= NSLOT) mbar_wait(empty + s, (n / NSLOT - 1) & 1);
       if (lane < PB) {
@@ -239,14 +245,14 @@ pair_kernel(const float2 *__restrict__ S, const float *__restrict__ Srsq, const 
       __syncwarp();
       if (lane == 0) {
         const uint32_t bytes = (list ? 0u : (uint32_t)Cfg::TILE_BYTES) + (rows ? (uint32_t)(PB * Cfg::ROW_BYTES) : 0u);
-        if (bytes) mbar_expect_tx(full + s, bytes); else mbar_arrive(full + s);
-        if (!list) bulk_g2s(st, S + (int64_t)tile * F * PB, (uint32_t)Cfg::TILE_BYTES, full + s);  // else: the groups gather
+        if (bytes) mbar_expect_tx(fullb, bytes); else mbar_arrive(fullb);
+        if (!list) bulk_g2s(st, S + (int64_t)tile * F * PB, (uint32_t)Cfg::TILE_BYTES, fullb);  // else: the groups gather
       }
       __syncwarp();
       // 1/sqrt(S_jj) row of every pair, from the copy of the table that is aligned for the pair's float4 groups
       if (rows && lane < PB)
         bulk_g2s(st + Cfg::OFF_ROWS + lane * Cfg::ROW_BYTES, Srsq + ((int64_t)((-pl) & 3) * lay.C + ij.y) * Cfg::FP,
-                 (uint32_t)Cfg::ROW_BYTES, full + s);
+                 (uint32_t)Cfg::ROW_BYTES, fullb);
       if (n + 1 < ncta) tables(n + 1);
     }
     return;
@@ -272,10 +278,10 @@ pair_kernel(const float2 *__restrict__ S, const float *__restrict__ Srsq, const 
 
   for (int n = team; n < ncta; n += NTEAM) {
     const int tile = blockIdx.x + n * gridDim.x;
-    const int s = n % NSLOT, use = n / NSLOT;
+    const int s = n % NSLOT;
     unsigned char *st = smem_raw + (size_t)s * Cfg::SLOT_BYTES;
     float2 *tl = reinterpret_cast<float2 *>(st);  // [F][PB], slot = (pl ^ s_swz(f)) & (PB-1)
-    mbar_wait(full + s, use & 1);
+    mbar_wait(full + n % Cfg::NFULL, (n / Cfg::NFULL) & 1);
     const ushort2 ij = reinterpret_cast<const ushort2 *>(st + Cfg::OFF_IJ)[pl];
     const int64_t p = (int64_t)tile * PB + pl;
     const bool valid = p < lay.Po;

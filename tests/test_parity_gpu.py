@@ -528,6 +528,37 @@ def test_three_views_576_channels():
     _full_size_check(x, w.nfft, w.hop, w.max_lag, "576 channels", 10, 7)
 
 
+@pytest.mark.parametrize("C", [192, 576])
+def test_output_subsets_on_a_reused_plan_are_bit_identical(C, mode):
+    """Every subset of the per-pair outputs, asked for over and over on one plan, carries the bits of the call that
+    asked for all of them.  A call for the cross-power alone makes the pair kernel's teams run far ahead of the
+    tile copies, which is where a ring whose teams could mistake a pending barrier phase for a completed one gave
+    wrong tiles (white-noise input: every tile differs from its neighbours)."""
+    b = binding()
+    w = es.WORKLOADS["single"]
+    x = dev(np.random.default_rng(1234).standard_normal((C, w.T)).astype(np.float32))
+    plan = b.Plan(C, w.T, w.nfft, w.hop, w.max_lag, contraction=mode)
+    full = plan.empty_outputs()
+    plan.analyze_chunk(x, full)
+    torch.cuda.synchronize()
+    full = {k: v.clone() for k, v in full.items()}
+    import fastcheck as fc
+    fc.check_all_pairs(x.cpu().numpy(), w.nfft, w.hop, w.max_lag, {"all": {k: v.cpu().numpy() for k, v in full.items()}},
+                       TOLS, f"white noise {C}")
+    subsets = [dict(G=False, A=False, R=False), dict(G=False, A=False, R=True), dict(G=True, A=False, R=False),
+               dict(G=False, A=True, R=False), dict(G=True, A=True, R=True)]
+    for rep in range(6):
+        for sub in subsets:
+            out = plan.empty_outputs(**sub)
+            out = {k: v for k, v in out.items() if v is not None}
+            for v in out.values():
+                v.fill_(float("nan"))
+            plan.analyze_chunk(x, out)
+            torch.cuda.synchronize()
+            for k, v in out.items():
+                assert torch.equal(v, full[k]), f"rep {rep} subset {sub}: {k} differs in {int((v != full[k]).any(dim=-1).sum())} rows"
+
+
 def test_staged_external_X_with_padding_not_zeroed():
     """A caller-supplied X buffer whose padding (rows C..Cp-1, segment blocks beyond ceil(K/8)) holds NaN before
     delta_stft: C = 192 and 128 have Cp == C and an odd number of segment blocks (K = 38: 5 of 6), the case where the
