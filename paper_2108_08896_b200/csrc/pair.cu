@@ -170,8 +170,10 @@ __device__ __forceinline__ void mbar_wait(uint64_t *b, uint32_t parity) {
     asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
                  : "=r"(ok) : "r"(addr), "r"(parity) : "memory");
     if (ok) return;
+    // a waiting warp must not take issue slots from the working ones: back off after a few quick polls
+    if (spins >= 4) __nanosleep(spins < 16 ? 100 : 400);
     if (spins == 64) t0 = clock64();
-    if (spins > 64 && (spins & 1023) == 0 && clock64() - t0 > 4000000000LL) __trap();
+    if (spins > 64 && (spins & 255) == 0 && clock64() - t0 > 4000000000LL) __trap();
   }
 }
 __device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t bytes, uint64_t *bar) {
@@ -392,10 +394,29 @@ pair_kernel(const float2 *__restrict__ S, const float *__restrict__ Srsq, const 
       fft_inplace_g<Geo, true, Sync>(v, FftPadMap{exch + pl * Geo::BUF}, ftab_s, gt);
     }
     float *Rp = R + p * lay.nlags;
-    if (!valid) {
-    } else if (FULL) {
-      // lag m = xi for xi <= L/2 and xi - L for xi >= L/2; row position q = m + L/2
-      const bool vec = (reinterpret_cast<uintptr_t>(Rp) & 7) == 0;  // q is even: float2 stores iff the row is 8-byte aligned
+    if (FULL && T <= 32) {
+      // lag m = xi for xi <= L/2 and xi - L for xi >= L/2; row position q = m + L/2.  Element nn holds xi = 2 nn, 2 nn + 1
+      // at the even position q: a float2 store if the row is 8-byte aligned.  Rows have 2 M + 1 floats, so every other
+      // row is not: there the pairs are taken one sample later, (x[2 nn + 1], x[2 nn + 2]) at q + 1, with x[2 nn + 2] from
+      // the next thread of the group (from the next element of thread 0 for the last thread).  That covers the
+      // positions 1 .. L (xi = L/2 at position L included); position 0, also xi = L/2, is stored on its own.  (Scalar
+      // stores for those rows, 64-byte pieces and twice the instructions, cost 3 us in a store-only replica.)
+      // (every thread of the warp takes part in the shuffles; the pairs beyond the last one of a ragged tile do not store)
+      const bool odd = (reinterpret_cast<uintptr_t>(Rp) & 7) != 0;
+#pragma unroll
+      for (int u = 0; u < E; ++u) {
+        const int nn = gt + T * u;
+        const float a = v[u].x * norm, b = v[u].y * norm;
+        const int q = (u < E / 2) ? 2 * nn + N : 2 * nn - N;
+        const float nxt = __shfl_sync(0xffffffffu, gt == 0 ? v[(u + 1) % E].x : v[u].x, (gt + 1) & (T - 1), T < 32 ? T : 32) * norm;
+        if (valid) {
+          ST2(Rp + q + (odd ? 1 : 0), odd ? make_float2(b, nxt) : make_float2(a, b));
+          if (u == E / 2 && gt == 0) ST1(Rp + (odd ? 0 : L), a);  // xi = L/2 is lag -L/2 and lag +L/2
+        }
+      }
+    } else if (!valid) {
+    } else if (FULL) {  // groups wider than a warp
+      const bool vec = (reinterpret_cast<uintptr_t>(Rp) & 7) == 0;
 #pragma unroll
       for (int u = 0; u < E; ++u) {
         const int nn = gt + T * u;

@@ -528,23 +528,25 @@ def test_three_views_576_channels():
     _full_size_check(x, w.nfft, w.hop, w.max_lag, "576 channels", 10, 7)
 
 
-@pytest.mark.parametrize("C", [192, 576])
-def test_output_subsets_on_a_reused_plan_are_bit_identical(C, mode):
+@pytest.mark.parametrize("C,L", [(192, 512), (576, 512), (320, 64), (320, 128), (320, 256), (224, 1024)])
+def test_output_subsets_on_a_reused_plan_are_bit_identical(C, L, mode):
     """Every subset of the per-pair outputs, asked for over and over on one plan, carries the bits of the call that
     asked for all of them.  A call for the cross-power alone makes the pair kernel's teams run far ahead of the
     tile copies, which is where a ring whose teams could mistake a pending barrier phase for a completed one gave
     wrong tiles (white-noise input: every tile differs from its neighbours)."""
     b = binding()
-    w = es.WORKLOADS["single"]
-    x = dev(np.random.default_rng(1234).standard_normal((C, w.T)).astype(np.float32))
-    plan = b.Plan(C, w.T, w.nfft, w.hop, w.max_lag, contraction=mode)
+    # the other transform lengths run more teams per CTA over shorter tiles: enough pairs for every CTA's ring to go
+    # round several times (51,040 pairs = 3,190 tiles at 320 channels), 20 segments
+    T, H, M = (es.WORKLOADS["single"].T, 256, 256) if L == 512 else (L // 2 * 21, L // 2, L // 2)
+    x = dev(np.random.default_rng(1234).standard_normal((C, T)).astype(np.float32))
+    plan = b.Plan(C, T, L, H, M, contraction=mode)
     full = plan.empty_outputs()
     plan.analyze_chunk(x, full)
     torch.cuda.synchronize()
     full = {k: v.clone() for k, v in full.items()}
     import fastcheck as fc
-    fc.check_all_pairs(x.cpu().numpy(), w.nfft, w.hop, w.max_lag, {"all": {k: v.cpu().numpy() for k, v in full.items()}},
-                       TOLS, f"white noise {C}")
+    fc.check_all_pairs(x.cpu().numpy(), L, H, M, {"all": {k: v.cpu().numpy() for k, v in full.items()}},
+                       TOLS, f"white noise {C} x {T}, nfft {L}")
     subsets = [dict(G=False, A=False, R=False), dict(G=False, A=False, R=True), dict(G=True, A=False, R=False),
                dict(G=False, A=True, R=False), dict(G=True, A=True, R=True)]
     for rep in range(6):
