@@ -445,7 +445,11 @@ stft_kernel(const void *__restrict__ x, int64_t ld, int in_dtype, int norm_mode,
     const float sc = !TC ? 1.f : (lay.estimator == DELTA_EST_PHASE_LOCK ? 8192.f : (CLUSTER ? csc[pcl] : chscale[c]));
     store_x_bin<TC>(Xout, lay, kb, c, f, sc, re, im);
   };
-  constexpr int HB = N / 2 + 1;  // f = 0 .. N/2
+  // Work items: (channel, f) with f = 0 .. N/2 - 1, i.e. CH N/2 of them; with 16 points per thread that is exactly the
+  // number of threads, so the loop runs once.  Bin N/2, its own partner (X[N/2] = conj Z[N/2]), rides with the item of
+  // f = 0 (as a 129th item per channel it sent two threads of the CTA through the loop a second time while all the
+  // others waited).
+  constexpr int HB = N / 2;
   for (int idx = tid; idx < CH * HB; idx += Cfg::THREADS) {
     const int pcl = idx % CH, f = idx / CH;
     const int c = c0 + pcl;
@@ -466,7 +470,17 @@ stft_kernel(const void *__restrict__ x, int64_t ld, int in_dtype, int norm_mode,
       im2[s] = -e.y - wd.x;
     }
     store_bin(c, pcl, f, re, im);
-    if (2 * f != N) store_bin(c, pcl, N - f, re2, im2);
+    store_bin(c, pcl, N - f, re2, im2);
+    if (f == 0) {
+      const int i_h = fft_pad(N / 2);
+#pragma unroll
+      for (int s = 0; s < kSegBlock; ++s) {
+        const float2 zh = zc[s * G::BUF + i_h];
+        re[s] = zh.x;
+        im[s] = -zh.y;
+      }
+      store_bin(c, pcl, N / 2, re, im);
+    }
   }
   if (CLUSTER) cg::this_cluster().barrier_wait();  // no CTA exits while its cmax may still be read
 }
