@@ -416,9 +416,22 @@ def run_ours(args):
             traffic = json.load(open(tpath)).get(w.name, {}).get(d["kernel"].split("+")[0])
         except Exception:
             traffic = None
+    # SM <-> L2 crossbar bytes of the dominant kernel per launch (ncu, profiles/r02_xbar.json.txt) held against the rates
+    # `bench.py --probe-fabric` measured (profiles/r02_probe_fabric.json.txt): reads and writes add up on that path, so
+    # bound_us = write / write rate + read / read rate.  Committed captures, not live values; null without them.
+    xbar = None
+    try:
+        xb = json.load(open(os.path.join(ROOT, "profiles", "r02_xbar.json.txt"))).get(w.name, {}).get(d["kernel"].split("+")[0])
+        pr = {c["case"].split(" ")[0]: c["gbs"] for c in json.load(open(os.path.join(ROOT, "profiles", "r02_probe_fabric.json.txt")))["cases"][:2]}
+        if xb:
+            bound_us = xb["write_bytes"] / pr["write"] / 1e3 + xb["read_bytes"] / pr["read"] / 1e3
+            xbar = {"read_bytes": xb["read_bytes"], "write_bytes": xb["write_bytes"], "probe_read_gbs": pr["read"],
+                    "probe_write_gbs": pr["write"], "bound_us": bound_us, "frac": bound_us / (d["ms"] * 1e3)}
+    except Exception:
+        xbar = None
     roofline = {"kernel": d["kernel"], "bound": d["bound"], "achieved": d["achieved"], "peak": peak, "unit": d["unit"],
                 "frac": d["achieved"] / peak, "traffic": traffic, "peak_source": peak_src,
-                "kernel_ms": d["ms"], "kernel_share_of_step": float(stage_mean[dom] / stage_mean.sum()),
+                "kernel_ms": d["ms"], "kernel_share_of_step": float(stage_mean[dom] / stage_mean.sum()), "xbar": xbar,
                 "stages": stages,
                 "pipeline": {"alg_bytes_per_step": ab["total"], "achieved": ab["total"] / (ms / K * 1e-3) / 1e9,
                              "unit": "GB/s", "frac_of_measured_hbm": ab["total"] / (ms / K * 1e-3) / 1e9 / peaks["hbm_gbs"],
@@ -493,6 +506,43 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def probe_fabric():
+    """What the path between the SMs and L2 sustains (paper_2108_08896_b200/csrc/probe.cu): the rate the crossbar bytes
+    of the kernels (ncu: l1tex__m_xbar2l1tex_read_bytes + l1tex__m_l1tex2xbar_write_bytes) are held against in
+    DESIGN.md section 7.  Sizes are those of config 2: S (37.9 MB, L2 resident) read, the outputs (94.2 MB, rotating over
+    six buffers so that they drain to HBM) written.  Prints one JSON line."""
+    import torch
+    from paper_2108_08896_b200 import binding as b
+    dev = torch.device("cuda", 0)
+    rbytes, wbytes = 37978112 // 32768 * 32768, 94173696 // 16 * 16
+    src = torch.ones(rbytes, dtype=torch.uint8, device=dev)
+    dsts = [torch.empty(wbytes, dtype=torch.uint8, device=dev) for _ in range(6)]
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    out = {"probe": "sm_l2_fabric", "unit": "GB/s", "launch": "one CTA per SM, 800 threads", "cases": []}
+    for name, rb, wb in (("read (bulk copy to shared memory)", rbytes, 0), ("write (16-byte streaming stores)", 0, wbytes),
+                         ("read + write", rbytes, wbytes)):
+        for r in range(12):
+            b._probe_fabric(src, rb, dsts[r % 6], wb)
+        torch.cuda.synchronize()
+        graph = torch.cuda.CUDAGraph()   # 60 launches back to back: a 5 us kernel is not to be timed at the host's launch rate
+        with torch.cuda.graph(graph):
+            for r in range(60):
+                b._probe_fabric(src, rb, dsts[r % 6], wb)
+        graph.replay()
+        torch.cuda.synchronize()
+        times = []
+        for rep in range(5):
+            e0.record()
+            graph.replay()
+            e1.record()
+            torch.cuda.synchronize()
+            times.append(e0.elapsed_time(e1) / 60)
+        ms = sorted(times)[2]
+        out["cases"].append({"case": name, "read_bytes": rb, "write_bytes": wb, "us_per_launch": round(ms * 1e3, 2),
+                             "gbs": round((rb + wb) / ms / 1e6, 1)})
+    print(json.dumps(out))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -504,7 +554,11 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--contraction", default="auto", choices=["auto", "fp32", "tc"])
     ap.add_argument("--inflight", type=int, default=2, help="independent chunks kept in flight (plans x streams)")
+    ap.add_argument("--probe-fabric", action="store_true", help="measure the SM <-> L2 rates instead of the workload")
     args = ap.parse_args()
+    if args.probe_fabric:
+        probe_fabric()
+        return
     if args.impl == "reference":
         args.steps = 20 if args.steps is None else args.steps   # defaults sized per arm
         args.warmup = 3 if args.warmup is None else args.warmup

@@ -62,6 +62,7 @@ def _load() -> C.CDLL:
     lib.delta_cross_spectra.argtypes = [vp, vp, vp, vp, vp]
     lib.delta_cross_spectra_unpack.argtypes = [vp, vp, vp, vp]
     lib.delta_internal_set_trace.argtypes = [vp, vp]   # development hook, not part of the C ABI
+    lib.delta_internal_probe_fabric.argtypes = [vp, C.c_size_t, vp, C.c_size_t, vp]   # measurement aid (csrc/probe.cu)
     lib.delta_coherence.argtypes = [vp, vp, vp, vp, vp]
     lib.delta_crossphase.argtypes = [vp, vp, vp, vp]
     lib.delta_crosspower.argtypes = [vp, vp, vp, vp]
@@ -266,3 +267,11 @@ class Plan:
     @property
     def last_launch_count(self):
         return LIB.delta_last_launch_count(self._h)
+
+
+def _probe_fabric(src, read_bytes, dst, write_bytes):
+    """One launch of the SM <-> L2 probe (csrc/probe.cu; not part of the C ABI): bulk-copies `read_bytes` of `src` into
+    shared memory and writes `write_bytes` of `dst`, one persistent CTA per SM."""
+    _check(LIB.delta_internal_probe_fabric(None if src is None else src.data_ptr(), read_bytes,
+                                           None if dst is None else dst.data_ptr(), write_bytes, _stream()),
+           "delta_internal_probe_fabric")
