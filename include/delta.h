@@ -41,7 +41,8 @@
 extern "C" {
 #endif
 
-#define DELTA_VERSION 200 /* 0.2.0: out_ring in delta_analyze_shot_host; scales inside X buffers; DELTA_ERR_NO_MEMORY */
+#define DELTA_VERSION 201 /* 0.2.1: delta_coherence_static, DELTA_ERR_TOO_LARGE (0.2.0: out_ring in
+                             delta_analyze_shot_host; scales inside X buffers; DELTA_ERR_NO_MEMORY) */
 
 typedef enum {
   DELTA_OK = 0,
@@ -52,7 +53,8 @@ typedef enum {
   DELTA_ERR_NO_WORKSPACE = -4,/* compute call before delta_plan_set_workspace(), or it is too small */
   DELTA_ERR_CUDA = -5,        /* a CUDA runtime call failed; see delta_last_cuda_error()            */
   DELTA_ERR_STATE = -6,       /* e.g. norm_mode needs offsets and delta_set_offsets() was not called */
-  DELTA_ERR_NO_MEMORY = -7    /* host allocation of the plan failed                                 */
+  DELTA_ERR_NO_MEMORY = -7,   /* host allocation of the plan failed                                 */
+  DELTA_ERR_TOO_LARGE = -8    /* delta_coherence_static: the plan needs more than DELTA_STATIC_SCRATCH_BYTES */
 } delta_status;
 
 /* periodic (DFT-even) windows, x = 2 pi n/L: Hann 1/2 - 1/2 cos x (R4, the default); the others are the f1 variants:
@@ -156,6 +158,21 @@ int delta_cross_spectra_unpack(delta_plan *plan, const float *d_S, float *d_out,
 
 /* a4, Eq. (1b): d_G float [P][F].  0 where S_ii S_jj = 0 (R16). */
 int delta_coherence(delta_plan *plan, const float *d_S, const float *d_Sauto, float *d_G, void *stream);
+/* a4, Eq. (1b) again, for callers that cannot let scratch be allocated or handed over: code under
+ * CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc.  Same arguments, same kernels and same
+ * result as delta_coherence, but the stage's scratch -- the table of 1/sqrt(S_cc[f]) in four shifted copies and
+ * 1/sqrt(L R_cc[0]), 4 C ceil4(F) + C floats, each part rounded up to 256 bytes -- lives in a device array of
+ * DELTA_STATIC_SCRATCH_BYTES inside the library (held by every GPU that loads the library, until the process exits)
+ * instead of the plan's workspace.  The call allocates nothing (no cudaMalloc, cudaFree or allocating library routine); the
+ * plan's workspace must still be set: the constant tables of the plan are read from it.
+ *   - A plan that needs more scratch than the array holds is refused with DELTA_ERR_TOO_LARGE (8 MiB covers every
+ *     BASELINE config: 0.8 MB at config 2, 6.3 MB at config 5; 576 channels at nfft 512 need 2.4 MB).
+ *   - The plan's device must be the current device (else DELTA_ERR_INVALID_ARG).
+ *   - ALL calls on a device, from any plan, share the one array.  Calls that overlap on the GPU (different streams
+ *     without an ordering between them) race on it: order them, or use delta_coherence, whose scratch is per plan.  The
+ *     array keeps the last call's contents; every call clears the part it uses before writing it. */
+#define DELTA_STATIC_SCRATCH_BYTES (8u << 20)
+int delta_coherence_static(delta_plan *plan, const float *d_S, const float *d_Sauto, float *d_G, void *stream);
 /* a4, Eq. (1c): d_A float [P][F], radians in [-pi, pi]. */
 int delta_crossphase(delta_plan *plan, const float *d_S, float *d_A, void *stream);
 /* a4, |Eq. (1a)|: d_P float [P][F]. */

@@ -16,6 +16,8 @@ from . import build as _build
 # ---- enums (include/delta.h) --------------------------------------------------------------
 OK = 0
 ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_ALIGNMENT, ERR_NO_WORKSPACE, ERR_CUDA, ERR_STATE, ERR_NO_MEMORY = -1, -2, -3, -4, -5, -6, -7
+ERR_TOO_LARGE = -8
+STATIC_SCRATCH_BYTES = 8 << 20   # DELTA_STATIC_SCRATCH_BYTES
 WIN_HANN_PERIODIC = 0
 SCALE_WINPOW, SCALE_NONE, SCALE_DENSITY, SCALE_SPECTRUM = 0, 1, 2, 3
 F32, I16 = 0, 1
@@ -40,7 +42,7 @@ class DeltaSizes(C.Structure):
 EXPORTS = ["delta_plan_create", "delta_plan_destroy", "delta_plan_sizes", "delta_plan_set_workspace",
            "delta_set_offsets", "delta_get_offsets", "delta_stft", "delta_stft_unpack", "delta_cross_spectra",
            "delta_cross_spectra_unpack",
-           "delta_coherence", "delta_crossphase", "delta_crosspower", "delta_crosscorr", "delta_accumulate", "delta_analyze_chunk",
+           "delta_coherence", "delta_coherence_static", "delta_crossphase", "delta_crosspower", "delta_crosscorr", "delta_accumulate", "delta_analyze_chunk",
            "delta_analyze_shot_host", "delta_plan_set_stage_events", "delta_last_launch_count", "delta_strerror", "delta_last_cuda_error",
            "delta_version"]
 
@@ -64,6 +66,7 @@ def _load() -> C.CDLL:
     lib.delta_internal_set_trace.argtypes = [vp, vp]   # development hook, not part of the C ABI
     lib.delta_internal_probe_fabric.argtypes = [vp, C.c_size_t, vp, C.c_size_t, vp]   # measurement aid (csrc/probe.cu)
     lib.delta_coherence.argtypes = [vp, vp, vp, vp, vp]
+    lib.delta_coherence_static.argtypes = [vp, vp, vp, vp, vp]
     lib.delta_crossphase.argtypes = [vp, vp, vp, vp]
     lib.delta_crosspower.argtypes = [vp, vp, vp, vp]
     lib.delta_crosscorr.argtypes = [vp, vp, vp, vp, vp]
@@ -209,6 +212,14 @@ class Plan:
     def coherence(self, S, Sauto, G=None):
         G = torch.empty((self.sizes.P, self.sizes.F), dtype=torch.float32, device=self.device) if G is None else G
         _check(LIB.delta_coherence(self._h, S.data_ptr(), Sauto.data_ptr(), G.data_ptr(), _stream()), "delta_coherence")
+        return G
+
+    def coherence_static(self, S, Sauto, G=None):
+        """delta_coherence with its scratch in the library's static device array: nothing is allocated by the call (pass
+        G to keep torch from allocating the output)."""
+        G = torch.empty((self.sizes.P, self.sizes.F), dtype=torch.float32, device=self.device) if G is None else G
+        _check(LIB.delta_coherence_static(self._h, S.data_ptr(), Sauto.data_ptr(), G.data_ptr(), _stream()),
+               "delta_coherence_static")
         return G
 
     def crossphase(self, S, A=None):

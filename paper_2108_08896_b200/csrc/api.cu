@@ -523,6 +523,7 @@ const char *delta_strerror(int status) {
     case DELTA_ERR_CUDA: return "CUDA runtime error (see delta_last_cuda_error)";
     case DELTA_ERR_STATE: return "call sequence error (offsets not set)";
     case DELTA_ERR_NO_MEMORY: return "host memory allocation failed";
+    case DELTA_ERR_TOO_LARGE: return "plan needs more scratch than DELTA_STATIC_SCRATCH_BYTES (use delta_coherence)";
     default: return "unknown status";
   }
 }

@@ -27,7 +27,7 @@ def test_library_exports_every_declared_symbol():
     for name in ("delta_stft", "delta_cross_spectra", "delta_coherence", "delta_crossphase", "delta_crosspower",
                  "delta_crosscorr"):   # the six calls BASELINE.json's north_star names
         assert name in syms
-    assert b.LIB.delta_version() == 200
+    assert b.LIB.delta_version() == 201
     assert os.path.dirname(b.LIB_PATH).endswith("paper_2108_08896_b200")  # in-tree, not site-packages
 
 
