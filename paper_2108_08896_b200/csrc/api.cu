@@ -306,6 +306,15 @@ int delta_internal_set_trace(delta_plan *p, void *d_trace) {
   return DELTA_OK;
 }
 
+// Test hook, not part of the C ABI: the epilogue warps of the tensor-core contraction sleep `ns` nanoseconds before every
+// accumulator unit but the first of an item.  With a slow epilogue, an MMA that reused the TMEM columns of a unit before
+// they were read out would corrupt S every time instead of once in a long while (tests/test_parity_gpu.py).
+int delta_internal_set_epilogue_delay(delta_plan *p, int ns) {
+  if (!p || ns < 0 || ns > 1000000) return DELTA_ERR_INVALID_ARG;
+  p->tc_epi_delay_ns = ns;
+  return DELTA_OK;
+}
+
 int delta_stft_unpack(delta_plan *p, const void *d_X, float *d_out, void *stream) {
   int rc = need_ws(p);
   if (rc) return rc;

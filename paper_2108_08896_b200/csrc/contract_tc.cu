@@ -122,6 +122,7 @@ struct TcParams {
   int nunits[kTcMaxGroups];
   TcUnit units[kTcMaxGroups][kTcMaxUnits];
   int nstage, ksteps, unit_major;
+  int epi_delay_ns;  // test hook (delta_internal_set_epilogue_delay): the epilogue sleeps before units of index >= 1
   uint32_t stage_bytes, plane_bytes;  // per stage: 4 planes of 2*Cp*16 bytes
   int64_t plane_elems;                // halves between planes in global memory: Kc*Cp*8
   int64_t kstep_elems;                // halves per K=16 step inside a plane: 2*Cp*8
@@ -250,10 +251,30 @@ contract_tc_kernel(const __half *__restrict__ X, Layout lay, TcParams prm, float
       }
       __syncwarp();
     };
-    auto wait_unit_free = [&](int u) {
+    // Before the first MMA of a unit its TMEM columns must have been read out.  tempty[u] says that for the last unit of
+    // index u.  But groups lay their units out differently (a 64-wide unit takes 128 columns, a 128-wide one 256), so the
+    // columns of unit u may also belong to a unit of HIGHER index of the CTA's previous item, which nothing above waits
+    // for: then the highest such index is awaited too.  That is enough: every epilogue warp reads the units in order, so
+    // a completed phase of tempty[m] means that all units before it (of that item and of the items before) are read out;
+    // indices below u have been awaited by this item's earlier units, and an index above u has not been used again yet,
+    // so its parity bit still stands for the previous item's phase.  (Found in round 2: 576 channels have such
+    // transitions, e.g. (64, 128, 64) -> (128, 128); it is also why 256-wide units "failed parity" on config 5 in round 1.)
+    int g = blockIdx.x % prm.ngroups, gp = -1;  // group of this item, of the previous item
+    auto wait_unit_free = [&](int u, const TcUnit &un) {
       if ((used >> u) & 1u) {  // epilogue has drained the previous use
         mbar_wait(tempty + u, ((par >> u) & 1u) ^ 1u);
         fence_after();
+      }
+      if (gp >= 0 && gp != g) {
+        int need = -1;
+        for (int up = u + 1; up < prm.nunits[gp]; ++up) {
+          const int otm = prm.units[gp][up].tm, oend = otm + 2 * prm.units[gp][up].N;
+          if (otm < un.tm + 2 * un.N && oend > un.tm) need = up;
+        }
+        if (need >= 0) {
+          mbar_wait(tempty + need, ((par >> need) & 1u) ^ 1u);
+          fence_after();
+        }
       }
     };
     auto unit_done = [&](int u) {
@@ -264,7 +285,6 @@ contract_tc_kernel(const __half *__restrict__ X, Layout lay, TcParams prm, float
     };
 
     uint32_t s0 = 0, pass0 = 0;  // stage and ring pass of the item's first K step
-    int g = blockIdx.x % prm.ngroups;
     const int gstep = gridDim.x % prm.ngroups;
     for (int item = blockIdx.x; item < nitems; item += gridDim.x) {
       const int nu = prm.nunits[g];
@@ -276,7 +296,7 @@ contract_tc_kernel(const __half *__restrict__ X, Layout lay, TcParams prm, float
           const uint32_t ao16 = (uint32_t)(un.row0 / 8) * 8u, bo16 = (uint32_t)(un.col0 / 8) * 8u;
           const uint32_t id = make_idesc(un.N, 0), idn = make_idesc(un.N, 1);
           const uint32_t d_re = tmem_base + (uint32_t)un.tm, d_im = d_re + (uint32_t)un.N;
-          wait_unit_free(u);
+          wait_unit_free(u, un);
           for (int ks = 0; ks < prm.ksteps; ++ks) {
             mbar_wait(full_bar + s, pass & 1u);
             fence_after();
@@ -294,7 +314,7 @@ contract_tc_kernel(const __half *__restrict__ X, Layout lay, TcParams prm, float
           const uint32_t ao16 = (uint32_t)(un.row0 / 8) * 8u, bo16 = (uint32_t)(un.col0 / 8) * 8u;
           const uint32_t id = make_idesc(un.N, 0), idn = make_idesc(un.N, 1);
           const uint32_t d_re = tmem_base + (uint32_t)un.tm, d_im = d_re + (uint32_t)un.N;
-          wait_unit_free(u);
+          wait_unit_free(u, un);
           uint32_t s = s0, pass = pass0;
           for (int ks = 0; ks < prm.ksteps; ++ks) {
             if (u == 0) {
@@ -314,6 +334,7 @@ contract_tc_kernel(const __half *__restrict__ X, Layout lay, TcParams prm, float
           if (u == nu - 1) { s0 = s; pass0 = pass; }
         }
       }
+      gp = g;
       g += gstep;
       if (g >= prm.ngroups) g -= prm.ngroups;
     }
@@ -339,6 +360,8 @@ contract_tc_kernel(const __half *__restrict__ X, Layout lay, TcParams prm, float
         par ^= 1u << u;
         fence_after();
         if (warp == 0) { TC_TRACE(2, tr); ++tr; }
+        // (test hook: a slow epilogue makes a too-early reuse of its TMEM columns by the next item show every time)
+        if (prm.epi_delay_ns && u > 0) __nanosleep((unsigned)prm.epi_delay_ns);
         if (32 * q >= un.lane_lo && 32 * q < un.lane_hi) {
           const int jw0 = un.row0 + 32 * q, j = jw0 + lane;
           const bool jok = j < C;
@@ -447,6 +470,7 @@ int launch_contract_tc(delta_plan *p, const void *d_X, float *d_S, float *d_auto
     }
   }
   prm.ksteps = lay.Kp / 16;
+  prm.epi_delay_ns = p->tc_epi_delay_ns;
   prm.plane_bytes = (uint32_t)lay.Cp * 32u;  // [2][Cp][8] halves
   prm.stage_bytes = 4u * prm.plane_bytes;
   prm.plane_elems = (int64_t)lay.Kc * lay.Cp * kSegBlock;

@@ -105,6 +105,7 @@ struct delta_plan {
   long long *d_trace = nullptr;  // debug: clock stamps of the tensor-core contraction (delta_debug_set_trace)
   bool band_on = false;  // band-pass filter or phase-lock estimator: rho is normalised from the autospectra, not from
                          // the windowed signal energy (Parseval does not apply to the modified spectra)
+  int tc_epi_delay_ns = 0;  // test hook, see delta_internal_set_epilogue_delay (api.cu)
   bool use_pdl = true;  // programmatic dependent launch between the hot-path kernels (DELTA_NO_PDL=1 switches it off)
   bool stage_events_on = false;
   cudaEvent_t stage_ev[4] = {nullptr, nullptr, nullptr, nullptr};

@@ -561,6 +561,31 @@ def test_output_subsets_on_a_reused_plan_are_bit_identical(C, L, mode):
                 assert torch.equal(v, full[k]), f"rep {rep} subset {sub}: {k} differs in {int((v != full[k]).any(dim=-1).sum())} rows"
 
 
+@pytest.mark.parametrize("C", [576, 704])
+def test_tmem_columns_are_not_reused_before_they_are_read_out(C):
+    """Tensor-core contraction, channel counts whose accumulator groups have different TMEM layouts (576: units of
+    (64, 128, 64) channels followed by (128, 128)): the first unit of an item shares columns with the SECOND unit of the
+    CTA's previous item, so its MMAs have to wait for that unit's read-out too, not only for the unit of their own index.
+    With the epilogue slowed down by the test hook a missing wait corrupts S every time."""
+    b = binding()
+    T, L, H, M = 3000, 512, 256, 16
+    x = np.random.default_rng(77).standard_normal((C, T)).astype(np.float32)
+    xd = dev(x)
+    ref_plan = b.Plan(C, T, L, H, M, contraction=b.CONTRACT_FP32)
+    S_ref = ref_plan.cross_spectra_unpack(ref_plan.cross_spectra(ref_plan.stft(xd))[0])
+    plan = b.Plan(C, T, L, H, M, contraction=b.CONTRACT_TC)
+    X = plan.stft(xd)
+    S_fast = plan.cross_spectra_unpack(plan.cross_spectra(X)[0])
+    plan._set_epilogue_delay(20000)
+    S_slow = plan.cross_spectra_unpack(plan.cross_spectra(X)[0])
+    plan._set_epilogue_delay(0)
+    torch.cuda.synchronize()
+    assert torch.equal(torch.view_as_real(S_slow), torch.view_as_real(S_fast)), \
+        f"{int((S_slow != S_fast).any(dim=1).sum())} pairs change with a slow epilogue"
+    scale = torch.abs(S_ref).max().item()
+    assert torch.max(torch.abs(S_fast - S_ref)).item() <= 2e-5 * scale   # split-fp16 tensor cores vs the FP32 pipe
+
+
 def test_staged_external_X_with_padding_not_zeroed():
     """A caller-supplied X buffer whose padding (rows C..Cp-1, segment blocks beyond ceil(K/8)) holds NaN before
     delta_stft: C = 192 and 128 have Cp == C and an odd number of segment blocks (K = 38: 5 of 6), the case where the
