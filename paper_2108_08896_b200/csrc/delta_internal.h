@@ -3,6 +3,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <mutex>
 #include <vector>
 
 #include "delta.h"
@@ -182,16 +183,32 @@ struct LaunchCfg {
   }
 };
 
-// opt in to more than 48 KB of dynamic shared memory
+// Opt in to more than 48 KB of dynamic shared memory.  The attribute belongs to the (kernel, device) pair and is a
+// maximum, so it is set once per pair and raised only when a launch needs more (the launchers call this every time).
+// Fixed-size table, no heap: the launch path allocates nothing.
+struct SmemOptIn {
+  const void *kern;
+  int dev;
+  size_t bytes;
+};
 template <typename Kern>
 static inline int opt_in_smem(Kern kern, size_t bytes) {
-  if (bytes > 48 * 1024) {
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
-    if (e != cudaSuccess) {
-      set_cuda_error(e);
-      return DELTA_ERR_CUDA;
-    }
-  }
+  if (bytes <= 48 * 1024) return DELTA_OK;
+  constexpr int kSlots = 256;
+  static std::mutex mu;  // one table per translation unit and kernel signature
+  static SmemOptIn seen[kSlots];
+  static int nseen = 0;
+  int dev = 0;
+  DELTA_CUDA_CHECK(cudaGetDevice(&dev));
+  const void *key = reinterpret_cast<const void *>(kern);
+  std::lock_guard<std::mutex> lock(mu);
+  SmemOptIn *slot = nullptr;
+  for (int i = 0; i < nseen; ++i)
+    if (seen[i].kern == key && seen[i].dev == dev) slot = &seen[i];
+  if (slot && slot->bytes >= bytes) return DELTA_OK;
+  DELTA_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
+  if (slot) slot->bytes = bytes;
+  else if (nseen < kSlots) seen[nseen++] = {key, dev, bytes};  // (a full table only costs the call again next time)
   return DELTA_OK;
 }
 
