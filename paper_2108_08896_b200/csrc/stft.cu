@@ -445,41 +445,33 @@ stft_kernel(const void *__restrict__ x, int64_t ld, int in_dtype, int norm_mode,
     const float sc = !TC ? 1.f : (lay.estimator == DELTA_EST_PHASE_LOCK ? 8192.f : (CLUSTER ? csc[pcl] : chscale[c]));
     store_x_bin<TC>(Xout, lay, kb, c, f, sc, re, im);
   };
-  // Work items: (channel, f) with f = 0 .. N/2 - 1, i.e. CH N/2 of them; with 16 points per thread that is exactly the
-  // number of threads, so the loop runs once.  Bin N/2, its own partner (X[N/2] = conj Z[N/2]), rides with the item of
-  // f = 0 (as a 129th item per channel it sent two threads of the CTA through the loop a second time while all the
-  // others waited).
+  // Work items: (channel, f0) with f0 = 0 .. N/2 - 1, i.e. CH N/2 of them; with 16 points per thread that is exactly the
+  // number of threads, so the loop runs once.  Bin N/2, its own partner, is a second turn of the item of f0 = 0 (as a 129th
+  // item per channel it sent two threads of the CTA through the whole loop again while all the others waited; as a third
+  // inline store of every thread it cost registers: spills at nfft 1024).
   constexpr int HB = N / 2;
   for (int idx = tid; idx < CH * HB; idx += Cfg::THREADS) {
-    const int pcl = idx % CH, f = idx / CH;
+    const int pcl = idx % CH, f0 = idx / CH;
     const int c = c0 + pcl;
     if (c >= lay.C) continue;
-    const float2 w = __ldg(tw + f);  // e^{-2 pi i f/L}
     const float2 *zc = zb + pcl * (kSegBlock * G::BUF + Cfg::CHPAD);
-    const int i_f = fft_pad(f), i_r = fft_pad((N - f) & (N - 1));
-    float re[kSegBlock], im[kSegBlock], re2[kSegBlock], im2[kSegBlock];
-#pragma unroll
-    for (int s = 0; s < kSegBlock; ++s) {
-      const float2 zf = zc[s * G::BUF + i_f], zr = zc[s * G::BUF + i_r];
-      const float2 e = make_float2(0.5f * (zf.x + zr.x), 0.5f * (zf.y - zr.y));
-      const float2 d = make_float2(0.5f * (zf.x - zr.x), 0.5f * (zf.y + zr.y));
-      const float2 wd = cmul(w, d);
-      re[s] = e.x + wd.y;
-      im[s] = e.y - wd.x;
-      re2[s] = e.x - wd.y;
-      im2[s] = -e.y - wd.x;
-    }
-    store_bin(c, pcl, f, re, im);
-    store_bin(c, pcl, N - f, re2, im2);
-    if (f == 0) {
-      const int i_h = fft_pad(N / 2);
+    for (int f = f0; f <= N / 2; f += (f0 == 0 ? N / 2 : N)) {  // f0 = 0: f = 0, N/2;  else: f = f0
+      const float2 w = __ldg(tw + f);  // e^{-2 pi i f/L}
+      const int i_f = fft_pad(f), i_r = fft_pad((N - f) & (N - 1));
+      float re[kSegBlock], im[kSegBlock], re2[kSegBlock], im2[kSegBlock];
 #pragma unroll
       for (int s = 0; s < kSegBlock; ++s) {
-        const float2 zh = zc[s * G::BUF + i_h];
-        re[s] = zh.x;
-        im[s] = -zh.y;
+        const float2 zf = zc[s * G::BUF + i_f], zr = zc[s * G::BUF + i_r];
+        const float2 e = make_float2(0.5f * (zf.x + zr.x), 0.5f * (zf.y - zr.y));
+        const float2 d = make_float2(0.5f * (zf.x - zr.x), 0.5f * (zf.y + zr.y));
+        const float2 wd = cmul(w, d);
+        re[s] = e.x + wd.y;
+        im[s] = e.y - wd.x;
+        re2[s] = e.x - wd.y;
+        im2[s] = -e.y - wd.x;
       }
-      store_bin(c, pcl, N / 2, re, im);
+      store_bin(c, pcl, f, re, im);
+      if (2 * f != N) store_bin(c, pcl, N - f, re2, im2);
     }
   }
   if (CLUSTER) cg::this_cluster().barrier_wait();  // no CTA exits while its cmax may still be read
