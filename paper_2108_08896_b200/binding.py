@@ -64,7 +64,7 @@ def _load() -> C.CDLL:
     lib.delta_cross_spectra.argtypes = [vp, vp, vp, vp, vp]
     lib.delta_cross_spectra_unpack.argtypes = [vp, vp, vp, vp]
     lib.delta_internal_set_trace.argtypes = [vp, vp]   # development hook, not part of the C ABI
-    lib.delta_internal_set_epilogue_delay.argtypes = [vp, i32]   # test hook, not part of the C ABI
+    lib.delta_internal_set_jitter.argtypes = [vp, i32, i32]   # test hook, not part of the C ABI
     lib.delta_internal_probe_fabric.argtypes = [vp, C.c_size_t, vp, C.c_size_t, vp]   # measurement aid (csrc/probe.cu)
     lib.delta_coherence.argtypes = [vp, vp, vp, vp, vp]
     lib.delta_coherence_static.argtypes = [vp, vp, vp, vp, vp]
@@ -210,8 +210,9 @@ class Plan:
     def _set_trace(self, buf):
         _check(LIB.delta_internal_set_trace(self._h, None if buf is None else buf.data_ptr()), "delta_internal_set_trace")
 
-    def _set_epilogue_delay(self, ns):
-        _check(LIB.delta_internal_set_epilogue_delay(self._h, ns), "delta_internal_set_epilogue_delay")
+    def _set_jitter(self, mask, ns):
+        """Test hook (kJit* bits in csrc/delta_internal.h): the kernels' roles sleep at the named places."""
+        _check(LIB.delta_internal_set_jitter(self._h, mask, ns), "delta_internal_set_jitter")
 
     def coherence(self, S, Sauto, G=None):
         G = torch.empty((self.sizes.P, self.sizes.F), dtype=torch.float32, device=self.device) if G is None else G

@@ -306,12 +306,13 @@ int delta_internal_set_trace(delta_plan *p, void *d_trace) {
   return DELTA_OK;
 }
 
-// Test hook, not part of the C ABI: the epilogue warps of the tensor-core contraction sleep `ns` nanoseconds before every
-// accumulator unit but the first of an item.  With a slow epilogue, an MMA that reused the TMEM columns of a unit before
-// they were read out would corrupt S every time instead of once in a long while (tests/test_parity_gpu.py).
-int delta_internal_set_epilogue_delay(delta_plan *p, int ns) {
-  if (!p || ns < 0 || ns > 1000000) return DELTA_ERR_INVALID_ARG;
-  p->tc_epi_delay_ns = ns;
+// Test hook, not part of the C ABI: the producer / consumer / neighbour roles of the kernels sleep `ns` nanoseconds at the
+// places the bits of `mask` name (kJit* in delta_internal.h).  Results must not depend on it: a wait that is missing in a
+// pipeline corrupts them every time under the right skew instead of once in a long while (tests/test_parity_gpu.py).
+int delta_internal_set_jitter(delta_plan *p, int mask, int ns) {
+  if (!p || mask < 0 || ns < 0 || ns > 1000000) return DELTA_ERR_INVALID_ARG;
+  p->lay.jitter_mask = ns ? mask : 0;
+  p->lay.jitter_ns = mask ? ns : 0;
   return DELTA_OK;
 }
 

@@ -122,7 +122,6 @@ struct TcParams {
   int nunits[kTcMaxGroups];
   TcUnit units[kTcMaxGroups][kTcMaxUnits];
   int nstage, ksteps, unit_major;
-  int epi_delay_ns;  // test hook (delta_internal_set_epilogue_delay): the epilogue sleeps before units of index >= 1
   uint32_t stage_bytes, plane_bytes;  // per stage: 4 planes of 2*Cp*16 bytes
   int64_t plane_elems;                // halves between planes in global memory: Kc*Cp*8
   int64_t kstep_elems;                // halves per K=16 step inside a plane: 2*Cp*8
@@ -205,6 +204,7 @@ contract_tc_kernel(const __half *__restrict__ X, Layout lay, TcParams prm, float
       const int reps = prm.unit_major == 2 ? prm.nunits[g] : 1;
       for (int kk = 0; kk < reps * prm.ksteps; ++kk, ++kidx) {
         const int ks = kk % prm.ksteps;
+        if (lay.jitter_mask & kJitTcProducer) __nanosleep((unsigned)lay.jitter_ns);  // (test hook)
         if (pass) mbar_wait(empty_bar + s, (pass - 1) & 1u);
         if (elect_one()) {
           mbar_expect_tx(full_bar + s, prm.stage_bytes);
@@ -261,6 +261,7 @@ contract_tc_kernel(const __half *__restrict__ X, Layout lay, TcParams prm, float
     // transitions, e.g. (64, 128, 64) -> (128, 128); it is also why 256-wide units "failed parity" on config 5 in round 1.)
     int g = blockIdx.x % prm.ngroups, gp = -1;  // group of this item, of the previous item
     auto wait_unit_free = [&](int u, const TcUnit &un) {
+      if (lay.jitter_mask & kJitTcMma) __nanosleep((unsigned)lay.jitter_ns);  // (test hook)
       if ((used >> u) & 1u) {  // epilogue has drained the previous use
         mbar_wait(tempty + u, ((par >> u) & 1u) ^ 1u);
         fence_after();
@@ -361,7 +362,8 @@ contract_tc_kernel(const __half *__restrict__ X, Layout lay, TcParams prm, float
         fence_after();
         if (warp == 0) { TC_TRACE(2, tr); ++tr; }
         // (test hook: a slow epilogue makes a too-early reuse of its TMEM columns by the next item show every time)
-        if (prm.epi_delay_ns && u > 0) __nanosleep((unsigned)prm.epi_delay_ns);
+        if (((lay.jitter_mask & kJitTcEpiLate) && u > 0) || ((lay.jitter_mask & kJitTcEpiSkew) && (warp & 1)))
+          __nanosleep((unsigned)lay.jitter_ns);
         if (32 * q >= un.lane_lo && 32 * q < un.lane_hi) {
           const int jw0 = un.row0 + 32 * q, j = jw0 + lane;
           const bool jok = j < C;
@@ -470,7 +472,6 @@ int launch_contract_tc(delta_plan *p, const void *d_X, float *d_S, float *d_auto
     }
   }
   prm.ksteps = lay.Kp / 16;
-  prm.epi_delay_ns = p->tc_epi_delay_ns;
   prm.plane_bytes = (uint32_t)lay.Cp * 32u;  // [2][Cp][8] halves
   prm.stage_bytes = 4u * prm.plane_bytes;
   prm.plane_elems = (int64_t)lay.Kc * lay.Cp * kSegBlock;

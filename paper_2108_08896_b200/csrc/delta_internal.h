@@ -55,6 +55,23 @@ struct Layout {
   int64_t P, Pblk;    // all pairs i < j: the S layout
   int64_t Po, Poblk;  // output rows: P, or the length of the explicit pair list (f2)
   int64_t x_elems_per_f;  // elements (float or half) per frequency
+  // Test hook (delta_internal_set_jitter, api.cu; both 0 in normal use): the roles of the kernels sleep jitter_ns nanoseconds
+  // at the places the bits of jitter_mask name, so that a protocol that only holds for the usual relative speeds of
+  // producer, consumer and neighbours fails every time instead of once in a long while.
+  int jitter_mask, jitter_ns;
+};
+enum : int {
+  kJitTcEpiLate = 1,     // contraction: epilogue warps sleep before every accumulator unit but the first of an item
+  kJitTcEpiSkew = 2,     //              odd epilogue warps sleep before every unit
+  kJitTcProducer = 4,    //              the operand producer sleeps before every stage
+  kJitTcMma = 8,         //              the MMA issuer sleeps before every unit
+  kJitPairProducer = 16, // pair kernel: the producer sleeps before every tile
+  kJitPairTeams = 32,    //              team t sleeps t x ns before every tile
+  kJitPairWarps = 64,    //              warp w sleeps (w mod 4) x ns between the two passes
+  kJitStftStart = 128,   // STFT: CTAs start skewed
+  kJitStftMid = 256,     //       CTAs are skewed again before the write-out
+  kJitPairReorder = 512  // pair kernel: the copy of every even tile of a CTA is issued after the next tile's copy and a pause
+                         //              (concurrent bulk copies may complete in any order; this makes them)
 };
 
 // Row swizzle of the S layout.  It is XOR-linear (s_swz(a ^ b) = s_swz(a) ^ s_swz(b)), and makes the three column
@@ -106,7 +123,6 @@ struct delta_plan {
   long long *d_trace = nullptr;  // debug: clock stamps of the tensor-core contraction (delta_debug_set_trace)
   bool band_on = false;  // band-pass filter or phase-lock estimator: rho is normalised from the autospectra, not from
                          // the windowed signal energy (Parseval does not apply to the modified spectra)
-  int tc_epi_delay_ns = 0;  // test hook, see delta_internal_set_epilogue_delay (api.cu)
   bool use_pdl = true;  // programmatic dependent launch between the hot-path kernels (DELTA_NO_PDL=1 switches it off)
   bool stage_events_on = false;
   cudaEvent_t stage_ev[4] = {nullptr, nullptr, nullptr, nullptr};

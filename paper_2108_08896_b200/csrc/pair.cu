@@ -238,6 +238,7 @@ pair_kernel(const float2 *__restrict__ S, const float *__restrict__ Srsq, const 
       const int s = n % NSLOT;
       uint64_t *fullb = full + n % Cfg::NFULL;
       unsigned char *st = smem_raw + (size_t)s * Cfg::SLOT_BYTES;
+      if (lay.jitter_mask & kJitPairProducer) __nanosleep((unsigned)lay.jitter_ns);  // (test hook)
       if (n >= NSLOT) mbar_wait(empty + s, (n / NSLOT - 1) & 1);
       if (lane < PB) {
         reinterpret_cast<ushort2 *>(st + Cfg::OFF_IJ)[lane] = ij;
@@ -248,7 +249,15 @@ pair_kernel(const float2 *__restrict__ S, const float *__restrict__ Srsq, const 
       if (lane == 0) {
         const uint32_t bytes = (list ? 0u : (uint32_t)Cfg::TILE_BYTES) + (rows ? (uint32_t)(PB * Cfg::ROW_BYTES) : 0u);
         if (bytes) mbar_expect_tx(fullb, bytes); else mbar_arrive(fullb);
-        if (!list) bulk_g2s(st, S + (int64_t)tile * F * PB, (uint32_t)Cfg::TILE_BYTES, fullb);  // else: the groups gather
+        // (test hook kJitPairReorder: the copy of an even tile waits until the next tile's copy is on its way)
+        const bool defer = (lay.jitter_mask & kJitPairReorder) && !(n & 1) && n + 1 < ncta;
+        if (!list && !defer) bulk_g2s(st, S + (int64_t)tile * F * PB, (uint32_t)Cfg::TILE_BYTES, fullb);  // else: the groups gather
+        if ((lay.jitter_mask & kJitPairReorder) && (n & 1) && !list) {
+          __nanosleep((unsigned)lay.jitter_ns);
+          const int m = n - 1;
+          bulk_g2s(smem_raw + (size_t)(m % NSLOT) * Cfg::SLOT_BYTES, S + (int64_t)(blockIdx.x + m * gridDim.x) * F * PB,
+                   (uint32_t)Cfg::TILE_BYTES, full + m % Cfg::NFULL);
+        }
       }
       __syncwarp();
       // 1/sqrt(S_jj) row of every pair, from the copy of the table that is aligned for the pair's float4 groups
@@ -283,6 +292,7 @@ pair_kernel(const float2 *__restrict__ S, const float *__restrict__ Srsq, const 
     const int s = n % NSLOT;
     unsigned char *st = smem_raw + (size_t)s * Cfg::SLOT_BYTES;
     float2 *tl = reinterpret_cast<float2 *>(st);  // [F][PB], slot = (pl ^ s_swz(f)) & (PB-1)
+    if (lay.jitter_mask & kJitPairTeams) __nanosleep((unsigned)(team * lay.jitter_ns));  // (test hook)
     mbar_wait(full + n % Cfg::NFULL, (n / Cfg::NFULL) & 1);
     const ushort2 ij = reinterpret_cast<const ushort2 *>(st + Cfg::OFF_IJ)[pl];
     const int64_t p = (int64_t)tile * PB + pl;
@@ -357,6 +367,7 @@ pair_kernel(const float2 *__restrict__ S, const float *__restrict__ Srsq, const 
         if (GAPALL || A) ST1(A + p * F + f, an);
       }
     }
+    if (lay.jitter_mask & kJitPairWarps) __nanosleep((unsigned)(((tid >> 5) & 3) * lay.jitter_ns));  // (test hook)
     if (!R) {  // the slot is free once every group of this warp has read it
       __syncwarp();
       if ((tid & 31) == 0) mbar_arrive(empty + s);

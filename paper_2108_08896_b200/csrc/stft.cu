@@ -280,6 +280,7 @@ stft_kernel(const void *__restrict__ x, int64_t ld, int in_dtype, int norm_mode,
     }
   }
   pdl_wait();  // the chunk may come from the caller's previous kernel; X, wpart and the scales are read by ours
+  if (lay.jitter_mask & kJitStftStart) __nanosleep((unsigned)(((blockIdx.x * 7 + blockIdx.y * 3) % 5) * lay.jitter_ns));  // (test hook)
 
   const int tid = threadIdx.x, g = tid / T, gt = tid % T;
   const int cl = g / kSegBlock, kk = g % kSegBlock;
@@ -437,6 +438,7 @@ stft_kernel(const void *__restrict__ x, int64_t ld, int in_dtype, int norm_mode,
     __syncthreads();           // csc is visible to the CTA
   }
 
+  if (lay.jitter_mask & kJitStftMid) __nanosleep((unsigned)(((blockIdx.x * 3 + blockIdx.y + 1) % 4) * lay.jitter_ns));  // (test hook)
   // Phase 2.  Bins f and N - f come from the same pair Z[f], Z[N-f]:  with e = (Z[f] + conj Z[N-f])/2,
   // d = (Z[f] - conj Z[N-f])/2 and (a, b) = e^{-2 pi i f/L} d:  X[f] = (e.x + b, e.y - a),  X[N-f] = (e.x - b, -e.y - a).
   // One thread does both for the 8 segments of the CTA; bin N/2 (its own partner) is done once.

@@ -576,9 +576,9 @@ def test_tmem_columns_are_not_reused_before_they_are_read_out(C):
     plan = b.Plan(C, T, L, H, M, contraction=b.CONTRACT_TC)
     X = plan.stft(xd)
     S_fast = plan.cross_spectra_unpack(plan.cross_spectra(X)[0])
-    plan._set_epilogue_delay(20000)
+    plan._set_jitter(1, 20000)   # kJitTcEpiLate
     S_slow = plan.cross_spectra_unpack(plan.cross_spectra(X)[0])
-    plan._set_epilogue_delay(0)
+    plan._set_jitter(0, 0)
     torch.cuda.synchronize()
     assert torch.equal(torch.view_as_real(S_slow), torch.view_as_real(S_fast)), \
         f"{int((S_slow != S_fast).any(dim=1).sum())} pairs change with a slow epilogue"
@@ -603,6 +603,42 @@ def test_many_channels_every_row(C):
     torch.cuda.synchronize()
     st = fc.check_all_pairs(x, L, H, M, {"auto": {k: v.cpu().numpy() for k, v in out.items()}}, TOLS, f"{C} channels")
     print(C, st)
+
+
+JITTER_BITS = {1: "tc epilogue late", 2: "tc epilogue warps skewed", 4: "tc producer slow", 8: "tc mma issuer slow",
+               16: "pair producer slow", 32: "pair teams skewed", 64: "pair warps skewed", 128: "stft CTAs skewed at start",
+               256: "stft CTAs skewed before the write-out", 512: "pair tile copies land out of order"}
+
+
+@pytest.mark.parametrize("C,T,L,H,M", [
+    (192, 10000, 512, 256, 256),   # config 2: cluster STFT, one accumulator group, three pair teams over a 4-slot ring
+    (576, 2600, 512, 256, 64),     # seven accumulator groups of three TMEM layouts
+    (320, 1400, 64, 32, 32),       # eight pair teams per CTA
+    (224, 6000, 1024, 512, 512),   # one pair team, two slots
+    (40, 9000, 2048, 1024, 1024),  # pair groups wider than a warp (private exchange buffers), chscale pass
+])
+def test_results_do_not_depend_on_the_relative_speed_of_the_roles(C, T, L, H, M):
+    """Producers, consumers and neighbouring CTAs of the three kernels are slowed down one role at a time (test hook
+    delta_internal_set_jitter): every output keeps its bits.  A pipeline whose waits only hold for the usual relative speeds
+    (the pair kernel's ring and the contraction's TMEM reuse both had such a gap until round 2) fails here every time."""
+    b = binding()
+    x = dev(np.random.default_rng(C + L).standard_normal((C, T)).astype(np.float32))
+    plan = b.Plan(C, T, L, H, M)
+    ref = plan.analyze_chunk(x)
+    torch.cuda.synchronize()
+    ref = {k: v.clone() for k, v in ref.items()}
+    for mask, what in list(JITTER_BITS.items()) + [(1023, "everything at once")]:
+        # all outputs, and the cross-power alone (the pair kernel's teams then run far ahead of the tile copies)
+        for subset in (dict(), dict(G=False, A=False, R=False)):
+            plan._set_jitter(mask, 20000 if mask == 512 else 3000)
+            out = {k: v for k, v in plan.empty_outputs(**subset).items() if v is not None}
+            for v in out.values():
+                v.fill_(float("nan"))
+            plan.analyze_chunk(x, out)
+            plan._set_jitter(0, 0)
+            torch.cuda.synchronize()
+            for k, v in out.items():
+                assert torch.equal(v, ref[k]), f"{what} {subset}: {k} differs in {int((v != ref[k]).any(dim=-1).sum())} rows"
 
 
 def test_staged_external_X_with_padding_not_zeroed():
