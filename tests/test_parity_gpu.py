@@ -621,9 +621,29 @@ def test_results_do_not_depend_on_the_relative_speed_of_the_roles(C, T, L, H, M)
     """Producers, consumers and neighbouring CTAs of the three kernels are slowed down one role at a time (test hook
     delta_internal_set_jitter): every output keeps its bits.  A pipeline whose waits only hold for the usual relative speeds
     (the pair kernel's ring and the contraction's TMEM reuse both had such a gap until round 2) fails here every time."""
+    _jitter_check(dict(n_channels=C, n_samples=T, nfft=L, hop=H, max_lag=M), C + L)
+
+
+def test_results_do_not_depend_on_timing_variants():
+    """The same for the variants that take other routes through the kernels: an explicit pair list (the groups gather
+    their tile columns themselves), the band-pass filter (autospectra tables from a separate kernel), int16 input."""
     b = binding()
-    x = dev(np.random.default_rng(C + L).standard_normal((C, T)).astype(np.float32))
-    plan = b.Plan(C, T, L, H, M)
+    allp = o.all_pairs(96)
+    pairs = allp[np.sort(np.random.default_rng(5).choice(len(allp), 1501, replace=False))]
+    _jitter_check(dict(n_channels=96, n_samples=5000, nfft=256, hop=128, max_lag=128, pairs=pairs), 1)
+    _jitter_check(dict(n_channels=128, n_samples=5000, nfft=512, hop=256, max_lag=256, band=(5e3, 9e3)), 2)
+    _jitter_check(dict(n_channels=64, n_samples=5000, nfft=512, hop=256, max_lag=100, in_dtype=b.I16), 3)
+
+
+def _jitter_check(plan_kw, seed):
+    b = binding()
+    C, T = plan_kw["n_channels"], plan_kw["n_samples"]
+    xf = np.random.default_rng(seed).standard_normal((C, T))
+    if plan_kw.get("in_dtype", b.F32) == b.I16:
+        x = dev((2000 + 200 * xf).astype(np.int16))
+    else:
+        x = dev(xf.astype(np.float32))
+    plan = b.Plan(**plan_kw)
     ref = plan.analyze_chunk(x)
     torch.cuda.synchronize()
     ref = {k: v.clone() for k, v in ref.items()}
