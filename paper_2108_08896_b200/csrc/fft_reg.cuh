@@ -211,6 +211,15 @@ struct FftNamedSync {
   }
 };
 
+// The same with one named barrier per group: group g of the CTA (threads g T .. g T + T - 1, T a multiple of 32) meets at
+// barrier 1 + g, so the groups of a CTA run free of each other.  At most 15 groups wider than a warp per CTA.
+template <int T>
+struct FftGroupBarSync {
+  static __device__ __forceinline__ void sync() {
+    if (T <= 32) __syncwarp(); else asm volatile("bar.sync %0, %1;" ::"r"(1 + (int)threadIdx.x / T), "n"(T) : "memory");
+  }
+};
+
 // v[u] <-> x[tid + T*u] in, X[tid + T*u] out (unnormalised).  The slots behind `m` are shared memory owned
 // by the group; other threads of the group may still be reading them when the call returns, so the group
 // must pass another Sync::sync() before it writes them again.

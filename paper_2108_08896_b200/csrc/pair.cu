@@ -71,6 +71,7 @@ struct PairCfg {
   static constexpr size_t OFF_BAR = (OFF_FTAB + FTAB_BYTES + 7) & ~(size_t)7;              // full[NFULL], empty[NSLOT]
   static constexpr size_t SMEM = OFF_BAR + (NFULL + NSLOT) * 8;
   static_assert(TTHREADS % 32 == 0 && THREADS <= 1024 && NTEAM >= 1, "block shape");
+  static_assert(T <= 32 || CTHREADS / T <= 15, "one named barrier per group wider than a warp");
   static_assert(TILE_BYTES % 16 == 0 && ROW_BYTES % 16 == 0 && PB % 4 == 0 && 2 * PB <= 32, "tile shape");
   static_assert((T & (T - 1)) == 0 && (PB & (PB - 1)) == 0 && E % 4 == 0, "powers of two");
   static_assert(NSLOT >= 2 && NSLOT >= NTEAM && SMEM <= kSmemPerSm, "shared memory");
@@ -271,7 +272,7 @@ pair_kernel(const float2 *__restrict__ S, const float *__restrict__ Srsq, const 
   // ===== compute warps =====
   const int team = tid / Cfg::TTHREADS, tt = tid % Cfg::TTHREADS;
 
-  using Sync = FftNamedSync<T, 1, Cfg::TTHREADS>;  // groups wider than a warp: NTEAM is 1 then
+  using Sync = FftGroupBarSync<T>;  // groups wider than a warp meet at a named barrier of their own
   float2 *exch = reinterpret_cast<float2 *>(smem_raw + Cfg::OFF_EXCH);  // [PB][BUF] (narrow tiles only)
   const int pl = tt / T, gt = tt % T;
   float2 wg = __ldg(tw + gt);  // e^{-2 pi i gt / L}
@@ -401,7 +402,7 @@ pair_kernel(const float2 *__restrict__ S, const float *__restrict__ Srsq, const 
       Sync::sync();  // the group's read-back is done: the slot can be refilled
       if ((tid & 31) == 0) mbar_arrive(empty + s);
     } else {
-      if ((tid & 31) == 0) mbar_arrive(empty + s);  // T >= 64 here: Sync is a barrier over all compute warps
+      if ((tid & 31) == 0) mbar_arrive(empty + s);  // this warp's S values are in registers (the slot counts every warp)
       fft_inplace_g<Geo, true, Sync>(v, FftPadMap{exch + pl * Geo::BUF}, ftab_s, gt);
     }
     float *Rp = R + p * lay.nlags;
