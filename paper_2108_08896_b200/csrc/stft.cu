@@ -200,7 +200,9 @@ struct StftCfg {
   static constexpr int N = L / 2;
   using G = FftGeom<N>;
   static constexpr int T = G::T;
-  static constexpr int CH = N <= 512 ? 2 : 1;  // channels per CTA
+  // channels per CTA: two adjacent channels make the 16-byte pieces of the write-out whole 32-byte sectors (one channel per
+  // CTA at nfft 2048 cost 25 % of the kernel: half-written sectors, twice the SM -> L2 bytes); nfft 4096 has room for one
+  static constexpr int CH = N <= 1024 ? 2 : 1;
   static constexpr int NFFT = CH * kSegBlock;                      // transforms per CTA
   static constexpr int THREADS = NFFT * T;
   static constexpr int CHPAD = CH > 1 ? 16 / CH : 0;                 // float2 skew between channels (bank spread)
