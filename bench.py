@@ -553,9 +553,13 @@ def main():
     ap.add_argument("--scaling", default="weak", choices=["weak", "strong"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--contraction", default="auto", choices=["auto", "fp32", "tc"])
-    ap.add_argument("--inflight", type=int, default=2, help="independent chunks kept in flight (plans x streams)")
+    ap.add_argument("--inflight", type=int, default=None,
+                    help="independent chunks kept in flight (plans x streams); default 2, 1 for `wide`, whose kernels are long "
+                         "enough to fill the GPU on their own (two in flight measured 919 vs 871 us per chunk)")
     ap.add_argument("--probe-fabric", action="store_true", help="measure the SM <-> L2 rates instead of the workload")
     args = ap.parse_args()
+    if args.inflight is None:
+        args.inflight = 1 if args.workload == "wide" else 2
     if args.probe_fabric:
         probe_fabric()
         return

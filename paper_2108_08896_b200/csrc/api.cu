@@ -53,10 +53,10 @@ static size_t x_buffer_bytes(const delta_plan *p) {
 }
 
 static bool tc_supported(const delta_config *c) {
-  // two pipeline stages of 128*Cp bytes must fit in shared memory, and the tile plan must exist
+  // the tile plan must exist (up to 16 groups of accumulator units per bin: 960 channels); the operand stages of many
+  // channels are packed per unit (contract_tc.cu, mode 3), so shared memory does not limit the channel count
   size_t Cp = align_up((size_t)c->n_channels, 64);
   if (Cp < 128) Cp = 128;
-  if (Cp > 768) return false;
   TcHostPlan tmp;
   return tc_plan_tiles((int)Cp, &tmp);
 }

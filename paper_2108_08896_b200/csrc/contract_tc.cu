@@ -200,23 +200,49 @@ contract_tc_kernel(const __half *__restrict__ X, Layout lay, TcParams prm, float
     const int fstep = gridDim.x / prm.ngroups, gstep = gridDim.x % prm.ngroups;
     for (int item = blockIdx.x; item < nitems; item += gridDim.x) {
       const __half *Xf = X + (int64_t)f * lay.x_elems_per_f;
-      // mode 2 (the K steps of a bin do not fit in the ring): every unit streams the bin's operands again (L2 hits)
-      const int reps = prm.unit_major == 2 ? prm.nunits[g] : 1;
-      for (int kk = 0; kk < reps * prm.ksteps; ++kk, ++kidx) {
-        const int ks = kk % prm.ksteps;
-        if (lay.jitter_mask & kJitTcProducer) __nanosleep((unsigned)lay.jitter_ns);  // (test hook)
-        if (pass) mbar_wait(empty_bar + s, (pass - 1) & 1u);
-        if (elect_one()) {
-          mbar_expect_tx(full_bar + s, prm.stage_bytes);
-          unsigned char *dst = stages + (size_t)s * prm.stage_bytes;
+      if (prm.unit_major == 3) {
+        // mode 3 (the K steps of a bin do not fit in the ring, many channels): every unit streams its own operands, and only those: per
+        // plane and K half the 128 rows of A (channels row0 ..) and the N rows of B (channels col0 ..), packed as
+        // [plane][K half][128 + N rows][8].  (Whole-Cp stages made every unit pull all channels through the crossbar.)
+        for (int u = 0; u < prm.nunits[g]; ++u) {
+          const TcUnit un = prm.units[g][u];
+          const uint32_t R = 128u + (uint32_t)un.N;
+          for (int ks = 0; ks < prm.ksteps; ++ks, ++kidx) {
+            if (lay.jitter_mask & kJitTcProducer) __nanosleep((unsigned)lay.jitter_ns);  // (test hook)
+            if (pass) mbar_wait(empty_bar + s, (pass - 1) & 1u);
+            if (elect_one()) {
+              mbar_expect_tx(full_bar + s, 8u * R * 16u);
+              unsigned char *dst = stages + (size_t)s * prm.stage_bytes;
 #pragma unroll
-          for (int pl = 0; pl < 4; ++pl)
-            bulk_g2s(dst + (size_t)pl * prm.plane_bytes, Xf + pl * prm.plane_elems + ks * prm.kstep_elems, prm.plane_bytes,
-                     full_bar + s);
-          TC_TRACE(0, kidx);
+              for (int pk = 0; pk < 8; ++pk) {  // plane pk / 2, K half pk % 2
+                const __half *src = Xf + (pk >> 1) * prm.plane_elems + ks * prm.kstep_elems + (int64_t)(pk & 1) * lay.Cp * kSegBlock;
+                bulk_g2s(dst + (size_t)pk * R * 16u, src + (int64_t)un.row0 * kSegBlock, 128u * 16u, full_bar + s);
+                bulk_g2s(dst + (size_t)pk * R * 16u + 128u * 16u, src + (int64_t)un.col0 * kSegBlock, (uint32_t)un.N * 16u, full_bar + s);
+              }
+            }
+            __syncwarp();
+            if (++s == (uint32_t)prm.nstage) { s = 0; ++pass; }
+          }
         }
-        __syncwarp();
-        if (++s == (uint32_t)prm.nstage) { s = 0; ++pass; }
+      } else {
+        // mode 2 (the K steps do not fit in the ring, few channels): every unit streams the bin's operands again (L2 hits)
+        const int reps = prm.unit_major == 2 ? prm.nunits[g] : 1;
+        for (int kk = 0; kk < reps * prm.ksteps; ++kk, ++kidx) {
+          const int ks = kk % prm.ksteps;
+          if (lay.jitter_mask & kJitTcProducer) __nanosleep((unsigned)lay.jitter_ns);  // (test hook)
+          if (pass) mbar_wait(empty_bar + s, (pass - 1) & 1u);
+          if (elect_one()) {
+            mbar_expect_tx(full_bar + s, prm.stage_bytes);
+            unsigned char *dst = stages + (size_t)s * prm.stage_bytes;
+#pragma unroll
+            for (int pl = 0; pl < 4; ++pl)
+              bulk_g2s(dst + (size_t)pl * prm.plane_bytes, Xf + pl * prm.plane_elems + ks * prm.kstep_elems, prm.plane_bytes,
+                       full_bar + s);
+            TC_TRACE(0, kidx);
+          }
+          __syncwarp();
+          if (++s == (uint32_t)prm.nstage) { s = 0; ++pass; }
+        }
       }
       f += fstep; g += gstep;
       if (g >= prm.ngroups) { g -= prm.ngroups; ++f; }
@@ -231,7 +257,8 @@ contract_tc_kernel(const __half *__restrict__ X, Layout lay, TcParams prm, float
     const uint32_t st16 = smem_u32(stages) >> 4, stage16 = prm.stage_bytes >> 4, plane16 = prm.plane_bytes >> 4;
 
     // the twelve MMAs of one (unit, K step): Re += A_j A_i + B_j B_i;  Im += A_j B_i - B_j A_i  (rows j, cols i)
-    auto issue = [&](uint32_t ao16, uint32_t bo16, uint32_t id, uint32_t idn, uint32_t d_re, uint32_t d_im, uint32_t s, uint32_t acc) {
+    auto issue = [&](uint64_t dbase, uint32_t plane16, uint32_t ao16, uint32_t bo16, uint32_t id, uint32_t idn, uint32_t d_re,
+                     uint32_t d_im, uint32_t s, uint32_t acc) {
       const uint64_t sb = dbase + (st16 + s * stage16);
       const uint64_t a_hr = sb + ao16, a_hi = a_hr + plane16, a_lr = a_hi + plane16, a_li = a_lr + plane16;
       const uint64_t b_hr = sb + bo16, b_hi = b_hr + plane16, b_lr = b_hi + plane16, b_li = b_lr + plane16;
@@ -289,19 +316,24 @@ contract_tc_kernel(const __half *__restrict__ X, Layout lay, TcParams prm, float
     const int gstep = gridDim.x % prm.ngroups;
     for (int item = blockIdx.x; item < nitems; item += gridDim.x) {
       const int nu = prm.nunits[g];
-      if (prm.unit_major == 2) {
+      if (prm.unit_major >= 2) {
         // unit after unit, each with its own pass over the K steps: the epilogue of unit u overlaps the MMAs of unit u+1
         uint32_t s = s0, pass = pass0;
         for (int u = 0; u < nu; ++u) {
           const TcUnit un = prm.units[g][u];
-          const uint32_t ao16 = (uint32_t)(un.row0 / 8) * 8u, bo16 = (uint32_t)(un.col0 / 8) * 8u;
+          // mode 3, packed stage of this unit: A rows at 0, B rows at 128, R = 128 + N rows per K half
+          const bool packed = prm.unit_major == 3;
+          const uint32_t R = 128u + (uint32_t)un.N;
+          const uint64_t dbase_u = packed ? make_sdesc(0, R * 16u, sbo) : dbase;
+          const uint32_t plane16_u = packed ? 2u * R : plane16;
+          const uint32_t ao16 = packed ? 0u : (uint32_t)(un.row0 / 8) * 8u, bo16 = packed ? 128u : (uint32_t)(un.col0 / 8) * 8u;
           const uint32_t id = make_idesc(un.N, 0), idn = make_idesc(un.N, 1);
           const uint32_t d_re = tmem_base + (uint32_t)un.tm, d_im = d_re + (uint32_t)un.N;
           wait_unit_free(u, un);
           for (int ks = 0; ks < prm.ksteps; ++ks) {
             mbar_wait(full_bar + s, pass & 1u);
             fence_after();
-            issue(ao16, bo16, id, idn, d_re, d_im, s, ks > 0 ? 1u : 0u);
+            issue(dbase_u, plane16_u, ao16, bo16, id, idn, d_re, d_im, s, ks > 0 ? 1u : 0u);
             if (elect_one()) mma_commit(empty_bar + s);
             __syncwarp();
             if (++s == (uint32_t)prm.nstage) { s = 0; ++pass; }
@@ -323,7 +355,7 @@ contract_tc_kernel(const __half *__restrict__ X, Layout lay, TcParams prm, float
               fence_after();
               if (lane == 0) TC_TRACE(4, tr);
             }
-            issue(ao16, bo16, id, idn, d_re, d_im, s, ks > 0 ? 1u : 0u);
+            issue(dbase, plane16, ao16, bo16, id, idn, d_re, d_im, s, ks > 0 ? 1u : 0u);
             if (u == nu - 1) {  // stage reusable once every unit has read it
               if (elect_one()) mma_commit(empty_bar + s);
               __syncwarp();
@@ -479,11 +511,18 @@ int launch_contract_tc(delta_plan *p, const void *d_X, float *d_S, float *d_auto
   const size_t fixed = (size_t)lay.Cp * sizeof(float2) + 64 * sizeof(uint64_t) + 64;
   int nstage = (int)((200 * 1024 - fixed) / prm.stage_bytes);
   if (nstage > 8) nstage = 8;
+  // 1: all K steps of a bin stay in the ring and are shared by its units;  2: every unit streams the bin's operands again;
+  // 3: every unit streams its own 128 + N <= 256 operand rows, packed (less than all channels from 320 channels on: at 192
+  //    the packed stages carry MORE rows, 84.9 vs 82.9 us at config 3; at 384 / 576 channels 222 vs 261 and 115 vs 125 us)
+  // (K-step-major order, all units advancing together, was measured slower: their epilogues cannot overlap the MMAs)
+  prm.unit_major = (nstage >= 2 && 2 * prm.ksteps <= nstage) ? 1 : (lay.Cp > 256 ? 3 : 2);
+  if (prm.unit_major == 3) {  // [4 planes][2 K halves][256 rows][8 halves]
+    prm.stage_bytes = 8u * 256u * 16u;
+    nstage = (int)((200 * 1024 - fixed) / prm.stage_bytes);
+    if (nstage > 6) nstage = 6;
+  }
   if (nstage < 2) return DELTA_ERR_UNSUPPORTED;
   prm.nstage = nstage;
-  // 1: all K steps of a bin stay in the ring and are shared by its units;  2: every unit streams them again
-  // (K-step-major order, all units advancing together, was measured slower: their epilogues cannot overlap the MMAs)
-  prm.unit_major = (2 * prm.ksteps <= nstage) ? 1 : 2;
   size_t smem = (size_t)nstage * prm.stage_bytes + fixed;
   if (smem < 120 * 1024) smem = 120 * 1024;  // one CTA per SM: each CTA allocates all 512 TMEM columns
   const int nitems = lay.F * prm.ngroups;

@@ -586,10 +586,10 @@ def test_tmem_columns_are_not_reused_before_they_are_read_out(C):
     assert torch.max(torch.abs(S_fast - S_ref)).item() <= 2e-5 * scale   # split-fp16 tensor cores vs the FP32 pipe
 
 
-@pytest.mark.parametrize("C", [448, 640, 768, 800])
+@pytest.mark.parametrize("C", [448, 640, 768, 960, 1000])
 def test_many_channels_every_row(C):
-    """Channel counts beyond the three-view array: up to 768 channels the tensor-core contraction is chosen (13 groups of
-    accumulator units per bin at 768), beyond that the FP32 one.  Short transform and few lags to keep it small; every row
+    """Channel counts beyond the three-view array: up to 960 channels the tensor-core contraction is chosen (16 groups of
+    accumulator units per bin at 960), beyond that the FP32 one.  Short transform and few lags to keep it small; every row
     of every output against the float64 pipeline (tests/fastcheck.py)."""
     import fastcheck as fc
     b = binding()
@@ -598,7 +598,7 @@ def test_many_channels_every_row(C):
     common = rng.standard_normal(T)
     x = (rng.uniform(0.0, 1.0, (C, 1)) * common + rng.standard_normal((C, T))).astype(np.float32)
     plan = b.Plan(C, T, L, H, M)
-    assert plan.sizes.contraction == (b.CONTRACT_TC if C <= 768 else b.CONTRACT_FP32)
+    assert plan.sizes.contraction == (b.CONTRACT_TC if C <= 960 else b.CONTRACT_FP32)
     out = plan.analyze_chunk(dev(x))
     torch.cuda.synchronize()
     st = fc.check_all_pairs(x, L, H, M, {"auto": {k: v.cpu().numpy() for k, v in out.items()}}, TOLS, f"{C} channels")
