@@ -74,9 +74,10 @@ enum { DELTA_F32 = 0, DELTA_I16 = 1 };               /* element type of the inpu
 enum { DELTA_NORM_NONE = 0,                          /* y = x                                         */
        DELTA_NORM_SUBTRACT = 1,                      /* y = x - o_c                                   */
        DELTA_NORM_RELATIVE = 2 };                    /* y = (x - o_c)/o_c   (delta T_e/<T_e>, L89)    */
-enum { DELTA_CONTRACT_AUTO = 0,                      /* library picks (tensor cores when available)   */
+enum { DELTA_CONTRACT_AUTO = 0,                      /* library picks: tensor cores up to 960 channels */
        DELTA_CONTRACT_FP32 = 1,                      /* Eq. (1a) on the FP32 FMA pipe                 */
-       DELTA_CONTRACT_TC = 2 };                      /* Eq. (1a) on tcgen05 tensor cores, split fp16  */
+       DELTA_CONTRACT_TC = 2 };                      /* Eq. (1a) on tcgen05 tensor cores, split fp16;
+                                                        more than 960 channels: DELTA_ERR_UNSUPPORTED */
 
 typedef struct {
   int32_t n_channels;   /* C >= 1                                                                     */
